@@ -1,0 +1,267 @@
+"""ctypes binding of the CPU oracle (oracle/libmco.so).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg
+may import this module.  It never imports the product package's CUDA binding.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_dp = C.POINTER(C.c_double)
+_fp = C.POINTER(C.c_float)
+_ip = C.POINTER(C.c_int32)
+
+
+class FieldParams(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("sigma", C.c_float), ("radius", C.c_int32),
+                ("coupling", C.c_float), ("n_sources", C.c_int32), ("sources", _fp)]
+
+
+class WorldParams(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("dt", C.c_float), ("nu", C.c_float),
+                ("trt_lambda", C.c_float), ("rho0", C.c_float), ("k_el", C.c_float),
+                ("pbd_iters", C.c_int32), ("n_fields", C.c_int32), ("fields", FieldParams * 4),
+                ("max_beads", C.c_int64)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        L.mco_phi.restype = C.c_double
+        L.mco_phi.argtypes = [C.c_double]
+        L.mco_last_error.restype = C.c_char_p
+        L.mco_last_error.argtypes = [C.c_void_p]
+        L.mco_destroy.restype = None
+        L.mco_destroy.argtypes = [C.c_void_p]
+        L.mco_radius.restype = C.c_int32
+        L.mco_radius.argtypes = [C.c_double, C.c_int32]
+        _lib = L
+    return _lib
+
+
+def _d(a):
+    return None if a is None else a.ctypes.data_as(_dp)
+
+
+def _f(a):
+    return None if a is None else a.ctypes.data_as(_fp)
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def make_params(p: dict):
+    """dict (worlds.py) -> (WorldParams, keepalive list)."""
+    wp = WorldParams()
+    keep = []
+    for k in ("nx", "ny", "pbd_iters"):
+        setattr(wp, k, int(p[k]))
+    for k in ("dt", "nu", "trt_lambda", "rho0", "k_el"):
+        setattr(wp, k, float(p[k]))
+    wp.n_fields = len(p["fields"])
+    wp.max_beads = int(p["max_beads"])
+    for i, fd in enumerate(p["fields"]):
+        fp = wp.fields[i]
+        fp.kind = int(fd["kind"])
+        fp.sigma = float(fd["sigma"])
+        fp.radius = int(fd["radius"])
+        fp.coupling = float(fd["coupling"])
+        src = fd.get("sources")
+        if src is not None:
+            src = _f32(src).reshape(-1, 4)
+            keep.append(src)
+            fp.n_sources = src.shape[0]
+            fp.sources = _f(src)
+        else:
+            fp.n_sources = 0
+            fp.sources = None
+    return wp, keep
+
+
+class World:
+    """Oracle world: mco_create + mco_load_filaments from a worlds.py dict."""
+
+    def __init__(self, world: dict, fp32_state: bool = False, threads: int = 0):
+        L = lib()
+        self.p = world["params"]
+        self.nx, self.ny = int(self.p["nx"]), int(self.p["ny"])
+        self.n_fields = len(self.p["fields"])
+        wp, self._keep = make_params(self.p)
+        h = C.c_void_p()
+        rc = L.mco_create(C.byref(wp), C.byref(h))
+        if rc != 0:
+            raise ValueError(f"mco_create failed: {rc}")
+        self.h = h
+        off = np.ascontiguousarray(world["offsets"], dtype=np.int32)
+        self.N = int(off[-1])
+        arrs = [_f32(world[k]) for k in ("xy", "L_rest", "theta_rest", "k_bend", "k_shear",
+                                        "k_stretch", "act_amp", "act_phase", "act_period")]
+        rc = L.mco_load_filaments(h, C.c_int32(len(off) - 1), off.ctypes.data_as(_ip),
+                                  *[_f(a) for a in arrs])
+        if rc != 0:
+            msg = L.mco_last_error(h).decode()
+            L.mco_destroy(h)
+            self.h = None
+            raise ValueError(f"mco_load_filaments failed: {rc} {msg}")
+        if fp32_state:
+            L.mco_set_fp32_state(h, 1)
+        L.mco_set_threads(h, int(threads))
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().mco_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        self.close()
+
+    def set_state(self, step: int, xy=None, fdev=None):
+        xy = None if xy is None else _f64(xy)
+        fdev = None if fdev is None else _f64(fdev)
+        rc = lib().mco_set_state(self.h, C.c_int64(step), _d(xy), _d(fdev))
+        if rc != 0:
+            raise ValueError(f"mco_set_state failed: {rc}")
+
+    def set_threads(self, k: int):
+        lib().mco_set_threads(self.h, int(k))
+
+    def step(self, n: int = 1):
+        rc = lib().mco_step(self.h, C.c_int32(n))
+        if rc != 0:
+            raise RuntimeError(f"mco_step failed: {rc} {lib().mco_last_error(self.h).decode()}")
+
+    def read_state(self) -> dict:
+        ny, nx, N = self.ny, self.nx, self.N
+        out = dict(xy=np.empty((N, 2)), u=np.empty((2, ny, nx)), rho=np.empty((ny, nx)),
+                   fdev=np.empty((9, ny, nx)), field=np.empty((self.n_fields, ny, nx)),
+                   force=np.empty((N, 2)), sense=np.empty(N))
+        st = C.c_int64()
+        rc = lib().mco_read_state(self.h, C.byref(st), _d(out["xy"]), _d(out["u"]), _d(out["rho"]),
+                                  _d(out["fdev"]), _d(out["field"]), _d(out["force"]),
+                                  _d(out["sense"]))
+        if rc != 0:
+            raise RuntimeError(f"mco_read_state failed: {rc}")
+        out["step"] = int(st.value)
+        return out
+
+    def read_intermediates(self) -> dict:
+        ny, nx, N = self.ny, self.nx, self.N
+        out = dict(D=np.empty((N, 2)), rho_b=np.empty((ny, nx)), G=np.empty((2, ny, nx)))
+        lib().mco_read_intermediates(self.h, _d(out["D"]), _d(out["rho_b"]), _d(out["G"]))
+        return out
+
+
+# ---- stateless components ----
+def phi(r: float) -> float:
+    return float(lib().mco_phi(float(r)))
+
+
+def support(x: float):
+    i0 = C.c_int32()
+    w = (C.c_double * 4)()
+    lib().mco_support(C.c_double(x), C.byref(i0), w)
+    return int(i0.value), np.array(w[:])
+
+
+def elastic(offsets, xy, L_rest, theta_rest, k_bend, k_shear, k_stretch, act_amp, act_phase,
+            act_period, dt: float, n: int) -> np.ndarray:
+    off = np.ascontiguousarray(offsets, dtype=np.int32)
+    xy = _f64(xy)
+    N = int(off[-1])
+    arrs = [_f32(a) for a in (L_rest, theta_rest, k_bend, k_shear, k_stretch, act_amp, act_phase,
+                              act_period)]
+    D = np.empty((N, 2))
+    rc = lib().mco_elastic(C.c_int32(len(off) - 1), off.ctypes.data_as(_ip), _d(xy),
+                           *[_f(a) for a in arrs], C.c_double(dt), C.c_int64(n), _d(D))
+    if rc != 0:
+        raise ValueError(f"mco_elastic failed: {rc}")
+    return D
+
+
+def deposit(nx, ny, xy) -> np.ndarray:
+    xy = _f64(xy)
+    out = np.empty((ny, nx))
+    lib().mco_deposit(C.c_int32(nx), C.c_int32(ny), C.c_int64(len(xy)), _d(xy), _d(out))
+    return out
+
+
+def spread(nx, ny, xy, F) -> np.ndarray:
+    xy, F = _f64(xy), _f64(F)
+    out = np.empty((2, ny, nx))
+    lib().mco_spread(C.c_int32(nx), C.c_int32(ny), C.c_int64(len(xy)), _d(xy), _d(F), _d(out))
+    return out
+
+
+def interp(planes, xy) -> np.ndarray:
+    planes, xy = _f64(planes), _f64(xy)
+    nch, ny, nx = planes.shape
+    out = np.empty((len(xy), nch))
+    lib().mco_interp(C.c_int32(nx), C.c_int32(ny), C.c_int32(nch), _d(planes), C.c_int64(len(xy)),
+                     _d(xy), _d(out))
+    return out
+
+
+def radius(sigma: float, r: int = 0) -> int:
+    return int(lib().mco_radius(float(sigma), int(r)))
+
+
+def gauss_taps(sigma: float, R: int) -> np.ndarray:
+    t = np.empty(2 * R + 1)
+    lib().mco_gauss_taps(C.c_double(sigma), C.c_int32(R), _d(t))
+    return t
+
+
+def blur(a, sigma: float, R: int) -> np.ndarray:
+    a = _f64(a)
+    ny, nx = a.shape
+    out = np.empty((ny, nx))
+    lib().mco_blur(C.c_int32(nx), C.c_int32(ny), _d(a), C.c_double(sigma), C.c_int32(R), _d(out))
+    return out
+
+
+def grad(a):
+    a = _f64(a)
+    ny, nx = a.shape
+    gx, gy = np.empty((ny, nx)), np.empty((ny, nx))
+    lib().mco_grad(C.c_int32(nx), C.c_int32(ny), _d(a), _d(gx), _d(gy))
+    return gx, gy
+
+
+def static_field(nx, ny, sources) -> np.ndarray:
+    s = _f32(sources).reshape(-1, 4)
+    out = np.empty((ny, nx))
+    lib().mco_static_field(C.c_int32(nx), C.c_int32(ny), C.c_int32(len(s)), _f(s), _d(out))
+    return out
+
+
+def lattice_constants(nu: float, dt: float, lam: float):
+    a, b = C.c_double(), C.c_double()
+    lib().mco_lattice_constants(C.c_double(nu), C.c_double(dt), C.c_double(lam), C.byref(a),
+                                C.byref(b))
+    return float(a.value), float(b.value)
+
+
+def lbm_step(f, G, omega_plus: float, omega_minus: float):
+    """f [9,ny,nx] un-shifted (modified copy returned), G [2,ny,nx] or None -> (f', u)."""
+    f = _f64(f).copy()
+    _, ny, nx = f.shape
+    G = None if G is None else _f64(G)
+    u = np.empty((2, ny, nx))
+    lib().mco_lbm_step(C.c_int32(nx), C.c_int32(ny), _d(f), _d(G), C.c_double(omega_plus),
+                       C.c_double(omega_minus), _d(u))
+    return f, u

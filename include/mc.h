@@ -1,0 +1,153 @@
+/* mc.h -- C ABI of the B200-native Microcosmos per-timestep update (libmc.so).
+ *
+ * The library advances a 2-D periodic world that holds many elastic filament chains
+ * two-way coupled to a D2Q9 lattice-Boltzmann fluid and to scalar fields, in the
+ * discretisation of arxiv/paper_2607_02954 (cited as P:L<line> of PAPER.md; readings of
+ * the paper's silences are numbered in DESIGN.md "Readings").  Every step of the path
+ * runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ *
+ * One step (state at step n -> n+1), in this order (north_star of BASELINE.json):
+ *   S0 actuation of the rest angle          P:L153, L171      (reading 18)
+ *   S1 elastic PBD displacement, Eq. 1-4     P:L91-113         (readings 1-5)
+ *   S2 deposit beads -> rho_b                P:L119            (reading 13)
+ *   S3 Gaussian filter + gradient            P:L119            (readings 14, 15)
+ *   S4 field forces at the beads             P:L119, L121, L175 (readings 16, 17)
+ *   S5 spread bead forces -> G               P:L125            (reading 7)
+ *   S6 D2Q9 TRT collide (Guo source) + stream P:L117-119, L127 (readings 10, 11)
+ *   S7 interpolate u at the beads, X += U    P:L125            (readings 11, 12, 19)
+ *
+ * Conventions.  Grid node (i,j) sits at position (i,j); cell size 1; periodic domain
+ * [0,nx) x [0,ny).  Grid arrays are row-major, x fastest (index j*nx+i); multi-channel
+ * arrays are planes ([q][j][i]).  Bead arrays are chain-ordered (bead offsets[f]+i).
+ * Bead positions are unwrapped; only grid indices wrap.  Everything is fp32 in memory.
+ * D2Q9 numbering: c0=(0,0) c1=(1,0) c2=(0,1) c3=(-1,0) c4=(0,-1) c5=(1,1) c6=(-1,1)
+ * c7=(-1,-1) c8=(1,-1); w0=4/9, w1..4=1/9, w5..8=1/36.
+ *
+ * Pointers: every pointer argument says HOST or DEVICE.  The caller owns all memory it
+ * passes in; the library copies what it needs into the workspace and keeps no caller
+ * pointer after the call returns.  No allocation of device memory happens inside the
+ * library: all device state lives in the caller-provided workspace.
+ *
+ * Errors: every call returns 0 (MC_OK) or a negative code; the message is available from
+ * mc_last_error.  Nothing throws or aborts across the ABI.
+ *
+ * Threading: one world = one stream; calls on one world are not re-entrant.
+ * Determinism: same inputs => bit-identical outputs of mc_read_state, run to run.
+ */
+#ifndef MC_H
+#define MC_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mc_world mc_world; /* opaque host-side handle */
+
+enum { MC_OK = 0, MC_EINVAL = -1, MC_ENOMEM = -2, MC_ECUDA = -3, MC_ESTATE = -4, MC_EDIVERGED = -5 };
+
+enum {
+  MC_FIELD_BEAD_DENSITY = 0, /* beads deposit; force = -k * grad(gauss * rho_b)  */
+  MC_FIELD_STATIC_SOURCE = 1 /* Gaussian packets; force = +k * grad(c); c is sensed P:L121 */
+};
+
+typedef struct {
+  int32_t kind;         /* MC_FIELD_*                                                     */
+  float sigma;          /* Gaussian filter width in cells (bead-density fields), > 0       */
+  int32_t radius;       /* truncation radius R of the filter; 0 => ceil(5*sigma); R <= 16  */
+  float coupling;       /* k_rep or chi in physical units; lattice value = coupling*dt^2   */
+  int32_t n_sources;    /* static-source fields: number of packets                         */
+  const float* sources; /* HOST [n_sources][4] = cx, cy, amplitude, width (cells)          */
+} mc_field_params;
+
+typedef struct {
+  int32_t nx, ny;    /* periodic grid, each a multiple of 32, >= 32                        */
+  float dt;          /* physical time per step (> 0)                                       */
+  float nu;          /* kinematic viscosity, cell^2/time; nu_lat = nu*dt; tau+ = 3nu_lat+.5 */
+  float trt_lambda;  /* TRT magic parameter Lambda (> 0), 0.25 is the usual choice         */
+  float rho0;        /* rest density of the fluid (> 0), 1.0                               */
+  float k_el;        /* elastic coupling, 1/time^2; kappa = k_el*dt^2 (reading 1)          */
+  int32_t pbd_iters; /* must be 1 (reading 3)                                              */
+  int32_t n_fields;  /* 0..4                                                               */
+  mc_field_params fields[4];
+  int64_t max_beads; /* capacity; mc_load_filaments may load up to this many beads         */
+} mc_world_params;
+
+/* Bytes of DEVICE workspace mc_create needs for these parameters (0 if they are invalid). */
+size_t mc_workspace_bytes(const mc_world_params* p /*HOST*/);
+
+/* Create a world: fluid at rest (f_q = w_q rho0), no filaments, step counter 0.
+ * workspace: DEVICE, >= mc_workspace_bytes(p) bytes, 256-byte aligned, owned by the caller and
+ * must outlive the world.  cuda_stream: a cudaStream_t (NULL = legacy default stream); all
+ * work of this world is enqueued on it.  *out receives the handle.
+ * Errors: MC_EINVAL (bad parameters, workspace too small or misaligned), MC_ENOMEM (host),
+ * MC_ECUDA. */
+int mc_create(const mc_world_params* p /*HOST*/, void* workspace /*DEVICE*/, size_t workspace_bytes,
+              void* cuda_stream, mc_world** out /*HOST*/);
+
+/* Load (replace) the filaments.  offsets: HOST int32 [n_fil+1], offsets[0] = 0, chain f owns
+ * beads offsets[f] .. offsets[f+1]-1, every chain >= 3 beads, N = offsets[n_fil] <= max_beads.
+ * All other arrays are DEVICE float arrays, chain-ordered:
+ *   xy [N][2] unwrapped positions;
+ *   L_rest[i], k_shear[i], k_stretch[i] belong to edge (i,i+1) (last entry of a chain unused);
+ *   theta_rest[i], k_bend[i], act_amp[i], act_phase[i], act_period[i] belong to the joint at
+ *   bead i (first/last entry of a chain unused);
+ *   theta*_i(n) = theta_rest[i] + act_amp[i]*sin(2*pi*n*dt/act_period[i] + act_phase[i]).
+ * Stiffnesses must lie in [0,1] and periods be > 0, else MC_EINVAL.  Synchronises the stream.
+ * The fluid state and the step counter are left as they are. */
+int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets /*HOST*/,
+                      const float* xy /*DEVICE*/, const float* L_rest /*DEVICE*/,
+                      const float* theta_rest /*DEVICE*/, const float* k_bend /*DEVICE*/,
+                      const float* k_shear /*DEVICE*/, const float* k_stretch /*DEVICE*/,
+                      const float* act_amp /*DEVICE*/, const float* act_phase /*DEVICE*/,
+                      const float* act_period /*DEVICE*/);
+
+/* Advance n >= 0 steps.  Asynchronous: kernels are enqueued on the world's stream and the
+ * call returns without synchronising.  Errors: MC_EINVAL, MC_ECUDA (launch failure),
+ * MC_EDIVERGED (a previous mc_read_state saw the sticky divergence flag: non-finite bead
+ * position or |u| > 0.3). */
+int mc_step(mc_world* w, int32_t n);
+
+/* Copy the state out.  Synchronises the stream.  Every output pointer is DEVICE memory of the
+ * stated size and may be NULL (skipped); step_out is HOST.
+ *   xy    [N][2]        bead positions
+ *   u     [2][ny][nx]   velocity stored by the last step's S6 (lattice units)
+ *   rho   [ny][nx]      fluid density sum_q f_q of the current (pre-collision) populations
+ *   fdev  [9][ny][nx]   current pre-collision populations as deviations f_q - w_q*rho0
+ *                       (the library stores populations shifted; un-shifting in fp32 would
+ *                       throw their low bits away)
+ *   field [n_fields][ny][nx]  last step's filtered bead density, or the static field c
+ *   force [N][2]        last step's total bead force F_i (lattice units)
+ *   sense [N]           last step's sum over static fields of c interpolated at the bead
+ * Returns MC_EDIVERGED (after filling the outputs) if the divergence flag is set. */
+int mc_read_state(mc_world* w, int64_t* step_out /*HOST*/, float* xy, float* u, float* rho,
+                  float* fdev, float* field, float* force, float* sense);
+
+/* Last step's intermediates, for parity checks (same rules as mc_read_state):
+ *   rho_b [ny][nx] deposited bead density (S2); G [2][ny][nx] spread force (S5). */
+int mc_read_intermediates(mc_world* w, float* rho_b, float* G);
+
+/* Optional per-kernel timing with CUDA events on the world's stream (used by bench.py for the
+ * roofline line; off by default, costs one event record per kernel group when on).
+ * Slots: 0 K0 bin, 1 K2a deposit, 2 K3a filter+gradient, 3 K1 filament force, 4 K2b spread,
+ * 5 K3b fluid, 6 K4 interpolate+integrate.  mc_profile_enable(w,1) starts a capture of up to
+ * 64 steps; mc_profile_read synchronises, writes the summed milliseconds per slot to
+ * ms (HOST float[MC_PROF_SLOTS]) and the number of captured steps, and restarts the capture. */
+#define MC_PROF_SLOTS 7
+int mc_profile_enable(mc_world* w, int32_t on);
+int mc_profile_read(mc_world* w, float* ms /*HOST*/, int32_t* steps /*HOST*/);
+
+/* Kernels launched on the world's stream since mc_create (a plain host counter). */
+int64_t mc_launch_count(const mc_world* w);
+
+/* Frees the host handle only (the workspace belongs to the caller).  NULL is allowed. */
+void mc_destroy(mc_world* w);
+
+/* Message of the last error on this world (handle-owned string; "" if none).  With
+ * w == NULL returns the message of the last failed mc_create on this thread. */
+const char* mc_last_error(const mc_world* w);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

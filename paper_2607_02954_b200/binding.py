@@ -1,0 +1,225 @@
+"""Thin ctypes binding of libmc.so (include/mc.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels.  PyTorch is used for device
+memory (the workspace and the in/out arrays) and the stream.  There is no CPU fallback:
+`load_library()` raises if libmc.so is missing and `World` raises without a CUDA device.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmc.so")
+
+MC_OK, MC_EINVAL, MC_ENOMEM, MC_ECUDA, MC_ESTATE, MC_EDIVERGED = 0, -1, -2, -3, -4, -5
+SYMBOLS = ("mc_workspace_bytes", "mc_create", "mc_load_filaments", "mc_step", "mc_read_state",
+           "mc_read_intermediates", "mc_launch_count", "mc_destroy", "mc_last_error",
+           "mc_profile_enable", "mc_profile_read")
+PROF_SLOTS = ("K0_bin", "K2a_deposit", "K3a_blur_grad", "K1_filament", "K2b_spread", "K3b_lbm",
+              "K4_interp_integrate")
+
+_fp = C.POINTER(C.c_float)
+
+
+class FieldParams(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("sigma", C.c_float), ("radius", C.c_int32),
+                ("coupling", C.c_float), ("n_sources", C.c_int32), ("sources", _fp)]
+
+
+class WorldParams(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("dt", C.c_float), ("nu", C.c_float),
+                ("trt_lambda", C.c_float), ("rho0", C.c_float), ("k_el", C.c_float),
+                ("pbd_iters", C.c_int32), ("n_fields", C.c_int32), ("fields", FieldParams * 4),
+                ("max_beads", C.c_int64)]
+
+
+class McError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libmc error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libmc.so and declare the prototypes.  Raises if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise FileNotFoundError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2607_02954_b200.build` "
+            "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+    L.mc_workspace_bytes.restype = C.c_size_t
+    L.mc_workspace_bytes.argtypes = [C.POINTER(WorldParams)]
+    L.mc_create.restype = C.c_int
+    L.mc_create.argtypes = [C.POINTER(WorldParams), vp, C.c_size_t, vp, C.POINTER(vp)]
+    L.mc_load_filaments.restype = C.c_int
+    L.mc_load_filaments.argtypes = [vp, i32, C.POINTER(i32)] + [vp] * 9
+    L.mc_step.restype = C.c_int
+    L.mc_step.argtypes = [vp, i32]
+    L.mc_read_state.restype = C.c_int
+    L.mc_read_state.argtypes = [vp, C.POINTER(i64)] + [vp] * 7
+    L.mc_read_intermediates.restype = C.c_int
+    L.mc_read_intermediates.argtypes = [vp, vp, vp]
+    L.mc_launch_count.restype = i64
+    L.mc_launch_count.argtypes = [vp]
+    L.mc_profile_enable.restype = C.c_int
+    L.mc_profile_enable.argtypes = [vp, i32]
+    L.mc_profile_read.restype = C.c_int
+    L.mc_profile_read.argtypes = [vp, _fp, C.POINTER(i32)]
+    L.mc_destroy.restype = None
+    L.mc_destroy.argtypes = [vp]
+    L.mc_last_error.restype = C.c_char_p
+    L.mc_last_error.argtypes = [vp]
+    _lib = L
+    return L
+
+
+def make_params(p: dict):
+    """worlds.py params dict -> (WorldParams, keepalive)."""
+    wp = WorldParams()
+    keep = []
+    for k in ("nx", "ny", "pbd_iters"):
+        setattr(wp, k, int(p[k]))
+    for k in ("dt", "nu", "trt_lambda", "rho0", "k_el"):
+        setattr(wp, k, float(p[k]))
+    wp.n_fields = len(p["fields"])
+    wp.max_beads = int(p["max_beads"])
+    for i, fd in enumerate(p["fields"][:4]):
+        fp = wp.fields[i]
+        fp.kind, fp.sigma = int(fd["kind"]), float(fd["sigma"])
+        fp.radius, fp.coupling = int(fd["radius"]), float(fd["coupling"])
+        src = fd.get("sources")
+        if src is not None:
+            src = np.ascontiguousarray(src, dtype=np.float32).reshape(-1, 4)
+            keep.append(src)
+            fp.n_sources = src.shape[0]
+            fp.sources = src.ctypes.data_as(_fp)
+        else:
+            fp.n_sources = 0
+            fp.sources = None
+    return wp, keep
+
+
+def workspace_bytes(params: dict) -> int:
+    wp, _keep = make_params(params)
+    return int(load_library().mc_workspace_bytes(C.byref(wp)))
+
+
+_CHAIN_KEYS = ("xy", "L_rest", "theta_rest", "k_bend", "k_shear", "k_stretch", "act_amp",
+               "act_phase", "act_period")
+
+
+class World:
+    """mc_create + mc_load_filaments from a worlds.py dict; mc_step; mc_read_state."""
+
+    def __init__(self, world: dict, device: str = "cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2607_02954_b200 needs a CUDA device (no CPU fallback)")
+        L = load_library()
+        self.torch = torch
+        self.device = torch.device(device)
+        self.p = world["params"]
+        self.nx, self.ny = int(self.p["nx"]), int(self.p["ny"])
+        self.n_fields = len(self.p["fields"])
+        self.h = None
+        with torch.cuda.device(self.device):
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            wp, keep = make_params(self.p)
+            nbytes = int(L.mc_workspace_bytes(C.byref(wp)))
+            if nbytes == 0:
+                raise McError(MC_EINVAL, "invalid world parameters")
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            h = C.c_void_p()
+            rc = L.mc_create(C.byref(wp), self.workspace.data_ptr(), nbytes,
+                             C.c_void_p(self.stream.cuda_stream), C.byref(h))
+            if rc != MC_OK:
+                raise McError(rc, L.mc_last_error(None).decode())
+            self.h = h
+            self.N = 0
+            if "offsets" in world:
+                self.load_filaments(world)
+
+    # -- mc_load_filaments: host numpy arrays or device tensors --
+    def load_filaments(self, world: dict):
+        torch = self.torch
+        off = np.ascontiguousarray(world["offsets"], dtype=np.int32)
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):
+            dev = []
+            for k in _CHAIN_KEYS:
+                a = world[k]
+                if not isinstance(a, torch.Tensor):
+                    a = torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32))
+                dev.append(a.to(self.device, dtype=torch.float32, non_blocking=False).contiguous())
+            rc = load_library().mc_load_filaments(
+                self.h, len(off) - 1, off.ctypes.data_as(C.POINTER(C.c_int32)),
+                *[C.c_void_p(t.data_ptr()) for t in dev])
+        self._check(rc)
+        self.N = int(off[-1])
+
+    def step(self, n: int = 1):
+        self._check(load_library().mc_step(self.h, int(n)))
+
+    def read_state(self, keys=("xy", "u", "rho", "fdev", "field", "force", "sense"), host: bool = True):
+        torch = self.torch
+        ny, nx, N = self.ny, self.nx, self.N
+        shapes = dict(xy=(N, 2), u=(2, ny, nx), rho=(ny, nx), fdev=(9, ny, nx),
+                      field=(self.n_fields, ny, nx), force=(N, 2), sense=(N,))
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):
+            out = {k: torch.empty(shapes[k], dtype=torch.float32, device=self.device) for k in keys}
+            ptr = [C.c_void_p(out[k].data_ptr()) if k in out and out[k].numel() else None
+                   for k in ("xy", "u", "rho", "fdev", "field", "force", "sense")]
+            st = C.c_int64()
+            rc = load_library().mc_read_state(self.h, C.byref(st), *ptr)
+        self._check(rc)
+        res = {k: (v.cpu().numpy() if host else v) for k, v in out.items()}
+        res["step"] = int(st.value)
+        return res
+
+    def read_intermediates(self, host: bool = True):
+        torch = self.torch
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):
+            rho_b = torch.empty((self.ny, self.nx), dtype=torch.float32, device=self.device)
+            G = torch.empty((2, self.ny, self.nx), dtype=torch.float32, device=self.device)
+            rc = load_library().mc_read_intermediates(self.h, C.c_void_p(rho_b.data_ptr()),
+                                                      C.c_void_p(G.data_ptr()))
+        self._check(rc)
+        return dict(rho_b=rho_b.cpu().numpy() if host else rho_b, G=G.cpu().numpy() if host else G)
+
+    def profile_enable(self, on: bool = True):
+        self._check(load_library().mc_profile_enable(self.h, int(bool(on))))
+
+    def profile_read(self):
+        """-> ({slot name: summed ms}, number of captured steps)"""
+        ms = (C.c_float * len(PROF_SLOTS))()
+        n = C.c_int32()
+        self._check(load_library().mc_profile_read(self.h, ms, C.byref(n)))
+        return {k: float(ms[i]) for i, k in enumerate(PROF_SLOTS)}, int(n.value)
+
+    def launch_count(self) -> int:
+        return int(load_library().mc_launch_count(self.h))
+
+    def _check(self, rc: int):
+        if rc != MC_OK:
+            raise McError(rc, load_library().mc_last_error(self.h).decode())
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.torch.cuda.synchronize(self.device)
+            load_library().mc_destroy(self.h)
+            self.h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,24 @@
+// k_g2p.cuh -- K4: S7 grid-to-particle interpolation fused with position integration.
+// U_i = sum_g u(g) delta_h(g - X_i) with the u stored by S6 and the same X as S1-S5;
+// X_i <- X_i + U_i (forward Euler in lattice units; readings 11, 12, 19).
+// P:L125 "the filaments' nodes sample the local fluid velocity".
+#pragma once
+#include "mc_common.cuh"
+
+namespace mc {
+
+__global__ void __launch_bounds__(256) k_interp_integrate(int N, float2* __restrict__ X,
+                                                          const float* __restrict__ u0,
+                                                          const float* __restrict__ u1, int nx, int ny,
+                                                          int* __restrict__ flag) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= N) return;
+  float2 p = X[b];
+  const float2 U = interp2(u0, u1, nx, ny, p.x, p.y);
+  p.x += U.x;
+  p.y += U.y;
+  X[b] = p;
+  if (!(isfinite(p.x) && isfinite(p.y))) atomicOr(flag, 8);
+}
+
+}  // namespace mc

@@ -1,0 +1,130 @@
+// k_lbm.cuh -- K3b: S6 fluid update.  D2Q9 (Qian et al. 1992), two-relaxation-time
+// collision (Ginzburg et al. 2008) with Guo's forcing split by parity, then streaming.
+// Readings 10 (scheme details) and 11 (beads see the collision-time velocity
+// u = (sum_q c_q f_q + G/2)/rho, which lets collide + stream + store-u be one pass).
+//
+// Storage: populations are kept SHIFTED, g_q = f_q - w_q*rho0 (fp32 velocities are small
+// differences of O(1) populations; the shift keeps ~3 more digits).
+// The array holds the POST-collision values of the previous step at their own node; streaming
+// is done on read ("pull"): the pre-collision population of this step is
+// g_q(x) = gpost_q(x - c_q).  Two buffers alternate.  Reads are coalesced rows shifted by
+// at most one cell; writes are aligned.
+//
+// With g: drho = sum g_q, rho = rho0 + drho, m = sum c_q g_q (sum c_q w_q = 0),
+//   geq+_q - w_q rho0 = w_q [drho + rho (4.5 (c_q.u)^2 - 1.5 u.u)]     (even part)
+//   geq-_q            = w_q rho 3 c_q.u                                 (odd part)
+//   S+_q = w_q [-3 u.G + 9 (c_q.u)(c_q.G)],  S-_q = 3 w_q c_q.G         (Guo source by parity)
+//   gpost_q = g_q - w+ (g+_q - geq+_q) - w- (g-_q - geq-_q) + (1 - w+/2) S+_q + (1 - w-/2) S-_q
+#pragma once
+#include "mc_common.cuh"
+
+namespace mc {
+
+struct LbmArgs {
+  const float* src;   // [9][ny][nx] post-collision, shifted
+  float* dst;         // [9][ny][nx]
+  const float* G0;    // spread force planes (may be NULL: zero force)
+  const float* G1;
+  float* u0;          // out: collision-time velocity
+  float* u1;
+  int nx, ny;
+  float rho0, omega_p, omega_m;
+  int* flag;          // sticky divergence flag (bit 2: |u| > 0.3 or non-finite)
+};
+
+// One TRT collision of a node given its pre-collision shifted populations g[9].
+__device__ __forceinline__ void trt_collide(float g[9], float Gx, float Gy, float rho0, float wp, float wm,
+                                            float& ux, float& uy) {
+  const float W0 = 4.0f / 9.0f, W1 = 1.0f / 9.0f, W5 = 1.0f / 36.0f;
+  const float drho = g[0] + ((g[1] + g[3]) + (g[2] + g[4])) + ((g[5] + g[7]) + (g[6] + g[8]));
+  const float mx = (g[1] - g[3]) + ((g[5] - g[7]) + (g[8] - g[6]));
+  const float my = (g[2] - g[4]) + ((g[5] - g[7]) + (g[6] - g[8]));
+  const float rho = rho0 + drho;
+  const float inv = 1.0f / rho;
+  ux = (mx + 0.5f * Gx) * inv;
+  uy = (my + 0.5f * Gy) * inv;
+  const float usq = ux * ux + uy * uy;
+  const float uG = ux * Gx + uy * Gy;
+  const float cp = 1.0f - 0.5f * wp, cm = 1.0f - 0.5f * wm;
+  // rest population (even only)
+  g[0] = g[0] - wp * (g[0] - W0 * (drho - 1.5f * rho * usq)) + cp * W0 * (-3.0f * uG);
+  // pairs (q, qbar) with c_qbar = -c_q:  (1,3) c=(1,0); (2,4) c=(0,1); (5,7) c=(1,1); (6,8) c=(-1,1)
+#define MC_PAIR(q, qb, w, cu, cG)                                                     \
+  {                                                                                   \
+    const float gp = 0.5f * (g[q] + g[qb]), gm = 0.5f * (g[q] - g[qb]);               \
+    const float ep = (w) * (drho + rho * (4.5f * (cu) * (cu) - 1.5f * usq));          \
+    const float em = (w) * rho * 3.0f * (cu);                                         \
+    const float Sp = (w) * (-3.0f * uG + 9.0f * (cu) * (cG));                         \
+    const float Sm = 3.0f * (w) * (cG);                                               \
+    const float even = -wp * (gp - ep) + cp * Sp;                                     \
+    const float odd = -wm * (gm - em) + cm * Sm;                                      \
+    g[q] += even + odd;                                                               \
+    g[qb] += even - odd;                                                              \
+  }
+  MC_PAIR(1, 3, W1, ux, Gx)
+  MC_PAIR(2, 4, W1, uy, Gy)
+  MC_PAIR(5, 7, W5, ux + uy, Gx + Gy)
+  MC_PAIR(6, 8, W5, uy - ux, Gy - Gx)
+#undef MC_PAIR
+}
+
+__global__ void __launch_bounds__(256) k_lbm_step(LbmArgs a) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y;
+  const int nx = a.nx, ny = a.ny;
+  const size_t nc = (size_t)nx * ny;
+  const int im = (i == 0) ? nx - 1 : i - 1, ip = (i == nx - 1) ? 0 : i + 1;
+  const int jm = (j == 0) ? ny - 1 : j - 1, jp = (j == ny - 1) ? 0 : j + 1;
+  const size_t r0 = (size_t)j * nx, rm = (size_t)jm * nx, rp = (size_t)jp * nx;
+  float g[9];
+  // pull: g_q(x) = src_q(x - c_q)
+  g[0] = __ldg(a.src + 0 * nc + r0 + i);
+  g[1] = __ldg(a.src + 1 * nc + r0 + im);
+  g[2] = __ldg(a.src + 2 * nc + rm + i);
+  g[3] = __ldg(a.src + 3 * nc + r0 + ip);
+  g[4] = __ldg(a.src + 4 * nc + rp + i);
+  g[5] = __ldg(a.src + 5 * nc + rm + im);
+  g[6] = __ldg(a.src + 6 * nc + rm + ip);
+  g[7] = __ldg(a.src + 7 * nc + rp + ip);
+  g[8] = __ldg(a.src + 8 * nc + rp + im);
+  const size_t c = r0 + i;
+  float Gx = 0.0f, Gy = 0.0f;
+  if (a.G0) { Gx = __ldg(a.G0 + c); Gy = __ldg(a.G1 + c); }
+  float ux, uy;
+  trt_collide(g, Gx, Gy, a.rho0, a.omega_p, a.omega_m, ux, uy);
+  a.u0[c] = ux;
+  a.u1[c] = uy;
+#pragma unroll
+  for (int q = 0; q < 9; ++q) a.dst[q * nc + c] = g[q];
+  if (!(fabsf(ux) <= 0.3f && fabsf(uy) <= 0.3f)) atomicOr(a.flag, 4);
+}
+
+// mc_read_state: current pre-collision populations (streamed) as deviations, and rho.
+__global__ void k_lbm_export(const float* __restrict__ src, int nx, int ny, float rho0,
+                             float* __restrict__ fdev, float* __restrict__ rho) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y;
+  if (i >= nx) return;
+  const size_t nc = (size_t)nx * ny;
+  const int im = (i == 0) ? nx - 1 : i - 1, ip = (i == nx - 1) ? 0 : i + 1;
+  const int jm = (j == 0) ? ny - 1 : j - 1, jp = (j == ny - 1) ? 0 : j + 1;
+  const size_t r0 = (size_t)j * nx, rm = (size_t)jm * nx, rp = (size_t)jp * nx;
+  float g[9];
+  g[0] = src[0 * nc + r0 + i];
+  g[1] = src[1 * nc + r0 + im];
+  g[2] = src[2 * nc + rm + i];
+  g[3] = src[3 * nc + r0 + ip];
+  g[4] = src[4 * nc + rp + i];
+  g[5] = src[5 * nc + rm + im];
+  g[6] = src[6 * nc + rm + ip];
+  g[7] = src[7 * nc + rp + ip];
+  g[8] = src[8 * nc + rp + im];
+  const size_t c = r0 + i;
+  if (fdev) {
+#pragma unroll
+    for (int q = 0; q < 9; ++q) fdev[q * nc + c] = g[q];
+  }
+  if (rho) rho[c] = rho0 + (g[0] + ((g[1] + g[3]) + (g[2] + g[4])) + ((g[5] + g[7]) + (g[6] + g[8])));
+}
+
+}  // namespace mc

@@ -1,0 +1,528 @@
+// mc_api.cu -- host side of libmc.so: the C ABI of include/mc.h, workspace layout, and the
+// per-step launch sequence K0 -> K2a -> K3a -> K1 -> K2b -> K3b -> K4.
+// No CPU implementation of any step lives here: without a CUDA device every call fails.
+#include "../../include/mc.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "k_bin.cuh"
+#include "k_blur.cuh"
+#include "k_filament.cuh"
+#include "k_g2p.cuh"
+#include "k_lbm.cuh"
+#include "k_p2g.cuh"
+
+namespace {
+
+thread_local std::string g_create_error;
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct Layout {
+  size_t fA, fB, u, rho_b, A, G, cfield, csum, As, cell_count, cell_start, block_sums;
+  size_t X, P0, P1, F, sense, bead_cell, bead_rank, slot_bead, W, offsets, flags, sources;
+  size_t total;
+};
+
+struct Derived {
+  int n_density = 0, n_static = 0;
+  int R[4] = {0, 0, 0, 0};
+  size_t n_src_floats = 0;
+};
+
+bool validate(const mc_world_params* p, Derived* d, std::string* why) {
+  if (!p) { *why = "null params"; return false; }
+  if (p->nx < 32 || p->ny < 32 || p->nx % 32 || p->ny % 32) { *why = "nx, ny must be multiples of 32, >= 32"; return false; }
+  if ((int64_t)p->nx * p->ny > (int64_t)1 << 30 || p->ny > 65535) { *why = "grid too large"; return false; }
+  if (!(p->dt > 0) || !(p->nu > 0) || !(p->trt_lambda > 0) || !(p->rho0 > 0)) { *why = "dt, nu, trt_lambda, rho0 must be > 0"; return false; }
+  if (p->pbd_iters != 1) { *why = "pbd_iters must be 1"; return false; }
+  if (p->n_fields < 0 || p->n_fields > 4) { *why = "n_fields must be 0..4"; return false; }
+  if (p->max_beads < 0 || p->max_beads > (int64_t)1 << 30) { *why = "max_beads out of range"; return false; }
+  for (int k = 0; k < p->n_fields; ++k) {
+    const mc_field_params& f = p->fields[k];
+    if (f.kind == MC_FIELD_BEAD_DENSITY) {
+      if (!(f.sigma > 0)) { *why = "field sigma must be > 0"; return false; }
+      const int R = f.radius > 0 ? f.radius : (int)std::ceil(5.0 * (double)f.sigma);
+      if (R < 1 || R > mc::BLUR_MAX_R) { *why = "filter radius must be 1..16"; return false; }
+      if (2 * R + 1 > p->nx || 2 * R + 1 > p->ny) { *why = "filter wider than the grid"; return false; }
+      d->R[k] = R;
+      d->n_density++;
+    } else if (f.kind == MC_FIELD_STATIC_SOURCE) {
+      if (f.n_sources < 0 || (f.n_sources > 0 && !f.sources)) { *why = "bad static sources"; return false; }
+      for (int s = 0; s < f.n_sources; ++s)
+        if (!(f.sources[4 * s + 3] > 0)) { *why = "source width must be > 0"; return false; }
+      d->n_static++;
+      d->n_src_floats += 4 * (size_t)f.n_sources;
+    } else {
+      *why = "unknown field kind";
+      return false;
+    }
+  }
+  return true;
+}
+
+Layout make_layout(const mc_world_params* p, const Derived& d) {
+  Layout L;
+  const size_t nc = (size_t)p->nx * p->ny, N = (size_t)p->max_beads, f4 = sizeof(float);
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes ? bytes : 1); return o; };
+  L.fA = take(9 * nc * f4);
+  L.fB = take(9 * nc * f4);
+  L.u = take(2 * nc * f4);
+  L.rho_b = take(nc * f4);
+  L.A = take(d.n_density ? 2 * nc * f4 : 0);
+  L.G = take(2 * nc * f4);
+  L.cfield = take(d.n_static * nc * f4);
+  L.csum = take(d.n_static ? nc * f4 : 0);
+  L.As = take(d.n_static ? 2 * nc * f4 : 0);
+  L.cell_count = take(nc * 4);
+  L.cell_start = take((nc + 4) * 4);
+  L.block_sums = take(((nc + mc::SCAN_CHUNK - 1) / mc::SCAN_CHUNK + 1) * 4);
+  L.X = take(N * 8);
+  L.P0 = take(N * 16);
+  L.P1 = take(N * 16);
+  L.F = take(N * 8);
+  L.sense = take(N * 4);
+  L.bead_cell = take(N * 4);
+  L.bead_rank = take(N * 4);
+  L.slot_bead = take(N * 4);
+  L.W = take(N * 8 * f4);
+  L.offsets = take((N / 3 + 2) * 4);
+  L.flags = take(64 * 4);
+  L.sources = take(d.n_src_floats * f4);
+  L.total = off;
+  return L;
+}
+
+}  // namespace
+
+struct mc_world {
+  mc_world_params p;
+  Derived d;
+  Layout L;
+  char* ws = nullptr;
+  cudaStream_t stream = nullptr;
+  int nx = 0, ny = 0;
+  size_t nc = 0;
+  int64_t step = 0;
+  int cur = 0;  // which of fA/fB holds the current post-collision populations
+  int n_fil = 0;
+  int N = 0;
+  float rho0 = 1, omega_p = 1, omega_m = 1, kappa = 0;
+  float coef[4] = {0, 0, 0, 0};  // lattice coupling with the sign of the force
+  mc::BlurTaps taps[4];
+  int static_slot[4] = {-1, -1, -1, -1};
+  int64_t launches = 0;
+  bool diverged = false;
+  std::string err;
+  // optional per-kernel timing (mc_profile_*): events at the 8 boundaries of a step
+  bool prof_on = false;
+  int prof_steps = 0;
+  std::vector<cudaEvent_t> prof_ev;  // [MC_PROF_MAX_STEPS][MC_PROF_SLOTS + 1]
+
+  template <class T>
+  T* ptr(size_t off) const { return reinterpret_cast<T*>(ws + off); }
+  float* fbuf(int which) const { return ptr<float>(which ? L.fB : L.fA); }
+};
+
+namespace {
+
+int fail(mc_world* w, int code, const std::string& msg) {
+  if (w) w->err = msg;
+  return code;
+}
+
+int check_cuda(mc_world* w, const char* what) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+  return MC_OK;
+}
+
+constexpr int PROF_MAX_STEPS = 64;
+
+inline void prof_mark(mc_world* w, int boundary) {
+  if (w->prof_on && w->prof_steps < PROF_MAX_STEPS)
+    cudaEventRecord(w->prof_ev[(size_t)w->prof_steps * (MC_PROF_SLOTS + 1) + boundary], w->stream);
+}
+
+int pick_bx(int nx) { return nx % 256 == 0 ? 256 : (nx % 128 == 0 ? 128 : (nx % 64 == 0 ? 64 : 32)); }
+
+// K3a for bead-density field k; accumulate: add to the planes already in A
+void launch_blur(mc_world* w, int k, bool first, float* field_out) {
+  const float* base0 = nullptr;
+  const float* base1 = nullptr;
+  float* A0 = w->ptr<float>(w->L.A);
+  float* A1 = A0 + w->nc;
+  if (first) {
+    if (w->d.n_static) { base0 = w->ptr<float>(w->L.As); base1 = base0 + w->nc; }
+  } else {
+    base0 = A0; base1 = A1;
+  }
+  dim3 grid(w->nx / mc::BLUR_T, w->ny / mc::BLUR_T);
+  mc::k_blur_grad<<<grid, 256, mc::blur_smem_bytes(w->d.R[k]), w->stream>>>(
+      w->nx, w->ny, w->d.R[k], w->taps[k], w->ptr<float>(w->L.rho_b), w->coef[k], base0, base1, A0, A1,
+      field_out);
+  w->launches++;
+}
+
+int enqueue_step(mc_world* w) {
+  const int N = w->N, nx = w->nx, ny = w->ny;
+  const int nc = (int)w->nc;
+  cudaStream_t st = w->stream;
+  float2* X = w->ptr<float2>(w->L.X);
+  float2* F = w->ptr<float2>(w->L.F);
+  int* cell_count = w->ptr<int>(w->L.cell_count);
+  int* cell_start = w->ptr<int>(w->L.cell_start);
+  int* block_sums = w->ptr<int>(w->L.block_sums);
+  int* bead_cell = w->ptr<int>(w->L.bead_cell);
+  int* bead_rank = w->ptr<int>(w->L.bead_rank);
+  int* slot_bead = w->ptr<int>(w->L.slot_bead);
+  float* W = w->ptr<float>(w->L.W);
+  const size_t plane = (size_t)(w->p.max_beads > 0 ? w->p.max_beads : 1);
+  float* rho_b = w->ptr<float>(w->L.rho_b);
+  float* G0 = w->ptr<float>(w->L.G);
+  float* G1 = G0 + w->nc;
+  int* flag = w->ptr<int>(w->L.flags);
+  const int bt = 256;
+  const int bgrid = (N + bt - 1) / bt;
+  const bool beads = N > 0;
+
+  prof_mark(w, 0);
+  if (beads) {
+    // K0: canonical cell binning
+    cudaMemsetAsync(cell_count, 0, (size_t)nc * 4, st);
+    mc::k_bin_count<<<bgrid, bt, 0, st>>>(X, N, nx, ny, cell_count, bead_cell, bead_rank);
+    const int nb = (nc + mc::SCAN_CHUNK - 1) / mc::SCAN_CHUNK;
+    mc::k_scan_block_sums<<<nb, mc::SCAN_THREADS, 0, st>>>(cell_count, nc, block_sums);
+    mc::k_scan_top<<<1, mc::SCAN_THREADS, 0, st>>>(block_sums, nb);
+    mc::k_scan_apply<<<nb, mc::SCAN_THREADS, 0, st>>>(cell_count, nc, block_sums, cell_start, N);
+    mc::k_bin_scatter<<<bgrid, bt, 0, st>>>(N, bead_cell, bead_rank, cell_start, slot_bead);
+    mc::k_bin_sort_cells<<<(nc + bt - 1) / bt, bt, 0, st>>>(nc, cell_start, slot_bead);
+    mc::k_bin_pack<<<bgrid, bt, 0, st>>>(N, slot_bead, X, W, plane);
+    w->launches += 8;
+    prof_mark(w, 1);
+    // K2a: S2 deposit
+    if (w->d.n_density) {
+      mc::k_p2g_gather<false><<<dim3(nx / 32, ny / 8), 256, 0, st>>>(nx, ny, cell_start, W, plane, slot_bead,
+                                                                      nullptr, rho_b, nullptr);
+      w->launches++;
+      prof_mark(w, 2);
+      // K3a: S3 filter + gradient -> force-gradient planes A
+      bool first = true;
+      for (int k = 0; k < w->p.n_fields; ++k)
+        if (w->p.fields[k].kind == MC_FIELD_BEAD_DENSITY) {
+          launch_blur(w, k, first, nullptr);
+          first = false;
+        }
+    }
+    if (!w->d.n_density) prof_mark(w, 2);
+    prof_mark(w, 3);
+    // K1: S0 + S1 + S4
+    mc::FilamentArgs fa;
+    fa.offsets = w->ptr<int>(w->L.offsets);
+    fa.n_fil = w->n_fil;
+    fa.X = X;
+    fa.P0 = w->ptr<float4>(w->L.P0);
+    fa.P1 = w->ptr<float4>(w->L.P1);
+    fa.F = F;
+    fa.sense = w->ptr<float>(w->L.sense);
+    fa.A0 = w->d.n_density ? w->ptr<float>(w->L.A) : (w->d.n_static ? w->ptr<float>(w->L.As) : nullptr);
+    fa.A1 = fa.A0 ? fa.A0 + w->nc : nullptr;
+    fa.csum = w->d.n_static ? w->ptr<float>(w->L.csum) : nullptr;
+    fa.nx = nx;
+    fa.ny = ny;
+    fa.kappa = w->kappa;
+    fa.t = (double)w->step * (double)w->p.dt;
+    const int warps_per_block = 8;
+    int fgrid = (w->n_fil + warps_per_block - 1) / warps_per_block;
+    if (fgrid > 148 * 64) fgrid = 148 * 64;
+    mc::k_filament_force<<<fgrid, warps_per_block * 32, 0, st>>>(fa);
+    prof_mark(w, 4);
+    // K2b: S5 spread
+    mc::k_p2g_gather<true><<<dim3(nx / 32, ny / 8), 256, 0, st>>>(nx, ny, cell_start, W, plane, slot_bead, F,
+                                                                   G0, G1);
+    w->launches += 2;
+  } else {
+    for (int b = 1; b <= 4; ++b) prof_mark(w, b);
+  }
+  prof_mark(w, 5);
+  // K3b: S6 fluid
+  mc::LbmArgs la;
+  la.src = w->fbuf(w->cur);
+  la.dst = w->fbuf(w->cur ^ 1);
+  la.G0 = beads ? G0 : nullptr;
+  la.G1 = beads ? G1 : nullptr;
+  la.u0 = w->ptr<float>(w->L.u);
+  la.u1 = la.u0 + w->nc;
+  la.nx = nx;
+  la.ny = ny;
+  la.rho0 = w->rho0;
+  la.omega_p = w->omega_p;
+  la.omega_m = w->omega_m;
+  la.flag = flag;
+  const int bx = pick_bx(nx);
+  mc::k_lbm_step<<<dim3(nx / bx, ny), bx, 0, st>>>(la);
+  w->launches++;
+  w->cur ^= 1;
+  prof_mark(w, 6);
+  // K4: S7
+  if (beads) {
+    mc::k_interp_integrate<<<bgrid, bt, 0, st>>>(N, X, la.u0, la.u1, nx, ny, flag);
+    w->launches++;
+  }
+  prof_mark(w, 7);
+  if (w->prof_on && w->prof_steps < PROF_MAX_STEPS) w->prof_steps++;
+  w->step += 1;
+  return MC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+#pragma GCC visibility push(default)
+
+size_t mc_workspace_bytes(const mc_world_params* p) {
+  Derived d;
+  std::string why;
+  if (!validate(p, &d, &why)) return 0;
+  return make_layout(p, d).total;
+}
+
+const char* mc_last_error(const mc_world* w) { return w ? w->err.c_str() : g_create_error.c_str(); }
+
+int64_t mc_launch_count(const mc_world* w) { return w ? w->launches : 0; }
+
+void mc_destroy(mc_world* w) {
+  if (!w) return;
+  for (cudaEvent_t e : w->prof_ev) cudaEventDestroy(e);
+  delete w;
+}
+
+int mc_profile_enable(mc_world* w, int32_t on) {
+  if (!w) return MC_EINVAL;
+  if (on && w->prof_ev.empty()) {
+    w->prof_ev.resize((size_t)PROF_MAX_STEPS * (MC_PROF_SLOTS + 1));
+    for (cudaEvent_t& e : w->prof_ev)
+      if (cudaEventCreate(&e) != cudaSuccess) return fail(w, MC_ECUDA, "cudaEventCreate failed");
+  }
+  w->prof_on = on != 0;
+  w->prof_steps = 0;
+  return MC_OK;
+}
+
+int mc_profile_read(mc_world* w, float* ms, int32_t* steps) {
+  if (!w || !ms) return MC_EINVAL;
+  for (int k = 0; k < MC_PROF_SLOTS; ++k) ms[k] = 0.0f;
+  if (steps) *steps = w->prof_steps;
+  cudaError_t e = cudaStreamSynchronize(w->stream);
+  if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_profile_read: ") + cudaGetErrorString(e));
+  for (int s = 0; s < w->prof_steps; ++s)
+    for (int k = 0; k < MC_PROF_SLOTS; ++k) {
+      float t = 0.0f;
+      const size_t base = (size_t)s * (MC_PROF_SLOTS + 1);
+      if (cudaEventElapsedTime(&t, w->prof_ev[base + k], w->prof_ev[base + k + 1]) == cudaSuccess) ms[k] += t;
+    }
+  w->prof_steps = 0;
+  return MC_OK;
+}
+
+int mc_create(const mc_world_params* p, void* workspace, size_t workspace_bytes, void* cuda_stream,
+              mc_world** out) {
+  g_create_error.clear();
+  if (!out) { g_create_error = "null out"; return MC_EINVAL; }
+  *out = nullptr;
+  Derived d;
+  std::string why;
+  if (!validate(p, &d, &why)) { g_create_error = why; return MC_EINVAL; }
+  Layout L = make_layout(p, d);
+  if (!workspace || workspace_bytes < L.total || ((uintptr_t)workspace % ALIGN) != 0) {
+    g_create_error = "workspace missing, too small or not 256-byte aligned";
+    return MC_EINVAL;
+  }
+  mc_world* w = new (std::nothrow) mc_world();
+  if (!w) { g_create_error = "host allocation failed"; return MC_ENOMEM; }
+  w->p = *p;
+  for (int k = 0; k < 4; ++k) w->p.fields[k].sources = nullptr;  // never keep caller pointers
+  w->d = d;
+  w->L = L;
+  w->ws = static_cast<char*>(workspace);
+  w->stream = static_cast<cudaStream_t>(cuda_stream);
+  w->nx = p->nx;
+  w->ny = p->ny;
+  w->nc = (size_t)p->nx * p->ny;
+  // lattice constants (reading 10, 12): nu_lat = nu dt; tau+ = 3 nu_lat + 1/2; tau- = Lambda/(tau+ - 1/2) + 1/2
+  const double dt = (double)p->dt, nu_lat = (double)p->nu * dt;
+  const double tau_p = 3.0 * nu_lat + 0.5, tau_m = (double)p->trt_lambda / (tau_p - 0.5) + 0.5;
+  w->omega_p = (float)(1.0 / tau_p);
+  w->omega_m = (float)(1.0 / tau_m);
+  w->rho0 = p->rho0;
+  w->kappa = (float)((double)p->k_el * dt * dt);
+
+  cudaStream_t st = w->stream;
+  cudaError_t e = cudaMemsetAsync(workspace, 0, L.total, st);  // fluid at rest: shifted populations = 0
+  if (e != cudaSuccess) {
+    g_create_error = std::string("cudaMemsetAsync: ") + cudaGetErrorString(e);
+    delete w;
+    return MC_ECUDA;
+  }
+  // fields
+  size_t src_off = 0;
+  int n_static_seen = 0;
+  for (int k = 0; k < p->n_fields; ++k) {
+    const mc_field_params& f = p->fields[k];
+    const double lat = (double)f.coupling * dt * dt;
+    if (f.kind == MC_FIELD_BEAD_DENSITY) {
+      w->coef[k] = (float)(-lat);  // F_rep = -kappa_rep * grad(rho~)
+      const int R = d.R[k];
+      double g[2 * mc::BLUR_MAX_R + 1], Z = 0.0;
+      for (int t = -R; t <= R; ++t) {
+        g[t + R] = std::exp(-(double)(t * t) / (2.0 * (double)f.sigma * (double)f.sigma));
+        Z += g[t + R];
+      }
+      for (int t = 0; t <= 2 * R; ++t) w->taps[k].g[t] = (float)(g[t] / Z);
+    } else {
+      w->coef[k] = (float)lat;  // F_chem = +kappa_chi * grad(c)
+      w->static_slot[k] = n_static_seen;
+      float* dsrc = w->ptr<float>(L.sources) + src_off;
+      if (f.n_sources > 0) {
+        e = cudaMemcpyAsync(dsrc, f.sources, 4 * (size_t)f.n_sources * sizeof(float), cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) {
+          g_create_error = std::string("cudaMemcpyAsync(sources): ") + cudaGetErrorString(e);
+          delete w;
+          return MC_ECUDA;
+        }
+        cudaStreamSynchronize(st);  // the host array belongs to the caller
+      }
+      float* As0 = w->ptr<float>(L.As);
+      mc::k_static_init<<<dim3((w->nx + 127) / 128, w->ny), 128, 0, st>>>(
+          w->nx, w->ny, f.n_sources, dsrc, w->coef[k], w->ptr<float>(L.cfield) + (size_t)n_static_seen * w->nc,
+          w->ptr<float>(L.csum), As0, As0 + w->nc);
+      w->launches++;
+      src_off += 4 * (size_t)f.n_sources;
+      n_static_seen++;
+    }
+  }
+  e = cudaStreamSynchronize(st);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    g_create_error = std::string("mc_create: ") + cudaGetErrorString(e);
+    delete w;
+    return MC_ECUDA;
+  }
+  *out = w;
+  return MC_OK;
+}
+
+int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const float* xy, const float* L_rest,
+                      const float* theta_rest, const float* k_bend, const float* k_shear,
+                      const float* k_stretch, const float* act_amp, const float* act_phase,
+                      const float* act_period) {
+  if (!w) return MC_EINVAL;
+  if (n_fil < 0 || !offsets || offsets[0] != 0) return fail(w, MC_EINVAL, "bad offsets");
+  for (int32_t f = 0; f < n_fil; ++f)
+    if (offsets[f + 1] - offsets[f] < 3) return fail(w, MC_EINVAL, "chain shorter than 3 beads");
+  const int64_t N = offsets[n_fil];
+  if (N > w->p.max_beads) return fail(w, MC_EINVAL, "N > max_beads");
+  if (N > 0 && (!xy || !L_rest || !theta_rest || !k_bend || !k_shear || !k_stretch || !act_amp || !act_phase ||
+                !act_period))
+    return fail(w, MC_EINVAL, "null array");
+  cudaStream_t st = w->stream;
+  int* flag = w->ptr<int>(w->L.flags) + 1;
+  cudaMemsetAsync(flag, 0, 4, st);
+  cudaMemcpyAsync(w->ptr<int>(w->L.offsets), offsets, (size_t)(n_fil + 1) * 4, cudaMemcpyHostToDevice, st);
+  if (N > 0) {
+    mc::k_pack_params<<<(int)((N + 255) / 256), 256, 0, st>>>((int)N, xy, L_rest, theta_rest, k_bend, k_shear,
+                                                              k_stretch, act_amp, act_phase, act_period,
+                                                              w->ptr<float2>(w->L.X), w->ptr<float4>(w->L.P0),
+                                                              w->ptr<float4>(w->L.P1), flag);
+    w->launches++;
+    cudaMemsetAsync(w->ptr<float>(w->L.F), 0, (size_t)N * 8, st);
+    cudaMemsetAsync(w->ptr<float>(w->L.sense), 0, (size_t)N * 4, st);
+  }
+  int h = 0;
+  cudaMemcpyAsync(&h, flag, 4, cudaMemcpyDeviceToHost, st);
+  cudaError_t e = cudaStreamSynchronize(st);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_load_filaments: ") + cudaGetErrorString(e));
+  if (h) {
+    w->N = 0;
+    w->n_fil = 0;
+    return fail(w, MC_EINVAL, (h & 1) ? "stiffness outside [0,1]" : "period <= 0");
+  }
+  w->N = (int)N;
+  w->n_fil = n_fil;
+  return MC_OK;
+}
+
+int mc_step(mc_world* w, int32_t n) {
+  if (!w) return MC_EINVAL;
+  if (n < 0) return fail(w, MC_EINVAL, "n < 0");
+  if (w->diverged) return fail(w, MC_EDIVERGED, "world diverged (non-finite bead or |u| > 0.3)");
+  for (int32_t s = 0; s < n; ++s) {
+    int rc = enqueue_step(w);
+    if (rc != MC_OK) return rc;
+  }
+  return check_cuda(w, "mc_step");
+}
+
+int mc_read_state(mc_world* w, int64_t* step_out, float* xy, float* u, float* rho, float* fdev, float* field,
+                  float* force, float* sense) {
+  if (!w) return MC_EINVAL;
+  cudaStream_t st = w->stream;
+  const size_t nc = w->nc, N = (size_t)w->N;
+  if (step_out) *step_out = w->step;
+  const cudaMemcpyKind d2d = cudaMemcpyDeviceToDevice;
+  if (xy && N) cudaMemcpyAsync(xy, w->ptr<float>(w->L.X), N * 8, d2d, st);
+  if (u) cudaMemcpyAsync(u, w->ptr<float>(w->L.u), 2 * nc * 4, d2d, st);
+  if (rho || fdev) {
+    const int bx = pick_bx(w->nx);
+    mc::k_lbm_export<<<dim3(w->nx / bx, w->ny), bx, 0, st>>>(w->fbuf(w->cur), w->nx, w->ny, w->rho0, fdev, rho);
+    w->launches++;
+  }
+  if (field) {
+    bool first = true;
+    for (int k = 0; k < w->p.n_fields; ++k) {
+      float* dst = field + (size_t)k * nc;
+      if (w->p.fields[k].kind == MC_FIELD_BEAD_DENSITY) {
+        // recompute the filtered density from the stored rho_b (A is rebuilt by every step anyway)
+        launch_blur(w, k, first, dst);
+        first = false;
+      } else {
+        cudaMemcpyAsync(dst, w->ptr<float>(w->L.cfield) + (size_t)w->static_slot[k] * nc, nc * 4, d2d, st);
+      }
+    }
+  }
+  if (force && N) cudaMemcpyAsync(force, w->ptr<float>(w->L.F), N * 8, d2d, st);
+  if (sense && N) cudaMemcpyAsync(sense, w->ptr<float>(w->L.sense), N * 4, d2d, st);
+  int h = 0;
+  cudaMemcpyAsync(&h, w->ptr<int>(w->L.flags), 4, cudaMemcpyDeviceToHost, st);
+  cudaError_t e = cudaStreamSynchronize(st);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_read_state: ") + cudaGetErrorString(e));
+  if (h) {
+    w->diverged = true;
+    return fail(w, MC_EDIVERGED, "world diverged (non-finite bead or |u| > 0.3)");
+  }
+  return MC_OK;
+}
+
+int mc_read_intermediates(mc_world* w, float* rho_b, float* G) {
+  if (!w) return MC_EINVAL;
+  cudaStream_t st = w->stream;
+  const size_t nc = w->nc;
+  if (rho_b) cudaMemcpyAsync(rho_b, w->ptr<float>(w->L.rho_b), nc * 4, cudaMemcpyDeviceToDevice, st);
+  if (G) cudaMemcpyAsync(G, w->ptr<float>(w->L.G), 2 * nc * 4, cudaMemcpyDeviceToDevice, st);
+  cudaError_t e = cudaStreamSynchronize(st);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_read_intermediates: ") + cudaGetErrorString(e));
+  return MC_OK;
+}
+
+#pragma GCC visibility pop
+}  // extern "C"

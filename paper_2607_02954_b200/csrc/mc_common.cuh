@@ -1,0 +1,98 @@
+// mc_common.cuh -- device helpers shared by the kernels of libmc.so (CUDA path only).
+// P:L<n> = PAPER.md line n; "reading k" = DESIGN.md "Readings" row k.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mc {
+
+// periodic wrap of a grid index (reading 9)
+__device__ __forceinline__ int wrapi(int i, int n) {
+  i %= n;
+  return i < 0 ? i + n : i;
+}
+// wrap when i is known to lie in [-n, 2n)
+__device__ __forceinline__ int wrap1(int i, int n) {
+  return i < 0 ? i + n : (i >= n ? i - n : i);
+}
+
+// Peskin's 4-point function (Peskin 2002, cited P:L125; reading 7) at the four nodes
+// fl-1, fl, fl+1, fl+2 of a bead with fractional coordinate fr = x - floor(x) in [0,1).
+// Node distances are 1+fr, fr, 1-fr, 2-fr.  The two inner weights are evaluated from
+// phi(r) = (3 - 2|r| + sqrt(1 + 4|r| - 4r^2))/8; the outer two follow from the kernel's
+// even/odd sum rule (w0 + w2 = w1 + w3 = 1/2), which is exact for phi and avoids the
+// cancellation in the outer branch's radicand.
+__device__ __forceinline__ void peskin4(float fr, float& w0, float& w1, float& w2, float& w3) {
+  const float a1 = fr, a2 = 1.0f - fr;
+  w1 = 0.125f * (3.0f - 2.0f * a1 + sqrtf(fmaf(4.0f * a1, a2, 1.0f)));  // 1+4a-4a^2 = 1+4a(1-a)
+  w2 = 0.125f * (3.0f - 2.0f * a2 + sqrtf(fmaf(4.0f * a2, a1, 1.0f)));
+  w0 = 0.5f - w2;
+  w3 = 0.5f - w1;
+}
+
+// Support of a coordinate: first node (unwrapped) and fractional part (reading 8).
+__device__ __forceinline__ void support(float x, int& i0, float& fr) {
+  const float fl = floorf(x);
+  fr = x - fl;  // exact in fp32
+  i0 = (int)fl - 1;
+}
+
+// Interpolate two planes at (x,y): sum over the 4x4 support of plane(g) * delta_h(g - X)
+// ("nodes sample the local fluid velocity"; also S4's gradient sampling).
+__device__ __forceinline__ float2 interp2(const float* __restrict__ p0, const float* __restrict__ p1,
+                                          int nx, int ny, float x, float y) {
+  int i0, j0;
+  float fx, fy, wx[4], wy[4];
+  support(x, i0, fx);
+  support(y, j0, fy);
+  peskin4(fx, wx[0], wx[1], wx[2], wx[3]);
+  peskin4(fy, wy[0], wy[1], wy[2], wy[3]);
+  i0 = wrapi(i0, nx);
+  j0 = wrapi(j0, ny);
+  int col[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) col[k] = (i0 + k >= nx) ? i0 + k - nx : i0 + k;
+  float ax = 0.0f, ay = 0.0f;
+#pragma unroll
+  for (int l = 0; l < 4; ++l) {
+    const int row = (j0 + l >= ny) ? j0 + l - ny : j0 + l;
+    const float* r0 = p0 + (size_t)row * nx;
+    const float* r1 = p1 + (size_t)row * nx;
+    float sx = 0.0f, sy = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      sx = fmaf(__ldg(r0 + col[k]), wx[k], sx);
+      sy = fmaf(__ldg(r1 + col[k]), wx[k], sy);
+    }
+    ax = fmaf(sx, wy[l], ax);
+    ay = fmaf(sy, wy[l], ay);
+  }
+  return make_float2(ax, ay);
+}
+
+__device__ __forceinline__ float interp1(const float* __restrict__ p0, int nx, int ny, float x, float y) {
+  int i0, j0;
+  float fx, fy, wx[4], wy[4];
+  support(x, i0, fx);
+  support(y, j0, fy);
+  peskin4(fx, wx[0], wx[1], wx[2], wx[3]);
+  peskin4(fy, wy[0], wy[1], wy[2], wy[3]);
+  i0 = wrapi(i0, nx);
+  j0 = wrapi(j0, ny);
+  float a = 0.0f;
+#pragma unroll
+  for (int l = 0; l < 4; ++l) {
+    const int row = (j0 + l >= ny) ? j0 + l - ny : j0 + l;
+    const float* r0 = p0 + (size_t)row * nx;
+    float s = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int c = (i0 + k >= nx) ? i0 + k - nx : i0 + k;
+      s = fmaf(__ldg(r0 + c), wx[k], s);
+    }
+    a = fmaf(s, wy[l], a);
+  }
+  return a;
+}
+
+}  // namespace mc

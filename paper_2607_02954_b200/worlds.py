@@ -193,3 +193,32 @@ def random_world(nx: int, ny: int, n_fil: int, m: int, seed: int = 0, *, kappa: 
     w["steps"] = 100
     w["name"] = tag
     return w
+
+
+def ragged_world(nx: int, ny: int, lengths, seed: int = 0, *, kappa: float = 2.0,
+                 kappa_rep: float | None = 0.01, static_source: bool = False,
+                 shift_some: bool = True, tag: str = "rg") -> dict:
+    """Chains of different lengths (edge cases of the one-warp-per-chain kernel: shorter than,
+    equal to and longer than a warp), uniformly placed so that some straddle the periodic
+    boundary; with shift_some every third chain is translated by a whole number of domain
+    periods, so unwrapped coordinates well outside [0,nx) x [0,ny) are exercised."""
+    parts = []
+    for g, m in enumerate(lengths):
+        parts.append(_random_chains(f"{tag}/{g}", seed, 1, int(m), nx, ny))
+    keys = ("xy", "L_rest", "theta_rest", "k_bend", "k_shear", "k_stretch", "act_amp",
+            "act_phase", "act_period")
+    w = {k: np.concatenate([p[k] for p in parts], axis=0) for k in keys}
+    w["offsets"] = np.concatenate([[0], np.cumsum([int(m) for m in lengths])]).astype(np.int32)
+    if shift_some:
+        for f in range(0, len(lengths), 3):
+            s, e = w["offsets"][f], w["offsets"][f + 1]
+            w["xy"][s:e, 0] += np.float32(nx * (1 if f % 2 else -2))
+            w["xy"][s:e, 1] += np.float32(ny * (-1 if f % 2 else 1))
+    base = random_world(nx, ny, 1, 4, seed=seed, kappa=kappa, kappa_rep=kappa_rep,
+                        static_source=static_source, tag=tag + "/p")
+    params = base["params"]
+    params["max_beads"] = int(w["offsets"][-1])
+    w["params"] = params
+    w["steps"] = 100
+    w["name"] = tag
+    return w

@@ -1,0 +1,314 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the whole hot path (mc_step) on synthetic Microcosmos worlds.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 4d] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path S0..S7 (all kernels K0..K4) over one seeded
+synthetic world.  Default workload: BASELINE.json config 4's largest world "4d" (10,000,000
+beads in 64-bead filaments on a 6272^2 grid) -- the largest single-GPU configuration, the one
+north_star's >= 60 % HBM-roofline bar is stated on.  Prints ONE JSON line (rank 0).
+
+  value        bead-steps/s, device-timed (CUDA events, max over ranks), state resident in HBM
+  e2e          the same metric through the public API with HOST buffers: every e2e step uploads
+               the filament arrays from pinned host memory (mc_load_filaments), runs mc_step(1)
+               and reads the bead positions back to pinned host memory (mc_read_state)
+  roofline     the step's dominant kernel (largest share of the step, measured live with CUDA
+               events on the world's stream through mc_profile_*), its algorithmic bytes per
+               launch / its mean duration, against the measured HBM peak
+  roofline_step  the same for the whole step (112 B/cell + 64 B/bead)
+  cpu_baseline the oracle (oracle/, as it stands) timed on this box's host cores on a bounded
+               sample: the same recipe at 1/100 size (world "4b": 100,032 beads, 640^2 grid)
+  --impl reference   times the oracle alone on that sample (there is no reference implementation
+               of the paper in this repository: the oracle is the reference arm)
+
+Multi-GPU (--gpus N under torchrun): the path does not shard (replicas
+only) -- every rank steps its own independent world (seed = rank); no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "bead-steps/sec for mc_step (whole hot path S0-S7)"
+UNIT = "bead-steps/s"
+SAMPLE_WORLD = "4b"  # the oracle's bounded sample: config-4 recipe at 1/100 of 4d
+
+
+def measured_peak_gbs():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+            except Exception:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# algorithmic HBM bytes per launch of each kernel group, fp32
+def kernel_bytes(n_cells: int, n_beads: int) -> dict:
+    return {
+        "K0_bin": 0,                                      # mechanism: no algorithmic traffic
+        "K2a_deposit": 4 * n_cells + 8 * n_beads,         # rho_b write; X read
+        "K3a_blur_grad": 12 * n_cells,                    # rho_b read; grad planes write
+        "K1_filament": 48 * n_beads,                      # X + 2 float4 params read; F write
+        "K2b_spread": 8 * n_cells + 8 * n_beads,          # G write; F read
+        "K3b_lbm": 88 * n_cells,                          # f read+write 72, G read 8, u write 8
+        "K4_interp_integrate": 16 * n_beads,              # X read + write
+    }
+
+
+def step_bytes(n_cells: int, n_beads: int) -> int:
+    return 112 * n_cells + 64 * n_beads  # SURVEY.md 8(d) / DESIGN.md
+
+
+def time_oracle(sample: str, seed: int, budget_s: float, min_steps: int, max_steps: int, warm: int = 1):
+    """Oracle as it stands, all host cores.  Returns (bead_steps_per_s, cores, steps, seconds)."""
+    from oracle import mco
+    from paper_2607_02954_b200 import worlds
+    cores = os.cpu_count() or 1
+    w = worlds.make_world(sample, seed)
+    O = mco.World(w, threads=cores)
+    O.step(warm)
+    n, t0 = 0, time.perf_counter()
+    while n < max_steps and (n < min_steps or time.perf_counter() - t0 < budget_s):
+        O.step(1)
+        n += 1
+    dt = time.perf_counter() - t0
+    N = int(w["offsets"][-1])
+    O.close()
+    return N * n / dt, cores, n, dt
+
+
+def run_reference(args, rank: int):
+    """--impl reference: the oracle alone, on the bounded sample, K timed steps after W warm-up."""
+    if rank != 0:
+        return
+    from oracle import mco
+    from paper_2607_02954_b200 import worlds
+    cores = os.cpu_count() or 1
+    w = worlds.make_world(SAMPLE_WORLD, 0)
+    N = int(w["offsets"][-1])
+    O = mco.World(w, threads=cores)
+    O.step(args.warmup)
+    t0 = time.perf_counter()
+    O.step(args.steps)
+    dt = time.perf_counter() - t0
+    val = N * args.steps / dt
+    p = w["params"]
+    sample = (f"world {SAMPLE_WORLD}: {N} beads in 64-bead filaments, {p['nx']}x{p['ny']} grid "
+              f"(config-4 recipe at 1/100 of 4d), {args.steps} steps")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic (seeded)", "config": {"workload": args.workload, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--workload", default="4d")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world_size = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if args.warmup < 3:
+        args.warmup = 3  # timing rule: W >= 3
+
+    import numpy as np
+    import torch
+    from paper_2607_02954_b200 import binding, worlds
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    dist = None
+    if world_size > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device(f"cuda:{local_rank}")
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # replicas only: every rank owns an independent world of the same recipe (seed = rank)
+    w = worlds.make_world(args.workload, seed=rank)
+    G = binding.World(w, device=str(dev))
+    N, nc = G.N, G.nx * G.ny
+    G.step(args.warmup)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    l0 = G.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    G.step(args.steps)
+    e1.record()
+    barrier()
+    ms = torch.tensor([e0.elapsed_time(e1)], device=dev, dtype=torch.float64)
+    launches = G.launch_count() - l0
+    if dist is not None:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms_total = float(ms.item())
+    clocks = sampler.stop() if rank == 0 else None
+    ms_step = ms_total / args.steps
+    value = world_size * N * args.steps / (ms_total * 1e-3)
+
+    # per-kernel durations, live, CUDA events on the world's stream (up to 64 steps)
+    G.profile_enable(True)
+    G.step(min(args.steps, 64))
+    prof, pn = G.profile_read()
+    G.profile_enable(False)
+    kms = {k: v / max(pn, 1) for k, v in prof.items()}
+    kb = kernel_bytes(nc, N)
+    peak, peak_src = measured_peak_gbs()
+    dom = max(kms, key=lambda k: kms[k])
+    ach = kb[dom] / (kms[dom] * 1e-3) / 1e9 if kms[dom] > 0 else 0.0
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
+                "frac": ach / peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": kb[dom], "ms_per_launch": kms[dom],
+                "share_of_step": kms[dom] / max(sum(kms.values()), 1e-12)}
+    ach_step = step_bytes(nc, N) / (ms_step * 1e-3) / 1e9
+    roofline_step = {"bound": "hbm", "achieved": ach_step, "peak": peak, "unit": "GB/s",
+                     "frac": ach_step / peak, "frac_of_8TBps_nominal": ach_step / 8000.0,
+                     "algorithmic_bytes_per_step": step_bytes(nc, N)}
+    kernels = {k: {"ms": round(kms[k], 5),
+                   "GBps": round(kb[k] / (kms[k] * 1e-3) / 1e9, 1) if kms[k] > 0 else None}
+               for k in kms}
+
+    # e2e: host buffers, copies inside the timed region, every step
+    keys = ("xy", "L_rest", "theta_rest", "k_bend", "k_shear", "k_stretch", "act_amp", "act_phase",
+            "act_period")
+    host = {k: torch.from_numpy(np.ascontiguousarray(w[k], dtype=np.float32)).pin_memory() for k in keys}
+    host["offsets"] = w["offsets"]
+    xy_back = torch.empty((N, 2), dtype=torch.float32).pin_memory()
+    h2d = sum(host[k].numel() * 4 for k in keys)
+    d2h = xy_back.numel() * 4
+
+    def e2e_step():
+        G.load_filaments(host)             # pinned host -> device + SoA packing (syncs)
+        G.step(1)
+        out = G.read_state(keys=("xy",), host=False)["xy"]
+        xy_back.copy_(out, non_blocking=True)
+        torch.cuda.synchronize(dev)
+        host["xy"].copy_(xy_back)          # the next step continues from the returned positions
+
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.e2e_steps):
+        e2e_step()
+    barrier()
+    te = torch.tensor([time.perf_counter() - t0], device=dev, dtype=torch.float64)
+    if dist is not None:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_val = world_size * N * args.e2e_steps / float(te.item())
+    G.close()
+
+    cpu = None
+    if rank == 0 and world_size == 1 and not args.no_cpu_baseline:
+        v, cores, n, secs = time_oracle(SAMPLE_WORLD, 0, budget_s=10.0, min_steps=3, max_steps=200)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"world {SAMPLE_WORLD} (config-4 recipe at 1/100 of 4d: 100,032 beads, 640x640 grid), "
+                         f"{n} steps in {secs:.1f} s, fp64, OpenMP over {cores} threads"}
+
+    if rank == 0:
+        p = w["params"]
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world_size, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic (seeded, DESIGN.md input recipe)",
+            "config": {"workload": f"BASELINE.json config {args.workload}", "beads": N,
+                       "filaments": len(w["offsets"]) - 1, "grid": [p["nx"], p["ny"]],
+                       "parallelism": "replicas only (one independent world per GPU)",
+                       "l2": f"working set {step_bytes(nc, N) / 1e6:.0f} MB per step vs 126 MB L2; no flush"},
+            "cell_steps_per_s": world_size * nc * args.steps / (ms_total * 1e-3),
+            "roofline": roofline, "roofline_step": roofline_step, "kernels": kernels,
+            "cpu_baseline": cpu,
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": args.e2e_steps,
+                    "what": "per step: mc_load_filaments from pinned host arrays + mc_step(1) + "
+                            "mc_read_state(xy) to pinned host"},
+            "gpu_launches": launches, "clocks": clocks,
+        }), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

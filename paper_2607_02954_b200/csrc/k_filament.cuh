@@ -1,133 +1,224 @@
 // k_filament.cuh -- K1: S0 actuation + S1 elastic PBD displacement (Eq. 1-4) + S4 field forces.
 //
-// One warp per chain; lane <-> bead; neighbour beads are exchanged with warp shuffles
-// (north_star (1)).  A chain longer than 32 beads is walked in windows of 32 beads that
-// overlap by 4 (D_i needs X_{i-2..i+2}).
-//
 // Paper: bending pass Eq. 1, position pass Eq. 2-4.
 // Readings: 1 the net PBD displacement D_i becomes the bead force kappa*D_i;
 // 2 edge angles come from the current geometry; 3 one Jacobi iteration; 4 joint angle =
-// atan2(cross, dot); 5 free ends; 18 theta*_i(n) = theta0_i + a_i sin(2 pi n dt/T_i + phi_i).
+// atan2(cross, dot) in (-pi, pi]; 5 free ends; 18 theta*_i(n) = theta0_i + a_i sin(2 pi n dt/T_i + phi_i).
 //
-// Precision.  State and parameters are fp32 and so is most of the arithmetic, but D_i is a
-// difference of differences: |D| ~ 1e-4 is formed from edge vectors of length ~1 and joint
-// angles ~0.3 rad, so plain fp32 leaves ~1e-5 relative error on the force (measured, DESIGN.md
-// "Precision") -- at the parity bar.  The three cancelling quantities are therefore formed
-// in fp64 from the exact fp32 inputs and rounded once: edge vector v = X_{i+1} - X_i,
-// |v|^2 - L^2, and the joint angle psi - theta* (cross, dot, atan2 and the actuation phase).
+// Mapping (north_star (1): one warp per chain, neighbours by warp shuffles, float4 SoA loads).
+// The beads of all chains form one flat chain-ordered array with a first/last flag per bead.
+// A warp owns a window of 64 consecutive beads, two per lane (positions arrive as one float4
+// per lane, parameters as three float4 per bead); D_i needs X_{i-2..i+2}, of which all but two
+// shuffles per quantity stay inside the lane.  When every chain has the same length m and m
+// divides 64 the windows are aligned to chain starts (one 64-bead chain, two 32-bead chains or
+// four 16-bead chains per warp) and all 64 beads are outputs; otherwise windows advance by 60
+// and overlap by 4, the two beads at either end being halo.
+//
+// Precision.  State and parameters are fp32 and so is almost all arithmetic.  But D_i is a
+// difference of differences (|D| ~ 1e-4 out of edge vectors ~1 and joint angles ~0.3 rad);
+// plain fp32 leaves ~1e-5 relative error on the force, which is the parity bar (measured,
+// DESIGN.md "Precision").  Three cancelling quantities are therefore formed in fp64 from the
+// exact fp32 inputs and rounded once: the edge vector v = X_{i+1} - X_i, |v|^2 - L^2, and
+// the joint's (cross, dot).  The joint angle itself never needs an fp64 atan2: (dot, cross) is
+// rotated by the rest angle first -- by the fp32 pair (cos, sin)(theta0) stored at load time,
+// whose own angle differs from theta0 by a stored residual eps -- so that the fp32 atan2f acts
+// on the SMALL angle psi - theta0, where its absolute error is ~1e-9.
 #pragma once
 #include "mc_common.cuh"
 
 namespace mc {
 
+constexpr int BEAD_FIRST = 1, BEAD_LAST = 2, BEAD_PAD = 4;
+
 struct FilamentArgs {
-  const int* offsets;     // [n_fil+1]
-  int n_fil;
-  const float2* X;        // [N]
-  const float4* P0;       // {L_rest, theta_rest, act_amp, act_phase}
-  const float4* P1;       // {k_bend, k_shear, k_stretch, act_period}
-  float2* F;              // [N] out: total bead force
-  float* sense;           // [N] out (only written when csum != NULL)
-  const float* A0;        // force-gradient planes (may be NULL: no field forces)
+  const float2* X;   // [N]
+  const float4* PA;  // {L_rest, act_amp, act_phase, k_bend}
+  const float4* PB;  // {k_shear, k_stretch, r_hi, r_lo}       r = dt / act_period (hi + lo)
+  const float4* PC;  // {cos theta0, sin theta0, eps, flags}   eps = theta0 - atan2(sin, cos)
+  float2* F;         // [N] out: total bead force
+  float* sense;      // [N] out (only written when csum != NULL)
+  const float* A0;   // force-gradient planes (may be NULL: no field forces)
   const float* A1;
-  const float* csum;      // sum of static fields (may be NULL)
+  const float* csum;  // sum of static fields (may be NULL)
+  int N;
   int nx, ny;
-  float kappa;            // k_el * dt^2
-  double t;               // n * dt (step index before the increment)
+  int stride;        // 64 (aligned windows) or 60 (overlapping windows)
+  int n_windows;
+  float kappa;       // k_el * dt^2
+  double n_step;     // step index n (before the increment)
 };
+
+struct BeadParams {
+  float L, amp, phase, kb, ks, kst, rhi, rlo, c0, s0, eps;
+  int flags;
+};
+
+__device__ __forceinline__ BeadParams load_params(const FilamentArgs& a, int b, bool valid) {
+  BeadParams p;
+  if (valid) {
+    const float4 pa = __ldg(a.PA + b), pb = __ldg(a.PB + b), pc = __ldg(a.PC + b);
+    p.L = pa.x; p.amp = pa.y; p.phase = pa.z; p.kb = pa.w;
+    p.ks = pb.x; p.kst = pb.y; p.rhi = pb.z; p.rlo = pb.w;
+    p.c0 = pc.x; p.s0 = pc.y; p.eps = pc.z; p.flags = __float_as_int(pc.w);
+  } else {
+    p.L = 1.f; p.amp = p.phase = p.kb = p.ks = p.kst = p.rhi = p.rlo = p.s0 = p.eps = 0.f;
+    p.c0 = 1.f;
+    p.flags = BEAD_FIRST | BEAD_LAST | BEAD_PAD;
+  }
+  return p;
+}
+
+// (1/2) k_bend C_bend of the joint between edge pv (incoming) and edge v (outgoing); Eq. 1.
+__device__ __forceinline__ float half_kC(double pvx, double pvy, double vx, double vy, const BeadParams& p,
+                                         double n_step) {
+  const double TWO_PI = 6.283185307179586476925286766559;
+  const double cross = pvx * vy - pvy * vx, dot = pvx * vx + pvy * vy;
+  // rotate by -theta0' (theta0' = angle of the stored fp32 pair): small-angle atan2f
+  const double c = (double)p.c0, s = (double)p.s0;
+  const double dotp = dot * c + cross * s, crossp = cross * c - dot * s;
+  float psi_p = atan2f((float)crossp, (float)dotp);  // = psi - theta0' (mod 2 pi)
+  if (!(dot > 0.0 && dotp > 0.0)) {
+    // rare: joint bent beyond +-pi/2.  Restore the oracle's branch, psi in (-pi, pi].
+    const float t = psi_p + atan2f(p.s0, p.c0);
+    if (t > 3.14159265358979f) psi_p -= 6.28318530717959f;
+    else if (t <= -3.14159265358979f) psi_p += 6.28318530717959f;
+  }
+  // actuation phase 2 pi n dt/T + phi, reduced in fp64 (n dt/T reaches thousands of turns)
+  double turns = n_step * (double)p.rhi + n_step * (double)p.rlo;
+  turns -= rint(turns);
+  double ph = TWO_PI * turns + (double)p.phase;
+  ph -= TWO_PI * rint(ph * (1.0 / TWO_PI));
+  const float C = psi_p - p.eps - p.amp * sinf((float)ph);
+  return 0.5f * p.kb * C;
+}
+
+// Delta x of an edge (Eq. 2-3) after the bending pass turned its director by delta.
+__device__ __forceinline__ float2 edge_delta(double vx, double vy, float delta, const BeadParams& p) {
+  const double l2 = vx * vx + vy * vy;
+  const float L = p.L;
+  const float ell = sqrtf((float)l2);
+  const float dl = (float)(l2 - (double)L * (double)L) / (ell + L);  // |v| - L_rest, no cancellation
+  const float inv = 1.0f / ell;
+  const float tx = (float)vx * inv, ty = (float)vy * inv;
+  const float sd = sinf(delta), sh = sinf(0.5f * delta);
+  const float omc = 2.0f * sh * sh;  // 1 - cos(delta)
+  // t - d with d = Rot(delta) t: Kirchhoff-Love error minus the stretch part, divided by L
+  const float ex = omc * tx + sd * ty, ey = omc * ty - sd * tx;
+  const float ksL = p.ks * L;
+  return make_float2(0.5f * p.kst * fmaf(ksL, ex, dl * tx), 0.5f * p.kst * fmaf(ksL, ey, dl * ty));
+}
 
 __global__ void __launch_bounds__(256) k_filament_force(FilamentArgs a) {
   const int lane = threadIdx.x & 31;
-  const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int n_warps = (gridDim.x * blockDim.x) >> 5;
-  const double TWO_PI = 6.283185307179586476925286766559;
+  const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (w >= a.n_windows) return;
   const unsigned FULL = 0xffffffffu;
-  for (int f = warp; f < a.n_fil; f += n_warps) {
-    const int b0 = a.offsets[f];
-    const int m = a.offsets[f + 1] - b0;
-    for (int base = 0;; base += 28) {
-      const bool last = (base + 32 >= m);
-      const int i = base + lane;
-      const bool valid = i < m;
-      float2 x = make_float2(0.f, 0.f);
-      float4 p0 = make_float4(1.f, 0.f, 0.f, 0.f), p1 = make_float4(0.f, 0.f, 0.f, 1.f);
-      if (valid) {
-        x = a.X[b0 + i];
-        p0 = a.P0[b0 + i];
-        p1 = a.P1[b0 + i];
-      }
-      // edge i = (i, i+1): v = X_{i+1} - X_i
-      const double xd = (double)x.x, yd = (double)x.y;
-      const double xn = __shfl_down_sync(FULL, xd, 1), yn = __shfl_down_sync(FULL, yd, 1);
-      const bool has_edge = (i + 1 < m) && (lane < 31);
-      const double vx = has_edge ? xn - xd : 1.0, vy = has_edge ? yn - yd : 0.0;
-      // joint i (between edge i-1 and edge i): C = psi - theta*   (Eq. 1's C_bend)
-      const double pvx = __shfl_up_sync(FULL, vx, 1), pvy = __shfl_up_sync(FULL, vy, 1);
-      const bool has_joint = (i >= 1) && (i + 1 < m) && (lane >= 1) && (lane < 31);
-      float hkC = 0.0f;  // (1/2) k_bend C
-      if (has_joint) {
-        const double cross = pvx * vy - pvy * vx, dot = pvx * vx + pvy * vy;
-        const double psi = atan2(cross, dot);
-        double ph = TWO_PI * (a.t / (double)p1.w) + (double)p0.w;
-        ph -= TWO_PI * rint(ph * (1.0 / TWO_PI));
-        const float s = sinf((float)ph);
-        const double theta_star = (double)p0.y + (double)(p0.z * s);
-        hkC = 0.5f * p1.x * (float)(psi - theta_star);
-      }
-      // Eq. 1 applied to edge i: theta_1 of joint i+1 (+), theta_2 of joint i (-)
-      const float hkC_next = __shfl_down_sync(FULL, hkC, 1);
-      const float delta = hkC_next - hkC;
-      float dx = 0.0f, dy = 0.0f;  // Delta x of edge i (Eq. 3)
-      if (has_edge) {
-        const double l2 = vx * vx + vy * vy;
-        const float L = p0.x;
-        const float ell = sqrtf((float)l2);
-        const float dl = (float)(l2 - (double)L * (double)L) / (ell + L);  // |v| - L_rest
-        const float inv = 1.0f / ell;
-        const float tx = (float)vx * inv, ty = (float)vy * inv;
-        const float sd = sinf(delta), sh = sinf(0.5f * delta);
-        const float omc = 2.0f * sh * sh;  // 1 - cos(delta)
-        // t - d, d = Rot(delta) t  (director after the bending pass)
-        const float ex = omc * tx + sd * ty, ey = omc * ty - sd * tx;
-        const float ksL = p1.y * L;
-        dx = 0.5f * p1.z * fmaf(ksL, ex, dl * tx);
-        dy = 0.5f * p1.z * fmaf(ksL, ey, dl * ty);
-      }
-      // Eq. 4 summed per bead: D_i = Delta_i - Delta_{i-1}
-      const float pdx = __shfl_up_sync(FULL, dx, 1), pdy = __shfl_up_sync(FULL, dy, 1);
-      float Dx = dx, Dy = dy;
-      if (lane >= 1) { Dx -= pdx; Dy -= pdy; }
-      const bool out = valid && (base == 0 || lane >= 2) && (last || lane <= 29);
-      if (out) {
-        float Fx = a.kappa * Dx, Fy = a.kappa * Dy;
-        if (a.A0) {
-          const float2 g = interp2(a.A0, a.A1, a.nx, a.ny, x.x, x.y);
-          Fx += g.x;
-          Fy += g.y;
-        }
-        a.F[b0 + i] = make_float2(Fx, Fy);
-        if (a.csum) a.sense[b0 + i] = interp1(a.csum, a.nx, a.ny, x.x, x.y);
-      }
-      if (last) break;
-    }
+  const bool aligned = (a.stride == 64);
+  const int base = w * a.stride - (aligned ? 0 : 2);  // even => float4-aligned pairs
+  const int bA = base + 2 * lane, bB = bA + 1;
+  const bool vA = bA >= 0 && bA < a.N, vB = bB >= 0 && bB < a.N;
+  float2 xa = make_float2(0.f, 0.f), xb = make_float2(1.f, 0.f);
+  if (vA && vB) {
+    const float4 q = __ldg(reinterpret_cast<const float4*>(a.X + bA));
+    xa = make_float2(q.x, q.y);
+    xb = make_float2(q.z, q.w);
+  } else {
+    if (vA) xa = __ldg(a.X + bA);
+    if (vB) xb = __ldg(a.X + bB);
+  }
+  const BeadParams pA = load_params(a, bA, vA), pB = load_params(a, bB, vB);
+  // neighbours across the lane boundary
+  const float nxa = __shfl_down_sync(FULL, xa.x, 1), nya = __shfl_down_sync(FULL, xa.y, 1);
+  const float pxb = __shfl_up_sync(FULL, xb.x, 1), pyb = __shfl_up_sync(FULL, xb.y, 1);
+  // edge vectors (fp64 differences of fp32 positions are exact)
+  const double eAx = (double)xb.x - (double)xa.x, eAy = (double)xb.y - (double)xa.y;  // A -> B
+  const double eBx = (double)nxa - (double)xb.x, eBy = (double)nya - (double)xb.y;    // B -> next A
+  const double ePx = (double)xa.x - (double)pxb, ePy = (double)xa.y - (double)pyb;    // prev B -> A
+  const bool edgeA = !(pA.flags & BEAD_LAST) && vB;
+  const bool edgeB = !(pB.flags & BEAD_LAST) && lane < 31;
+  const bool jointA = !(pA.flags & (BEAD_FIRST | BEAD_LAST)) && lane >= 1;
+  const bool jointB = !(pB.flags & (BEAD_FIRST | BEAD_LAST)) && lane < 31;
+  const float hA = jointA ? half_kC(ePx, ePy, eAx, eAy, pA, a.n_step) : 0.0f;
+  const float hB = jointB ? half_kC(eAx, eAy, eBx, eBy, pB, a.n_step) : 0.0f;
+  // Eq. 1 on an edge: theta_1 of its far joint (+), theta_2 of its near joint (-)
+  const float hA_next = __shfl_down_sync(FULL, hA, 1);
+  float2 dA = make_float2(0.f, 0.f), dB = make_float2(0.f, 0.f);
+  if (edgeA) dA = edge_delta(eAx, eAy, hB - hA, pA);
+  if (edgeB) dB = edge_delta(eBx, eBy, hA_next - hB, pB);
+  // Eq. 4 summed per bead: D_i = Delta_i - Delta_{i-1}
+  float pdx = __shfl_up_sync(FULL, dB.x, 1), pdy = __shfl_up_sync(FULL, dB.y, 1);
+  if ((pA.flags & BEAD_FIRST) || lane == 0) { pdx = 0.f; pdy = 0.f; }
+  float DAx = dA.x - pdx, DAy = dA.y - pdy;
+  float DBx = dB.x, DBy = dB.y;
+  if (!(pB.flags & BEAD_FIRST)) { DBx -= dA.x; DBy -= dA.y; }
+  const bool out = aligned || (lane >= 1 && lane <= 30);
+  if (!out) return;
+  float2 FA = make_float2(a.kappa * DAx, a.kappa * DAy), FB = make_float2(a.kappa * DBx, a.kappa * DBy);
+  if (a.A0) {
+    if (vA) { const float2 g = interp2(a.A0, a.A1, a.nx, a.ny, xa.x, xa.y); FA.x += g.x; FA.y += g.y; }
+    if (vB) { const float2 g = interp2(a.A0, a.A1, a.nx, a.ny, xb.x, xb.y); FB.x += g.x; FB.y += g.y; }
+  }
+  if (vA && vB) {
+    *reinterpret_cast<float4*>(a.F + bA) = make_float4(FA.x, FA.y, FB.x, FB.y);
+  } else {
+    if (vA) a.F[bA] = FA;
+    if (vB) a.F[bB] = FB;
+  }
+  if (a.csum) {
+    if (vA) a.sense[bA] = interp1(a.csum, a.nx, a.ny, xa.x, xa.y);
+    if (vB) a.sense[bB] = interp1(a.csum, a.nx, a.ny, xb.x, xb.y);
   }
 }
 
-// mc_load_filaments: pack the per-bead parameters and validate them (flag != 0 => invalid)
-__global__ void k_pack_params(int N, const float* __restrict__ xy, const float* __restrict__ L_rest,
-                              const float* __restrict__ theta_rest, const float* __restrict__ k_bend,
-                              const float* __restrict__ k_shear, const float* __restrict__ k_stretch,
-                              const float* __restrict__ act_amp, const float* __restrict__ act_phase,
-                              const float* __restrict__ act_period, float2* __restrict__ X,
-                              float4* __restrict__ P0, float4* __restrict__ P1, int* __restrict__ flag) {
+// mc_load_filaments: gather the caller's arrays into the internal (spatially sorted) chain
+// order, pack the per-bead parameters and validate them (flag != 0 => invalid input).
+struct PackArgs {
+  int N;
+  const int* src;  // internal bead -> caller's bead
+  const unsigned char* flags;
+  const float *xy, *L_rest, *theta_rest, *k_bend, *k_shear, *k_stretch, *act_amp, *act_phase, *act_period;
+  float2* X;
+  float4 *PA, *PB, *PC;
+  double dt;
+  int* bad;
+};
+
+__global__ void k_pack_params(PackArgs a) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
-  if (b >= N) return;
-  X[b] = make_float2(xy[2 * b], xy[2 * b + 1]);
-  const float kb = k_bend[b], ks = k_shear[b], kst = k_stretch[b], T = act_period[b];
-  P0[b] = make_float4(L_rest[b], theta_rest[b], act_amp[b], act_phase[b]);
-  P1[b] = make_float4(kb, ks, kst, T);
-  if (!(kb >= 0.f && kb <= 1.f && ks >= 0.f && ks <= 1.f && kst >= 0.f && kst <= 1.f)) atomicOr(flag, 1);
-  if (!(T > 0.f)) atomicOr(flag, 2);
+  if (b >= a.N) return;
+  const int s = a.src[b];
+  a.X[b] = make_float2(a.xy[2 * s], a.xy[2 * s + 1]);
+  const float kb = a.k_bend[s], ks = a.k_shear[s], kst = a.k_stretch[s], T = a.act_period[s];
+  const double th = (double)a.theta_rest[s];
+  const float c0 = (float)cos(th), s0 = (float)sin(th);
+  const float eps = (float)(th - atan2((double)s0, (double)c0));
+  const double r = a.dt / (double)T;
+  const float rhi = (float)r, rlo = (float)(r - (double)rhi);
+  a.PA[b] = make_float4(a.L_rest[s], a.act_amp[s], a.act_phase[s], kb);
+  a.PB[b] = make_float4(ks, kst, rhi, rlo);
+  a.PC[b] = make_float4(c0, s0, eps, __int_as_float((int)a.flags[b]));
+  if (!(kb >= 0.f && kb <= 1.f && ks >= 0.f && ks <= 1.f && kst >= 0.f && kst <= 1.f)) atomicOr(a.bad, 1);
+  if (!(T > 0.f)) atomicOr(a.bad, 2);
+}
+
+// first-bead tile key of every chain (for the spatial sort of the chains at load time)
+__global__ void k_chain_keys(int n_fil, const int* __restrict__ offsets, const float* __restrict__ xy, int nx,
+                             int ny, int key_tile, int* __restrict__ keys) {
+  const int f = blockIdx.x * blockDim.x + threadIdx.x;
+  if (f >= n_fil) return;
+  const int b = offsets[f];
+  const int ci = wrapi((int)floorf(xy[2 * b]), nx), cj = wrapi((int)floorf(xy[2 * b + 1]), ny);
+  keys[f] = (cj / key_tile) * ((nx + key_tile - 1) / key_tile) + ci / key_tile;
+}
+
+// mc_read_state: internal order -> caller's order
+__global__ void k_unpermute2(int N, const int* __restrict__ src, const float2* __restrict__ in, float2* __restrict__ out) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b < N) out[src[b]] = in[b];
+}
+__global__ void k_unpermute1(int N, const int* __restrict__ src, const float* __restrict__ in, float* __restrict__ out) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b < N) out[src[b]] = in[b];
 }
 
 }  // namespace mc

@@ -1,52 +1,171 @@
-// k_p2g.cuh -- K2a scalar deposition (S2) and K2b force spreading (S5) as gathers by node.
+// k_p2g.cuh -- K2a scalar deposition (S2) and K2b force spreading (S5): shared-memory tile
+// accumulation (north_star (2)).
 //
 // S2: rho_b(g) = sum_i delta_h(g - X_i)            ("node positions are deposited")
 // S5: G(g)     = sum_i F_i delta_h(g - X_i)        ("broadcasts ... onto the grid")
-// delta_h = Peskin 4-point product kernel (reading 7, 13).
+// delta_h = Peskin 4-point product kernel (readings 7, 13).
 //
-// A bead whose cell is (ci,cj) = floor(X) touches nodes ci-1..ci+2, cj-1..cj+2, so node
-// (i,j) receives from the beads of cells (i+di, j+dj), di,dj in -2..1, with weight planes
-// wx[1-di] * wy[1-dj].  One thread per node walks those 16 bead lists in the canonical order
-// K0 built: no float atomics, fixed summation order => bit-reproducible.
+// One CTA per TS x TS tile.  Each thread takes beads from the tile's list (k_tile.cuh), forms
+// the 4+4 weights and adds its up-to-16 contributions into the tile's accumulators in shared
+// memory with the native 32-bit integer atomic (ATOMS.ADD).  Accumulating in FIXED POINT
+// makes the sum independent of the order in which the atomics land, so the result is
+// bit-reproducible run to run without sorting the lists (a float atomic would not be, and on
+// sm_100a it is a CAS loop ~4x slower than the integer one; profiles/atoms_microbench.md).
+// The fixed-point scale is a power of two chosen per tile from a bound on the largest
+// possible accumulator, so no overflow can occur and the quantisation is ~2^-30 of that bound:
+//   S2: every contribution is <= 1/4, so |acc| <= n_list/4;
+//   S5: |sum_i F_i w_i| <= max|F| * sum_i w_i = max|F| * rho_b(g) <= max|F| * max_tile(rho_b),
+//       with max_tile(rho_b) left behind by S2 of the same step (same X, same weights).
 #pragma once
+#include "k_tile.cuh"
 #include "mc_common.cuh"
 
 namespace mc {
 
-template <bool SPREAD>
-__global__ void __launch_bounds__(256) k_p2g_gather(int nx, int ny, const int* __restrict__ cell_start,
-                                                    const float* __restrict__ W, size_t plane,
-                                                    const int* __restrict__ slot_bead,
-                                                    const float2* __restrict__ F,
-                                                    float* __restrict__ out0, float* __restrict__ out1) {
-  const int i = blockIdx.x * 32 + (threadIdx.x & 31);
-  const int j = blockIdx.y * 8 + (threadIdx.x >> 5);
-  float a0 = 0.0f, a1 = 0.0f;
+struct TileBead {
+  int lx[4], ly[4];  // local node indices in the tile, or -1 when outside it
+  float wx[4], wy[4];
+};
+
+__device__ __forceinline__ void tile_bead(float2 p, int nx, int ny, int x0, int y0, TileBead& tb) {
+  int i0, j0;
+  float fx, fy;
+  support(p.x, i0, fx);
+  support(p.y, j0, fy);
+  peskin4(fx, tb.wx[0], tb.wx[1], tb.wx[2], tb.wx[3]);
+  peskin4(fy, tb.wy[0], tb.wy[1], tb.wy[2], tb.wy[3]);
+  i0 = wrapi(i0, nx);
+  j0 = wrapi(j0, ny);
 #pragma unroll
-  for (int dj = -2; dj <= 1; ++dj) {
-    const int row = wrap1(j + dj, ny);
-    const float* wy = W + (size_t)(4 + 1 - dj) * plane;
+  for (int k = 0; k < 4; ++k) {
+    const int c = ((i0 + k >= nx) ? i0 + k - nx : i0 + k) - x0;
+    const int r = ((j0 + k >= ny) ? j0 + k - ny : j0 + k) - y0;
+    tb.lx[k] = ((unsigned)c < (unsigned)TS) ? c : -1;
+    tb.ly[k] = ((unsigned)r < (unsigned)TS) ? r : -1;
+  }
+}
+
+__device__ __forceinline__ float block_max(float v, float* sm /*[32]*/) {
 #pragma unroll
-    for (int di = -2; di <= 1; ++di) {
-      const int col = wrap1(i + di, nx);
-      const int c = row * nx + col;
-      const int s = __ldg(cell_start + c), e = __ldg(cell_start + c + 1);
-      const float* wx = W + (size_t)(1 - di) * plane;
-      for (int k = s; k < e; ++k) {
-        const float w = __ldg(wx + k) * __ldg(wy + k);
-        if (SPREAD) {
-          const float2 f = __ldg(F + __ldg(slot_bead + k));
-          a0 = fmaf(w, f.x, a0);
-          a1 = fmaf(w, f.y, a1);
-        } else {
-          a0 += w;
-        }
-      }
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+  __syncthreads();
+  v = (threadIdx.x < (blockDim.x >> 5)) ? sm[threadIdx.x] : 0.0f;
+  if (threadIdx.x < 32) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if (threadIdx.x == 0) sm[0] = v;
+  }
+  __syncthreads();
+  v = sm[0];
+  __syncthreads();
+  return v;
+}
+
+// power-of-two scale s with bound * s < 2^30
+__device__ __forceinline__ float pow2_scale(float bound) {
+  int ex;
+  frexpf(bound, &ex);  // bound = m * 2^ex, m in [0.5, 1)
+  return ldexpf(1.0f, 30 - ex);
+}
+
+// K2a: S2 deposit.  tile_rho_max[t] receives max over the tile of rho_b (for K2b's scale).
+__global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int* __restrict__ tile_start,
+                                                      const int* __restrict__ list,
+                                                      const float2* __restrict__ X,
+                                                      float* __restrict__ rho_b,
+                                                      float* __restrict__ tile_rho_max) {
+  __shared__ int acc[TS * TS];
+  __shared__ float red[32];
+  const int t = blockIdx.x, ntx = nx / TS;
+  const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
+  const int s = tile_start[t], e = tile_start[t + 1];
+  for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) acc[c] = 0;
+  const float scale = pow2_scale(fmaxf(0.25f * (float)(e - s), 1.0f));
+  __syncthreads();
+  for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
+    TileBead tb;
+    tile_bead(__ldg(X + __ldg(list + k)), nx, ny, x0, y0, tb);
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      if (tb.ly[l] < 0) continue;
+      const float wys = tb.wy[l] * scale;
+#pragma unroll
+      for (int kx = 0; kx < 4; ++kx)
+        if (tb.lx[kx] >= 0) atomicAdd(&acc[tb.ly[l] * TS + tb.lx[kx]], __float2int_rn(tb.wx[kx] * wys));
     }
   }
-  const size_t g = (size_t)j * nx + i;
-  out0[g] = a0;
-  if (SPREAD) out1[g] = a1;
+  __syncthreads();
+  const float inv = 1.0f / scale;
+  float mx = 0.0f;
+  for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) {
+    const float v = (float)acc[c] * inv;
+    rho_b[(size_t)(y0 + (c >> 5)) * nx + x0 + (c & 31)] = v;
+    mx = fmaxf(mx, v);
+  }
+  mx = block_max(mx, red);
+  if (threadIdx.x == 0) tile_rho_max[t] = mx;
+}
+
+// Accumulate the spread force of one tile into shared memory (two planes), return the scale.
+// Shared by the stand-alone spread kernel and by the fused spread + fluid kernel (k_lbm.cuh).
+__device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, int y0, int s, int e,
+                                                        const int* __restrict__ list,
+                                                        const float2* __restrict__ X,
+                                                        const float2* __restrict__ F, float rho_max,
+                                                        int* acc0, int* acc1, float* red) {
+  for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) { acc0[c] = 0; acc1[c] = 0; }
+  float fm = 0.0f;
+  for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
+    const float2 f = __ldg(F + __ldg(list + k));
+    fm = fmaxf(fm, fmaxf(fabsf(f.x), fabsf(f.y)));
+  }
+  fm = block_max(fm, red);  // also orders the zeroing before the atomics
+  const float sum_w = (rho_max > 0.0f) ? 1.0625f * rho_max : fmaxf(0.25f * (float)(e - s), 1.0f);
+  const float scale = pow2_scale(fmaxf(fm * sum_w, 1e-18f));
+  for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
+    const int b = __ldg(list + k);
+    TileBead tb;
+    tile_bead(__ldg(X + b), nx, ny, x0, y0, tb);
+    const float2 f = __ldg(F + b);
+    const float fxs = f.x * scale, fys = f.y * scale;
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      if (tb.ly[l] < 0) continue;
+#pragma unroll
+      for (int kx = 0; kx < 4; ++kx)
+        if (tb.lx[kx] >= 0) {
+          const float w = tb.wx[kx] * tb.wy[l];
+          const int a = tb.ly[l] * TS + tb.lx[kx];
+          atomicAdd(&acc0[a], __float2int_rn(w * fxs));
+          atomicAdd(&acc1[a], __float2int_rn(w * fys));
+        }
+    }
+  }
+  __syncthreads();
+  return scale;
+}
+
+// K2b: S5 spread (stand-alone form; the hot path uses the fused spread + fluid kernel)
+__global__ void __launch_bounds__(256) k_spread_tile(int nx, int ny, const int* __restrict__ tile_start,
+                                                     const int* __restrict__ list,
+                                                     const float2* __restrict__ X,
+                                                     const float2* __restrict__ F,
+                                                     const float* __restrict__ tile_rho_max,
+                                                     float* __restrict__ G0, float* __restrict__ G1) {
+  __shared__ int acc0[TS * TS], acc1[TS * TS];
+  __shared__ float red[32];
+  const int t = blockIdx.x, ntx = nx / TS;
+  const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
+  const int s = tile_start[t], e = tile_start[t + 1];
+  const float scale = spread_tile_accumulate(nx, ny, x0, y0, s, e, list, X, F,
+                                             tile_rho_max ? tile_rho_max[t] : 0.0f, acc0, acc1, red);
+  const float inv = 1.0f / scale;
+  for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) {
+    const size_t g = (size_t)(y0 + (c >> 5)) * nx + x0 + (c & 31);
+    G0[g] = (float)acc0[c] * inv;
+    G1[g] = (float)acc1[c] * inv;
+  }
 }
 
 }  // namespace mc

@@ -1,0 +1,113 @@
+// k_tile.cuh -- K0: bin the beads by grid TILE (north_star (2): "bead sort by cell tile
+// followed by shared-memory tile accumulation, so global atomics are minimised").
+//
+// A tile is TS x TS nodes.  A bead is listed in every tile its 4x4 Peskin support overlaps
+// (1, 2 or 4 tiles), so a tile's CTA can accumulate ALL contributions to its own nodes from its
+// own list and never writes outside the tile: no global float atomics, no halo exchange.
+//   count : per bead, +1 on each overlapped tile (integer atomics, warp-aggregated)
+//   scan  : exclusive prefix sum over the tiles (one block; there are few tiles)
+//   fill  : per bead, claim a slot in each overlapped tile's segment and store the bead index
+// The order inside a tile's list is the arrival order of the atomics and is NOT reproducible;
+// that is harmless because the accumulation that consumes the lists (k_p2g.cuh) adds integers
+// (fixed point), which is order-independent.
+#pragma once
+#include "mc_common.cuh"
+
+namespace mc {
+
+constexpr int TS = 32;  // tile side in nodes
+
+// The (up to 4) tiles overlapped by the support of a bead at (x,y): tiles of the first and
+// the last support node along each axis (periodic).  Returns the number of distinct tiles.
+__device__ __forceinline__ int bead_tiles(float x, float y, int nx, int ny, int ntx, int t[4]) {
+  const int i0 = wrapi((int)floorf(x) - 1, nx), j0 = wrapi((int)floorf(y) - 1, ny);
+  const int i3 = (i0 + 3 >= nx) ? i0 + 3 - nx : i0 + 3, j3 = (j0 + 3 >= ny) ? j0 + 3 - ny : j0 + 3;
+  const int txa = i0 / TS, txb = i3 / TS, tya = j0 / TS, tyb = j3 / TS;
+  int n = 0;
+  t[n++] = tya * ntx + txa;
+  if (txb != txa) t[n++] = tya * ntx + txb;
+  if (tyb != tya) {
+    t[n++] = tyb * ntx + txa;
+    if (txb != txa) t[n++] = tyb * ntx + txb;
+  }
+  return n;
+}
+
+// warp-aggregated atomicAdd(&ctr[key], 1) for the lanes with act set; returns the claimed value
+__device__ __forceinline__ int warp_claim(int* ctr, int key, bool act) {
+  const unsigned m = __ballot_sync(0xffffffffu, act);
+  int slot = 0;
+  if (act) {
+    const unsigned peers = __match_any_sync(m, key);
+    const int lane = threadIdx.x & 31;
+    const int leader = __ffs(peers) - 1;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(&ctr[key], __popc(peers));
+    base = __shfl_sync(peers, base, leader);
+    slot = base + __popc(peers & ((1u << lane) - 1u));
+  }
+  return slot;
+}
+
+// FILL = false: tile_ctr[t] += 1 per listed bead.  FILL = true: tile_ctr holds the running
+// cursor (initialised to tile_start) and the bead index is stored at the claimed slot.
+template <bool FILL>
+__global__ void __launch_bounds__(256) k_tile_bin(const float2* __restrict__ X, int N, int nx, int ny,
+                                                  int* __restrict__ tile_ctr, int* __restrict__ list) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  int t[4] = {0, 0, 0, 0};
+  int n = 0;
+  if (b < N) {
+    const float2 p = X[b];
+    n = bead_tiles(p.x, p.y, nx, ny, nx / TS, t);
+  }
+#pragma unroll
+  for (int s = 0; s < 4; ++s) {
+    const int slot = warp_claim(tile_ctr, t[s], s < n);
+    if (FILL && s < n) list[slot] = b;
+  }
+}
+
+// one block: tile_start = exclusive scan of tile_count (n_tiles + 1 entries); the cursor array
+// for the fill pass is initialised to tile_start; counts are zeroed for the next step.
+__global__ void __launch_bounds__(1024) k_tile_scan(int* __restrict__ tile_count, int n_tiles,
+                                                    int* __restrict__ tile_start, int* __restrict__ tile_cursor) {
+  __shared__ int sm[33];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  int carry = 0;
+  for (int base = 0; base < n_tiles; base += 1024) {
+    const int i = base + threadIdx.x;
+    const int v = (i < n_tiles) ? tile_count[i] : 0;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int u = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += u;
+    }
+    if (lane == 31) sm[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+      const int s = sm[lane];
+      int si = s;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int u = __shfl_up_sync(0xffffffffu, si, o);
+        if (lane >= o) si += u;
+      }
+      sm[lane] = si - s;
+      if (lane == 31) sm[32] = si;
+    }
+    __syncthreads();
+    if (i < n_tiles) {
+      const int ex = carry + sm[wid] + inc - v;
+      tile_start[i] = ex;
+      tile_cursor[i] = ex;
+      tile_count[i] = 0;
+    }
+    carry += sm[32];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) tile_start[n_tiles] = carry;
+}
+
+}  // namespace mc

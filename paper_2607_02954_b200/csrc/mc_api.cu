@@ -1,5 +1,5 @@
 // mc_api.cu -- host side of libmc.so: the C ABI of include/mc.h, workspace layout, and the
-// per-step launch sequence K0 -> K2a -> K3a -> K1 -> K2b -> K3b -> K4.
+// per-step launch sequence K0 -> K2a -> K3a -> K1 -> K2b -> K3b -> K4 (DESIGN.md "Kernels").
 // No CPU implementation of any step lives here: without a CUDA device every call fails.
 #include "../../include/mc.h"
 
@@ -8,14 +8,16 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <algorithm>
+#include <numeric>
 #include <vector>
 
-#include "k_bin.cuh"
 #include "k_blur.cuh"
 #include "k_filament.cuh"
 #include "k_g2p.cuh"
 #include "k_lbm.cuh"
 #include "k_p2g.cuh"
+#include "k_tile.cuh"
 
 namespace {
 
@@ -25,8 +27,8 @@ constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
-  size_t fA, fB, u, rho_b, A, G, cfield, csum, As, cell_count, cell_start, block_sums;
-  size_t X, P0, P1, F, sense, bead_cell, bead_rank, slot_bead, W, offsets, flags, sources;
+  size_t fA, fB, u, rho_b, A, G, cfield, csum, As, tile_count, tile_start, tile_cursor, tile_rho_max;
+  size_t X, PA, PB, PC, F, sense, list, src, bflags, scratch, flags, sources;
   size_t total;
 };
 
@@ -81,19 +83,21 @@ Layout make_layout(const mc_world_params* p, const Derived& d) {
   L.cfield = take(d.n_static * nc * f4);
   L.csum = take(d.n_static ? nc * f4 : 0);
   L.As = take(d.n_static ? 2 * nc * f4 : 0);
-  L.cell_count = take(nc * 4);
-  L.cell_start = take((nc + 4) * 4);
-  L.block_sums = take(((nc + mc::SCAN_CHUNK - 1) / mc::SCAN_CHUNK + 1) * 4);
+  const size_t nt = nc / (mc::TS * mc::TS);
+  L.tile_count = take(nt * 4);
+  L.tile_start = take((nt + 1) * 4);
+  L.tile_cursor = take(nt * 4);
+  L.tile_rho_max = take(nt * 4);
   L.X = take(N * 8);
-  L.P0 = take(N * 16);
-  L.P1 = take(N * 16);
+  L.PA = take(N * 16);
+  L.PB = take(N * 16);
+  L.PC = take(N * 16);
   L.F = take(N * 8);
   L.sense = take(N * 4);
-  L.bead_cell = take(N * 4);
-  L.bead_rank = take(N * 4);
-  L.slot_bead = take(N * 4);
-  L.W = take(N * 8 * f4);
-  L.offsets = take((N / 3 + 2) * 4);
+  L.list = take(N * 4 * 4);   // a bead is listed in at most 4 tiles
+  L.src = take(N * 4);        // internal bead -> caller's bead
+  L.bflags = take(N);         // first/last flags (load-time scratch; PC.w carries them)
+  L.scratch = take((N / 3 + 2) * 8);  // load-time: chain offsets and sort keys
   L.flags = take(64 * 4);
   L.sources = take(d.n_src_floats * f4);
   L.total = off;
@@ -114,6 +118,8 @@ struct mc_world {
   int cur = 0;  // which of fA/fB holds the current post-collision populations
   int n_fil = 0;
   int N = 0;
+  int stride = 60;   // K1 window advance: 64 when all chains share a length dividing 64
+  int n_windows = 0;
   float rho0 = 1, omega_p = 1, omega_m = 1, kappa = 0;
   float coef[4] = {0, 0, 0, 0};  // lattice coupling with the sign of the force
   mc::BlurTaps taps[4];
@@ -173,44 +179,34 @@ void launch_blur(mc_world* w, int k, bool first, float* field_out) {
 
 int enqueue_step(mc_world* w) {
   const int N = w->N, nx = w->nx, ny = w->ny;
-  const int nc = (int)w->nc;
   cudaStream_t st = w->stream;
   float2* X = w->ptr<float2>(w->L.X);
   float2* F = w->ptr<float2>(w->L.F);
-  int* cell_count = w->ptr<int>(w->L.cell_count);
-  int* cell_start = w->ptr<int>(w->L.cell_start);
-  int* block_sums = w->ptr<int>(w->L.block_sums);
-  int* bead_cell = w->ptr<int>(w->L.bead_cell);
-  int* bead_rank = w->ptr<int>(w->L.bead_rank);
-  int* slot_bead = w->ptr<int>(w->L.slot_bead);
-  float* W = w->ptr<float>(w->L.W);
-  const size_t plane = (size_t)(w->p.max_beads > 0 ? w->p.max_beads : 1);
+  int* tile_count = w->ptr<int>(w->L.tile_count);
+  int* tile_start = w->ptr<int>(w->L.tile_start);
+  int* tile_cursor = w->ptr<int>(w->L.tile_cursor);
+  float* tile_rho_max = w->ptr<float>(w->L.tile_rho_max);
+  int* list = w->ptr<int>(w->L.list);
   float* rho_b = w->ptr<float>(w->L.rho_b);
   float* G0 = w->ptr<float>(w->L.G);
   float* G1 = G0 + w->nc;
   int* flag = w->ptr<int>(w->L.flags);
+  const int n_tiles = (nx / mc::TS) * (ny / mc::TS);
   const int bt = 256;
   const int bgrid = (N + bt - 1) / bt;
   const bool beads = N > 0;
 
   prof_mark(w, 0);
   if (beads) {
-    // K0: canonical cell binning
-    cudaMemsetAsync(cell_count, 0, (size_t)nc * 4, st);
-    mc::k_bin_count<<<bgrid, bt, 0, st>>>(X, N, nx, ny, cell_count, bead_cell, bead_rank);
-    const int nb = (nc + mc::SCAN_CHUNK - 1) / mc::SCAN_CHUNK;
-    mc::k_scan_block_sums<<<nb, mc::SCAN_THREADS, 0, st>>>(cell_count, nc, block_sums);
-    mc::k_scan_top<<<1, mc::SCAN_THREADS, 0, st>>>(block_sums, nb);
-    mc::k_scan_apply<<<nb, mc::SCAN_THREADS, 0, st>>>(cell_count, nc, block_sums, cell_start, N);
-    mc::k_bin_scatter<<<bgrid, bt, 0, st>>>(N, bead_cell, bead_rank, cell_start, slot_bead);
-    mc::k_bin_sort_cells<<<(nc + bt - 1) / bt, bt, 0, st>>>(nc, cell_start, slot_bead);
-    mc::k_bin_pack<<<bgrid, bt, 0, st>>>(N, slot_bead, X, W, plane);
-    w->launches += 8;
+    // K0: tile binning (count, scan, fill)
+    mc::k_tile_bin<false><<<bgrid, bt, 0, st>>>(X, N, nx, ny, tile_count, nullptr);
+    mc::k_tile_scan<<<1, 1024, 0, st>>>(tile_count, n_tiles, tile_start, tile_cursor);
+    mc::k_tile_bin<true><<<bgrid, bt, 0, st>>>(X, N, nx, ny, tile_cursor, list);
+    w->launches += 3;
     prof_mark(w, 1);
     // K2a: S2 deposit
     if (w->d.n_density) {
-      mc::k_p2g_gather<false><<<dim3(nx / 32, ny / 8), 256, 0, st>>>(nx, ny, cell_start, W, plane, slot_bead,
-                                                                      nullptr, rho_b, nullptr);
+      mc::k_deposit_tile<<<n_tiles, 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max);
       w->launches++;
       prof_mark(w, 2);
       // K3a: S3 filter + gradient -> force-gradient planes A
@@ -225,28 +221,27 @@ int enqueue_step(mc_world* w) {
     prof_mark(w, 3);
     // K1: S0 + S1 + S4
     mc::FilamentArgs fa;
-    fa.offsets = w->ptr<int>(w->L.offsets);
-    fa.n_fil = w->n_fil;
     fa.X = X;
-    fa.P0 = w->ptr<float4>(w->L.P0);
-    fa.P1 = w->ptr<float4>(w->L.P1);
+    fa.PA = w->ptr<float4>(w->L.PA);
+    fa.PB = w->ptr<float4>(w->L.PB);
+    fa.PC = w->ptr<float4>(w->L.PC);
     fa.F = F;
     fa.sense = w->ptr<float>(w->L.sense);
     fa.A0 = w->d.n_density ? w->ptr<float>(w->L.A) : (w->d.n_static ? w->ptr<float>(w->L.As) : nullptr);
     fa.A1 = fa.A0 ? fa.A0 + w->nc : nullptr;
     fa.csum = w->d.n_static ? w->ptr<float>(w->L.csum) : nullptr;
+    fa.N = N;
     fa.nx = nx;
     fa.ny = ny;
+    fa.stride = w->stride;
+    fa.n_windows = w->n_windows;
     fa.kappa = w->kappa;
-    fa.t = (double)w->step * (double)w->p.dt;
-    const int warps_per_block = 8;
-    int fgrid = (w->n_fil + warps_per_block - 1) / warps_per_block;
-    if (fgrid > 148 * 64) fgrid = 148 * 64;
-    mc::k_filament_force<<<fgrid, warps_per_block * 32, 0, st>>>(fa);
+    fa.n_step = (double)w->step;
+    mc::k_filament_force<<<(w->n_windows + 7) / 8, 256, 0, st>>>(fa);
     prof_mark(w, 4);
     // K2b: S5 spread
-    mc::k_p2g_gather<true><<<dim3(nx / 32, ny / 8), 256, 0, st>>>(nx, ny, cell_start, W, plane, slot_bead, F,
-                                                                   G0, G1);
+    mc::k_spread_tile<<<n_tiles, 256, 0, st>>>(nx, ny, tile_start, list, X, F,
+                                               w->d.n_density ? tile_rho_max : nullptr, G0, G1);
     w->launches += 2;
   } else {
     for (int b = 1; b <= 4; ++b) prof_mark(w, b);
@@ -433,30 +428,73 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
                 !act_period))
     return fail(w, MC_EINVAL, "null array");
   cudaStream_t st = w->stream;
-  int* flag = w->ptr<int>(w->L.flags) + 1;
-  cudaMemsetAsync(flag, 0, 4, st);
-  cudaMemcpyAsync(w->ptr<int>(w->L.offsets), offsets, (size_t)(n_fil + 1) * 4, cudaMemcpyHostToDevice, st);
-  if (N > 0) {
-    mc::k_pack_params<<<(int)((N + 255) / 256), 256, 0, st>>>((int)N, xy, L_rest, theta_rest, k_bend, k_shear,
-                                                              k_stretch, act_amp, act_phase, act_period,
-                                                              w->ptr<float2>(w->L.X), w->ptr<float4>(w->L.P0),
-                                                              w->ptr<float4>(w->L.P1), flag);
-    w->launches++;
-    cudaMemsetAsync(w->ptr<float>(w->L.F), 0, (size_t)N * 8, st);
-    cudaMemsetAsync(w->ptr<float>(w->L.sense), 0, (size_t)N * 4, st);
-  }
-  int h = 0;
-  cudaMemcpyAsync(&h, flag, 4, cudaMemcpyDeviceToHost, st);
+  w->N = 0;
+  w->n_fil = 0;
+  w->n_windows = 0;
+  if (N == 0) return MC_OK;
+  // 1. spatial sort of the CHAINS (not of the beads): chains whose first bead falls in the same
+  //    64x64 block of nodes become neighbours in memory, so the per-bead grid gathers of K1/K4
+  //    and the per-tile bead gathers of K2 hit L2 instead of re-fetching sectors from HBM.
+  //    The internal order is a mechanism only: every output is returned in the caller's order.
+  int* d_off = w->ptr<int>(w->L.scratch);
+  int* d_keys = d_off + (n_fil + 1);
+  std::vector<int> keys(n_fil);
+  cudaMemcpyAsync(d_off, offsets, (size_t)(n_fil + 1) * 4, cudaMemcpyHostToDevice, st);
+  mc::k_chain_keys<<<(n_fil + 255) / 256, 256, 0, st>>>(n_fil, d_off, xy, w->nx, w->ny, 64, d_keys);
+  w->launches++;
+  cudaMemcpyAsync(keys.data(), d_keys, (size_t)n_fil * 4, cudaMemcpyDeviceToHost, st);
   cudaError_t e = cudaStreamSynchronize(st);
   if (e == cudaSuccess) e = cudaGetLastError();
   if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_load_filaments: ") + cudaGetErrorString(e));
-  if (h) {
-    w->N = 0;
-    w->n_fil = 0;
-    return fail(w, MC_EINVAL, (h & 1) ? "stiffness outside [0,1]" : "period <= 0");
+  std::vector<int> order(n_fil);
+  std::iota(order.begin(), order.end(), 0);
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return keys[a] < keys[b]; });
+  std::vector<int> src((size_t)N);
+  std::vector<unsigned char> bflags((size_t)N, 0);
+  bool uniform = true;
+  const int m0 = offsets[1] - offsets[0];
+  size_t pos = 0;
+  for (int c = 0; c < n_fil; ++c) {
+    const int f = order[c];
+    const int b0 = offsets[f], m = offsets[f + 1] - b0;
+    uniform = uniform && (m == m0);
+    for (int i = 0; i < m; ++i) src[pos + i] = b0 + i;
+    bflags[pos] |= mc::BEAD_FIRST;
+    bflags[pos + m - 1] |= mc::BEAD_LAST;
+    pos += m;
   }
+  int* bad = w->ptr<int>(w->L.flags) + 1;
+  cudaMemsetAsync(bad, 0, 4, st);
+  cudaMemcpyAsync(w->ptr<int>(w->L.src), src.data(), (size_t)N * 4, cudaMemcpyHostToDevice, st);
+  cudaMemcpyAsync(w->ptr<unsigned char>(w->L.bflags), bflags.data(), (size_t)N, cudaMemcpyHostToDevice, st);
+  // 2. gather + pack the per-bead parameters in the internal order, validate
+  mc::PackArgs pa;
+  pa.N = (int)N;
+  pa.src = w->ptr<int>(w->L.src);
+  pa.flags = w->ptr<unsigned char>(w->L.bflags);
+  pa.xy = xy; pa.L_rest = L_rest; pa.theta_rest = theta_rest; pa.k_bend = k_bend; pa.k_shear = k_shear;
+  pa.k_stretch = k_stretch; pa.act_amp = act_amp; pa.act_phase = act_phase; pa.act_period = act_period;
+  pa.X = w->ptr<float2>(w->L.X);
+  pa.PA = w->ptr<float4>(w->L.PA);
+  pa.PB = w->ptr<float4>(w->L.PB);
+  pa.PC = w->ptr<float4>(w->L.PC);
+  pa.dt = (double)w->p.dt;
+  pa.bad = bad;
+  mc::k_pack_params<<<(int)((N + 255) / 256), 256, 0, st>>>(pa);
+  w->launches++;
+  cudaMemsetAsync(w->ptr<float>(w->L.F), 0, (size_t)N * 8, st);
+  cudaMemsetAsync(w->ptr<float>(w->L.sense), 0, (size_t)N * 4, st);
+  int h = 0;
+  cudaMemcpyAsync(&h, bad, 4, cudaMemcpyDeviceToHost, st);
+  e = cudaStreamSynchronize(st);  // src/bflags are host vectors of this call
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_load_filaments: ") + cudaGetErrorString(e));
+  if (h) return fail(w, MC_EINVAL, (h & 1) ? "stiffness outside [0,1]" : "period <= 0");
   w->N = (int)N;
   w->n_fil = n_fil;
+  const bool aligned = uniform && (64 % m0 == 0);
+  w->stride = aligned ? 64 : 60;
+  w->n_windows = aligned ? (int)((N + 63) / 64) : (int)((N + 59) / 60);
   return MC_OK;
 }
 
@@ -478,7 +516,12 @@ int mc_read_state(mc_world* w, int64_t* step_out, float* xy, float* u, float* rh
   const size_t nc = w->nc, N = (size_t)w->N;
   if (step_out) *step_out = w->step;
   const cudaMemcpyKind d2d = cudaMemcpyDeviceToDevice;
-  if (xy && N) cudaMemcpyAsync(xy, w->ptr<float>(w->L.X), N * 8, d2d, st);
+  const int* src = w->ptr<int>(w->L.src);
+  const int pg = (int)((N + 255) / 256);
+  if (xy && N) {
+    mc::k_unpermute2<<<pg, 256, 0, st>>>((int)N, src, w->ptr<float2>(w->L.X), reinterpret_cast<float2*>(xy));
+    w->launches++;
+  }
   if (u) cudaMemcpyAsync(u, w->ptr<float>(w->L.u), 2 * nc * 4, d2d, st);
   if (rho || fdev) {
     const int bx = pick_bx(w->nx);
@@ -498,8 +541,14 @@ int mc_read_state(mc_world* w, int64_t* step_out, float* xy, float* u, float* rh
       }
     }
   }
-  if (force && N) cudaMemcpyAsync(force, w->ptr<float>(w->L.F), N * 8, d2d, st);
-  if (sense && N) cudaMemcpyAsync(sense, w->ptr<float>(w->L.sense), N * 4, d2d, st);
+  if (force && N) {
+    mc::k_unpermute2<<<pg, 256, 0, st>>>((int)N, src, w->ptr<float2>(w->L.F), reinterpret_cast<float2*>(force));
+    w->launches++;
+  }
+  if (sense && N) {
+    mc::k_unpermute1<<<pg, 256, 0, st>>>((int)N, src, w->ptr<float>(w->L.sense), sense);
+    w->launches++;
+  }
   int h = 0;
   cudaMemcpyAsync(&h, w->ptr<int>(w->L.flags), 4, cudaMemcpyDeviceToHost, st);
   cudaError_t e = cudaStreamSynchronize(st);

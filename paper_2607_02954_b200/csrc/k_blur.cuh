@@ -22,58 +22,95 @@ struct BlurTaps {
   float g[2 * BLUR_MAX_R + 1];
 };
 
-__host__ __device__ inline size_t blur_smem_bytes(int R) {
-  const int H = BLUR_T + 2 * R + 2;
-  return sizeof(float) * ((size_t)H * H + (size_t)H * (BLUR_T + 2));
+// shared-memory geometry for radius R (all pitches multiples of 4 floats => 16-byte rows)
+__host__ __device__ constexpr int blur_H(int R) { return BLUR_T + 2 * R + 2; }                  // input tile side
+__host__ __device__ constexpr int blur_HP(int R) { return BLUR_T + 4 * ((4 + 2 * R + 3) / 4); } // input row pitch
+constexpr int BLUR_TW = BLUR_T + 2;   // filtered tile side (one-node halo for the gradient)
+constexpr int BLUR_TWP = 36;          // its row pitch
+__host__ __device__ constexpr size_t blur_smem_bytes(int R) {
+  return sizeof(float) * ((size_t)(blur_H(R) + 1) * blur_HP(R) + (size_t)(blur_H(R) + 4) * BLUR_TWP);
 }
 
-// coef: lattice coupling with sign.  base0/base1: planes added to the result (static part or the
-// running sum over earlier bead-density fields), may be NULL.  field_out may be NULL.
-__global__ void __launch_bounds__(256) k_blur_grad(int nx, int ny, int R, BlurTaps taps,
+// One CTA filters one 32x32 tile.  Stages (all in shared memory, one read of rho_b per node plus
+// the halo, one write of the two gradient planes):
+//   load  (32+2R+2)^2 nodes of rho_b, periodic indices
+//   x pass: each thread produces 4 consecutive outputs of one row from a register window
+//           (4+2R inputs fetched with 16-byte LDS)                       -> tmp[H][34]
+//   y pass: each thread produces 4 consecutive outputs of one column    -> bl[34][34]
+//   central difference, scale by the signed coupling, add the base planes, store float2.
+// coef: lattice coupling with the sign of the force.  base: interleaved planes added to the
+// result (static part, or the running sum over earlier bead-density fields), may be NULL.
+// A: interleaved (x,y) force-gradient planes.  field_out (filtered density) may be NULL.
+template <int R>
+__global__ void __launch_bounds__(256) k_blur_grad(int nx, int ny, BlurTaps taps,
                                                    const float* __restrict__ rho_b, float coef,
-                                                   const float* base0, const float* base1,
-                                                   float* A0, float* A1, float* __restrict__ field_out) {
-  extern __shared__ float sm[];
-  const int H = BLUR_T + 2 * R + 2;   // input tile side
-  const int TW = BLUR_T + 2;          // blurred tile side (one-cell halo for the gradient)
-  float* in = sm;                     // [H][H]
-  float* tmp = sm + (size_t)H * H;    // [H][TW]
+                                                   const float2* base, float2* A,
+                                                   float* __restrict__ field_out) {
+  extern __shared__ __align__(16) float sm[];
+  constexpr int H = blur_H(R), HP = blur_HP(R), TW = BLUR_TW, TWP = BLUR_TWP;
+  constexpr int NV = 4 + 2 * R, NV4 = (NV + 3) / 4;
+  float* in = sm;                          // [H+1][HP]
+  float* tmp = sm + (size_t)(H + 1) * HP;  // [H+4][TWP]
   const int i0 = blockIdx.x * BLUR_T, j0 = blockIdx.y * BLUR_T;
-  for (int t = threadIdx.x; t < H * H; t += blockDim.x) {
-    const int y = t / H, x = t - y * H;
-    const int gi = wrapi(i0 - R - 1 + x, nx), gj = wrapi(j0 - R - 1 + y, ny);
-    in[t] = __ldg(rho_b + (size_t)gj * nx + gi);
+  float g[2 * R + 1];
+#pragma unroll
+  for (int k = 0; k <= 2 * R; ++k) g[k] = taps.g[k];
+  // load: a warp reads one row (H <= 64 => two coalesced requests)
+  for (int y = threadIdx.x >> 5; y < H; y += 8) {
+    const int gj = wrap1(j0 - R - 1 + y, ny);  // |halo| <= R+1 < ny
+    const float* row = rho_b + (size_t)gj * nx;
+    for (int x = threadIdx.x & 31; x < HP; x += 32)
+      in[y * HP + x] = (x < H) ? __ldg(row + wrap1(i0 - R - 1 + x, nx)) : 0.0f;
   }
+  for (int x = threadIdx.x; x < HP; x += 256) in[H * HP + x] = 0.0f;  // pad row (16-byte over-read)
   __syncthreads();
-  // along x
-  for (int t = threadIdx.x; t < H * TW; t += blockDim.x) {
-    const int y = t / TW, x = t - y * TW;
-    const float* r = in + y * H + x;
-    float s = 0.0f;
-    for (int k = 0; k <= 2 * R; ++k) s = fmaf(taps.g[k], r[k], s);
-    tmp[t] = s;
+  // x pass: items (row y, chunk c of 4 outputs), 9 chunks cover 34(+2) outputs
+  for (int it = threadIdx.x; it < H * 9; it += 256) {
+    const int y = it / 9, c = it - y * 9;
+    float v[4 * NV4];
+    const float4* p = reinterpret_cast<const float4*>(in + y * HP + 4 * c);
+#pragma unroll
+    for (int q = 0; q < NV4; ++q) {
+      const float4 t = p[q];
+      v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+    }
+    float o[4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+      float s = 0.0f;
+#pragma unroll
+      for (int k = 0; k <= 2 * R; ++k) s = fmaf(g[k], v[a + k], s);
+      o[a] = s;
+    }
+    *reinterpret_cast<float4*>(tmp + y * TWP + 4 * c) = make_float4(o[0], o[1], o[2], o[3]);
   }
+  for (int x = threadIdx.x; x < 4 * TWP; x += 256) tmp[H * TWP + x] = 0.0f;  // pad rows
   __syncthreads();
-  // along y; result bl[TW][TW] overwrites the front of `in`
+  // y pass: items (chunk c of 4 output rows, column x); result bl[36][TWP] overwrites `in`
   float* bl = in;
-  for (int t = threadIdx.x; t < TW * TW; t += blockDim.x) {
-    const int y = t / TW, x = t - y * TW;
-    const float* c = tmp + y * TW + x;
-    float s = 0.0f;
-    for (int k = 0; k <= 2 * R; ++k) s = fmaf(taps.g[k], c[k * TW], s);
-    bl[t] = s;
+  for (int it = threadIdx.x; it < 9 * TWP; it += 256) {
+    const int c = it / TWP, x = it - c * TWP;
+    float v[NV];
+#pragma unroll
+    for (int k = 0; k < NV; ++k) v[k] = tmp[(4 * c + k) * TWP + x];
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+      float s = 0.0f;
+#pragma unroll
+      for (int k = 0; k <= 2 * R; ++k) s = fmaf(g[k], v[a + k], s);
+      bl[(4 * c + a) * TWP + x] = s;
+    }
   }
   __syncthreads();
-  for (int t = threadIdx.x; t < BLUR_T * BLUR_T; t += blockDim.x) {
+  for (int t = threadIdx.x; t < BLUR_T * BLUR_T; t += 256) {
     const int y = t >> 5, x = t & 31;
-    const float gx = 0.5f * (bl[(y + 1) * TW + x + 2] - bl[(y + 1) * TW + x]);
-    const float gy = 0.5f * (bl[(y + 2) * TW + x + 1] - bl[y * TW + x + 1]);
-    const size_t g = (size_t)(j0 + y) * nx + (i0 + x);
-    float a0 = coef * gx, a1 = coef * gy;
-    if (base0) { a0 += base0[g]; a1 += base1[g]; }
-    A0[g] = a0;
-    A1[g] = a1;
-    if (field_out) field_out[g] = bl[(y + 1) * TW + x + 1];
+    const float gx = 0.5f * (bl[(y + 1) * TWP + x + 2] - bl[(y + 1) * TWP + x]);
+    const float gy = 0.5f * (bl[(y + 2) * TWP + x + 1] - bl[y * TWP + x + 1]);
+    const size_t gidx = (size_t)(j0 + y) * nx + (i0 + x);
+    float2 a = make_float2(coef * gx, coef * gy);
+    if (base) { const float2 b = base[gidx]; a.x += b.x; a.y += b.y; }
+    A[gidx] = a;
+    if (field_out) field_out[gidx] = bl[(y + 1) * TWP + x + 1];
   }
 }
 
@@ -97,7 +134,7 @@ __device__ inline double static_c(int nx, int ny, int n_src, const float* __rest
 // cost two digits of the force.
 __global__ void k_static_init(int nx, int ny, int n_src, const float* __restrict__ src, float coef,
                               float* __restrict__ c_out, float* __restrict__ csum,
-                              float* __restrict__ As0, float* __restrict__ As1) {
+                              float2* __restrict__ As) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
   if (i >= nx) return;
   const size_t g = (size_t)j * nx + i;
@@ -108,8 +145,10 @@ __global__ void k_static_init(int nx, int ny, int n_src, const float* __restrict
                            static_c(nx, ny, n_src, src, i, wrap1(j - 1, ny)));
   c_out[g] = (float)c;
   csum[g] += (float)c;
-  As0[g] += (float)((double)coef * gx);
-  As1[g] += (float)((double)coef * gy);
+  float2 a = As[g];
+  a.x += (float)((double)coef * gx);
+  a.y += (float)((double)coef * gy);
+  As[g] = a;
 }
 
 }  // namespace mc

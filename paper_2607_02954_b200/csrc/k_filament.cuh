@@ -37,8 +37,7 @@ struct FilamentArgs {
   const float4* PC;  // {cos theta0, sin theta0, eps, flags}   eps = theta0 - atan2(sin, cos)
   float2* F;         // [N] out: total bead force
   float* sense;      // [N] out (only written when csum != NULL)
-  const float* A0;   // force-gradient planes (may be NULL: no field forces)
-  const float* A1;
+  const float2* A;   // interleaved force-gradient field (may be NULL: no field forces)
   const float* csum;  // sum of static fields (may be NULL)
   int N;
   int nx, ny;
@@ -154,9 +153,9 @@ __global__ void __launch_bounds__(256) k_filament_force(FilamentArgs a) {
   const bool out = aligned || (lane >= 1 && lane <= 30);
   if (!out) return;
   float2 FA = make_float2(a.kappa * DAx, a.kappa * DAy), FB = make_float2(a.kappa * DBx, a.kappa * DBy);
-  if (a.A0) {
-    if (vA) { const float2 g = interp2(a.A0, a.A1, a.nx, a.ny, xa.x, xa.y); FA.x += g.x; FA.y += g.y; }
-    if (vB) { const float2 g = interp2(a.A0, a.A1, a.nx, a.ny, xb.x, xb.y); FB.x += g.x; FB.y += g.y; }
+  if (a.A) {
+    if (vA) { const float2 g = interp2(a.A, a.nx, a.ny, xa.x, xa.y); FA.x += g.x; FA.y += g.y; }
+    if (vB) { const float2 g = interp2(a.A, a.nx, a.ny, xb.x, xb.y); FB.x += g.x; FB.y += g.y; }
   }
   if (vA && vB) {
     *reinterpret_cast<float4*>(a.F + bA) = make_float4(FA.x, FA.y, FB.x, FB.y);

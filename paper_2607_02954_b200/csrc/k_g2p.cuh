@@ -8,13 +8,12 @@
 namespace mc {
 
 __global__ void __launch_bounds__(256) k_interp_integrate(int N, float2* __restrict__ X,
-                                                          const float* __restrict__ u0,
-                                                          const float* __restrict__ u1, int nx, int ny,
+                                                          const float2* __restrict__ u, int nx, int ny,
                                                           int* __restrict__ flag) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b >= N) return;
   float2 p = X[b];
-  const float2 U = interp2(u0, u1, nx, ny, p.x, p.y);
+  const float2 U = interp2(u, nx, ny, p.x, p.y);
   p.x += U.x;
   p.y += U.y;
   X[b] = p;

@@ -25,8 +25,7 @@ struct LbmArgs {
   float* dst;         // [9][ny][nx]
   const float* G0;    // spread force planes (may be NULL: zero force)
   const float* G1;
-  float* u0;          // out: collision-time velocity
-  float* u1;
+  float2* u;          // out: collision-time velocity, interleaved (ux, uy)
   int nx, ny;
   float rho0, omega_p, omega_m;
   int* flag;          // sticky divergence flag (bit 2: |u| > 0.3 or non-finite)
@@ -92,8 +91,7 @@ __global__ void __launch_bounds__(256) k_lbm_step(LbmArgs a) {
   if (a.G0) { Gx = __ldg(a.G0 + c); Gy = __ldg(a.G1 + c); }
   float ux, uy;
   trt_collide(g, Gx, Gy, a.rho0, a.omega_p, a.omega_m, ux, uy);
-  a.u0[c] = ux;
-  a.u1[c] = uy;
+  a.u[c] = make_float2(ux, uy);
 #pragma unroll
   for (int q = 0; q < 9; ++q) a.dst[q * nc + c] = g[q];
   if (!(fabsf(ux) <= 0.3f && fabsf(uy) <= 0.3f)) atomicOr(a.flag, 4);
@@ -125,6 +123,12 @@ __global__ void k_lbm_export(const float* __restrict__ src, int nx, int ny, floa
     for (int q = 0; q < 9; ++q) fdev[q * nc + c] = g[q];
   }
   if (rho) rho[c] = rho0 + (g[0] + ((g[1] + g[3]) + (g[2] + g[4])) + ((g[5] + g[7]) + (g[6] + g[8])));
+}
+
+// mc_read_state: interleaved (x,y) field -> two planes
+__global__ void k_split2(size_t n, const float2* __restrict__ in, float* __restrict__ out0, float* __restrict__ out1) {
+  const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c < n) { const float2 v = in[c]; out0[c] = v.x; out1[c] = v.y; }
 }
 
 }  // namespace mc

@@ -159,21 +159,25 @@ inline void prof_mark(mc_world* w, int boundary) {
 
 int pick_bx(int nx) { return nx % 256 == 0 ? 256 : (nx % 128 == 0 ? 128 : (nx % 64 == 0 ? 64 : 32)); }
 
-// K3a for bead-density field k; accumulate: add to the planes already in A
-void launch_blur(mc_world* w, int k, bool first, float* field_out) {
-  const float* base0 = nullptr;
-  const float* base1 = nullptr;
-  float* A0 = w->ptr<float>(w->L.A);
-  float* A1 = A0 + w->nc;
-  if (first) {
-    if (w->d.n_static) { base0 = w->ptr<float>(w->L.As); base1 = base0 + w->nc; }
-  } else {
-    base0 = A0; base1 = A1;
-  }
+template <int R>
+void launch_blur_R(mc_world* w, int k, const float2* base, float2* A, float* field_out) {
   dim3 grid(w->nx / mc::BLUR_T, w->ny / mc::BLUR_T);
-  mc::k_blur_grad<<<grid, 256, mc::blur_smem_bytes(w->d.R[k]), w->stream>>>(
-      w->nx, w->ny, w->d.R[k], w->taps[k], w->ptr<float>(w->L.rho_b), w->coef[k], base0, base1, A0, A1,
-      field_out);
+  mc::k_blur_grad<R><<<grid, 256, mc::blur_smem_bytes(R), w->stream>>>(
+      w->nx, w->ny, w->taps[k], w->ptr<float>(w->L.rho_b), w->coef[k], base, A, field_out);
+}
+
+// K3a for bead-density field k; first: start from the static part, else add to the planes in A
+void launch_blur(mc_world* w, int k, bool first, float* field_out) {
+  float2* A = w->ptr<float2>(w->L.A);
+  const float2* base = first ? (w->d.n_static ? w->ptr<float2>(w->L.As) : nullptr) : A;
+  switch (w->d.R[k]) {
+#define MC_BLUR_CASE(R) case R: launch_blur_R<R>(w, k, base, A, field_out); break;
+    MC_BLUR_CASE(1) MC_BLUR_CASE(2) MC_BLUR_CASE(3) MC_BLUR_CASE(4) MC_BLUR_CASE(5) MC_BLUR_CASE(6)
+    MC_BLUR_CASE(7) MC_BLUR_CASE(8) MC_BLUR_CASE(9) MC_BLUR_CASE(10) MC_BLUR_CASE(11) MC_BLUR_CASE(12)
+    MC_BLUR_CASE(13) MC_BLUR_CASE(14) MC_BLUR_CASE(15) MC_BLUR_CASE(16)
+#undef MC_BLUR_CASE
+    default: break;
+  }
   w->launches++;
 }
 
@@ -227,8 +231,7 @@ int enqueue_step(mc_world* w) {
     fa.PC = w->ptr<float4>(w->L.PC);
     fa.F = F;
     fa.sense = w->ptr<float>(w->L.sense);
-    fa.A0 = w->d.n_density ? w->ptr<float>(w->L.A) : (w->d.n_static ? w->ptr<float>(w->L.As) : nullptr);
-    fa.A1 = fa.A0 ? fa.A0 + w->nc : nullptr;
+    fa.A = w->d.n_density ? w->ptr<float2>(w->L.A) : (w->d.n_static ? w->ptr<float2>(w->L.As) : nullptr);
     fa.csum = w->d.n_static ? w->ptr<float>(w->L.csum) : nullptr;
     fa.N = N;
     fa.nx = nx;
@@ -253,8 +256,7 @@ int enqueue_step(mc_world* w) {
   la.dst = w->fbuf(w->cur ^ 1);
   la.G0 = beads ? G0 : nullptr;
   la.G1 = beads ? G1 : nullptr;
-  la.u0 = w->ptr<float>(w->L.u);
-  la.u1 = la.u0 + w->nc;
+  la.u = w->ptr<float2>(w->L.u);
   la.nx = nx;
   la.ny = ny;
   la.rho0 = w->rho0;
@@ -268,7 +270,7 @@ int enqueue_step(mc_world* w) {
   prof_mark(w, 6);
   // K4: S7
   if (beads) {
-    mc::k_interp_integrate<<<bgrid, bt, 0, st>>>(N, X, la.u0, la.u1, nx, ny, flag);
+    mc::k_interp_integrate<<<bgrid, bt, 0, st>>>(N, X, la.u, nx, ny, flag);
     w->launches++;
   }
   prof_mark(w, 7);
@@ -394,10 +396,9 @@ int mc_create(const mc_world_params* p, void* workspace, size_t workspace_bytes,
         }
         cudaStreamSynchronize(st);  // the host array belongs to the caller
       }
-      float* As0 = w->ptr<float>(L.As);
       mc::k_static_init<<<dim3((w->nx + 127) / 128, w->ny), 128, 0, st>>>(
           w->nx, w->ny, f.n_sources, dsrc, w->coef[k], w->ptr<float>(L.cfield) + (size_t)n_static_seen * w->nc,
-          w->ptr<float>(L.csum), As0, As0 + w->nc);
+          w->ptr<float>(L.csum), w->ptr<float2>(L.As));
       w->launches++;
       src_off += 4 * (size_t)f.n_sources;
       n_static_seen++;
@@ -522,7 +523,10 @@ int mc_read_state(mc_world* w, int64_t* step_out, float* xy, float* u, float* rh
     mc::k_unpermute2<<<pg, 256, 0, st>>>((int)N, src, w->ptr<float2>(w->L.X), reinterpret_cast<float2*>(xy));
     w->launches++;
   }
-  if (u) cudaMemcpyAsync(u, w->ptr<float>(w->L.u), 2 * nc * 4, d2d, st);
+  if (u) {
+    mc::k_split2<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(nc, w->ptr<float2>(w->L.u), u, u + nc);
+    w->launches++;
+  }
   if (rho || fdev) {
     const int bx = pick_bx(w->nx);
     mc::k_lbm_export<<<dim3(w->nx / bx, w->ny), bx, 0, st>>>(w->fbuf(w->cur), w->nx, w->ny, w->rho0, fdev, rho);

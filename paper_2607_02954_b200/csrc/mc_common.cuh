@@ -6,14 +6,16 @@
 
 namespace mc {
 
-// periodic wrap of a grid index (reading 9)
-__device__ __forceinline__ int wrapi(int i, int n) {
-  i %= n;
-  return i < 0 ? i + n : i;
-}
 // wrap when i is known to lie in [-n, 2n)
 __device__ __forceinline__ int wrap1(int i, int n) {
   return i < 0 ? i + n : (i >= n ? i - n : i);
+}
+// periodic wrap of a grid index (reading 9).  Beads are almost always within one period of the
+// domain, so the integer division (~35 instructions) is kept off the common path.
+__device__ __forceinline__ int wrapi(int i, int n) {
+  if ((unsigned)(i + n) < (unsigned)(3 * n)) return wrap1(i, n);
+  i %= n;
+  return i < 0 ? i + n : i;
 }
 
 // Peskin's 4-point function (Peskin 2002, cited P:L125; reading 7) at the four nodes
@@ -37,10 +39,10 @@ __device__ __forceinline__ void support(float x, int& i0, float& fr) {
   i0 = (int)fl - 1;
 }
 
-// Interpolate two planes at (x,y): sum over the 4x4 support of plane(g) * delta_h(g - X)
-// ("nodes sample the local fluid velocity"; also S4's gradient sampling).
-__device__ __forceinline__ float2 interp2(const float* __restrict__ p0, const float* __restrict__ p1,
-                                          int nx, int ny, float x, float y) {
+// Interpolate an interleaved two-component field at (x,y): sum over the 4x4 support of
+// field(g) * delta_h(g - X)  ("nodes sample the local fluid velocity"; also S4's
+// gradient sampling).  One 8-byte load per support node.
+__device__ __forceinline__ float2 interp2(const float2* __restrict__ p, int nx, int ny, float x, float y) {
   int i0, j0;
   float fx, fy, wx[4], wy[4];
   support(x, i0, fx);
@@ -56,13 +58,13 @@ __device__ __forceinline__ float2 interp2(const float* __restrict__ p0, const fl
 #pragma unroll
   for (int l = 0; l < 4; ++l) {
     const int row = (j0 + l >= ny) ? j0 + l - ny : j0 + l;
-    const float* r0 = p0 + (size_t)row * nx;
-    const float* r1 = p1 + (size_t)row * nx;
+    const float2* r = p + (size_t)row * nx;
     float sx = 0.0f, sy = 0.0f;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-      sx = fmaf(__ldg(r0 + col[k]), wx[k], sx);
-      sy = fmaf(__ldg(r1 + col[k]), wx[k], sy);
+      const float2 v = __ldg(r + col[k]);
+      sx = fmaf(v.x, wx[k], sx);
+      sy = fmaf(v.y, wx[k], sy);
     }
     ax = fmaf(sx, wy[l], ax);
     ay = fmaf(sy, wy[l], ay);

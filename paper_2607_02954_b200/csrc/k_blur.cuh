@@ -22,51 +22,55 @@ struct BlurTaps {
   float g[2 * BLUR_MAX_R + 1];
 };
 
-// shared-memory geometry for radius R (all pitches multiples of 4 floats => 16-byte rows)
-__host__ __device__ constexpr int blur_H(int R) { return BLUR_T + 2 * R + 2; }                  // input tile side
-__host__ __device__ constexpr int blur_HP(int R) { return BLUR_T + 4 * ((4 + 2 * R + 3) / 4); } // input row pitch
-constexpr int BLUR_TW = BLUR_T + 2;   // filtered tile side (one-node halo for the gradient)
-constexpr int BLUR_TWP = 36;          // its row pitch
+// shared-memory geometry for radius R.  The input tile starts P nodes left of the output tile,
+// P the smallest multiple of 4 >= R+1, so that every global and shared access of the x pass is
+// a 16-byte one; the x pass then produces its outputs from column i0 - 1 - S on, S = P - 1 - R.
+__host__ __device__ constexpr int blur_P(int R) { return 4 * ((R + 1 + 3) / 4); }
+__host__ __device__ constexpr int blur_S(int R) { return blur_P(R) - 1 - R; }
+__host__ __device__ constexpr int blur_NC(int R) { return (BLUR_T + 2 + blur_S(R) + 3) / 4; }  // x chunks
+__host__ __device__ constexpr int blur_TWP(int R) { return 4 * blur_NC(R); }                    // filtered pitch
+__host__ __device__ constexpr int blur_HP(int R) { return 4 * ((blur_TWP(R) + 2 * R + 3) / 4); } // input pitch
+__host__ __device__ constexpr int blur_H(int R) { return BLUR_T + 2 * R + 2; }                  // input rows
 __host__ __device__ constexpr size_t blur_smem_bytes(int R) {
-  return sizeof(float) * ((size_t)(blur_H(R) + 1) * blur_HP(R) + (size_t)(blur_H(R) + 4) * BLUR_TWP);
+  return sizeof(float) * ((size_t)blur_H(R) * blur_HP(R) + (size_t)(blur_H(R) + 4) * blur_TWP(R));
 }
 
 // One CTA filters one 32x32 tile.  Stages (all in shared memory, one read of rho_b per node plus
-// the halo, one write of the two gradient planes):
-//   load  (32+2R+2)^2 nodes of rho_b, periodic indices
+// the halo, one write of the gradient):
+//   load  H x HP nodes of rho_b with 16-byte loads, periodic indices
 //   x pass: each thread produces 4 consecutive outputs of one row from a register window
-//           (4+2R inputs fetched with 16-byte LDS)                       -> tmp[H][34]
-//   y pass: each thread produces 4 consecutive outputs of one column    -> bl[34][34]
-//   central difference, scale by the signed coupling, add the base planes, store float2.
-// coef: lattice coupling with the sign of the force.  base: interleaved planes added to the
+//           (4+2R inputs fetched with 16-byte LDS)                       -> tmp[H][TWP]
+//   y pass: each thread produces 4 consecutive outputs of one column    -> bl[36][TWP]
+//   central difference, scale by the signed coupling, add the base field, store float2.
+// coef: lattice coupling with the sign of the force.  base: interleaved field added to the
 // result (static part, or the running sum over earlier bead-density fields), may be NULL.
-// A: interleaved (x,y) force-gradient planes.  field_out (filtered density) may be NULL.
+// A: interleaved (x,y) force-gradient field.  field_out (filtered density) may be NULL.
 template <int R>
 __global__ void __launch_bounds__(256) k_blur_grad(int nx, int ny, BlurTaps taps,
                                                    const float* __restrict__ rho_b, float coef,
                                                    const float2* base, float2* A,
                                                    float* __restrict__ field_out) {
   extern __shared__ __align__(16) float sm[];
-  constexpr int H = blur_H(R), HP = blur_HP(R), TW = BLUR_TW, TWP = BLUR_TWP;
-  constexpr int NV = 4 + 2 * R, NV4 = (NV + 3) / 4;
-  float* in = sm;                          // [H+1][HP]
-  float* tmp = sm + (size_t)(H + 1) * HP;  // [H+4][TWP]
+  constexpr int H = blur_H(R), HP = blur_HP(R), TWP = blur_TWP(R), NC = blur_NC(R);
+  constexpr int P = blur_P(R), S = blur_S(R);
+  constexpr int NV = 4 + 2 * R, NV4 = (NV + 3) / 4, HP4 = HP / 4;
+  float* in = sm;                    // [H][HP]    in[y][x]  <-> node (j0-R-1+y, i0-P+x)
+  float* tmp = sm + (size_t)H * HP;  // [H+4][TWP] tmp[y][t] <-> node (j0-R-1+y, i0-1-S+t)
   const int i0 = blockIdx.x * BLUR_T, j0 = blockIdx.y * BLUR_T;
   float g[2 * R + 1];
 #pragma unroll
   for (int k = 0; k <= 2 * R; ++k) g[k] = taps.g[k];
-  // load: a warp reads one row (H <= 64 => two coalesced requests)
-  for (int y = threadIdx.x >> 5; y < H; y += 8) {
-    const int gj = wrap1(j0 - R - 1 + y, ny);  // |halo| <= R+1 < ny
-    const float* row = rho_b + (size_t)gj * nx;
-    for (int x = threadIdx.x & 31; x < HP; x += 32)
-      in[y * HP + x] = (x < H) ? __ldg(row + wrap1(i0 - R - 1 + x, nx)) : 0.0f;
+  const int nx4 = nx >> 2, gc0 = (i0 - P) >> 2;  // arithmetic shift: i0 - P may be negative
+  for (int it = threadIdx.x; it < H * HP4; it += 256) {
+    const int y = it / HP4, v = it - y * HP4;
+    const int gj = wrap1(j0 - R - 1 + y, ny);  // halo <= R+1 < ny
+    const int gc = wrap1(gc0 + v, nx4);
+    reinterpret_cast<float4*>(in)[it] = __ldg(reinterpret_cast<const float4*>(rho_b + (size_t)gj * nx) + gc);
   }
-  for (int x = threadIdx.x; x < HP; x += 256) in[H * HP + x] = 0.0f;  // pad row (16-byte over-read)
   __syncthreads();
-  // x pass: items (row y, chunk c of 4 outputs), 9 chunks cover 34(+2) outputs
-  for (int it = threadIdx.x; it < H * 9; it += 256) {
-    const int y = it / 9, c = it - y * 9;
+  // x pass: items (row y, chunk c of 4 outputs)
+  for (int it = threadIdx.x; it < H * NC; it += 256) {
+    const int y = it / NC, c = it - y * NC;
     float v[4 * NV4];
     const float4* p = reinterpret_cast<const float4*>(in + y * HP + 4 * c);
 #pragma unroll
@@ -86,8 +90,8 @@ __global__ void __launch_bounds__(256) k_blur_grad(int nx, int ny, BlurTaps taps
   }
   for (int x = threadIdx.x; x < 4 * TWP; x += 256) tmp[H * TWP + x] = 0.0f;  // pad rows
   __syncthreads();
-  // y pass: items (chunk c of 4 output rows, column x); result bl[36][TWP] overwrites `in`
-  float* bl = in;
+  // y pass: items (chunk c of 4 output rows, column t); bl[36][TWP] overwrites `in`
+  float* bl = in;                    // bl[y][t] <-> node (j0-1+y, i0-1-S+t)
   for (int it = threadIdx.x; it < 9 * TWP; it += 256) {
     const int c = it / TWP, x = it - c * TWP;
     float v[NV];
@@ -103,10 +107,10 @@ __global__ void __launch_bounds__(256) k_blur_grad(int nx, int ny, BlurTaps taps
   }
   __syncthreads();
   for (int t = threadIdx.x; t < BLUR_T * BLUR_T; t += 256) {
-    const int y = t >> 5, x = t & 31;
+    const int y = t >> 5, x = (t & 31) + S;
     const float gx = 0.5f * (bl[(y + 1) * TWP + x + 2] - bl[(y + 1) * TWP + x]);
     const float gy = 0.5f * (bl[(y + 2) * TWP + x + 1] - bl[y * TWP + x + 1]);
-    const size_t gidx = (size_t)(j0 + y) * nx + (i0 + x);
+    const size_t gidx = (size_t)(j0 + y) * nx + (i0 + (t & 31));
     float2 a = make_float2(coef * gx, coef * gy);
     if (base) { const float2 b = base[gidx]; a.x += b.x; a.y += b.y; }
     A[gidx] = a;

@@ -22,9 +22,17 @@
 
 namespace mc {
 
+// A listed bead seen from one tile: node offsets clamped into the tile and weights MASKED to
+// zero outside it, so that the 16 accumulations below need no branch (a bead overlapping the
+// tile only partly adds exact zeros to a clamped address, which changes nothing).
+// Row pitch of the shared accumulator tiles.  Lanes of a warp hold consecutive beads of a chain,
+// i.e. nodes about one cell apart in an arbitrary direction; with pitch 32 a vertical chain would
+// put all 32 lanes on one bank.  37 = 5 (mod 32) has no bank collision for offsets |dr|,|dc| <= 2.
+constexpr int TSP = 37;
+
 struct TileBead {
-  int lx[4], ly[4];  // local node indices in the tile, or -1 when outside it
-  float wx[4], wy[4];
+  int col[4], row[4];    // col: local x (0..TS-1); row: local y * TSP
+  float wx[4], wy[4];    // 0 where the support node lies outside the tile
 };
 
 __device__ __forceinline__ void tile_bead(float2 p, int nx, int ny, int x0, int y0, TileBead& tb) {
@@ -40,8 +48,11 @@ __device__ __forceinline__ void tile_bead(float2 p, int nx, int ny, int x0, int 
   for (int k = 0; k < 4; ++k) {
     const int c = ((i0 + k >= nx) ? i0 + k - nx : i0 + k) - x0;
     const int r = ((j0 + k >= ny) ? j0 + k - ny : j0 + k) - y0;
-    tb.lx[k] = ((unsigned)c < (unsigned)TS) ? c : -1;
-    tb.ly[k] = ((unsigned)r < (unsigned)TS) ? r : -1;
+    const bool cin = (unsigned)c < (unsigned)TS, rin = (unsigned)r < (unsigned)TS;
+    tb.col[k] = cin ? c : 0;
+    tb.row[k] = rin ? r * TSP : 0;
+    tb.wx[k] = cin ? tb.wx[k] : 0.0f;
+    tb.wy[k] = rin ? tb.wy[k] : 0.0f;
   }
 }
 
@@ -75,12 +86,12 @@ __global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int*
                                                       const float2* __restrict__ X,
                                                       float* __restrict__ rho_b,
                                                       float* __restrict__ tile_rho_max) {
-  __shared__ int acc[TS * TS];
+  __shared__ int acc[TS * TSP];
   __shared__ float red[32];
   const int t = blockIdx.x, ntx = nx / TS;
   const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
   const int s = tile_start[t], e = tile_start[t + 1];
-  for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) acc[c] = 0;
+  for (int c = threadIdx.x; c < TS * TSP; c += blockDim.x) acc[c] = 0;
   const float scale = pow2_scale(fmaxf(0.25f * (float)(e - s), 1.0f));
   __syncthreads();
   for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
@@ -88,18 +99,17 @@ __global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int*
     tile_bead(__ldg(X + __ldg(list + k)), nx, ny, x0, y0, tb);
 #pragma unroll
     for (int l = 0; l < 4; ++l) {
-      if (tb.ly[l] < 0) continue;
       const float wys = tb.wy[l] * scale;
 #pragma unroll
       for (int kx = 0; kx < 4; ++kx)
-        if (tb.lx[kx] >= 0) atomicAdd(&acc[tb.ly[l] * TS + tb.lx[kx]], __float2int_rn(tb.wx[kx] * wys));
+        atomicAdd(&acc[tb.row[l] + tb.col[kx]], __float2int_rn(tb.wx[kx] * wys));
     }
   }
   __syncthreads();
   const float inv = 1.0f / scale;
   float mx = 0.0f;
   for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) {
-    const float v = (float)acc[c] * inv;
+    const float v = (float)acc[(c >> 5) * TSP + (c & 31)] * inv;
     rho_b[(size_t)(y0 + (c >> 5)) * nx + x0 + (c & 31)] = v;
     mx = fmaxf(mx, v);
   }
@@ -114,7 +124,7 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
                                                         const float2* __restrict__ X,
                                                         const float2* __restrict__ F, float rho_max,
                                                         int* acc0, int* acc1, float* red) {
-  for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) { acc0[c] = 0; acc1[c] = 0; }
+  for (int c = threadIdx.x; c < TS * TSP; c += blockDim.x) { acc0[c] = 0; acc1[c] = 0; }
   float fm = 0.0f;
   for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
     const float2 f = __ldg(F + __ldg(list + k));
@@ -131,15 +141,13 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
     const float fxs = f.x * scale, fys = f.y * scale;
 #pragma unroll
     for (int l = 0; l < 4; ++l) {
-      if (tb.ly[l] < 0) continue;
+      const float wyx = tb.wy[l] * fxs, wyy = tb.wy[l] * fys;
 #pragma unroll
-      for (int kx = 0; kx < 4; ++kx)
-        if (tb.lx[kx] >= 0) {
-          const float w = tb.wx[kx] * tb.wy[l];
-          const int a = tb.ly[l] * TS + tb.lx[kx];
-          atomicAdd(&acc0[a], __float2int_rn(w * fxs));
-          atomicAdd(&acc1[a], __float2int_rn(w * fys));
-        }
+      for (int kx = 0; kx < 4; ++kx) {
+        const int a = tb.row[l] + tb.col[kx];
+        atomicAdd(&acc0[a], __float2int_rn(tb.wx[kx] * wyx));
+        atomicAdd(&acc1[a], __float2int_rn(tb.wx[kx] * wyy));
+      }
     }
   }
   __syncthreads();
@@ -153,7 +161,7 @@ __global__ void __launch_bounds__(256) k_spread_tile(int nx, int ny, const int* 
                                                      const float2* __restrict__ F,
                                                      const float* __restrict__ tile_rho_max,
                                                      float* __restrict__ G0, float* __restrict__ G1) {
-  __shared__ int acc0[TS * TS], acc1[TS * TS];
+  __shared__ int acc0[TS * TSP], acc1[TS * TSP];
   __shared__ float red[32];
   const int t = blockIdx.x, ntx = nx / TS;
   const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
@@ -163,8 +171,8 @@ __global__ void __launch_bounds__(256) k_spread_tile(int nx, int ny, const int* 
   const float inv = 1.0f / scale;
   for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) {
     const size_t g = (size_t)(y0 + (c >> 5)) * nx + x0 + (c & 31);
-    G0[g] = (float)acc0[c] * inv;
-    G1[g] = (float)acc1[c] * inv;
+    G0[g] = (float)acc0[(c >> 5) * TSP + (c & 31)] * inv;
+    G1[g] = (float)acc1[(c >> 5) * TSP + (c & 31)] * inv;
   }
 }
 

@@ -127,6 +127,12 @@ int mc_read_state(mc_world* w, int64_t* step_out /*HOST*/, float* xy, float* u, 
  *   rho_b [ny][nx] deposited bead density (S2); G [2][ny][nx] spread force (S5). */
 int mc_read_intermediates(mc_world* w, float* rho_b, float* G);
 
+/* The hot path fuses S5 into the fluid kernel and never stores G.  mc_keep_intermediates(w, 1)
+ * makes the following steps store it too (slower; for parity checks); without it
+ * mc_read_intermediates with a non-NULL G returns MC_ESTATE.  rho_b is always stored while the
+ * world has a bead-density field. */
+int mc_keep_intermediates(mc_world* w, int32_t on);
+
 /* Optional per-kernel timing with CUDA events on the world's stream (used by bench.py for the
  * roofline line; off by default, costs one event record per kernel group when on).
  * Slots: 0 K0 bin, 1 K2a deposit, 2 K3a filter+gradient, 3 K1 filament force, 4 K2b spread,

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libmc.so")
 MC_OK, MC_EINVAL, MC_ENOMEM, MC_ECUDA, MC_ESTATE, MC_EDIVERGED = 0, -1, -2, -3, -4, -5
 SYMBOLS = ("mc_workspace_bytes", "mc_create", "mc_load_filaments", "mc_step", "mc_read_state",
            "mc_read_intermediates", "mc_launch_count", "mc_destroy", "mc_last_error",
-           "mc_profile_enable", "mc_profile_read")
+           "mc_profile_enable", "mc_profile_read", "mc_keep_intermediates")
 PROF_SLOTS = ("K0_bin", "K2a_deposit", "K3a_blur_grad", "K1_filament", "K2b_spread", "K3b_lbm",
               "K4_interp_integrate")
 
@@ -74,6 +74,8 @@ def load_library():
     L.mc_profile_enable.argtypes = [vp, i32]
     L.mc_profile_read.restype = C.c_int
     L.mc_profile_read.argtypes = [vp, _fp, C.POINTER(i32)]
+    L.mc_keep_intermediates.restype = C.c_int
+    L.mc_keep_intermediates.argtypes = [vp, i32]
     L.mc_destroy.restype = None
     L.mc_destroy.argtypes = [vp]
     L.mc_last_error.restype = C.c_char_p
@@ -193,6 +195,9 @@ class World:
                                                       C.c_void_p(G.data_ptr()))
         self._check(rc)
         return dict(rho_b=rho_b.cpu().numpy() if host else rho_b, G=G.cpu().numpy() if host else G)
+
+    def keep_intermediates(self, on: bool = True):
+        self._check(load_library().mc_keep_intermediates(self.h, int(bool(on))))
 
     def profile_enable(self, on: bool = True):
         self._check(load_library().mc_profile_enable(self.h, int(bool(on))))

@@ -16,6 +16,7 @@
 //   S+_q = w_q [-3 u.G + 9 (c_q.u)(c_q.G)],  S-_q = 3 w_q c_q.G         (Guo source by parity)
 //   gpost_q = g_q - w+ (g+_q - geq+_q) - w- (g-_q - geq-_q) + (1 - w+/2) S+_q + (1 - w-/2) S-_q
 #pragma once
+#include "k_p2g.cuh"
 #include "mc_common.cuh"
 
 namespace mc {
@@ -25,6 +26,8 @@ struct LbmArgs {
   float* dst;         // [9][ny][nx]
   const float* G0;    // spread force planes (may be NULL: zero force)
   const float* G1;
+  float* G0out;       // fused kernel only: where G is stored when KEEP_G
+  float* G1out;
   float2* u;          // out: collision-time velocity, interleaved (ux, uy)
   int nx, ny;
   float rho0, omega_p, omega_m;
@@ -95,6 +98,63 @@ __global__ void __launch_bounds__(256) k_lbm_step(LbmArgs a) {
 #pragma unroll
   for (int q = 0; q < 9; ++q) a.dst[q * nc + c] = g[q];
   if (!(fabsf(ux) <= 0.3f && fabsf(uy) <= 0.3f)) atomicOr(a.flag, 4);
+}
+
+// Fused K2b + K3b: one CTA per TS x TS tile first accumulates the spread force of its tile in
+// shared memory (S5, k_p2g.cuh) and then updates the fluid of the same nodes with it (S6), so G
+// never travels through HBM (-16 B/node).  CTAs in their atomic phase overlap on an SM with
+// CTAs in their streaming phase.  KEEP_G also stores G (parity tests: mc_keep_intermediates).
+struct LbmSpreadArgs {
+  LbmArgs lbm;             // G0/G1 are OUTPUTS here, used only when KEEP_G
+  const int* tile_start;
+  const int* list;
+  const float2* X;
+  const float2* F;
+  const float* tile_rho_max;  // may be NULL
+};
+
+template <bool KEEP_G>
+__global__ void __launch_bounds__(256) k_lbm_spread_tile(LbmSpreadArgs p) {
+  __shared__ int acc0[TS * TSP], acc1[TS * TSP];
+  __shared__ float red[32];
+  const LbmArgs& a = p.lbm;
+  const int nx = a.nx, ny = a.ny;
+  const int t = blockIdx.x, ntx = nx / TS;
+  const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
+  const int s = p.tile_start[t], e = p.tile_start[t + 1];
+  const float scale = spread_tile_accumulate(nx, ny, x0, y0, s, e, p.list, p.X, p.F,
+                                             p.tile_rho_max ? p.tile_rho_max[t] : 0.0f, acc0, acc1, red);
+  const float inv = 1.0f / scale;
+  const size_t nc = (size_t)nx * ny;
+  const int lx = threadIdx.x & 31;
+  const int i = x0 + lx;
+  const int im = (i == 0) ? nx - 1 : i - 1, ip = (i == nx - 1) ? 0 : i + 1;
+  bool bad = false;
+  for (int ly = threadIdx.x >> 5; ly < TS; ly += 8) {
+    const int j = y0 + ly;
+    const int jm = (j == 0) ? ny - 1 : j - 1, jp = (j == ny - 1) ? 0 : j + 1;
+    const size_t r0 = (size_t)j * nx, rm = (size_t)jm * nx, rp = (size_t)jp * nx;
+    float g[9];
+    g[0] = __ldg(a.src + 0 * nc + r0 + i);
+    g[1] = __ldg(a.src + 1 * nc + r0 + im);
+    g[2] = __ldg(a.src + 2 * nc + rm + i);
+    g[3] = __ldg(a.src + 3 * nc + r0 + ip);
+    g[4] = __ldg(a.src + 4 * nc + rp + i);
+    g[5] = __ldg(a.src + 5 * nc + rm + im);
+    g[6] = __ldg(a.src + 6 * nc + rm + ip);
+    g[7] = __ldg(a.src + 7 * nc + rp + ip);
+    g[8] = __ldg(a.src + 8 * nc + rp + im);
+    const size_t c = r0 + i;
+    const float Gx = (float)acc0[ly * TSP + lx] * inv, Gy = (float)acc1[ly * TSP + lx] * inv;
+    if (KEEP_G) { a.G0out[c] = Gx; a.G1out[c] = Gy; }
+    float ux, uy;
+    trt_collide(g, Gx, Gy, a.rho0, a.omega_p, a.omega_m, ux, uy);
+    a.u[c] = make_float2(ux, uy);
+#pragma unroll
+    for (int q = 0; q < 9; ++q) a.dst[q * nc + c] = g[q];
+    bad = bad || !(fabsf(ux) <= 0.3f && fabsf(uy) <= 0.3f);
+  }
+  if (bad) atomicOr(a.flag, 4);
 }
 
 // mc_read_state: current pre-collision populations (streamed) as deviations, and rho.

@@ -126,6 +126,7 @@ struct mc_world {
   int static_slot[4] = {-1, -1, -1, -1};
   int64_t launches = 0;
   bool diverged = false;
+  bool keep_G = false;  // mc_keep_intermediates: the fused spread+fluid kernel also stores G
   std::string err;
   // optional per-kernel timing (mc_profile_*): events at the 8 boundaries of a step
   bool prof_on = false;
@@ -242,10 +243,7 @@ int enqueue_step(mc_world* w) {
     fa.n_step = (double)w->step;
     mc::k_filament_force<<<(w->n_windows + 7) / 8, 256, 0, st>>>(fa);
     prof_mark(w, 4);
-    // K2b: S5 spread
-    mc::k_spread_tile<<<n_tiles, 256, 0, st>>>(nx, ny, tile_start, list, X, F,
-                                               w->d.n_density ? tile_rho_max : nullptr, G0, G1);
-    w->launches += 2;
+    w->launches++;
   } else {
     for (int b = 1; b <= 4; ++b) prof_mark(w, b);
   }
@@ -263,8 +261,25 @@ int enqueue_step(mc_world* w) {
   la.omega_p = w->omega_p;
   la.omega_m = w->omega_m;
   la.flag = flag;
-  const int bx = pick_bx(nx);
-  mc::k_lbm_step<<<dim3(nx / bx, ny), bx, 0, st>>>(la);
+  la.G0out = G0;
+  la.G1out = G1;
+  if (beads) {
+    // K2b + K3b fused: S5 spread into shared memory, S6 fluid update of the same tile
+    la.G0 = nullptr;
+    la.G1 = nullptr;
+    mc::LbmSpreadArgs ls;
+    ls.lbm = la;
+    ls.tile_start = tile_start;
+    ls.list = list;
+    ls.X = X;
+    ls.F = F;
+    ls.tile_rho_max = w->d.n_density ? tile_rho_max : nullptr;
+    if (w->keep_G) mc::k_lbm_spread_tile<true><<<n_tiles, 256, 0, st>>>(ls);
+    else mc::k_lbm_spread_tile<false><<<n_tiles, 256, 0, st>>>(ls);
+  } else {
+    const int bx = pick_bx(nx);
+    mc::k_lbm_step<<<dim3(nx / bx, ny), bx, 0, st>>>(la);
+  }
   w->launches++;
   w->cur ^= 1;
   prof_mark(w, 6);
@@ -565,8 +580,15 @@ int mc_read_state(mc_world* w, int64_t* step_out, float* xy, float* u, float* rh
   return MC_OK;
 }
 
+int mc_keep_intermediates(mc_world* w, int32_t on) {
+  if (!w) return MC_EINVAL;
+  w->keep_G = on != 0;
+  return MC_OK;
+}
+
 int mc_read_intermediates(mc_world* w, float* rho_b, float* G) {
   if (!w) return MC_EINVAL;
+  if (G && !w->keep_G) return fail(w, MC_ESTATE, "G is only stored after mc_keep_intermediates(w, 1)");
   cudaStream_t st = w->stream;
   const size_t nc = w->nc;
   if (rho_b) cudaMemcpyAsync(rho_b, w->ptr<float>(w->L.rho_b), nc * 4, cudaMemcpyDeviceToDevice, st);

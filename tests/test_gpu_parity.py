@@ -76,6 +76,7 @@ def step_parity(G, w, threads=0, check=True):
 def run_protocol(w, steps_at, threads=0):
     from paper_2607_02954_b200 import binding
     G = binding.World(w)
+    G.keep_intermediates(True)
     done = 0
     worst = {}
     for s in steps_at:
@@ -154,6 +155,7 @@ def test_bitwise_reproducible(name):
     outs = []
     for _ in range(2):
         G = binding.World(SMALL[name]())
+        G.keep_intermediates(True)
         G.step(25)
         s = G.read_state()
         i = G.read_intermediates()

@@ -1,9 +1,15 @@
 // k_tile.cuh -- K0: bin the beads by grid TILE (north_star (2): "bead sort by cell tile
 // followed by shared-memory tile accumulation, so global atomics are minimised").
 //
-// A tile is TS x TS nodes.  A bead is listed in every tile its 4x4 Peskin support overlaps
-// (1, 2 or 4 tiles), so a tile's CTA can accumulate ALL contributions to its own nodes from its
-// own list and never writes outside the tile: no global float atomics, no halo exchange.
+// A tile is TS x TS nodes.  A bead is listed in every tile its 4x4 Peskin support, widened by a
+// SKIN of one node on every side, overlaps (1, 2 or 4 tiles), so a tile's CTA can accumulate ALL
+// contributions to its own nodes from its own list and never writes outside the tile: no global
+// float atomics, no halo exchange.  The skin makes a list valid for several steps: a bead moves
+// by at most 0.3 nodes per axis per step (U is a convex combination of u, and |u| > 0.3 raises
+// the divergence flag), so lists built at step n0 still cover every support at steps n0+1..n0+3
+// (drift <= 0.9 < 1) and K0 runs only every LIST_STEPS = 4 steps.  Entries whose support no
+// longer (or not yet) overlaps the tile add exact zeros (k_p2g.cuh), so the result does not
+// depend on when the lists were built.
 //   count : per bead, +1 on each overlapped tile (integer atomics, warp-aggregated)
 //   scan  : exclusive prefix sum over the tiles (one block; there are few tiles)
 //   fill  : per bead, claim a slot in each overlapped tile's segment and store the bead index
@@ -15,13 +21,16 @@
 
 namespace mc {
 
-constexpr int TS = 32;  // tile side in nodes
+constexpr int TS = 32;          // tile side in nodes
+constexpr int LIST_SKIN = 1;    // nodes added on every side of the support when listing
+constexpr int LIST_STEPS = 4;   // steps a list stays valid: (LIST_STEPS-1) * 0.3 < LIST_SKIN
 
-// The (up to 4) tiles overlapped by the support of a bead at (x,y): tiles of the first and
-// the last support node along each axis (periodic).  Returns the number of distinct tiles.
+// The (up to 4) tiles overlapped by the skinned support of a bead at (x,y): tiles of the first
+// and the last listed node along each axis (periodic).  Returns the number of distinct tiles.
 __device__ __forceinline__ int bead_tiles(float x, float y, int nx, int ny, int ntx, int t[4]) {
-  const int i0 = wrapi((int)floorf(x) - 1, nx), j0 = wrapi((int)floorf(y) - 1, ny);
-  const int i3 = (i0 + 3 >= nx) ? i0 + 3 - nx : i0 + 3, j3 = (j0 + 3 >= ny) ? j0 + 3 - ny : j0 + 3;
+  constexpr int W = 3 + 2 * LIST_SKIN;  // last listed node relative to the first
+  const int i0 = wrapi((int)floorf(x) - 1 - LIST_SKIN, nx), j0 = wrapi((int)floorf(y) - 1 - LIST_SKIN, ny);
+  const int i3 = (i0 + W >= nx) ? i0 + W - nx : i0 + W, j3 = (j0 + W >= ny) ? j0 + W - ny : j0 + W;
   const int txa = i0 / TS, txb = i3 / TS, tya = j0 / TS, tyb = j3 / TS;
   int n = 0;
   t[n++] = tya * ntx + txa;

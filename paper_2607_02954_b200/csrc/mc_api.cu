@@ -120,6 +120,7 @@ struct mc_world {
   int N = 0;
   int stride = 60;   // K1 window advance: 64 when all chains share a length dividing 64
   int n_windows = 0;
+  int list_age = 0;  // steps since the tile lists were built (rebuilt when 0)
   float rho0 = 1, omega_p = 1, omega_m = 1, kappa = 0;
   float coef[4] = {0, 0, 0, 0};  // lattice coupling with the sign of the force
   mc::BlurTaps taps[4];
@@ -203,11 +204,14 @@ int enqueue_step(mc_world* w) {
 
   prof_mark(w, 0);
   if (beads) {
-    // K0: tile binning (count, scan, fill)
-    mc::k_tile_bin<false><<<bgrid, bt, 0, st>>>(X, N, nx, ny, tile_count, nullptr);
-    mc::k_tile_scan<<<1, 1024, 0, st>>>(tile_count, n_tiles, tile_start, tile_cursor);
-    mc::k_tile_bin<true><<<bgrid, bt, 0, st>>>(X, N, nx, ny, tile_cursor, list);
-    w->launches += 3;
+    // K0: tile binning (count, scan, fill), every LIST_STEPS steps (skinned lists, k_tile.cuh)
+    if (w->list_age == 0) {
+      mc::k_tile_bin<false><<<bgrid, bt, 0, st>>>(X, N, nx, ny, tile_count, nullptr);
+      mc::k_tile_scan<<<1, 1024, 0, st>>>(tile_count, n_tiles, tile_start, tile_cursor);
+      mc::k_tile_bin<true><<<bgrid, bt, 0, st>>>(X, N, nx, ny, tile_cursor, list);
+      w->launches += 3;
+    }
+    w->list_age = (w->list_age + 1) % mc::LIST_STEPS;
     prof_mark(w, 1);
     // K2a: S2 deposit
     if (w->d.n_density) {
@@ -508,6 +512,7 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   if (h) return fail(w, MC_EINVAL, (h & 1) ? "stiffness outside [0,1]" : "period <= 0");
   w->N = (int)N;
   w->n_fil = n_fil;
+  w->list_age = 0;
   const bool aligned = uniform && (64 % m0 == 0);
   w->stride = aligned ? 64 : 60;
   w->n_windows = aligned ? (int)((N + 63) / 64) : (int)((N + 59) / 60);

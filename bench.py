@@ -107,10 +107,10 @@ def kernel_bytes(n_cells: int, n_beads: int) -> dict:
     return {
         "K0_bin": 0,                                      # mechanism: no algorithmic traffic
         "K2a_deposit": 4 * n_cells + 8 * n_beads,         # rho_b write; X read
-        "K3a_blur_grad": 12 * n_cells,                    # rho_b read; grad planes write
-        "K1_filament": 48 * n_beads,                      # X + 2 float4 params read; F write
-        "K2b_spread": 8 * n_cells + 8 * n_beads,          # G write; F read
-        "K3b_lbm": 88 * n_cells,                          # f read+write 72, G read 8, u write 8
+        "K3a_blur_grad": 12 * n_cells,                    # rho_b read; gradient field write
+        "K1_filament": 48 * n_beads,                      # X + params read; F write (model: 32 B params)
+        "K2b_spread": 0,                                  # fused into K3b (slot measures nothing)
+        "K3b_lbm": 80 * n_cells + 16 * n_beads,           # f read+write 72, u write 8; X, F read (S5 fused)
         "K4_interp_integrate": 16 * n_beads,              # X read + write
     }
 

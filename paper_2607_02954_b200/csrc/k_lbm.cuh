@@ -114,16 +114,18 @@ struct LbmSpreadArgs {
 };
 
 template <bool KEEP_G>
-__global__ void __launch_bounds__(256) k_lbm_spread_tile(LbmSpreadArgs p) {
-  __shared__ int acc0[TS * TSP], acc1[TS * TSP];
+__global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
+  __shared__ int acc0[TS * TSP], acc1[TS * TSP], accl0[TS * TSP], accl1[TS * TSP];
   __shared__ float red[32];
   const LbmArgs& a = p.lbm;
   const int nx = a.nx, ny = a.ny;
   const int t = blockIdx.x, ntx = nx / TS;
   const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
   const int s = p.tile_start[t], e = p.tile_start[t + 1];
+  float linv;
   const float scale = spread_tile_accumulate(nx, ny, x0, y0, s, e, p.list, p.X, p.F,
-                                             p.tile_rho_max ? p.tile_rho_max[t] : 0.0f, acc0, acc1, red);
+                                             p.tile_rho_max ? p.tile_rho_max[t] : 0.0f, acc0, acc1, accl0,
+                                             accl1, red, linv);
   const float inv = 1.0f / scale;
   const size_t nc = (size_t)nx * ny;
   const int lx = threadIdx.x & 31;
@@ -145,7 +147,8 @@ __global__ void __launch_bounds__(256) k_lbm_spread_tile(LbmSpreadArgs p) {
     g[7] = __ldg(a.src + 7 * nc + rp + ip);
     g[8] = __ldg(a.src + 8 * nc + rp + im);
     const size_t c = r0 + i;
-    const float Gx = (float)acc0[ly * TSP + lx] * inv, Gy = (float)acc1[ly * TSP + lx] * inv;
+    const float Gx = tile_value(acc0, accl0, ly * TSP + lx, linv) * inv;
+    const float Gy = tile_value(acc1, accl1, ly * TSP + lx, linv) * inv;
     if (KEEP_G) { a.G0out[c] = Gx; a.G1out[c] = Gy; }
     float ux, uy;
     trt_collide(g, Gx, Gy, a.rho0, a.omega_p, a.omega_m, ux, uy);

@@ -16,6 +16,11 @@
 //   S2: every contribution is <= 1/4, so |acc| <= n_list/4;
 //   S5: |sum_i F_i w_i| <= max|F| * sum_i w_i = max|F| * rho_b(g) <= max|F| * max_tile(rho_b),
 //       with max_tile(rho_b) left behind by S2 of the same step (same X, same weights).
+// Crowded tiles (more than WIDE_N listed beads, e.g. the cluster of config 5) would lose digits
+// that way: their bound is far above the typical node value (many contributions, cancelling
+// forces).  They accumulate every contribution as TWO integers -- the rounded value and its
+// remainder scaled by a further 2^LB -- into a second accumulator plane, which restores fp32
+// accuracy per contribution at twice the atomics, in those tiles only.
 #pragma once
 #include "k_tile.cuh"
 #include "mc_common.cuh"
@@ -29,6 +34,7 @@ namespace mc {
 // i.e. nodes about one cell apart in an arbitrary direction; with pitch 32 a vertical chain would
 // put all 32 lanes on one bank.  37 = 5 (mod 32) has no bank collision for offsets |dr|,|dc| <= 2.
 constexpr int TSP = 37;
+constexpr int WIDE_N = 1024;  // listed beads above which a tile accumulates hi + lo words
 
 struct TileBead {
   int col[4], row[4];    // col: local x (0..TS-1); row: local y * TSP
@@ -80,20 +86,16 @@ __device__ __forceinline__ float pow2_scale(float bound) {
   return ldexpf(1.0f, 30 - ex);
 }
 
-// K2a: S2 deposit.  tile_rho_max[t] receives max over the tile of rho_b (for K2b's scale).
-__global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int* __restrict__ tile_start,
-                                                      const int* __restrict__ list,
-                                                      const float2* __restrict__ X,
-                                                      float* __restrict__ rho_b,
-                                                      float* __restrict__ tile_rho_max) {
-  __shared__ int acc[TS * TSP];
-  __shared__ float red[32];
-  const int t = blockIdx.x, ntx = nx / TS;
-  const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
-  const int s = tile_start[t], e = tile_start[t + 1];
-  for (int c = threadIdx.x; c < TS * TSP; c += blockDim.x) acc[c] = 0;
-  const float scale = pow2_scale(fmaxf(0.25f * (float)(e - s), 1.0f));
-  __syncthreads();
+// number of extra fraction bits the lo word can carry without overflowing for n contributions
+__device__ __forceinline__ int lo_bits(int n) {
+  const int lg = 32 - __clz(max(n, 2) - 1);  // ceil(log2 n)
+  return min(20, max(0, 30 - lg));
+}
+
+template <bool WIDE>
+__device__ __forceinline__ void deposit_loop(int nx, int ny, int x0, int y0, int s, int e,
+                                             const int* __restrict__ list, const float2* __restrict__ X,
+                                             float scale, float lscale, int* acc, int* accl) {
   for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
     TileBead tb;
     tile_bead(__ldg(X + __ldg(list + k)), nx, ny, x0, y0, tb);
@@ -101,38 +103,26 @@ __global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int*
     for (int l = 0; l < 4; ++l) {
       const float wys = tb.wy[l] * scale;
 #pragma unroll
-      for (int kx = 0; kx < 4; ++kx)
-        atomicAdd(&acc[tb.row[l] + tb.col[kx]], __float2int_rn(tb.wx[kx] * wys));
+      for (int kx = 0; kx < 4; ++kx) {
+        const int a = tb.row[l] + tb.col[kx];
+        const float v = tb.wx[kx] * wys;
+        if (WIDE) {
+          const float h = rintf(v);
+          atomicAdd(&acc[a], (int)h);
+          atomicAdd(&accl[a], __float2int_rn((v - h) * lscale));
+        } else {
+          atomicAdd(&acc[a], __float2int_rn(v));
+        }
+      }
     }
   }
-  __syncthreads();
-  const float inv = 1.0f / scale;
-  float mx = 0.0f;
-  for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) {
-    const float v = (float)acc[(c >> 5) * TSP + (c & 31)] * inv;
-    rho_b[(size_t)(y0 + (c >> 5)) * nx + x0 + (c & 31)] = v;
-    mx = fmaxf(mx, v);
-  }
-  mx = block_max(mx, red);
-  if (threadIdx.x == 0) tile_rho_max[t] = mx;
 }
 
-// Accumulate the spread force of one tile into shared memory (two planes), return the scale.
-// Shared by the stand-alone spread kernel and by the fused spread + fluid kernel (k_lbm.cuh).
-__device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, int y0, int s, int e,
-                                                        const int* __restrict__ list,
-                                                        const float2* __restrict__ X,
-                                                        const float2* __restrict__ F, float rho_max,
-                                                        int* acc0, int* acc1, float* red) {
-  for (int c = threadIdx.x; c < TS * TSP; c += blockDim.x) { acc0[c] = 0; acc1[c] = 0; }
-  float fm = 0.0f;
-  for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
-    const float2 f = __ldg(F + __ldg(list + k));
-    fm = fmaxf(fm, fmaxf(fabsf(f.x), fabsf(f.y)));
-  }
-  fm = block_max(fm, red);  // also orders the zeroing before the atomics
-  const float sum_w = (rho_max > 0.0f) ? 1.0625f * rho_max : fmaxf(0.25f * (float)(e - s), 1.0f);
-  const float scale = pow2_scale(fmaxf(fm * sum_w, 1e-18f));
+template <bool WIDE>
+__device__ __forceinline__ void spread_loop(int nx, int ny, int x0, int y0, int s, int e,
+                                            const int* __restrict__ list, const float2* __restrict__ X,
+                                            const float2* __restrict__ F, float scale, float lscale,
+                                            int* acc0, int* acc1, int* accl0, int* accl1) {
   for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
     const int b = __ldg(list + k);
     TileBead tb;
@@ -145,11 +135,95 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
 #pragma unroll
       for (int kx = 0; kx < 4; ++kx) {
         const int a = tb.row[l] + tb.col[kx];
-        atomicAdd(&acc0[a], __float2int_rn(tb.wx[kx] * wyx));
-        atomicAdd(&acc1[a], __float2int_rn(tb.wx[kx] * wyy));
+        const float vx = tb.wx[kx] * wyx, vy = tb.wx[kx] * wyy;
+        if (WIDE) {
+          const float hx = rintf(vx), hy = rintf(vy);
+          atomicAdd(&acc0[a], (int)hx);
+          atomicAdd(&acc1[a], (int)hy);
+          atomicAdd(&accl0[a], __float2int_rn((vx - hx) * lscale));
+          atomicAdd(&accl1[a], __float2int_rn((vy - hy) * lscale));
+        } else {
+          atomicAdd(&acc0[a], __float2int_rn(vx));
+          atomicAdd(&acc1[a], __float2int_rn(vy));
+        }
       }
     }
   }
+}
+
+// the rare crowded-tile variants are kept out of line so that their registers do not count
+// against the occupancy of the common path
+__device__ __noinline__ void deposit_loop_wide(int nx, int ny, int x0, int y0, int s, int e, const int* list,
+                                               const float2* X, float scale, float lscale, int* acc, int* accl) {
+  deposit_loop<true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
+}
+__device__ __noinline__ void spread_loop_wide(int nx, int ny, int x0, int y0, int s, int e, const int* list,
+                                              const float2* X, const float2* F, float scale, float lscale,
+                                              int* acc0, int* acc1, int* accl0, int* accl1) {
+  spread_loop<true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
+}
+
+// K2a: S2 deposit.  tile_rho_max[t] receives max over the tile of rho_b (for K2b's scale).
+__global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int* __restrict__ tile_start,
+                                                      const int* __restrict__ list,
+                                                      const float2* __restrict__ X,
+                                                      float* __restrict__ rho_b,
+                                                      float* __restrict__ tile_rho_max) {
+  __shared__ int acc[TS * TSP], accl[TS * TSP];
+  __shared__ float red[32];
+  const int t = blockIdx.x, ntx = nx / TS;
+  const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
+  const int s = tile_start[t], e = tile_start[t + 1];
+  const bool wide = (e - s) > WIDE_N;
+  for (int c = threadIdx.x; c < TS * TSP; c += blockDim.x) { acc[c] = 0; if (wide) accl[c] = 0; }
+  const float scale = pow2_scale(fmaxf(0.25f * (float)(e - s), 1.0f));
+  const float lscale = ldexpf(1.0f, lo_bits(e - s));
+  __syncthreads();
+  if (wide) deposit_loop_wide(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
+  else deposit_loop<false>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
+  __syncthreads();
+  const float inv = 1.0f / scale, linv = 1.0f / lscale;
+  float mx = 0.0f;
+  for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) {
+    const int a = (c >> 5) * TSP + (c & 31);
+    const float v = (wide ? fmaf((float)accl[a], linv, (float)acc[a]) : (float)acc[a]) * inv;
+    rho_b[(size_t)(y0 + (c >> 5)) * nx + x0 + (c & 31)] = v;
+    mx = fmaxf(mx, v);
+  }
+  mx = block_max(mx, red);
+  if (threadIdx.x == 0) tile_rho_max[t] = mx;
+}
+
+// accumulator -> float (before the 1/scale): hi word, plus the lo word in wide tiles (linv != 0)
+__device__ __forceinline__ float tile_value(const int* acc, const int* accl, int a, float linv) {
+  return (linv != 0.0f) ? fmaf((float)accl[a], linv, (float)acc[a]) : (float)acc[a];
+}
+
+// Accumulate the spread force of one tile into shared memory (two planes), return the scale.
+// Shared by the stand-alone spread kernel and by the fused spread + fluid kernel (k_lbm.cuh).
+__device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, int y0, int s, int e,
+                                                        const int* __restrict__ list,
+                                                        const float2* __restrict__ X,
+                                                        const float2* __restrict__ F, float rho_max,
+                                                        int* acc0, int* acc1, int* accl0, int* accl1,
+                                                        float* red, float& linv) {
+  const bool wide = (e - s) > WIDE_N;
+  const float lscale = ldexpf(1.0f, lo_bits(e - s));
+  linv = wide ? 1.0f / lscale : 0.0f;  // 0 => the readers skip the lo planes (not zeroed then)
+  for (int c = threadIdx.x; c < TS * TSP; c += blockDim.x) {
+    acc0[c] = 0; acc1[c] = 0;
+    if (wide) { accl0[c] = 0; accl1[c] = 0; }
+  }
+  float fm = 0.0f;
+  for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
+    const float2 f = __ldg(F + __ldg(list + k));
+    fm = fmaxf(fm, fmaxf(fabsf(f.x), fabsf(f.y)));
+  }
+  fm = block_max(fm, red);  // also orders the zeroing before the atomics
+  const float sum_w = (rho_max > 0.0f) ? 1.0625f * rho_max : fmaxf(0.25f * (float)(e - s), 1.0f);
+  const float scale = pow2_scale(fmaxf(fm * sum_w, 1e-18f));
+  if (wide) spread_loop_wide(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
+  else spread_loop<false>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
   __syncthreads();
   return scale;
 }
@@ -161,18 +235,20 @@ __global__ void __launch_bounds__(256) k_spread_tile(int nx, int ny, const int* 
                                                      const float2* __restrict__ F,
                                                      const float* __restrict__ tile_rho_max,
                                                      float* __restrict__ G0, float* __restrict__ G1) {
-  __shared__ int acc0[TS * TSP], acc1[TS * TSP];
+  __shared__ int acc0[TS * TSP], acc1[TS * TSP], accl0[TS * TSP], accl1[TS * TSP];
   __shared__ float red[32];
   const int t = blockIdx.x, ntx = nx / TS;
   const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
   const int s = tile_start[t], e = tile_start[t + 1];
+  float linv;
   const float scale = spread_tile_accumulate(nx, ny, x0, y0, s, e, list, X, F,
-                                             tile_rho_max ? tile_rho_max[t] : 0.0f, acc0, acc1, red);
+                                             tile_rho_max ? tile_rho_max[t] : 0.0f, acc0, acc1, accl0, accl1,
+                                             red, linv);
   const float inv = 1.0f / scale;
   for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) {
     const size_t g = (size_t)(y0 + (c >> 5)) * nx + x0 + (c & 31);
-    G0[g] = (float)acc0[(c >> 5) * TSP + (c & 31)] * inv;
-    G1[g] = (float)acc1[(c >> 5) * TSP + (c & 31)] * inv;
+    G0[g] = tile_value(acc0, accl0, (c >> 5) * TSP + (c & 31), linv) * inv;
+    G1[g] = tile_value(acc1, accl1, (c >> 5) * TSP + (c & 31), linv) * inv;
   }
 }
 

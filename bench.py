@@ -115,6 +115,23 @@ def kernel_bytes(n_cells: int, n_beads: int) -> dict:
     }
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
+# (profiles/r1_traffic.json, world 4d); None for other workloads or kernels not captured
+_SLOT_KERNEL = {"K2a_deposit": "k_deposit_tile", "K3a_blur_grad": "k_blur_grad", "K1_filament": "k_filament_force",
+                "K3b_lbm": "k_lbm_spread_tile", "K4_interp_integrate": "k_interp_integrate"}
+
+
+def ncu_traffic(slot: str, workload: str):
+    try:
+        with open(os.path.join(ROOT, "profiles", "r1_traffic.json")) as fh:
+            d = json.load(fh)
+        if d.get("world") != workload:
+            return None
+        return d["dram_bytes_per_launch"].get(_SLOT_KERNEL.get(slot, ""))
+    except Exception:
+        return None
+
+
 def step_bytes(n_cells: int, n_beads: int) -> int:
     return 112 * n_cells + 64 * n_beads  # SURVEY.md 8(d) / DESIGN.md
 
@@ -239,7 +256,7 @@ def main():
     dom = max(kms, key=lambda k: kms[k])
     ach = kb[dom] / (kms[dom] * 1e-3) / 1e9 if kms[dom] > 0 else 0.0
     roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
-                "frac": ach / peak, "traffic": None, "peak_source": peak_src,
+                "frac": ach / peak, "traffic": ncu_traffic(dom, args.workload), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": kb[dom], "ms_per_launch": kms[dom],
                 "share_of_step": kms[dom] / max(sum(kms.values()), 1e-12)}
     ach_step = step_bytes(nc, N) / (ms_step * 1e-3) / 1e9

@@ -121,6 +121,7 @@ struct mc_world {
   int stride = 60;   // K1 window advance: 64 when all chains share a length dividing 64
   int n_windows = 0;
   int list_age = 0;  // steps since the tile lists were built (rebuilt when 0)
+  std::vector<int32_t> loaded_offsets;  // offsets of the last load: same chains => keep the internal order
   float rho0 = 1, omega_p = 1, omega_m = 1, kappa = 0;
   float coef[4] = {0, 0, 0, 0};  // lattice coupling with the sign of the force
   mc::BlurTaps taps[4];
@@ -448,6 +449,9 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
                 !act_period))
     return fail(w, MC_EINVAL, "null array");
   cudaStream_t st = w->stream;
+  const bool reuse_order = w->N == N && w->n_fil == n_fil && (int64_t)w->loaded_offsets.size() == n_fil + 1 &&
+                           std::equal(w->loaded_offsets.begin(), w->loaded_offsets.end(), offsets);
+  const int prev_stride = w->stride, prev_windows = w->n_windows;
   w->N = 0;
   w->n_fil = 0;
   w->n_windows = 0;
@@ -456,6 +460,14 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   //    64x64 block of nodes become neighbours in memory, so the per-bead grid gathers of K1/K4
   //    and the per-tile bead gathers of K2 hit L2 instead of re-fetching sectors from HBM.
   //    The internal order is a mechanism only: every output is returned in the caller's order.
+  bool uniform = true;
+  const int m0 = offsets[1] - offsets[0];
+  int* bad = w->ptr<int>(w->L.flags) + 1;
+  cudaMemsetAsync(bad, 0, 4, st);
+  cudaError_t e = cudaSuccess;
+  std::vector<int> src;                 // host staging of this call; must outlive the final sync
+  std::vector<unsigned char> bflags;
+  if (!reuse_order) {
   int* d_off = w->ptr<int>(w->L.scratch);
   int* d_keys = d_off + (n_fil + 1);
   std::vector<int> keys(n_fil);
@@ -463,16 +475,14 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   mc::k_chain_keys<<<(n_fil + 255) / 256, 256, 0, st>>>(n_fil, d_off, xy, w->nx, w->ny, 64, d_keys);
   w->launches++;
   cudaMemcpyAsync(keys.data(), d_keys, (size_t)n_fil * 4, cudaMemcpyDeviceToHost, st);
-  cudaError_t e = cudaStreamSynchronize(st);
+  e = cudaStreamSynchronize(st);
   if (e == cudaSuccess) e = cudaGetLastError();
   if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_load_filaments: ") + cudaGetErrorString(e));
   std::vector<int> order(n_fil);
   std::iota(order.begin(), order.end(), 0);
   std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return keys[a] < keys[b]; });
-  std::vector<int> src((size_t)N);
-  std::vector<unsigned char> bflags((size_t)N, 0);
-  bool uniform = true;
-  const int m0 = offsets[1] - offsets[0];
+  src.resize((size_t)N);
+  bflags.assign((size_t)N, 0);
   size_t pos = 0;
   for (int c = 0; c < n_fil; ++c) {
     const int f = order[c];
@@ -483,10 +493,9 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
     bflags[pos + m - 1] |= mc::BEAD_LAST;
     pos += m;
   }
-  int* bad = w->ptr<int>(w->L.flags) + 1;
-  cudaMemsetAsync(bad, 0, 4, st);
   cudaMemcpyAsync(w->ptr<int>(w->L.src), src.data(), (size_t)N * 4, cudaMemcpyHostToDevice, st);
   cudaMemcpyAsync(w->ptr<unsigned char>(w->L.bflags), bflags.data(), (size_t)N, cudaMemcpyHostToDevice, st);
+  }
   // 2. gather + pack the per-bead parameters in the internal order, validate
   mc::PackArgs pa;
   pa.N = (int)N;
@@ -509,13 +518,22 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   e = cudaStreamSynchronize(st);  // src/bflags are host vectors of this call
   if (e == cudaSuccess) e = cudaGetLastError();
   if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_load_filaments: ") + cudaGetErrorString(e));
-  if (h) return fail(w, MC_EINVAL, (h & 1) ? "stiffness outside [0,1]" : "period <= 0");
+  if (h) {
+    w->loaded_offsets.clear();
+    return fail(w, MC_EINVAL, (h & 1) ? "stiffness outside [0,1]" : "period <= 0");
+  }
   w->N = (int)N;
   w->n_fil = n_fil;
   w->list_age = 0;
-  const bool aligned = uniform && (64 % m0 == 0);
-  w->stride = aligned ? 64 : 60;
-  w->n_windows = aligned ? (int)((N + 63) / 64) : (int)((N + 59) / 60);
+  if (reuse_order) {
+    w->stride = prev_stride;
+    w->n_windows = prev_windows;
+  } else {
+    const bool aligned = uniform && (64 % m0 == 0);
+    w->stride = aligned ? 64 : 60;
+    w->n_windows = aligned ? (int)((N + 63) / 64) : (int)((N + 59) / 60);
+    w->loaded_offsets.assign(offsets, offsets + n_fil + 1);
+  }
   return MC_OK;
 }
 

@@ -39,6 +39,7 @@ struct FilamentArgs {
   float* sense;      // [N] out (only written when csum != NULL)
   const float2* A;   // interleaved force-gradient field (may be NULL: no field forces)
   const float* csum;  // sum of static fields (may be NULL)
+  unsigned* tile_fmax;  // per 32x32 tile: bits of max |F| over the beads whose floor(X) lies in it (may be NULL)
   int N;
   int nx, ny;
   int stride;        // 64 (aligned windows) or 60 (overlapping windows)
@@ -156,6 +157,26 @@ __global__ void __launch_bounds__(256) k_filament_force(FilamentArgs a) {
   if (a.A) {
     if (vA) { const float2 g = interp2(a.A, a.nx, a.ny, xa.x, xa.y); FA.x += g.x; FA.y += g.y; }
     if (vB) { const float2 g = interp2(a.A, a.nx, a.ny, xb.x, xb.y); FB.x += g.x; FB.y += g.y; }
+  }
+  if (a.tile_fmax) {
+    // Bound for the fixed-point scale of S5 (k_p2g.cuh): tile_fmax[t] >= max |F| over the beads
+    // whose floor(X) lies in tile t.  The warp's own maximum is used for every tile its beads
+    // touch (a valid, slightly looser bound) so that one lane per distinct tile issues at most
+    // one atomicMax, and none once the stored value is high enough.  Positive floats order like
+    // their bit patterns.
+    float m = 0.0f;
+    if (vA) m = fmaxf(fabsf(FA.x), fabsf(FA.y));
+    if (vB) m = fmaxf(m, fmaxf(fabsf(FB.x), fabsf(FB.y)));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(__activemask(), m, o));
+    const unsigned mb = __float_as_uint(m);
+    const int ntx = a.nx >> 5;
+    const int tA = vA ? (wrapi((int)floorf(xa.y), a.ny) >> 5) * ntx + (wrapi((int)floorf(xa.x), a.nx) >> 5) : -1;
+    const int tB = vB ? (wrapi((int)floorf(xb.y), a.ny) >> 5) * ntx + (wrapi((int)floorf(xb.x), a.nx) >> 5) : -1;
+    const unsigned act = __activemask();
+    const unsigned pa = __match_any_sync(act, tA), pb = __match_any_sync(act, tB);
+    if (tA >= 0 && lane == __ffs(pa) - 1 && mb > a.tile_fmax[tA]) atomicMax(a.tile_fmax + tA, mb);
+    if (tB >= 0 && tB != tA && lane == __ffs(pb) - 1 && mb > a.tile_fmax[tB]) atomicMax(a.tile_fmax + tB, mb);
   }
   if (vA && vB) {
     *reinterpret_cast<float4*>(a.F + bA) = make_float4(FA.x, FA.y, FB.x, FB.y);

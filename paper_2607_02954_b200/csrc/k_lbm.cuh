@@ -111,6 +111,7 @@ struct LbmSpreadArgs {
   const float2* X;
   const float2* F;
   const float* tile_rho_max;  // may be NULL
+  const unsigned* tile_fmax;  // may be NULL
 };
 
 template <bool KEEP_G>
@@ -122,10 +123,20 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
   const int t = blockIdx.x, ntx = nx / TS;
   const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
   const int s = p.tile_start[t], e = p.tile_start[t + 1];
+  {
+    // start pulling this tile's populations towards L2 while the atomic phase runs: 9 planes x
+    // 32 rows x one 128-byte line (the +-1 halo columns/rows come with the neighbours' tiles)
+    const size_t ncp = (size_t)nx * ny;
+    for (int it = threadIdx.x; it < 9 * TS; it += 256) {
+      const int q = it >> 5, r = it & 31;
+      const float* ptr = a.src + q * ncp + (size_t)(y0 + r) * nx + x0;
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
+    }
+  }
   float linv;
   const float scale = spread_tile_accumulate(nx, ny, x0, y0, s, e, p.list, p.X, p.F,
-                                             p.tile_rho_max ? p.tile_rho_max[t] : 0.0f, acc0, acc1, accl0,
-                                             accl1, red, linv);
+                                             p.tile_rho_max ? p.tile_rho_max[t] : 0.0f, p.tile_fmax, t, acc0, acc1,
+                                             accl0, accl1, red, linv);
   const float inv = 1.0f / scale;
   const size_t nc = (size_t)nx * ny;
   const int lx = threadIdx.x & 31;

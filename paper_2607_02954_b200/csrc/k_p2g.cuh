@@ -168,7 +168,8 @@ __global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int*
                                                       const int* __restrict__ list,
                                                       const float2* __restrict__ X,
                                                       float* __restrict__ rho_b,
-                                                      float* __restrict__ tile_rho_max) {
+                                                      float* __restrict__ tile_rho_max,
+                                                      unsigned* __restrict__ tile_fmax) {
   __shared__ int acc[TS * TSP], accl[TS * TSP];
   __shared__ float red[32];
   const int t = blockIdx.x, ntx = nx / TS;
@@ -191,7 +192,10 @@ __global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int*
     mx = fmaxf(mx, v);
   }
   mx = block_max(mx, red);
-  if (threadIdx.x == 0) tile_rho_max[t] = mx;
+  if (threadIdx.x == 0) {
+    tile_rho_max[t] = mx;
+    tile_fmax[t] = 0u;  // K1 of this step raises it (atomicMax), K2b reads it
+  }
 }
 
 // accumulator -> float (before the 1/scale): hi word, plus the lo word in wide tiles (linv != 0)
@@ -205,6 +209,7 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
                                                         const int* __restrict__ list,
                                                         const float2* __restrict__ X,
                                                         const float2* __restrict__ F, float rho_max,
+                                                        const unsigned* __restrict__ tile_fmax, int t,
                                                         int* acc0, int* acc1, int* accl0, int* accl1,
                                                         float* red, float& linv) {
   const bool wide = (e - s) > WIDE_N;
@@ -215,11 +220,29 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
     if (wide) { accl0[c] = 0; accl1[c] = 0; }
   }
   float fm = 0.0f;
-  for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
-    const float2 f = __ldg(F + __ldg(list + k));
-    fm = fmaxf(fm, fmaxf(fabsf(f.x), fabsf(f.y)));
+  if (tile_fmax) {
+    // max |F| over the beads owned by this tile and its 8 neighbours (every listed bead whose
+    // support overlaps the tile is owned by one of them), left by K1: no pass over the list
+    if (threadIdx.x < 32) {
+      const int ntx = nx / TS, nty = ny / TS;
+      const int tx = t % ntx, ty = t / ntx;
+      if (threadIdx.x < 9) {
+        const int dx = (int)threadIdx.x % 3 - 1, dy = (int)threadIdx.x / 3 - 1;
+        fm = __uint_as_float(tile_fmax[wrap1(ty + dy, nty) * ntx + wrap1(tx + dx, ntx)]);
+      }
+#pragma unroll
+      for (int o = 8; o > 0; o >>= 1) fm = fmaxf(fm, __shfl_xor_sync(0xffffffffu, fm, o));
+      if (threadIdx.x == 0) red[0] = fm;
+    }
+    __syncthreads();  // also orders the zeroing before the atomics
+    fm = red[0];
+  } else {
+    for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
+      const float2 f = __ldg(F + __ldg(list + k));
+      fm = fmaxf(fm, fmaxf(fabsf(f.x), fabsf(f.y)));
+    }
+    fm = block_max(fm, red);  // also orders the zeroing before the atomics
   }
-  fm = block_max(fm, red);  // also orders the zeroing before the atomics
   const float sum_w = (rho_max > 0.0f) ? 1.0625f * rho_max : fmaxf(0.25f * (float)(e - s), 1.0f);
   const float scale = pow2_scale(fmaxf(fm * sum_w, 1e-18f));
   if (wide) spread_loop_wide(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
@@ -234,6 +257,7 @@ __global__ void __launch_bounds__(256) k_spread_tile(int nx, int ny, const int* 
                                                      const float2* __restrict__ X,
                                                      const float2* __restrict__ F,
                                                      const float* __restrict__ tile_rho_max,
+                                                     const unsigned* __restrict__ tile_fmax,
                                                      float* __restrict__ G0, float* __restrict__ G1) {
   __shared__ int acc0[TS * TSP], acc1[TS * TSP], accl0[TS * TSP], accl1[TS * TSP];
   __shared__ float red[32];
@@ -242,8 +266,8 @@ __global__ void __launch_bounds__(256) k_spread_tile(int nx, int ny, const int* 
   const int s = tile_start[t], e = tile_start[t + 1];
   float linv;
   const float scale = spread_tile_accumulate(nx, ny, x0, y0, s, e, list, X, F,
-                                             tile_rho_max ? tile_rho_max[t] : 0.0f, acc0, acc1, accl0, accl1,
-                                             red, linv);
+                                             tile_rho_max ? tile_rho_max[t] : 0.0f, tile_fmax, t, acc0, acc1,
+                                             accl0, accl1, red, linv);
   const float inv = 1.0f / scale;
   for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) {
     const size_t g = (size_t)(y0 + (c >> 5)) * nx + x0 + (c & 31);

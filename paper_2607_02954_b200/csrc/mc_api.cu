@@ -27,7 +27,7 @@ constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
-  size_t fA, fB, u, rho_b, A, G, cfield, csum, As, tile_count, tile_start, tile_cursor, tile_rho_max;
+  size_t fA, fB, u, rho_b, A, G, cfield, csum, As, tile_count, tile_start, tile_cursor, tile_rho_max, tile_fmax;
   size_t X, PA, PB, PC, F, sense, list, src, bflags, scratch, flags, sources;
   size_t total;
 };
@@ -88,6 +88,7 @@ Layout make_layout(const mc_world_params* p, const Derived& d) {
   L.tile_start = take((nt + 1) * 4);
   L.tile_cursor = take(nt * 4);
   L.tile_rho_max = take(nt * 4);
+  L.tile_fmax = take(nt * 4);
   L.X = take(N * 8);
   L.PA = take(N * 16);
   L.PB = take(N * 16);
@@ -193,6 +194,7 @@ int enqueue_step(mc_world* w) {
   int* tile_start = w->ptr<int>(w->L.tile_start);
   int* tile_cursor = w->ptr<int>(w->L.tile_cursor);
   float* tile_rho_max = w->ptr<float>(w->L.tile_rho_max);
+  unsigned* tile_fmax = w->d.n_density ? w->ptr<unsigned>(w->L.tile_fmax) : nullptr;
   int* list = w->ptr<int>(w->L.list);
   float* rho_b = w->ptr<float>(w->L.rho_b);
   float* G0 = w->ptr<float>(w->L.G);
@@ -216,7 +218,7 @@ int enqueue_step(mc_world* w) {
     prof_mark(w, 1);
     // K2a: S2 deposit
     if (w->d.n_density) {
-      mc::k_deposit_tile<<<n_tiles, 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max);
+      mc::k_deposit_tile<<<n_tiles, 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax);
       w->launches++;
       prof_mark(w, 2);
       // K3a: S3 filter + gradient -> force-gradient planes A
@@ -239,6 +241,7 @@ int enqueue_step(mc_world* w) {
     fa.sense = w->ptr<float>(w->L.sense);
     fa.A = w->d.n_density ? w->ptr<float2>(w->L.A) : (w->d.n_static ? w->ptr<float2>(w->L.As) : nullptr);
     fa.csum = w->d.n_static ? w->ptr<float>(w->L.csum) : nullptr;
+    fa.tile_fmax = tile_fmax;
     fa.N = N;
     fa.nx = nx;
     fa.ny = ny;
@@ -279,6 +282,7 @@ int enqueue_step(mc_world* w) {
     ls.X = X;
     ls.F = F;
     ls.tile_rho_max = w->d.n_density ? tile_rho_max : nullptr;
+    ls.tile_fmax = tile_fmax;
     if (w->keep_G) mc::k_lbm_spread_tile<true><<<n_tiles, 256, 0, st>>>(ls);
     else mc::k_lbm_spread_tile<false><<<n_tiles, 256, 0, st>>>(ls);
   } else {

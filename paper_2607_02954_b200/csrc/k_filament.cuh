@@ -45,7 +45,7 @@ struct FilamentArgs {
   int stride;        // 64 (aligned windows) or 60 (overlapping windows)
   int n_windows;
   float kappa;       // k_el * dt^2
-  double n_step;     // step index n (before the increment)
+  const long long* step;  // DEVICE: step index n (before the increment); K4 increments it
 };
 
 struct BeadParams {
@@ -108,7 +108,7 @@ __device__ __forceinline__ float2 edge_delta(double vx, double vy, float delta, 
   return make_float2(0.5f * p.kst * fmaf(ksL, ex, dl * tx), 0.5f * p.kst * fmaf(ksL, ey, dl * ty));
 }
 
-__global__ void __launch_bounds__(256) k_filament_force(FilamentArgs a) {
+__global__ void __launch_bounds__(256, 5) k_filament_force(FilamentArgs a) {
   const int lane = threadIdx.x & 31;
   const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (w >= a.n_windows) return;
@@ -138,8 +138,9 @@ __global__ void __launch_bounds__(256) k_filament_force(FilamentArgs a) {
   const bool edgeB = !(pB.flags & BEAD_LAST) && lane < 31;
   const bool jointA = !(pA.flags & (BEAD_FIRST | BEAD_LAST)) && lane >= 1;
   const bool jointB = !(pB.flags & (BEAD_FIRST | BEAD_LAST)) && lane < 31;
-  const float hA = jointA ? half_kC(ePx, ePy, eAx, eAy, pA, a.n_step) : 0.0f;
-  const float hB = jointB ? half_kC(eAx, eAy, eBx, eBy, pB, a.n_step) : 0.0f;
+  const double n_step = (double)*a.step;
+  const float hA = jointA ? half_kC(ePx, ePy, eAx, eAy, pA, n_step) : 0.0f;
+  const float hB = jointB ? half_kC(eAx, eAy, eBx, eBy, pB, n_step) : 0.0f;
   // Eq. 1 on an edge: theta_1 of its far joint (+), theta_2 of its near joint (-)
   const float hA_next = __shfl_down_sync(FULL, hA, 1);
   float2 dA = make_float2(0.f, 0.f), dB = make_float2(0.f, 0.f);

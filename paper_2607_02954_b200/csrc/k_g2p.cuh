@@ -9,8 +9,9 @@ namespace mc {
 
 __global__ void __launch_bounds__(256) k_interp_integrate(int N, float2* __restrict__ X,
                                                           const float2* __restrict__ u, int nx, int ny,
-                                                          int* __restrict__ flag) {
+                                                          int* __restrict__ flag, long long* __restrict__ step) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b == 0) *step += 1;  // device copy of the step counter (K1 of the next step reads it)
   if (b >= N) return;
   float2 p = X[b];
   const float2 U = interp2(u, nx, ny, p.x, p.y);

@@ -248,7 +248,7 @@ int enqueue_step(mc_world* w) {
     fa.stride = w->stride;
     fa.n_windows = w->n_windows;
     fa.kappa = w->kappa;
-    fa.n_step = (double)w->step;
+    fa.step = w->ptr<long long>(w->L.flags) + 4;  // flags[8..9]: device copy of the step counter
     mc::k_filament_force<<<(w->n_windows + 7) / 8, 256, 0, st>>>(fa);
     prof_mark(w, 4);
     w->launches++;
@@ -294,7 +294,7 @@ int enqueue_step(mc_world* w) {
   prof_mark(w, 6);
   // K4: S7
   if (beads) {
-    mc::k_interp_integrate<<<bgrid, bt, 0, st>>>(N, X, la.u, nx, ny, flag);
+    mc::k_interp_integrate<<<bgrid, bt, 0, st>>>(N, X, la.u, nx, ny, flag, w->ptr<long long>(w->L.flags) + 4);
     w->launches++;
   }
   prof_mark(w, 7);
@@ -517,6 +517,8 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   w->launches++;
   cudaMemsetAsync(w->ptr<float>(w->L.F), 0, (size_t)N * 8, st);
   cudaMemsetAsync(w->ptr<float>(w->L.sense), 0, (size_t)N * 4, st);
+  const long long host_step = w->step;  // steps without beads do not advance the device copy
+  cudaMemcpyAsync(w->ptr<long long>(w->L.flags) + 4, &host_step, 8, cudaMemcpyHostToDevice, st);
   int h = 0;
   cudaMemcpyAsync(&h, bad, 4, cudaMemcpyDeviceToHost, st);
   e = cudaStreamSynchronize(st);  // src/bflags are host vectors of this call

@@ -232,9 +232,9 @@ def main():
     l0 = G.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
-    e0.record()
+    e0.record(G.stream)   # events on the stream the kernels are launched on (the world's own)
     G.step(args.steps)
-    e1.record()
+    e1.record(G.stream)
     barrier()
     ms = torch.tensor([e0.elapsed_time(e1)], device=dev, dtype=torch.float64)
     launches = G.launch_count() - l0

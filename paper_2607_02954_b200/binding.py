@@ -134,7 +134,8 @@ class World:
         self.n_fields = len(self.p["fields"])
         self.h = None
         with torch.cuda.device(self.device):
-            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            # a stream of its own: the legacy default stream cannot be captured into CUDA graphs
+            self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
             wp, keep = make_params(self.p)
             nbytes = int(L.mc_workspace_bytes(C.byref(wp)))
             if nbytes == 0:

@@ -122,6 +122,11 @@ struct mc_world {
   int stride = 60;   // K1 window advance: 64 when all chains share a length dividing 64
   int n_windows = 0;
   int list_age = 0;  // steps since the tile lists were built (rebuilt when 0)
+  // CUDA graphs of GRAPH_STEPS consecutive steps, one per ping-pong phase, captured on first use
+  // when the tile lists are due (list_age == 0); GRAPH_STEPS is a multiple of LIST_STEPS and of 2
+  cudaGraphExec_t graph[2] = {nullptr, nullptr};
+  int64_t graph_launches[2] = {0, 0};
+  bool graph_off = false;  // the stream cannot be captured (e.g. the legacy default stream): direct launches
   std::vector<int32_t> loaded_offsets;  // offsets of the last load: same chains => keep the internal order
   float rho0 = 1, omega_p = 1, omega_m = 1, kappa = 0;
   float coef[4] = {0, 0, 0, 0};  // lattice coupling with the sign of the force
@@ -155,6 +160,13 @@ int check_cuda(mc_world* w, const char* what) {
 }
 
 constexpr int PROF_MAX_STEPS = 64;
+constexpr int GRAPH_STEPS = 4;
+static_assert(GRAPH_STEPS % mc::LIST_STEPS == 0 && GRAPH_STEPS % 2 == 0, "graph period");
+
+void drop_graphs(mc_world* w) {
+  for (int k = 0; k < 2; ++k)
+    if (w->graph[k]) { cudaGraphExecDestroy(w->graph[k]); w->graph[k] = nullptr; }
+}
 
 inline void prof_mark(mc_world* w, int boundary) {
   if (w->prof_on && w->prof_steps < PROF_MAX_STEPS)
@@ -322,6 +334,7 @@ int64_t mc_launch_count(const mc_world* w) { return w ? w->launches : 0; }
 void mc_destroy(mc_world* w) {
   if (!w) return;
   for (cudaEvent_t e : w->prof_ev) cudaEventDestroy(e);
+  drop_graphs(w);
   delete w;
 }
 
@@ -456,6 +469,7 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   const bool reuse_order = w->N == N && w->n_fil == n_fil && (int64_t)w->loaded_offsets.size() == n_fil + 1 &&
                            std::equal(w->loaded_offsets.begin(), w->loaded_offsets.end(), offsets);
   const int prev_stride = w->stride, prev_windows = w->n_windows;
+  drop_graphs(w);
   w->N = 0;
   w->n_fil = 0;
   w->n_windows = 0;
@@ -547,9 +561,39 @@ int mc_step(mc_world* w, int32_t n) {
   if (!w) return MC_EINVAL;
   if (n < 0) return fail(w, MC_EINVAL, "n < 0");
   if (w->diverged) return fail(w, MC_EDIVERGED, "world diverged (non-finite bead or |u| > 0.3)");
-  for (int32_t s = 0; s < n; ++s) {
+  int32_t done = 0;
+  while (done < n) {
+    // Blocks of GRAPH_STEPS steps that start where the tile lists are due replay a captured CUDA
+    // graph (same kernels, same order, same arguments: results are bit-identical to direct
+    // launches); small worlds are bound by launch overhead, not by the kernels.
+    if (!w->prof_on && !w->graph_off && w->list_age == 0 && n - done >= GRAPH_STEPS) {
+      const int ph = w->cur;
+      if (!w->graph[ph]) {
+        cudaGraph_t g = nullptr;
+        const int64_t l0 = w->launches;
+        if (w->stream == nullptr ||
+            cudaStreamBeginCapture(w->stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+          cudaGetLastError();  // not an error of the world: this stream just cannot be captured
+          w->graph_off = true;
+          continue;
+        }
+        for (int s = 0; s < GRAPH_STEPS; ++s) enqueue_step(w);  // advances the host-side state
+        cudaError_t e = cudaStreamEndCapture(w->stream, &g);
+        if (e == cudaSuccess) e = cudaGraphInstantiate(&w->graph[ph], g, 0);
+        if (g) cudaGraphDestroy(g);
+        if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
+        w->graph_launches[ph] = w->launches - l0;
+      } else {
+        w->step += GRAPH_STEPS;  // cur and list_age return to their values after GRAPH_STEPS steps
+        w->launches += w->graph_launches[ph];
+      }
+      if (cudaGraphLaunch(w->graph[ph], w->stream) != cudaSuccess) return fail(w, MC_ECUDA, "cudaGraphLaunch failed");
+      done += GRAPH_STEPS;
+      continue;
+    }
     int rc = enqueue_step(w);
     if (rc != MC_OK) return rc;
+    ++done;
   }
   return check_cuda(w, "mc_step");
 }
@@ -611,6 +655,7 @@ int mc_read_state(mc_world* w, int64_t* step_out, float* xy, float* u, float* rh
 
 int mc_keep_intermediates(mc_world* w, int32_t on) {
   if (!w) return MC_EINVAL;
+  if (w->keep_G != (on != 0)) drop_graphs(w);
   w->keep_G = on != 0;
   return MC_OK;
 }

@@ -168,16 +168,22 @@ def test_bitwise_reproducible(name):
 
 
 def test_step_batching_is_equivalent():
-    # mc_step(10) == 10 x mc_step(1), bit for bit
+    # mc_step(23) (CUDA-graph replay of 4-step blocks + direct launches) == 23 x mc_step(1)
+    # (direct launches only) == 3 + 20 split across calls, bit for bit
     from paper_2607_02954_b200 import binding
     w = SMALL["uniform_m32"]()
-    A, B = binding.World(w), binding.World(w)
-    A.step(10)
-    for _ in range(10):
+    A, B, C = binding.World(w), binding.World(w), binding.World(w)
+    A.step(23)
+    for _ in range(23):
         B.step(1)
+    C.step(3)
+    C.step(20)
+    c = C.read_state()
+    assert c["step"] == 23
     a, b = A.read_state(), B.read_state()
     for k in ("xy", "u", "fdev", "force"):
         assert a[k].tobytes() == b[k].tobytes(), k
+        assert a[k].tobytes() == c[k].tobytes(), k
 
 
 def test_empty_world_stays_at_rest():

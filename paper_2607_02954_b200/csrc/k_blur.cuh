@@ -107,13 +107,16 @@ __global__ void __launch_bounds__(256) k_blur_grad(int nx, int ny, BlurTaps taps
   }
   __syncthreads();
   for (int t = threadIdx.x; t < BLUR_T * BLUR_T; t += 256) {
-    const int y = t >> 5, x = (t & 31) + S;
+    // 16 consecutive threads own one 4x4 block of the blocked output: a warp stores two full lines
+    const int bl_id = t >> 4, n = t & 15;
+    const int y = ((bl_id >> 3) << 2) + (n >> 2), xo = ((bl_id & 7) << 2) + (n & 3), x = xo + S;
     const float gx = 0.5f * (bl[(y + 1) * TWP + x + 2] - bl[(y + 1) * TWP + x]);
     const float gy = 0.5f * (bl[(y + 2) * TWP + x + 1] - bl[y * TWP + x + 1]);
-    const size_t gidx = (size_t)(j0 + y) * nx + (i0 + (t & 31));
+    const size_t gidx = (size_t)(j0 + y) * nx + (i0 + xo);
     float2 a = make_float2(coef * gx, coef * gy);
-    if (base) { const float2 b = base[gidx]; a.x += b.x; a.y += b.y; }
-    A[gidx] = a;
+    const size_t bidx = blk_index(i0 + xo, j0 + y, nx);  // A and base are blocked (mc_common.cuh)
+    if (base) { const float2 b = base[bidx]; a.x += b.x; a.y += b.y; }
+    A[bidx] = a;
     if (field_out) field_out[gidx] = bl[(y + 1) * TWP + x + 1];
   }
 }
@@ -149,10 +152,11 @@ __global__ void k_static_init(int nx, int ny, int n_src, const float* __restrict
                            static_c(nx, ny, n_src, src, i, wrap1(j - 1, ny)));
   c_out[g] = (float)c;
   csum[g] += (float)c;
-  float2 a = As[g];
+  const size_t bg = blk_index(i, j, nx);  // blocked like A
+  float2 a = As[bg];
   a.x += (float)((double)coef * gx);
   a.y += (float)((double)coef * gy);
-  As[g] = a;
+  As[bg] = a;
 }
 
 }  // namespace mc

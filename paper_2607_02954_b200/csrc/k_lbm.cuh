@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(256) k_lbm_step(LbmArgs a) {
   if (a.G0) { Gx = __ldg(a.G0 + c); Gy = __ldg(a.G1 + c); }
   float ux, uy;
   trt_collide(g, Gx, Gy, a.rho0, a.omega_p, a.omega_m, ux, uy);
-  a.u[c] = make_float2(ux, uy);
+  a.u[blk_index(i, j, nx)] = make_float2(ux, uy);
 #pragma unroll
   for (int q = 0; q < 9; ++q) a.dst[q * nc + c] = g[q];
   if (!(fabsf(ux) <= 0.3f && fabsf(uy) <= 0.3f)) atomicOr(a.flag, 4);
@@ -163,7 +163,7 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
     if (KEEP_G) { a.G0out[c] = Gx; a.G1out[c] = Gy; }
     float ux, uy;
     trt_collide(g, Gx, Gy, a.rho0, a.omega_p, a.omega_m, ux, uy);
-    a.u[c] = make_float2(ux, uy);
+    a.u[blk_index(i, j, nx)] = make_float2(ux, uy);
 #pragma unroll
     for (int q = 0; q < 9; ++q) a.dst[q * nc + c] = g[q];
     bad = bad || !(fabsf(ux) <= 0.3f && fabsf(uy) <= 0.3f);
@@ -199,10 +199,13 @@ __global__ void k_lbm_export(const float* __restrict__ src, int nx, int ny, floa
   if (rho) rho[c] = rho0 + (g[0] + ((g[1] + g[3]) + (g[2] + g[4])) + ((g[5] + g[7]) + (g[6] + g[8])));
 }
 
-// mc_read_state: interleaved (x,y) field -> two planes
-__global__ void k_split2(size_t n, const float2* __restrict__ in, float* __restrict__ out0, float* __restrict__ out1) {
-  const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (c < n) { const float2 v = in[c]; out0[c] = v.x; out1[c] = v.y; }
+// mc_read_state: blocked interleaved (x,y) field -> two row-major planes
+__global__ void k_split2(int nx, int ny, const float2* __restrict__ in, float* __restrict__ out0, float* __restrict__ out1) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+  if (i >= nx) return;
+  const float2 v = in[blk_index(i, j, nx)];
+  out0[(size_t)j * nx + i] = v.x;
+  out1[(size_t)j * nx + i] = v.y;
 }
 
 }  // namespace mc

@@ -612,7 +612,10 @@ int mc_read_state(mc_world* w, int64_t* step_out, float* xy, float* u, float* rh
     w->launches++;
   }
   if (u) {
-    mc::k_split2<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(nc, w->ptr<float2>(w->L.u), u, u + nc);
+    {
+      const int bx = pick_bx(w->nx);
+      mc::k_split2<<<dim3(w->nx / bx, w->ny), bx, 0, st>>>(w->nx, w->ny, w->ptr<float2>(w->L.u), u, u + nc);
+    }
     w->launches++;
   }
   if (rho || fdev) {

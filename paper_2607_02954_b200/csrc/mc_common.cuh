@@ -39,6 +39,14 @@ __device__ __forceinline__ void support(float x, int& i0, float& fr) {
   i0 = (int)fl - 1;
 }
 
+// The two gathered fields (velocity u, force-gradient field A) are stored BLOCKED: 4x4 nodes of
+// float2 = one 128-byte line.  Consecutive beads of a chain are ~1 node apart in an arbitrary
+// direction; in a row-major field every lane of a gather instruction then sits on its own line
+// (vertical chains), while 4x4 blocks are shared by ~4 consecutive beads whatever the direction.
+__device__ __forceinline__ size_t blk_index(int i, int j, int nx) {
+  return ((size_t)(j >> 2) * (nx >> 2) + (i >> 2)) * 16 + ((j & 3) << 2) + (i & 3);
+}
+
 // Interpolate an interleaved two-component field at (x,y): sum over the 4x4 support of
 // field(g) * delta_h(g - X)  ("nodes sample the local fluid velocity"; also S4's
 // gradient sampling).  One 8-byte load per support node.
@@ -51,14 +59,18 @@ __device__ __forceinline__ float2 interp2(const float2* __restrict__ p, int nx, 
   peskin4(fy, wy[0], wy[1], wy[2], wy[3]);
   i0 = wrapi(i0, nx);
   j0 = wrapi(j0, ny);
-  int col[4];
+  int col[4];  // column part of the blocked index
 #pragma unroll
-  for (int k = 0; k < 4; ++k) col[k] = (i0 + k >= nx) ? i0 + k - nx : i0 + k;
+  for (int k = 0; k < 4; ++k) {
+    const int c = (i0 + k >= nx) ? i0 + k - nx : i0 + k;
+    col[k] = ((c >> 2) << 4) + (c & 3);
+  }
+  const int nbx = nx >> 2;
   float ax = 0.0f, ay = 0.0f;
 #pragma unroll
   for (int l = 0; l < 4; ++l) {
     const int row = (j0 + l >= ny) ? j0 + l - ny : j0 + l;
-    const float2* r = p + (size_t)row * nx;
+    const float2* r = p + ((size_t)(row >> 2) * nbx * 16 + ((row & 3) << 2));
     float sx = 0.0f, sy = 0.0f;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {

@@ -41,6 +41,23 @@ struct TileBead {
   float wx[4], wy[4];    // 0 where the support node lies outside the tile
 };
 
+// distance (in nodes, periodic) from the tile origin to the first support node, in [-n/2, n/2)
+__device__ __forceinline__ int tile_delta(int i0, int origin, int n) {
+  int d = i0 - origin;
+  const int h = n >> 1;
+  if ((unsigned)(d + h + n) < (unsigned)(3 * n)) {  // within one period of the window: common case
+    if (d >= h) d -= n;
+    else if (d < -h) d += n;
+  } else {
+    d = wrapi(d + h, n) - h;
+  }
+  return d;
+}
+
+// WRAP_IN_TILE: the domain is a single tile wide along some axis, so a support can wrap around
+// onto the SAME tile; then every node is folded individually.  Otherwise one periodic fold of the
+// first support node is enough and the other three follow by +1.
+template <bool WRAP_IN_TILE>
 __device__ __forceinline__ void tile_bead(float2 p, int nx, int ny, int x0, int y0, TileBead& tb) {
   int i0, j0;
   float fx, fy;
@@ -48,12 +65,23 @@ __device__ __forceinline__ void tile_bead(float2 p, int nx, int ny, int x0, int 
   support(p.y, j0, fy);
   peskin4(fx, tb.wx[0], tb.wx[1], tb.wx[2], tb.wx[3]);
   peskin4(fy, tb.wy[0], tb.wy[1], tb.wy[2], tb.wy[3]);
-  i0 = wrapi(i0, nx);
-  j0 = wrapi(j0, ny);
+  if (WRAP_IN_TILE) {
+    i0 = wrapi(i0, nx);
+    j0 = wrapi(j0, ny);
+  } else {
+    i0 = tile_delta(i0, x0, nx);
+    j0 = tile_delta(j0, y0, ny);
+  }
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
-    const int c = ((i0 + k >= nx) ? i0 + k - nx : i0 + k) - x0;
-    const int r = ((j0 + k >= ny) ? j0 + k - ny : j0 + k) - y0;
+    int c, r;
+    if (WRAP_IN_TILE) {
+      c = ((i0 + k >= nx) ? i0 + k - nx : i0 + k) - x0;
+      r = ((j0 + k >= ny) ? j0 + k - ny : j0 + k) - y0;
+    } else {
+      c = i0 + k;
+      r = j0 + k;
+    }
     const bool cin = (unsigned)c < (unsigned)TS, rin = (unsigned)r < (unsigned)TS;
     tb.col[k] = cin ? c : 0;
     tb.row[k] = rin ? r * TSP : 0;
@@ -92,13 +120,13 @@ __device__ __forceinline__ int lo_bits(int n) {
   return min(20, max(0, 30 - lg));
 }
 
-template <bool WIDE>
+template <bool WIDE, bool WRAP>
 __device__ __forceinline__ void deposit_loop(int nx, int ny, int x0, int y0, int s, int e,
                                              const int* __restrict__ list, const float2* __restrict__ X,
                                              float scale, float lscale, int* acc, int* accl) {
   for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
     TileBead tb;
-    tile_bead(__ldg(X + __ldg(list + k)), nx, ny, x0, y0, tb);
+    tile_bead<WRAP>(__ldg(X + __ldg(list + k)), nx, ny, x0, y0, tb);
 #pragma unroll
     for (int l = 0; l < 4; ++l) {
       const float wys = tb.wy[l] * scale;
@@ -118,7 +146,7 @@ __device__ __forceinline__ void deposit_loop(int nx, int ny, int x0, int y0, int
   }
 }
 
-template <bool WIDE>
+template <bool WIDE, bool WRAP>
 __device__ __forceinline__ void spread_loop(int nx, int ny, int x0, int y0, int s, int e,
                                             const int* __restrict__ list, const float2* __restrict__ X,
                                             const float2* __restrict__ F, float scale, float lscale,
@@ -126,7 +154,7 @@ __device__ __forceinline__ void spread_loop(int nx, int ny, int x0, int y0, int 
   for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
     const int b = __ldg(list + k);
     TileBead tb;
-    tile_bead(__ldg(X + b), nx, ny, x0, y0, tb);
+    tile_bead<WRAP>(__ldg(X + b), nx, ny, x0, y0, tb);
     const float2 f = __ldg(F + b);
     const float fxs = f.x * scale, fys = f.y * scale;
 #pragma unroll
@@ -155,12 +183,12 @@ __device__ __forceinline__ void spread_loop(int nx, int ny, int x0, int y0, int 
 // against the occupancy of the common path
 __device__ __noinline__ void deposit_loop_wide(int nx, int ny, int x0, int y0, int s, int e, const int* list,
                                                const float2* X, float scale, float lscale, int* acc, int* accl) {
-  deposit_loop<true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
+  deposit_loop<true, true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
 }
 __device__ __noinline__ void spread_loop_wide(int nx, int ny, int x0, int y0, int s, int e, const int* list,
                                               const float2* X, const float2* F, float scale, float lscale,
                                               int* acc0, int* acc1, int* accl0, int* accl1) {
-  spread_loop<true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
+  spread_loop<true, true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
 }
 
 // K2a: S2 deposit.  tile_rho_max[t] receives max over the tile of rho_b (for K2b's scale).
@@ -181,7 +209,8 @@ __global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int*
   const float lscale = ldexpf(1.0f, lo_bits(e - s));
   __syncthreads();
   if (wide) deposit_loop_wide(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
-  else deposit_loop<false>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
+  else if (nx == TS || ny == TS) deposit_loop<false, true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
+  else deposit_loop<false, false>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
   __syncthreads();
   const float inv = 1.0f / scale, linv = 1.0f / lscale;
   float mx = 0.0f;
@@ -246,7 +275,8 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
   const float sum_w = (rho_max > 0.0f) ? 1.0625f * rho_max : fmaxf(0.25f * (float)(e - s), 1.0f);
   const float scale = pow2_scale(fmaxf(fm * sum_w, 1e-18f));
   if (wide) spread_loop_wide(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
-  else spread_loop<false>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
+  else if (nx == TS || ny == TS) spread_loop<false, true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
+  else spread_loop<false, false>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
   __syncthreads();
   return scale;
 }

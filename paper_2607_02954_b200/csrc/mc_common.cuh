@@ -24,10 +24,19 @@ __device__ __forceinline__ int wrapi(int i, int n) {
 // phi(r) = (3 - 2|r| + sqrt(1 + 4|r| - 4r^2))/8; the outer two follow from the kernel's
 // even/odd sum rule (w0 + w2 = w1 + w3 = 1/2), which is exact for phi and avoids the
 // cancellation in the outer branch's radicand.
+// sqrt.approx (one MUFU, relative error ~1e-7, radicand in [1,2]) instead of the IEEE-rounded
+// sqrtf (MUFU.RSQ + Newton + a slow-path call, ~10 instructions): four of them per bead in each
+// of the four bead-grid kernels.
+__device__ __forceinline__ float sqrt_fast(float v) {
+  float r;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(v));
+  return r;
+}
+
 __device__ __forceinline__ void peskin4(float fr, float& w0, float& w1, float& w2, float& w3) {
   const float a1 = fr, a2 = 1.0f - fr;
-  w1 = 0.125f * (3.0f - 2.0f * a1 + sqrtf(fmaf(4.0f * a1, a2, 1.0f)));  // 1+4a-4a^2 = 1+4a(1-a)
-  w2 = 0.125f * (3.0f - 2.0f * a2 + sqrtf(fmaf(4.0f * a2, a1, 1.0f)));
+  w1 = 0.125f * (3.0f - 2.0f * a1 + sqrt_fast(fmaf(4.0f * a1, a2, 1.0f)));  // 1+4a-4a^2 = 1+4a(1-a)
+  w2 = 0.125f * (3.0f - 2.0f * a2 + sqrt_fast(fmaf(4.0f * a2, a1, 1.0f)));
   w0 = 0.5f - w2;
   w3 = 0.5f - w1;
 }

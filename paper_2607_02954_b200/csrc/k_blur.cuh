@@ -56,7 +56,9 @@ __global__ void __launch_bounds__(256) k_blur_grad(int nx, int ny, BlurTaps taps
   constexpr int NV = 4 + 2 * R, NV4 = (NV + 3) / 4, HP4 = HP / 4;
   float* in = sm;                    // [H][HP]    in[y][x]  <-> node (j0-R-1+y, i0-P+x)
   float* tmp = sm + (size_t)H * HP;  // [H+4][TWP] tmp[y][t] <-> node (j0-R-1+y, i0-1-S+t)
-  const int i0 = blockIdx.x * BLUR_T, j0 = blockIdx.y * BLUR_T;
+  // 1-D grid in row-major tile order (2-D grids are rasterised in an order that streams worse)
+  const int ntx = nx / BLUR_T;
+  const int i0 = (blockIdx.x % ntx) * BLUR_T, j0 = (blockIdx.x / ntx) * BLUR_T;
   float g[2 * R + 1];
 #pragma unroll
   for (int k = 0; k <= 2 * R; ++k) g[k] = taps.g[k];

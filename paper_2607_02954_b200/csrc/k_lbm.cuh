@@ -110,7 +110,7 @@ struct LbmSpreadArgs {
   const int* list;
   const float2* X;
   const float2* F;
-  const float* tile_rho_max;  // may be NULL
+  float* tile_rho_max;        // may be NULL; read, then reset to 0 for the next step's S2 (atomicMax)
   const unsigned* tile_fmax;  // may be NULL
 };
 
@@ -120,6 +120,8 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
   __shared__ float red[32];
   const LbmArgs& a = p.lbm;
   const int nx = a.nx, ny = a.ny;
+  // 1-D grid in row-major tile order (a 2-D grid is rasterised differently by the hardware and
+  // cost the streaming phase 20 % on world 4d)
   const int t = blockIdx.x, ntx = nx / TS;
   const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
   const int s = p.tile_start[t], e = p.tile_start[t + 1];
@@ -138,6 +140,7 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
                                              p.tile_rho_max ? p.tile_rho_max[t] : 0.0f, p.tile_fmax, t, acc0, acc1,
                                              accl0, accl1, red, linv);
   const float inv = 1.0f / scale;
+  if (threadIdx.x == 0 && p.tile_rho_max) p.tile_rho_max[t] = 0.0f;  // all reads happened before the barrier
   const size_t nc = (size_t)nx * ny;
   const int lx = threadIdx.x & 31;
   const int i = x0 + lx;

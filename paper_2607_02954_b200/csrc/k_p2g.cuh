@@ -200,8 +200,8 @@ __global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int*
                                                       unsigned* __restrict__ tile_fmax) {
   __shared__ int acc[TS * TSP], accl[TS * TSP];
   __shared__ float red[32];
-  const int t = blockIdx.x, ntx = nx / TS;
-  const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
+  const int t = blockIdx.y * gridDim.x + blockIdx.x;  // grid = (nx/TS, ny/TS)
+  const int x0 = blockIdx.x * TS, y0 = blockIdx.y * TS;
   const int s = tile_start[t], e = tile_start[t + 1];
   const bool wide = (e - s) > WIDE_N;
   for (int c = threadIdx.x; c < TS * TSP; c += blockDim.x) { acc[c] = 0; if (wide) accl[c] = 0; }
@@ -220,11 +220,12 @@ __global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int*
     rho_b[(size_t)(y0 + (c >> 5)) * nx + x0 + (c & 31)] = v;
     mx = fmaxf(mx, v);
   }
-  mx = block_max(mx, red);
-  if (threadIdx.x == 0) {
-    tile_rho_max[t] = mx;
-    tile_fmax[t] = 0u;  // K1 of this step raises it (atomicMax), K2b reads it
-  }
+  // tile maximum: rho_b >= 0, so the float bits order like unsigned integers; one global
+  // atomicMax per warp onto tile_rho_max[t] (zeroed by the tile-list scan of this step)
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<unsigned*>(tile_rho_max) + t, __float_as_uint(mx));
+  if (threadIdx.x == 0) tile_fmax[t] = 0u;  // K1 of this step raises it (atomicMax), K2b reads it
 }
 
 // accumulator -> float (before the 1/scale): hi word, plus the lo word in wide tiles (linv != 0)
@@ -233,7 +234,7 @@ __device__ __forceinline__ float tile_value(const int* acc, const int* accl, int
 }
 
 // Accumulate the spread force of one tile into shared memory (two planes), return the scale.
-// Shared by the stand-alone spread kernel and by the fused spread + fluid kernel (k_lbm.cuh).
+// Used by the fused spread + fluid kernel (k_lbm.cuh).
 __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, int y0, int s, int e,
                                                         const int* __restrict__ list,
                                                         const float2* __restrict__ X,
@@ -279,31 +280,6 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
   else spread_loop<false, false>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
   __syncthreads();
   return scale;
-}
-
-// K2b: S5 spread (stand-alone form; the hot path uses the fused spread + fluid kernel)
-__global__ void __launch_bounds__(256) k_spread_tile(int nx, int ny, const int* __restrict__ tile_start,
-                                                     const int* __restrict__ list,
-                                                     const float2* __restrict__ X,
-                                                     const float2* __restrict__ F,
-                                                     const float* __restrict__ tile_rho_max,
-                                                     const unsigned* __restrict__ tile_fmax,
-                                                     float* __restrict__ G0, float* __restrict__ G1) {
-  __shared__ int acc0[TS * TSP], acc1[TS * TSP], accl0[TS * TSP], accl1[TS * TSP];
-  __shared__ float red[32];
-  const int t = blockIdx.x, ntx = nx / TS;
-  const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
-  const int s = tile_start[t], e = tile_start[t + 1];
-  float linv;
-  const float scale = spread_tile_accumulate(nx, ny, x0, y0, s, e, list, X, F,
-                                             tile_rho_max ? tile_rho_max[t] : 0.0f, tile_fmax, t, acc0, acc1,
-                                             accl0, accl1, red, linv);
-  const float inv = 1.0f / scale;
-  for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) {
-    const size_t g = (size_t)(y0 + (c >> 5)) * nx + x0 + (c & 31);
-    G0[g] = tile_value(acc0, accl0, (c >> 5) * TSP + (c & 31), linv) * inv;
-    G1[g] = tile_value(acc1, accl1, (c >> 5) * TSP + (c & 31), linv) * inv;
-  }
 }
 
 }  // namespace mc

@@ -177,7 +177,7 @@ int pick_bx(int nx) { return nx % 256 == 0 ? 256 : (nx % 128 == 0 ? 128 : (nx % 
 
 template <int R>
 void launch_blur_R(mc_world* w, int k, const float2* base, float2* A, float* field_out) {
-  dim3 grid(w->nx / mc::BLUR_T, w->ny / mc::BLUR_T);
+  const int grid = (w->nx / mc::BLUR_T) * (w->ny / mc::BLUR_T);
   mc::k_blur_grad<R><<<grid, 256, mc::blur_smem_bytes(R), w->stream>>>(
       w->nx, w->ny, w->taps[k], w->ptr<float>(w->L.rho_b), w->coef[k], base, A, field_out);
 }
@@ -213,6 +213,7 @@ int enqueue_step(mc_world* w) {
   float* G1 = G0 + w->nc;
   int* flag = w->ptr<int>(w->L.flags);
   const int n_tiles = (nx / mc::TS) * (ny / mc::TS);
+  const dim3 tgrid(nx / mc::TS, ny / mc::TS);
   const int bt = 256;
   const int bgrid = (N + bt - 1) / bt;
   const bool beads = N > 0;
@@ -230,7 +231,7 @@ int enqueue_step(mc_world* w) {
     prof_mark(w, 1);
     // K2a: S2 deposit
     if (w->d.n_density) {
-      mc::k_deposit_tile<<<n_tiles, 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax);
+      mc::k_deposit_tile<<<tgrid, 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax);
       w->launches++;
       prof_mark(w, 2);
       // K3a: S3 filter + gradient -> force-gradient planes A

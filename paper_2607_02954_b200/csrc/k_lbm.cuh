@@ -141,35 +141,49 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
                                              accl0, accl1, red, linv);
   const float inv = 1.0f / scale;
   if (threadIdx.x == 0 && p.tile_rho_max) p.tile_rho_max[t] = 0.0f;  // all reads happened before the barrier
+  // S6 on the tile: each thread owns the node PAIR (i, i+1), i even, in rows ry and ry + 16.
+  // Two nodes per thread halve the address arithmetic and turn the unshifted planes, all nine
+  // stores and the blocked u store into 8/16-byte accesses: the kernel is bound by issue slots
+  // (5.8e8 warp instructions per launch on world 4d), not by DRAM.
   const size_t nc = (size_t)nx * ny;
-  const int lx = threadIdx.x & 31;
+  const int lx = (threadIdx.x & 15) << 1, ry = threadIdx.x >> 4;
   const int i = x0 + lx;
-  const int im = (i == 0) ? nx - 1 : i - 1, ip = (i == nx - 1) ? 0 : i + 1;
+  const int im = (i == 0) ? nx - 1 : i - 1, ip2 = (i + 2 == nx) ? 0 : i + 2;
   bool bad = false;
-  for (int ly = threadIdx.x >> 5; ly < TS; ly += 8) {
-    const int j = y0 + ly;
+#pragma unroll 1
+  for (int h = 0; h < 2; ++h) {
+    const int ly = ry + 16 * h, j = y0 + ly;
     const int jm = (j == 0) ? ny - 1 : j - 1, jp = (j == ny - 1) ? 0 : j + 1;
     const size_t r0 = (size_t)j * nx, rm = (size_t)jm * nx, rp = (size_t)jp * nx;
-    float g[9];
-    g[0] = __ldg(a.src + 0 * nc + r0 + i);
-    g[1] = __ldg(a.src + 1 * nc + r0 + im);
-    g[2] = __ldg(a.src + 2 * nc + rm + i);
-    g[3] = __ldg(a.src + 3 * nc + r0 + ip);
-    g[4] = __ldg(a.src + 4 * nc + rp + i);
-    g[5] = __ldg(a.src + 5 * nc + rm + im);
-    g[6] = __ldg(a.src + 6 * nc + rm + ip);
-    g[7] = __ldg(a.src + 7 * nc + rp + ip);
-    g[8] = __ldg(a.src + 8 * nc + rp + im);
+    float gA[9], gB[9];  // pre-collision populations of nodes i and i+1 (pull: g_q(x) = src_q(x - c_q))
+    {
+      const float2 v0 = __ldg(reinterpret_cast<const float2*>(a.src + 0 * nc + r0 + i));
+      const float2 v2 = __ldg(reinterpret_cast<const float2*>(a.src + 2 * nc + rm + i));
+      const float2 v4 = __ldg(reinterpret_cast<const float2*>(a.src + 4 * nc + rp + i));
+      gA[0] = v0.x; gB[0] = v0.y; gA[2] = v2.x; gB[2] = v2.y; gA[4] = v4.x; gB[4] = v4.y;
+      gA[1] = __ldg(a.src + 1 * nc + r0 + im);     gB[1] = __ldg(a.src + 1 * nc + r0 + i);
+      gA[3] = __ldg(a.src + 3 * nc + r0 + i + 1);  gB[3] = __ldg(a.src + 3 * nc + r0 + ip2);
+      gA[5] = __ldg(a.src + 5 * nc + rm + im);     gB[5] = __ldg(a.src + 5 * nc + rm + i);
+      gA[6] = __ldg(a.src + 6 * nc + rm + i + 1);  gB[6] = __ldg(a.src + 6 * nc + rm + ip2);
+      gA[7] = __ldg(a.src + 7 * nc + rp + i + 1);  gB[7] = __ldg(a.src + 7 * nc + rp + ip2);
+      gA[8] = __ldg(a.src + 8 * nc + rp + im);     gB[8] = __ldg(a.src + 8 * nc + rp + i);
+    }
     const size_t c = r0 + i;
-    const float Gx = tile_value(acc0, accl0, ly * TSP + lx, linv) * inv;
-    const float Gy = tile_value(acc1, accl1, ly * TSP + lx, linv) * inv;
-    if (KEEP_G) { a.G0out[c] = Gx; a.G1out[c] = Gy; }
-    float ux, uy;
-    trt_collide(g, Gx, Gy, a.rho0, a.omega_p, a.omega_m, ux, uy);
-    a.u[blk_index(i, j, nx)] = make_float2(ux, uy);
+    const int sa = ly * TSP + lx;
+    const float GAx = tile_value(acc0, accl0, sa, linv) * inv, GAy = tile_value(acc1, accl1, sa, linv) * inv;
+    const float GBx = tile_value(acc0, accl0, sa + 1, linv) * inv, GBy = tile_value(acc1, accl1, sa + 1, linv) * inv;
+    if (KEEP_G) {
+      *reinterpret_cast<float2*>(a.G0out + c) = make_float2(GAx, GBx);
+      *reinterpret_cast<float2*>(a.G1out + c) = make_float2(GAy, GBy);
+    }
+    float uAx, uAy, uBx, uBy;
+    trt_collide(gA, GAx, GAy, a.rho0, a.omega_p, a.omega_m, uAx, uAy);
+    trt_collide(gB, GBx, GBy, a.rho0, a.omega_p, a.omega_m, uBx, uBy);
+    // blocked u: nodes i and i+1 (i even) are neighbours inside one 4x4 block
+    *reinterpret_cast<float4*>(a.u + blk_index(i, j, nx)) = make_float4(uAx, uAy, uBx, uBy);
 #pragma unroll
-    for (int q = 0; q < 9; ++q) a.dst[q * nc + c] = g[q];
-    bad = bad || !(fabsf(ux) <= 0.3f && fabsf(uy) <= 0.3f);
+    for (int q = 0; q < 9; ++q) *reinterpret_cast<float2*>(a.dst + q * nc + c) = make_float2(gA[q], gB[q]);
+    bad = bad || !(fabsf(uAx) <= 0.3f && fabsf(uAy) <= 0.3f && fabsf(uBx) <= 0.3f && fabsf(uBy) <= 0.3f);
   }
   if (bad) atomicOr(a.flag, 4);
 }

@@ -35,6 +35,11 @@ struct LbmArgs {
 };
 
 // One TRT collision of a node given its pre-collision shifted populations g[9].
+// The formulae of the header with the common factors pulled out (the kernel is issue bound):
+//   even_q = -w+ g+_q + w_q [E0 + (c.u)(a (c.u) + b (c.G))],  E0 = w+ (drho - 1.5 rho u.u) - 3 (1 - w+/2) u.G,
+//                                                              a = 4.5 w+ rho, b = 9 (1 - w+/2)
+//   odd_q  = -w- g-_q + w_q [c1 (c.u) + c2 (c.G)],             c1 = 3 w- rho, c2 = 3 (1 - w-/2)
+//   gpost_q = g_q + even_q + odd_q,  gpost_qbar = g_qbar + even_q - odd_q
 __device__ __forceinline__ void trt_collide(float g[9], float Gx, float Gy, float rho0, float wp, float wm,
                                             float& ux, float& uy) {
   const float W0 = 4.0f / 9.0f, W1 = 1.0f / 9.0f, W5 = 1.0f / 36.0f;
@@ -48,18 +53,17 @@ __device__ __forceinline__ void trt_collide(float g[9], float Gx, float Gy, floa
   const float usq = ux * ux + uy * uy;
   const float uG = ux * Gx + uy * Gy;
   const float cp = 1.0f - 0.5f * wp, cm = 1.0f - 0.5f * wm;
-  // rest population (even only)
-  g[0] = g[0] - wp * (g[0] - W0 * (drho - 1.5f * rho * usq)) + cp * W0 * (-3.0f * uG);
-  // pairs (q, qbar) with c_qbar = -c_q:  (1,3) c=(1,0); (2,4) c=(0,1); (5,7) c=(1,1); (6,8) c=(-1,1)
+  const float E0 = wp * (drho - 1.5f * rho * usq) - 3.0f * cp * uG;
+  const float ca = 4.5f * wp * rho, cb = 9.0f * cp;
+  const float c1 = 3.0f * wm * rho, c2 = 3.0f * cm;
+  const float hwp = 0.5f * wp, hwm = 0.5f * wm;
+  // rest population (even only, c = 0)
+  g[0] = fmaf(W0, E0, g[0] - wp * g[0]);
 #define MC_PAIR(q, qb, w, cu, cG)                                                     \
   {                                                                                   \
-    const float gp = 0.5f * (g[q] + g[qb]), gm = 0.5f * (g[q] - g[qb]);               \
-    const float ep = (w) * (drho + rho * (4.5f * (cu) * (cu) - 1.5f * usq));          \
-    const float em = (w) * rho * 3.0f * (cu);                                         \
-    const float Sp = (w) * (-3.0f * uG + 9.0f * (cu) * (cG));                         \
-    const float Sm = 3.0f * (w) * (cG);                                               \
-    const float even = -wp * (gp - ep) + cp * Sp;                                     \
-    const float odd = -wm * (gm - em) + cm * Sm;                                      \
+    const float cu_ = (cu), cG_ = (cG);                                               \
+    const float even = fmaf((w), fmaf(cu_, fmaf(ca, cu_, cb * cG_), E0), -hwp * (g[q] + g[qb])); \
+    const float odd = fmaf((w), fmaf(c1, cu_, c2 * cG_), -hwm * (g[q] - g[qb]));      \
     g[q] += even + odd;                                                               \
     g[qb] += even - odd;                                                              \
   }

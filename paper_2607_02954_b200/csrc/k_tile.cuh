@@ -119,4 +119,13 @@ __global__ void __launch_bounds__(1024) k_tile_scan(int* __restrict__ tile_count
   if (threadIdx.x == 0) tile_start[n_tiles] = carry;
 }
 
+// mc_load_filaments: largest tile list (chooses the CTA size of the P2G kernels)
+__global__ void k_max_int(const int* __restrict__ v, int n, int* __restrict__ out) {
+  int m = 0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) m = max(m, v[i]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) atomicMax(out, m);
+}
+
 }  // namespace mc

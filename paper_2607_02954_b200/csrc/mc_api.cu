@@ -122,6 +122,7 @@ struct mc_world {
   int stride = 60;   // K1 window advance: 64 when all chains share a length dividing 64
   int n_windows = 0;
   int list_age = 0;  // steps since the tile lists were built (rebuilt when 0)
+  int deposit_threads = 128;  // CTA size of K2a: 128 hides the per-tile latency better, crowded worlds want 256
   // CUDA graphs of GRAPH_STEPS consecutive steps, one per ping-pong phase, captured on first use
   // when the tile lists are due (list_age == 0); GRAPH_STEPS is a multiple of LIST_STEPS and of 2
   cudaGraphExec_t graph[2] = {nullptr, nullptr};
@@ -231,7 +232,7 @@ int enqueue_step(mc_world* w) {
     prof_mark(w, 1);
     // K2a: S2 deposit
     if (w->d.n_density) {
-      mc::k_deposit_tile<<<tgrid, 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax);
+      mc::k_deposit_tile<<<tgrid, w->deposit_threads, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax);
       w->launches++;
       prof_mark(w, 2);
       // K3a: S3 filter + gradient -> force-gradient planes A
@@ -532,6 +533,20 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   w->launches++;
   cudaMemsetAsync(w->ptr<float>(w->L.F), 0, (size_t)N * 8, st);
   cudaMemsetAsync(w->ptr<float>(w->L.sense), 0, (size_t)N * 4, st);
+  // largest tile list of the loaded configuration -> CTA size of the deposit kernel
+  int* maxlist = w->ptr<int>(w->L.flags) + 2;
+  {
+    const int n_tiles = (w->nx / mc::TS) * (w->ny / mc::TS);
+    int* tile_count = w->ptr<int>(w->L.tile_count);
+    cudaMemsetAsync(maxlist, 0, 4, st);
+    mc::k_tile_bin<false><<<(int)((N + 255) / 256), 256, 0, st>>>(w->ptr<float2>(w->L.X), (int)N, w->nx, w->ny,
+                                                                  tile_count, nullptr);
+    mc::k_max_int<<<64, 256, 0, st>>>(tile_count, n_tiles, maxlist);
+    cudaMemsetAsync(tile_count, 0, (size_t)n_tiles * 4, st);
+    w->launches += 2;
+  }
+  int h_maxlist = 0;
+  cudaMemcpyAsync(&h_maxlist, maxlist, 4, cudaMemcpyDeviceToHost, st);
   const long long host_step = w->step;  // steps without beads do not advance the device copy
   cudaMemcpyAsync(w->ptr<long long>(w->L.flags) + 4, &host_step, 8, cudaMemcpyHostToDevice, st);
   int h = 0;
@@ -546,6 +561,7 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   w->N = (int)N;
   w->n_fil = n_fil;
   w->list_age = 0;
+  w->deposit_threads = h_maxlist > 1024 ? 256 : 128;
   if (reuse_order) {
     w->stride = prev_stride;
     w->n_windows = prev_windows;

@@ -91,6 +91,13 @@ def run_protocol(w, steps_at, threads=0):
     return worst
 
 
+def _with_sigma(w, sigma, radius):
+    for f in w["params"]["fields"]:
+        if f["kind"] == 0:
+            f["sigma"], f["radius"] = sigma, radius
+    return w
+
+
 SMALL = {
     # several tiles + ragged chain lengths (3 .. 100 beads: shorter/equal/longer than a warp),
     # chains straddling the periodic boundary and translated by whole periods
@@ -106,6 +113,10 @@ SMALL = {
     # crowded: many short chains clustered (many beads per cell; contention case of config 5)
     "crowded_64": lambda: worlds.random_world(64, 64, 96, 16, seed=7, kappa=0.25, kappa_rep=2e-4,
                                               clustered=3.0),
+    # smallest legal grid: one tile in each direction, every support wraps onto the same tile
+    "single_tile_32": lambda: worlds.ragged_world(32, 32, [5, 12, 20], seed=11),
+    # wide and flat: one tile high, several wide; R = 3 filter; sigma != 1
+    "flat_160x32": lambda: _with_sigma(worlds.ragged_world(160, 32, [16, 30, 64, 9], seed=12), 0.6, 3),
     # uniform 64-bead and 32-bead chains (the shapes of configs 2-4)
     "uniform_m64": lambda: worlds.random_world(128, 96, 40, 64, seed=8),
     "uniform_m32": lambda: worlds.random_world(96, 128, 70, 32, seed=9, static_source=True),

@@ -103,7 +103,9 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets /*HOST*
                       const float* act_period /*DEVICE*/);
 
 /* Advance n >= 0 steps.  Asynchronous: kernels are enqueued on the world's stream and the
- * call returns without synchronising.  Errors: MC_EINVAL, MC_ECUDA (launch failure),
+ * call returns without synchronising.  Blocks of four steps are replayed from a CUDA graph when
+ * the stream can be captured (not the legacy default stream); the results are bit-identical to
+ * direct launches, so mc_step(a) then mc_step(b) equals mc_step(a + b).  Errors: MC_EINVAL, MC_ECUDA (launch failure),
  * MC_EDIVERGED (a previous mc_read_state saw the sticky divergence flag: non-finite bead
  * position or |u| > 0.3). */
 int mc_step(mc_world* w, int32_t n);
@@ -135,7 +137,8 @@ int mc_keep_intermediates(mc_world* w, int32_t on);
 
 /* Optional per-kernel timing with CUDA events on the world's stream (used by bench.py for the
  * roofline line; off by default, costs one event record per kernel group when on).
- * Slots: 0 K0 bin, 1 K2a deposit, 2 K3a filter+gradient, 3 K1 filament force, 4 K2b spread,
+ * Slots: 0 K0 bin, 1 K2a deposit, 2 K3a filter+gradient, 3 K1 filament force, 4 K2b spread (empty:
+ * S5 is fused into the fluid kernel and is timed in slot 5),
  * 5 K3b fluid, 6 K4 interpolate+integrate.  mc_profile_enable(w,1) starts a capture of up to
  * 64 steps; mc_profile_read synchronises, writes the summed milliseconds per slot to
  * ms (HOST float[MC_PROF_SLOTS]) and the number of captured steps, and restarts the capture. */

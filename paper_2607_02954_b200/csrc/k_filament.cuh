@@ -92,6 +92,15 @@ __device__ __forceinline__ float half_kC(double pvx, double pvy, double vx, doub
   return 0.5f * p.kb * C;
 }
 
+// sin(x) for the small director rotations of Eq. 1 (|delta| is a fraction of the joint error):
+// odd Taylor polynomial to x^9 for |x| <= 0.5 (relative error < 2e-10 there), sinf beyond.
+__device__ __forceinline__ float sin_small(float x) {
+  if (fabsf(x) > 0.5f) return sinf(x);
+  const float x2 = x * x;
+  const float p = fmaf(x2, fmaf(x2, fmaf(x2, 2.7557319e-6f, -1.9841270e-4f), 8.3333333e-3f), -1.6666667e-1f);
+  return fmaf(x * x2, p, x);
+}
+
 // Delta x of an edge (Eq. 2-3) after the bending pass turned its director by delta.
 __device__ __forceinline__ float2 edge_delta(double vx, double vy, float delta, const BeadParams& p) {
   const double l2 = vx * vx + vy * vy;
@@ -100,7 +109,7 @@ __device__ __forceinline__ float2 edge_delta(double vx, double vy, float delta, 
   const float dl = (float)(l2 - (double)L * (double)L) / (ell + L);  // |v| - L_rest, no cancellation
   const float inv = 1.0f / ell;
   const float tx = (float)vx * inv, ty = (float)vy * inv;
-  const float sd = sinf(delta), sh = sinf(0.5f * delta);
+  const float sd = sin_small(delta), sh = sin_small(0.5f * delta);
   const float omc = 2.0f * sh * sh;  // 1 - cos(delta)
   // t - d with d = Rot(delta) t: Kirchhoff-Love error minus the stretch part, divided by L
   const float ex = omc * tx + sd * ty, ey = omc * ty - sd * tx;
@@ -152,12 +161,14 @@ __global__ void __launch_bounds__(256, 5) k_filament_force(FilamentArgs a) {
   float DAx = dA.x - pdx, DAy = dA.y - pdy;
   float DBx = dB.x, DBy = dB.y;
   if (!(pB.flags & BEAD_FIRST)) { DBx -= dA.x; DBy -= dA.y; }
+  // halo lanes of an overlapping window stay in the warp (the reductions below are warp-wide)
+  // but own no output
   const bool out = aligned || (lane >= 1 && lane <= 30);
-  if (!out) return;
+  const bool oA = out && vA, oB = out && vB;
   float2 FA = make_float2(a.kappa * DAx, a.kappa * DAy), FB = make_float2(a.kappa * DBx, a.kappa * DBy);
   if (a.A) {
-    if (vA) { const float2 g = interp2(a.A, a.nx, a.ny, xa.x, xa.y); FA.x += g.x; FA.y += g.y; }
-    if (vB) { const float2 g = interp2(a.A, a.nx, a.ny, xb.x, xb.y); FB.x += g.x; FB.y += g.y; }
+    if (oA) { const float2 g = interp2(a.A, a.nx, a.ny, xa.x, xa.y); FA.x += g.x; FA.y += g.y; }
+    if (oB) { const float2 g = interp2(a.A, a.nx, a.ny, xb.x, xb.y); FB.x += g.x; FB.y += g.y; }
   }
   if (a.tile_fmax) {
     // Bound for the fixed-point scale of S5 (k_p2g.cuh): tile_fmax[t] >= max |F| over the beads
@@ -166,28 +177,27 @@ __global__ void __launch_bounds__(256, 5) k_filament_force(FilamentArgs a) {
     // one atomicMax, and none once the stored value is high enough.  Positive floats order like
     // their bit patterns.
     float m = 0.0f;
-    if (vA) m = fmaxf(fabsf(FA.x), fabsf(FA.y));
-    if (vB) m = fmaxf(m, fmaxf(fabsf(FB.x), fabsf(FB.y)));
+    if (oA) m = fmaxf(fabsf(FA.x), fabsf(FA.y));
+    if (oB) m = fmaxf(m, fmaxf(fabsf(FB.x), fabsf(FB.y)));
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(__activemask(), m, o));
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(FULL, m, o));
     const unsigned mb = __float_as_uint(m);
     const int ntx = a.nx >> 5;
-    const int tA = vA ? (wrapi((int)floorf(xa.y), a.ny) >> 5) * ntx + (wrapi((int)floorf(xa.x), a.nx) >> 5) : -1;
-    const int tB = vB ? (wrapi((int)floorf(xb.y), a.ny) >> 5) * ntx + (wrapi((int)floorf(xb.x), a.nx) >> 5) : -1;
-    const unsigned act = __activemask();
-    const unsigned pa = __match_any_sync(act, tA), pb = __match_any_sync(act, tB);
+    const int tA = oA ? (wrapi((int)floorf(xa.y), a.ny) >> 5) * ntx + (wrapi((int)floorf(xa.x), a.nx) >> 5) : -1;
+    const int tB = oB ? (wrapi((int)floorf(xb.y), a.ny) >> 5) * ntx + (wrapi((int)floorf(xb.x), a.nx) >> 5) : -1;
+    const unsigned pa = __match_any_sync(FULL, tA), pb = __match_any_sync(FULL, tB);
     if (tA >= 0 && lane == __ffs(pa) - 1 && mb > a.tile_fmax[tA]) atomicMax(a.tile_fmax + tA, mb);
     if (tB >= 0 && tB != tA && lane == __ffs(pb) - 1 && mb > a.tile_fmax[tB]) atomicMax(a.tile_fmax + tB, mb);
   }
-  if (vA && vB) {
+  if (oA && oB) {
     *reinterpret_cast<float4*>(a.F + bA) = make_float4(FA.x, FA.y, FB.x, FB.y);
   } else {
-    if (vA) a.F[bA] = FA;
-    if (vB) a.F[bB] = FB;
+    if (oA) a.F[bA] = FA;
+    if (oB) a.F[bB] = FB;
   }
   if (a.csum) {
-    if (vA) a.sense[bA] = interp1(a.csum, a.nx, a.ny, xa.x, xa.y);
-    if (vB) a.sense[bB] = interp1(a.csum, a.nx, a.ny, xb.x, xb.y);
+    if (oA) a.sense[bA] = interp1(a.csum, a.nx, a.ny, xa.x, xa.y);
+    if (oB) a.sense[bB] = interp1(a.csum, a.nx, a.ny, xb.x, xb.y);
   }
 }
 

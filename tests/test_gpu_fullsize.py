@@ -28,6 +28,15 @@ def test_per_step_parity_config(name, steps_at):
     print(name, {k: f"{v:.2e}" for k, v in worst.items()})
 
 
+def test_per_step_parity_many_ragged_chains():
+    # 400 chains of 3..150 beads (K1's overlapping-window mode across thousands of windows)
+    import os
+    lengths = (3 + (worlds.uniform(5, "ragged/len", 400) * 148).astype(int)).tolist()
+    w = worlds.ragged_world(256, 192, lengths, seed=21, static_source=True)
+    worst = run_protocol(w, steps_at=[0, 7, 30], threads=os.cpu_count() or 1)
+    print("ragged400", {k: f"{v:.2e}" for k, v in worst.items()})
+
+
 @pytest.mark.parametrize("name", ["4c", "5"])
 def test_one_parity_step_large(name):
     import os

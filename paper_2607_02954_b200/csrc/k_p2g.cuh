@@ -107,12 +107,13 @@ __device__ __forceinline__ float block_max(float v, float* sm /*[32]*/) {
   return v;
 }
 
-// power-of-two scale s with bound * s < 2^30
+// power-of-two scale s with bound * s < 2^30, for a normal positive bound (exponent arithmetic on
+// the bits: frexpf/ldexpf cost ~60 instructions in every thread of every tile)
 __device__ __forceinline__ float pow2_scale(float bound) {
-  int ex;
-  frexpf(bound, &ex);  // bound = m * 2^ex, m in [0.5, 1)
-  return ldexpf(1.0f, 30 - ex);
+  const int e = (int)((__float_as_uint(bound) >> 23) & 0xffu);  // bound in [2^(e-127), 2^(e-126))
+  return __uint_as_float((unsigned)(127 + 30 - (e - 126)) << 23);  // 2^(30 - (e - 126))
 }
+__device__ __forceinline__ float pow2f(int k) { return __uint_as_float((unsigned)(127 + k) << 23); }
 
 // number of extra fraction bits the lo word can carry without overflowing for n contributions
 __device__ __forceinline__ int lo_bits(int n) {
@@ -206,7 +207,7 @@ __global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int*
   const bool wide = (e - s) > WIDE_N;
   for (int c = threadIdx.x; c < TS * TSP; c += blockDim.x) { acc[c] = 0; if (wide) accl[c] = 0; }
   const float scale = pow2_scale(fmaxf(0.25f * (float)(e - s), 1.0f));
-  const float lscale = ldexpf(1.0f, lo_bits(e - s));
+  const float lscale = pow2f(lo_bits(e - s));
   __syncthreads();
   if (wide) deposit_loop_wide(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
   else if (nx == TS || ny == TS) deposit_loop<false, true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
@@ -243,7 +244,7 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
                                                         int* acc0, int* acc1, int* accl0, int* accl1,
                                                         float* red, float& linv) {
   const bool wide = (e - s) > WIDE_N;
-  const float lscale = ldexpf(1.0f, lo_bits(e - s));
+  const float lscale = pow2f(lo_bits(e - s));
   linv = wide ? 1.0f / lscale : 0.0f;  // 0 => the readers skip the lo planes (not zeroed then)
   for (int c = threadIdx.x; c < TS * TSP; c += blockDim.x) {
     acc0[c] = 0; acc1[c] = 0;

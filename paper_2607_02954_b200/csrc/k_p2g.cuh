@@ -151,12 +151,21 @@ template <bool WIDE, bool WRAP>
 __device__ __forceinline__ void spread_loop(int nx, int ny, int x0, int y0, int s, int e,
                                             const int* __restrict__ list, const float2* __restrict__ X,
                                             const float2* __restrict__ F, float scale, float lscale,
-                                            int* acc0, int* acc1, int* accl0, int* accl1) {
+                                            int* acc0, int* acc1, int* accl0, int* accl1,
+                                            float2 xpre, float2 fpre) {
+  // the caller loaded this thread's FIRST entry (xpre, fpre) before the zeroing and the barrier,
+  // so that the list -> X/F gather latency is spent under them; later entries are software-
+  // pipelined one iteration ahead
+  float2 xc = xpre, fc = fpre;
   for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
-    const int b = __ldg(list + k);
+    const float2 xb = xc, f = fc;
+    if (k + (int)blockDim.x < e) {
+      const int bn = __ldg(list + k + blockDim.x);
+      xc = __ldg(X + bn);
+      fc = __ldg(F + bn);
+    }
     TileBead tb;
-    tile_bead<WRAP>(__ldg(X + b), nx, ny, x0, y0, tb);
-    const float2 f = __ldg(F + b);
+    tile_bead<WRAP>(xb, nx, ny, x0, y0, tb);
     const float fxs = f.x * scale, fys = f.y * scale;
 #pragma unroll
     for (int l = 0; l < 4; ++l) {
@@ -188,8 +197,9 @@ __device__ __noinline__ void deposit_loop_wide(int nx, int ny, int x0, int y0, i
 }
 __device__ __noinline__ void spread_loop_wide(int nx, int ny, int x0, int y0, int s, int e, const int* list,
                                               const float2* X, const float2* F, float scale, float lscale,
-                                              int* acc0, int* acc1, int* accl0, int* accl1) {
-  spread_loop<true, true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
+                                              int* acc0, int* acc1, int* accl0, int* accl1, float2 xpre,
+                                              float2 fpre) {
+  spread_loop<true, true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre);
 }
 
 // K2a: S2 deposit.  tile_rho_max[t] receives max over the tile of rho_b (for K2b's scale).
@@ -244,6 +254,12 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
                                                         int* acc0, int* acc1, int* accl0, int* accl1,
                                                         float* red, float& linv) {
   const bool wide = (e - s) > WIDE_N;
+  float2 xpre = make_float2(0.f, 0.f), fpre = make_float2(0.f, 0.f);
+  if (s + (int)threadIdx.x < e) {  // first entry of this thread: start its gather now
+    const int b = __ldg(list + s + threadIdx.x);
+    xpre = __ldg(X + b);
+    fpre = __ldg(F + b);
+  }
   const float lscale = pow2f(lo_bits(e - s));
   linv = wide ? 1.0f / lscale : 0.0f;  // 0 => the readers skip the lo planes (not zeroed then)
   for (int c = threadIdx.x; c < TS * TSP; c += blockDim.x) {
@@ -276,9 +292,9 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
   }
   const float sum_w = (rho_max > 0.0f) ? 1.0625f * rho_max : fmaxf(0.25f * (float)(e - s), 1.0f);
   const float scale = pow2_scale(fmaxf(fm * sum_w, 1e-18f));
-  if (wide) spread_loop_wide(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
-  else if (nx == TS || ny == TS) spread_loop<false, true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
-  else spread_loop<false, false>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1);
+  if (wide) spread_loop_wide(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre);
+  else if (nx == TS || ny == TS) spread_loop<false, true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre);
+  else spread_loop<false, false>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre);
   __syncthreads();
   return scale;
 }

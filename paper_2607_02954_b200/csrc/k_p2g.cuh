@@ -124,10 +124,13 @@ __device__ __forceinline__ int lo_bits(int n) {
 template <bool WIDE, bool WRAP>
 __device__ __forceinline__ void deposit_loop(int nx, int ny, int x0, int y0, int s, int e,
                                              const int* __restrict__ list, const float2* __restrict__ X,
-                                             float scale, float lscale, int* acc, int* accl) {
+                                             float scale, float lscale, int* acc, int* accl, float2 xpre) {
+  float2 xc = xpre;  // first entry preloaded by the caller, later ones one iteration ahead
   for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
+    const float2 xb = xc;
+    if (k + (int)blockDim.x < e) xc = __ldg(X + __ldg(list + k + blockDim.x));
     TileBead tb;
-    tile_bead<WRAP>(__ldg(X + __ldg(list + k)), nx, ny, x0, y0, tb);
+    tile_bead<WRAP>(xb, nx, ny, x0, y0, tb);
 #pragma unroll
     for (int l = 0; l < 4; ++l) {
       const float wys = tb.wy[l] * scale;
@@ -192,8 +195,9 @@ __device__ __forceinline__ void spread_loop(int nx, int ny, int x0, int y0, int 
 // the rare crowded-tile variants are kept out of line so that their registers do not count
 // against the occupancy of the common path
 __device__ __noinline__ void deposit_loop_wide(int nx, int ny, int x0, int y0, int s, int e, const int* list,
-                                               const float2* X, float scale, float lscale, int* acc, int* accl) {
-  deposit_loop<true, true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
+                                               const float2* X, float scale, float lscale, int* acc, int* accl,
+                                               float2 xpre) {
+  deposit_loop<true, true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl, xpre);
 }
 __device__ __noinline__ void spread_loop_wide(int nx, int ny, int x0, int y0, int s, int e, const int* list,
                                               const float2* X, const float2* F, float scale, float lscale,
@@ -215,13 +219,15 @@ __global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int*
   const int x0 = blockIdx.x * TS, y0 = blockIdx.y * TS;
   const int s = tile_start[t], e = tile_start[t + 1];
   const bool wide = (e - s) > WIDE_N;
+  float2 xpre = make_float2(0.f, 0.f);
+  if (s + (int)threadIdx.x < e) xpre = __ldg(X + __ldg(list + s + threadIdx.x));  // gather starts before the zeroing
   for (int c = threadIdx.x; c < TS * TSP; c += blockDim.x) { acc[c] = 0; if (wide) accl[c] = 0; }
   const float scale = pow2_scale(fmaxf(0.25f * (float)(e - s), 1.0f));
   const float lscale = pow2f(lo_bits(e - s));
   __syncthreads();
-  if (wide) deposit_loop_wide(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
-  else if (nx == TS || ny == TS) deposit_loop<false, true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
-  else deposit_loop<false, false>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl);
+  if (wide) deposit_loop_wide(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl, xpre);
+  else if (nx == TS || ny == TS) deposit_loop<false, true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl, xpre);
+  else deposit_loop<false, false>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl, xpre);
   __syncthreads();
   const float inv = 1.0f / scale, linv = 1.0f / lscale;
   float mx = 0.0f;

@@ -154,24 +154,31 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
   const int i = x0 + lx;
   const int im = (i == 0) ? nx - 1 : i - 1, ip2 = (i + 2 == nx) ? 0 : i + 2;
   bool bad = false;
+  float gA[9], gB[9];  // pre-collision populations of nodes i and i+1 (pull: g_q(x) = src_q(x - c_q))
+  auto load_pair = [&](int ly) {
+    const int j = y0 + ly;
+    const int jm = (j == 0) ? ny - 1 : j - 1, jp = (j == ny - 1) ? 0 : j + 1;
+    const size_t r0 = (size_t)j * nx, rm = (size_t)jm * nx, rp = (size_t)jp * nx;
+    const float2 v0 = __ldg(reinterpret_cast<const float2*>(a.src + 0 * nc + r0 + i));
+    const float2 v2 = __ldg(reinterpret_cast<const float2*>(a.src + 2 * nc + rm + i));
+    const float2 v4 = __ldg(reinterpret_cast<const float2*>(a.src + 4 * nc + rp + i));
+    gA[0] = v0.x; gB[0] = v0.y; gA[2] = v2.x; gB[2] = v2.y; gA[4] = v4.x; gB[4] = v4.y;
+    gA[1] = __ldg(a.src + 1 * nc + r0 + im);     gB[1] = __ldg(a.src + 1 * nc + r0 + i);
+    gA[3] = __ldg(a.src + 3 * nc + r0 + i + 1);  gB[3] = __ldg(a.src + 3 * nc + r0 + ip2);
+    gA[5] = __ldg(a.src + 5 * nc + rm + im);     gB[5] = __ldg(a.src + 5 * nc + rm + i);
+    gA[6] = __ldg(a.src + 6 * nc + rm + i + 1);  gB[6] = __ldg(a.src + 6 * nc + rm + ip2);
+    gA[7] = __ldg(a.src + 7 * nc + rp + i + 1);  gB[7] = __ldg(a.src + 7 * nc + rp + ip2);
+    gA[8] = __ldg(a.src + 8 * nc + rp + im);     gB[8] = __ldg(a.src + 8 * nc + rp + i);
+  };
+  // the first pass's 15 loads are issued BEFORE the barrier that ends the atomic phase, so their
+  // DRAM latency is spent while the slower warps finish their atomics
+  load_pair(ry);
+  __syncthreads();
 #pragma unroll 1
   for (int h = 0; h < 2; ++h) {
     const int ly = ry + 16 * h, j = y0 + ly;
-    const int jm = (j == 0) ? ny - 1 : j - 1, jp = (j == ny - 1) ? 0 : j + 1;
-    const size_t r0 = (size_t)j * nx, rm = (size_t)jm * nx, rp = (size_t)jp * nx;
-    float gA[9], gB[9];  // pre-collision populations of nodes i and i+1 (pull: g_q(x) = src_q(x - c_q))
-    {
-      const float2 v0 = __ldg(reinterpret_cast<const float2*>(a.src + 0 * nc + r0 + i));
-      const float2 v2 = __ldg(reinterpret_cast<const float2*>(a.src + 2 * nc + rm + i));
-      const float2 v4 = __ldg(reinterpret_cast<const float2*>(a.src + 4 * nc + rp + i));
-      gA[0] = v0.x; gB[0] = v0.y; gA[2] = v2.x; gB[2] = v2.y; gA[4] = v4.x; gB[4] = v4.y;
-      gA[1] = __ldg(a.src + 1 * nc + r0 + im);     gB[1] = __ldg(a.src + 1 * nc + r0 + i);
-      gA[3] = __ldg(a.src + 3 * nc + r0 + i + 1);  gB[3] = __ldg(a.src + 3 * nc + r0 + ip2);
-      gA[5] = __ldg(a.src + 5 * nc + rm + im);     gB[5] = __ldg(a.src + 5 * nc + rm + i);
-      gA[6] = __ldg(a.src + 6 * nc + rm + i + 1);  gB[6] = __ldg(a.src + 6 * nc + rm + ip2);
-      gA[7] = __ldg(a.src + 7 * nc + rp + i + 1);  gB[7] = __ldg(a.src + 7 * nc + rp + ip2);
-      gA[8] = __ldg(a.src + 8 * nc + rp + im);     gB[8] = __ldg(a.src + 8 * nc + rp + i);
-    }
+    if (h) load_pair(ly);
+    const size_t r0 = (size_t)j * nx;
     const size_t c = r0 + i;
     const int sa = ly * TSP + lx;
     const float GAx = tile_value(acc0, accl0, sa, linv) * inv, GAy = tile_value(acc1, accl1, sa, linv) * inv;

@@ -251,7 +251,8 @@ __device__ __forceinline__ float tile_value(const int* acc, const int* accl, int
 }
 
 // Accumulate the spread force of one tile into shared memory (two planes), return the scale.
-// Used by the fused spread + fluid kernel (k_lbm.cuh).
+// Used by the fused spread + fluid kernel (k_lbm.cuh), which must __syncthreads() before it
+// reads the accumulators.
 __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, int y0, int s, int e,
                                                         const int* __restrict__ list,
                                                         const float2* __restrict__ X,
@@ -301,7 +302,7 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
   if (wide) spread_loop_wide(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre);
   else if (nx == TS || ny == TS) spread_loop<false, true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre);
   else spread_loop<false, false>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre);
-  __syncthreads();
+  // NO barrier here: the caller issues its next global loads first, then synchronises
   return scale;
 }
 

@@ -9,16 +9,28 @@ namespace mc {
 
 __global__ void __launch_bounds__(256) k_interp_integrate(int N, float2* __restrict__ X,
                                                           const float2* __restrict__ u, int nx, int ny,
-                                                          int* __restrict__ flag, long long* __restrict__ step) {
+                                                          int* __restrict__ flag, long long* __restrict__ step,
+                                                          unsigned* __restrict__ step_max) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b == 0) *step += 1;  // device copy of the step counter (K1 of the next step reads it)
-  if (b >= N) return;
-  float2 p = X[b];
-  const float2 U = interp2(u, nx, ny, p.x, p.y);
-  p.x += U.x;
-  p.y += U.y;
-  X[b] = p;
-  if (!(isfinite(p.x) && isfinite(p.y))) atomicOr(flag, 8);
+  float m = 0.0f;
+  if (b < N) {
+    float2 p = X[b];
+    const float2 U = interp2(u, nx, ny, p.x, p.y);
+    p.x += U.x;
+    p.y += U.y;
+    X[b] = p;
+    if (!(isfinite(p.x) && isfinite(p.y))) atomicOr(flag, 8);
+    m = fmaxf(fabsf(U.x), fabsf(U.y));
+  }
+  // largest displacement component of this step: feeds the drift bound of the tile lists
+  // (k_tile.cuh).  One guarded atomicMax per warp; positive floats order like their bits.
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) {
+    const unsigned mb = __float_as_uint(m);
+    if (mb > *step_max) atomicMax(step_max, mb);
+  }
 }
 
 }  // namespace mc

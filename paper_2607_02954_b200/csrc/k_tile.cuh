@@ -4,12 +4,12 @@
 // A tile is TS x TS nodes.  A bead is listed in every tile its 4x4 Peskin support, widened by a
 // SKIN of one node on every side, overlaps (1, 2 or 4 tiles), so a tile's CTA can accumulate ALL
 // contributions to its own nodes from its own list and never writes outside the tile: no global
-// float atomics, no halo exchange.  The skin makes a list valid for several steps: a bead moves
-// by at most 0.3 nodes per axis per step (U is a convex combination of u, and |u| > 0.3 raises
-// the divergence flag), so lists built at step n0 still cover every support at steps n0+1..n0+3
-// (drift <= 0.9 < 1) and K0 runs only every LIST_STEPS = 4 steps.  Entries whose support no
-// longer (or not yet) overlaps the tile add exact zeros (k_p2g.cuh), so the result does not
-// depend on when the lists were built.
+// float atomics, no halo exchange.  The skin makes a list valid for many steps: K4 records the
+// largest bead displacement component of every step, a one-thread policy kernel (k_list_policy)
+// adds it to the drift accumulated since the lists were built and orders a rebuild only when
+// the drift could reach the skin; until then the three K0 kernels return at once.  Entries
+// whose support no longer (or not yet) overlaps the tile add exact zeros (k_p2g.cuh), so the
+// result does not depend on when the lists were built (any rebuild schedule gives the same bits).
 //   count : per bead, +1 on each overlapped tile (integer atomics, warp-aggregated)
 //   scan  : exclusive prefix sum over the tiles (one block; there are few tiles)
 //   fill  : per bead, claim a slot in each overlapped tile's segment and store the bead index
@@ -23,7 +23,22 @@ namespace mc {
 
 constexpr int TS = 32;          // tile side in nodes
 constexpr int LIST_SKIN = 1;    // nodes added on every side of the support when listing
-constexpr int LIST_STEPS = 4;   // steps a list stays valid: (LIST_STEPS-1) * 0.3 < LIST_SKIN
+constexpr float LIST_DRIFT_MAX = 0.9f;  // rebuild when the accumulated drift bound exceeds this (< LIST_SKIN)
+
+// device-side list state, in the world's flag words
+struct ListState {
+  int need;            // 1: the K0 kernels of this step rebuild the lists
+  float drift;         // bound on the per-axis displacement of any bead since the lists were built
+  unsigned step_max;   // bits of max |U_x|,|U_y| over the beads in the last step (K4, atomicMax)
+};
+
+__global__ void k_list_policy(ListState* st) {
+  const float d = st->drift + __uint_as_float(st->step_max);
+  st->step_max = 0u;
+  const bool need = !(d <= LIST_DRIFT_MAX);  // also true for NaN
+  st->need = need ? 1 : 0;
+  st->drift = need ? 0.0f : d;
+}
 
 // The (up to 4) tiles overlapped by the skinned support of a bead at (x,y): tiles of the first
 // and the last listed node along each axis (periodic).  Returns the number of distinct tiles.
@@ -61,27 +76,34 @@ __device__ __forceinline__ int warp_claim(int* ctr, int key, bool act) {
 // FILL = false: tile_ctr[t] += 1 per listed bead.  FILL = true: tile_ctr holds the running
 // cursor (initialised to tile_start) and the bead index is stored at the claimed slot.
 template <bool FILL>
-__global__ void __launch_bounds__(256) k_tile_bin(const float2* __restrict__ X, int N, int nx, int ny,
-                                                  int* __restrict__ tile_ctr, int* __restrict__ list) {
-  const int b = blockIdx.x * blockDim.x + threadIdx.x;
-  int t[4] = {0, 0, 0, 0};
-  int n = 0;
-  if (b < N) {
-    const float2 p = X[b];
-    n = bead_tiles(p.x, p.y, nx, ny, nx / TS, t);
-  }
+__global__ void __launch_bounds__(256) k_tile_bin(const ListState* __restrict__ st, const float2* __restrict__ X,
+                                                  int N, int nx, int ny, int* __restrict__ tile_ctr,
+                                                  int* __restrict__ list) {
+  if (!st->need) return;
+  // grid-stride over whole blocks of beads: every lane of a warp takes part in warp_claim
+  for (int base = blockIdx.x * blockDim.x; base < N; base += gridDim.x * blockDim.x) {
+    const int b = base + threadIdx.x;
+    int t[4] = {0, 0, 0, 0};
+    int n = 0;
+    if (b < N) {
+      const float2 p = X[b];
+      n = bead_tiles(p.x, p.y, nx, ny, nx / TS, t);
+    }
 #pragma unroll
-  for (int s = 0; s < 4; ++s) {
-    const int slot = warp_claim(tile_ctr, t[s], s < n);
-    if (FILL && s < n) list[slot] = b;
+    for (int s = 0; s < 4; ++s) {
+      const int slot = warp_claim(tile_ctr, t[s], s < n);
+      if (FILL && s < n) list[slot] = b;
+    }
   }
 }
 
 // one block: tile_start = exclusive scan of tile_count (n_tiles + 1 entries); the cursor array
 // for the fill pass is initialised to tile_start; counts are zeroed for the next step.
-__global__ void __launch_bounds__(1024) k_tile_scan(int* __restrict__ tile_count, int n_tiles,
-                                                    int* __restrict__ tile_start, int* __restrict__ tile_cursor) {
+__global__ void __launch_bounds__(1024) k_tile_scan(const ListState* __restrict__ st, int* __restrict__ tile_count,
+                                                    int n_tiles, int* __restrict__ tile_start,
+                                                    int* __restrict__ tile_cursor) {
   __shared__ int sm[33];
+  if (!st->need) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   int carry = 0;
   for (int base = 0; base < n_tiles; base += 1024) {

@@ -121,10 +121,9 @@ struct mc_world {
   int N = 0;
   int stride = 60;   // K1 window advance: 64 when all chains share a length dividing 64
   int n_windows = 0;
-  int list_age = 0;  // steps since the tile lists were built (rebuilt when 0)
   int deposit_threads = 128;  // CTA size of K2a: 128 hides the per-tile latency better, crowded worlds want 256
   // CUDA graphs of GRAPH_STEPS consecutive steps, one per ping-pong phase, captured on first use
-  // when the tile lists are due (list_age == 0); GRAPH_STEPS is a multiple of LIST_STEPS and of 2
+  // (the ping-pong phase is the only host-side state a step depends on); GRAPH_STEPS is even
   cudaGraphExec_t graph[2] = {nullptr, nullptr};
   int64_t graph_launches[2] = {0, 0};
   bool graph_off = false;  // the stream cannot be captured (e.g. the legacy default stream): direct launches
@@ -162,7 +161,7 @@ int check_cuda(mc_world* w, const char* what) {
 
 constexpr int PROF_MAX_STEPS = 64;
 constexpr int GRAPH_STEPS = 4;
-static_assert(GRAPH_STEPS % mc::LIST_STEPS == 0 && GRAPH_STEPS % 2 == 0, "graph period");
+static_assert(GRAPH_STEPS % 2 == 0, "graph period");
 
 void drop_graphs(mc_world* w) {
   for (int k = 0; k < 2; ++k)
@@ -221,14 +220,15 @@ int enqueue_step(mc_world* w) {
 
   prof_mark(w, 0);
   if (beads) {
-    // K0: tile binning (count, scan, fill), every LIST_STEPS steps (skinned lists, k_tile.cuh)
-    if (w->list_age == 0) {
-      mc::k_tile_bin<false><<<bgrid, bt, 0, st>>>(X, N, nx, ny, tile_count, nullptr);
-      mc::k_tile_scan<<<1, 1024, 0, st>>>(tile_count, n_tiles, tile_start, tile_cursor);
-      mc::k_tile_bin<true><<<bgrid, bt, 0, st>>>(X, N, nx, ny, tile_cursor, list);
-      w->launches += 3;
-    }
-    w->list_age = (w->list_age + 1) % mc::LIST_STEPS;
+    // K0: policy + tile binning (count, scan, fill).  The three binning kernels return at once
+    // unless the policy kernel found the lists' drift bound used up (k_tile.cuh).
+    mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16);
+    const int k0grid = bgrid < 148 * 8 ? bgrid : 148 * 8;
+    mc::k_list_policy<<<1, 1, 0, st>>>(ls_state);
+    mc::k_tile_bin<false><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, tile_count, nullptr);
+    mc::k_tile_scan<<<1, 1024, 0, st>>>(ls_state, tile_count, n_tiles, tile_start, tile_cursor);
+    mc::k_tile_bin<true><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, tile_cursor, list);
+    w->launches += 4;
     prof_mark(w, 1);
     // K2a: S2 deposit
     if (w->d.n_density) {
@@ -308,7 +308,8 @@ int enqueue_step(mc_world* w) {
   prof_mark(w, 6);
   // K4: S7
   if (beads) {
-    mc::k_interp_integrate<<<bgrid, bt, 0, st>>>(N, X, la.u, nx, ny, flag, w->ptr<long long>(w->L.flags) + 4);
+    mc::k_interp_integrate<<<bgrid, bt, 0, st>>>(N, X, la.u, nx, ny, flag, w->ptr<long long>(w->L.flags) + 4,
+                                                 reinterpret_cast<unsigned*>(w->ptr<int>(w->L.flags) + 18));
     w->launches++;
   }
   prof_mark(w, 7);
@@ -539,8 +540,15 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
     const int n_tiles = (w->nx / mc::TS) * (w->ny / mc::TS);
     int* tile_count = w->ptr<int>(w->L.tile_count);
     cudaMemsetAsync(maxlist, 0, 4, st);
-    mc::k_tile_bin<false><<<(int)((N + 255) / 256), 256, 0, st>>>(w->ptr<float2>(w->L.X), (int)N, w->nx, w->ny,
-                                                                  tile_count, nullptr);
+    // force the next step to rebuild the lists (drift = +inf), and count once now with need = 1
+    mc::ListState force;
+    force.need = 1;
+    force.drift = INFINITY;
+    force.step_max = 0u;
+    mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16);
+    cudaMemcpyAsync(ls_state, &force, sizeof(force), cudaMemcpyHostToDevice, st);
+    mc::k_tile_bin<false><<<(int)((N + 255) / 256), 256, 0, st>>>(ls_state, w->ptr<float2>(w->L.X), (int)N, w->nx,
+                                                                  w->ny, tile_count, nullptr);
     mc::k_max_int<<<64, 256, 0, st>>>(tile_count, n_tiles, maxlist);
     cudaMemsetAsync(tile_count, 0, (size_t)n_tiles * 4, st);
     w->launches += 2;
@@ -560,7 +568,6 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   }
   w->N = (int)N;
   w->n_fil = n_fil;
-  w->list_age = 0;
   w->deposit_threads = h_maxlist > 1024 ? 256 : 128;
   if (reuse_order) {
     w->stride = prev_stride;
@@ -580,10 +587,10 @@ int mc_step(mc_world* w, int32_t n) {
   if (w->diverged) return fail(w, MC_EDIVERGED, "world diverged (non-finite bead or |u| > 0.3)");
   int32_t done = 0;
   while (done < n) {
-    // Blocks of GRAPH_STEPS steps that start where the tile lists are due replay a captured CUDA
+    // Blocks of GRAPH_STEPS steps replay a captured CUDA
     // graph (same kernels, same order, same arguments: results are bit-identical to direct
     // launches); small worlds are bound by launch overhead, not by the kernels.
-    if (!w->prof_on && !w->graph_off && w->list_age == 0 && n - done >= GRAPH_STEPS) {
+    if (!w->prof_on && !w->graph_off && n - done >= GRAPH_STEPS) {
       const int ph = w->cur;
       if (!w->graph[ph]) {
         cudaGraph_t g = nullptr;
@@ -601,7 +608,7 @@ int mc_step(mc_world* w, int32_t n) {
         if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
         w->graph_launches[ph] = w->launches - l0;
       } else {
-        w->step += GRAPH_STEPS;  // cur and list_age return to their values after GRAPH_STEPS steps
+        w->step += GRAPH_STEPS;  // cur returns to its value after GRAPH_STEPS steps
         w->launches += w->graph_launches[ph];
       }
       if (cudaGraphLaunch(w->graph[ph], w->stream) != cudaSuccess) return fail(w, MC_ECUDA, "cudaGraphLaunch failed");

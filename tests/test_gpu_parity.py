@@ -268,3 +268,36 @@ def test_reload_same_chains_keeps_results():
     D.step(1)
     c, d = C.read_state(keys=("xy", "force")), D.read_state(keys=("xy", "force"))
     assert c["xy"].tobytes() == d["xy"].tobytes() and c["force"].tobytes() == d["force"].tobytes()
+
+
+def test_list_rebuild_schedule_does_not_change_the_bits():
+    # The tile lists are rebuilt only when a drift bound is used up (k_tile.cuh).  Entries whose
+    # support left the tile add exact zeros, so ANY rebuild schedule must give the same bits:
+    # world A free-runs (few rebuilds), world B is reloaded with its own positions before every
+    # step, which forces a rebuild each step.  kappa = 8 moves the beads fast enough for A to
+    # rebuild several times within the run.
+    from oracle import mco
+    from paper_2607_02954_b200 import binding
+    w = worlds.random_world(96, 64, 24, 32, seed=13, kappa=8.0)
+    A, B = binding.World(w), binding.World(w)
+    n = 240
+    A.step(n)
+    for _ in range(n):
+        xy = B.read_state(keys=("xy",))["xy"]
+        w2 = dict(w)
+        w2["xy"] = xy
+        B.load_filaments(w2)
+        B.step(1)
+    a, b = A.read_state(keys=("xy", "u", "fdev")), B.read_state(keys=("xy", "u", "fdev"))
+    for k in ("xy", "u", "fdev"):
+        assert a[k].tobytes() == b[k].tobytes(), k
+    # and the run agrees with the oracle (positions, 1e-3)
+    O = mco.World(w)
+    drift, prev = 0.0, w["xy"].astype(np.float64)
+    for _ in range(n):
+        O.step(1)
+        cur = O.read_state()["xy"]
+        drift += np.abs(cur - prev).max()  # what the policy kernel accumulates
+        prev = cur
+    assert_close("X after 240 steps", a["xy"], prev, TOL_TRAJ)
+    assert drift > 1.8, drift  # the drift bound (0.9) was used up at least twice in world A

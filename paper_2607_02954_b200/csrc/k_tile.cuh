@@ -2,14 +2,16 @@
 // followed by shared-memory tile accumulation, so global atomics are minimised").
 //
 // A tile is TS x TS nodes.  A bead is listed in every tile its 4x4 Peskin support, widened by a
-// SKIN of one node on every side, overlaps (1, 2 or 4 tiles), so a tile's CTA can accumulate ALL
+// SKIN (a quarter node of bead motion in every direction), overlaps (1, 2 or 4 tiles), so a tile's CTA can accumulate ALL
 // contributions to its own nodes from its own list and never writes outside the tile: no global
 // float atomics, no halo exchange.  The skin makes a list valid for many steps: K4 records the
 // largest bead displacement component of every step, a one-thread policy kernel (k_list_policy)
 // adds it to the drift accumulated since the lists were built and orders a rebuild only when
 // the drift could reach the skin; until then the three K0 kernels return at once.  Entries
 // whose support no longer (or not yet) overlaps the tile add exact zeros (k_p2g.cuh), so the
-// result does not depend on when the lists were built (any rebuild schedule gives the same bits).
+// schedule touches the results only through the per-tile fixed-point scales (powers of two
+// chosen from the list lengths), i.e. at rounding level; it is a function of the state alone,
+// so runs stay bit-reproducible and mc_step(a), mc_step(b) equals mc_step(a + b).
 //   count : per bead, +1 on each overlapped tile (integer atomics, warp-aggregated)
 //   scan  : exclusive prefix sum over the tiles (one block; there are few tiles)
 //   fill  : per bead, claim a slot in each overlapped tile's segment and store the bead index
@@ -22,8 +24,8 @@
 namespace mc {
 
 constexpr int TS = 32;          // tile side in nodes
-constexpr int LIST_SKIN = 1;    // nodes added on every side of the support when listing
-constexpr float LIST_DRIFT_MAX = 0.9f;  // rebuild when the accumulated drift bound exceeds this (< LIST_SKIN)
+constexpr float LIST_SKIN = 0.25f;  // a bead is listed as if it sat anywhere within +-LIST_SKIN of its position
+constexpr float LIST_DRIFT_MAX = 0.22f;  // rebuild when the accumulated drift bound exceeds this (< LIST_SKIN)
 
 // device-side list state, in the world's flag words
 struct ListState {
@@ -43,9 +45,11 @@ __global__ void k_list_policy(ListState* st) {
 // The (up to 4) tiles overlapped by the skinned support of a bead at (x,y): tiles of the first
 // and the last listed node along each axis (periodic).  Returns the number of distinct tiles.
 __device__ __forceinline__ int bead_tiles(float x, float y, int nx, int ny, int ntx, int t[4]) {
-  constexpr int W = 3 + 2 * LIST_SKIN;  // last listed node relative to the first
-  const int i0 = wrapi((int)floorf(x) - 1 - LIST_SKIN, nx), j0 = wrapi((int)floorf(y) - 1 - LIST_SKIN, ny);
-  const int i3 = (i0 + W >= nx) ? i0 + W - nx : i0 + W, j3 = (j0 + W >= ny) ? j0 + W - ny : j0 + W;
+  // first and last node any support can reach while the bead stays within the skin
+  const int ia = (int)floorf(x - LIST_SKIN) - 1, ja = (int)floorf(y - LIST_SKIN) - 1;
+  const int wx = (int)floorf(x + LIST_SKIN) + 2 - ia, wy = (int)floorf(y + LIST_SKIN) + 2 - ja;  // 3 or 4
+  const int i0 = wrapi(ia, nx), j0 = wrapi(ja, ny);
+  const int i3 = (i0 + wx >= nx) ? i0 + wx - nx : i0 + wx, j3 = (j0 + wy >= ny) ? j0 + wy - ny : j0 + wy;
   const int txa = i0 / TS, txb = i3 / TS, tya = j0 / TS, tyb = j3 / TS;
   int n = 0;
   t[n++] = tya * ntx + txa;

@@ -1,11 +1,11 @@
-// k_blur.cuh -- K3a: S3 Gaussian filter + gradient of the deposited bead density, one pass
-// through shared memory.
+// k_blur.cuh -- K3a: S3 Gaussian filter + gradient of the deposited bead density, one kernel,
+// intermediates in shared memory.
 //
 // "node positions are deposited onto a grid, diffused with a Gaussian filter via FFT
 // convolution to produce a density field, and the gradient of this density field generates
 // repulsive forces."  Reading 14: the filter is the periodic convolution with the sampled,
-// normalised Gaussian truncated at R (= the paper's filter to 2.6e-8 at R = 5 sigma), applied
-// along x then along y; reading 15: second-order central difference.
+// normalised Gaussian truncated at R (= the paper's filter to 2.6e-8 at R = 5 sigma), separable
+// (applied here along y, then along x); reading 15: second-order central difference.
 //
 // Output: the force-gradient planes A = sum_fields coupling_k * grad(field_k) with the sign of
 // the force (-kappa_rep for bead-density fields, +kappa_chi for static ones; S4 then needs one
@@ -22,104 +22,126 @@ struct BlurTaps {
   float g[2 * BLUR_MAX_R + 1];
 };
 
-// shared-memory geometry for radius R.  The input tile starts P nodes left of the output tile,
-// P the smallest multiple of 4 >= R+1, so that every global and shared access of the x pass is
-// a 16-byte one; the x pass then produces its outputs from column i0 - 1 - S on, S = P - 1 - R.
-__host__ __device__ constexpr int blur_P(int R) { return 4 * ((R + 1 + 3) / 4); }
-__host__ __device__ constexpr int blur_S(int R) { return blur_P(R) - 1 - R; }
-__host__ __device__ constexpr int blur_NC(int R) { return (BLUR_T + 2 + blur_S(R) + 3) / 4; }  // x chunks
-__host__ __device__ constexpr int blur_TWP(int R) { return 4 * blur_NC(R); }                    // filtered pitch
-__host__ __device__ constexpr int blur_HP(int R) { return 4 * ((blur_TWP(R) + 2 * R + 3) / 4); } // input pitch
-__host__ __device__ constexpr int blur_H(int R) { return BLUR_T + 2 * R + 2; }                  // input rows
-__host__ __device__ constexpr size_t blur_smem_bytes(int R) {
-  return sizeof(float) * ((size_t)blur_H(R) * blur_HP(R) + (size_t)(blur_H(R) + 4) * blur_TWP(R));
-}
+// shared-memory geometry for radius R.  The two intermediate planes hold the 32 rows of the tile
+// and the columns from node i0 - (R+1) on, so that the x pass of the 8 outputs starting at node
+// i0 + 8c reads its window from column 8c: every shared access of the x pass is a 16-byte one.
+constexpr int BLUR_THREADS = 192;
+__host__ __device__ constexpr int blur_NV(int R) { return 10 + 2 * R; }               // window: 8 outputs + 2 + 2R
+__host__ __device__ constexpr int blur_NV4(int R) { return (blur_NV(R) + 3) / 4; }
+__host__ __device__ constexpr int blur_CW(int R) { return 24 + 4 * blur_NV4(R); }     // plane pitch >= 34 + 2R
 
-// One CTA filters one 32x32 tile.  Stages (all in shared memory, one read of rho_b per node plus
-// the halo, one write of the gradient):
-//   load  H x HP nodes of rho_b with 16-byte loads, periodic indices
-//   x pass: each thread produces 4 consecutive outputs of one row from a register window
-//           (4+2R inputs fetched with 16-byte LDS)                       -> tmp[H][TWP]
-//   y pass: each thread produces 4 consecutive outputs of one column    -> bl[36][TWP]
-//   central difference, scale by the signed coupling, add the base field, store float2.
-// coef: lattice coupling with the sign of the force.  base: interleaved field added to the
-// result (static part, or the running sum over earlier bead-density fields), may be NULL.
-// A: interleaved (x,y) force-gradient field.  field_out (filtered density) may be NULL.
+// One CTA filters one 32x32 tile; rho_b is read once per node plus the halo (through L1), the
+// gradient is written once, nothing else touches global memory.  The y pass comes first because
+// its loads are then coalesced straight from global memory (lanes = columns) and the y-derivative
+// is a register operation on its outputs:
+//   y pass: thread = (column of the tile + x halo, chunk of 8 rows): 10 + 2R loads of its
+//           column, ty = G_y rho_b on 10 rows, of which 8 are stored together with
+//           dy = (ty[y+1] - ty[y-1]) / 2                                   -> ty, dy [32][CW]
+//   x pass: thread = (row, chunk of 8 nodes): register windows of ty and dy (16-byte LDS),
+//           B = G_x ty on 10 nodes, grad_x = (B[x+1] - B[x-1]) / 2, grad_y = G_x dy on 8 nodes,
+//           scaled by the signed coupling, plus the base field, stored as 16-byte pieces of the
+//           blocked layout.
+// (G_x G_y = G_y G_x and the differences commute with both: the result is the oracle's central
+// difference of the filtered field up to rounding order.)
+// coef: lattice coupling with the sign of the force.  base: blocked field added to the result
+// (static part, or the running sum over earlier bead-density fields), may be NULL.
+// A: blocked (x,y) force-gradient field.  field_out (filtered density, row-major) may be NULL.
 template <int R>
-__global__ void __launch_bounds__(256) k_blur_grad(int nx, int ny, BlurTaps taps,
-                                                   const float* __restrict__ rho_b, float coef,
-                                                   const float2* base, float2* A,
-                                                   float* __restrict__ field_out) {
-  extern __shared__ __align__(16) float sm[];
-  constexpr int H = blur_H(R), HP = blur_HP(R), TWP = blur_TWP(R), NC = blur_NC(R);
-  constexpr int P = blur_P(R), S = blur_S(R);
-  constexpr int NV = 4 + 2 * R, NV4 = (NV + 3) / 4, HP4 = HP / 4;
-  float* in = sm;                    // [H][HP]    in[y][x]  <-> node (j0-R-1+y, i0-P+x)
-  float* tmp = sm + (size_t)H * HP;  // [H+4][TWP] tmp[y][t] <-> node (j0-R-1+y, i0-1-S+t)
+__global__ void __launch_bounds__(BLUR_THREADS, 7) k_blur_grad(int nx, int ny, BlurTaps taps,
+                                                            const float* __restrict__ rho_b, float coef,
+                                                            const float2* base, float2* A,
+                                                            float* __restrict__ field_out) {
+  constexpr int NV = blur_NV(R), NV4 = blur_NV4(R), CW = blur_CW(R);
+  __shared__ __align__(16) float ty[BLUR_T * CW], dy[BLUR_T * CW];
   // 1-D grid in row-major tile order (2-D grids are rasterised in an order that streams worse)
   const int ntx = nx / BLUR_T;
   const int i0 = (blockIdx.x % ntx) * BLUR_T, j0 = (blockIdx.x / ntx) * BLUR_T;
-  float g[2 * R + 1];
-#pragma unroll
-  for (int k = 0; k <= 2 * R; ++k) g[k] = taps.g[k];
-  const int nx4 = nx >> 2, gc0 = (i0 - P) >> 2;  // arithmetic shift: i0 - P may be negative
-  for (int it = threadIdx.x; it < H * HP4; it += 256) {
-    const int y = it / HP4, v = it - y * HP4;
-    const int gj = wrap1(j0 - R - 1 + y, ny);  // halo <= R+1 < ny
-    const int gc = wrap1(gc0 + v, nx4);
-    reinterpret_cast<float4*>(in)[it] = __ldg(reinterpret_cast<const float4*>(rho_b + (size_t)gj * nx) + gc);
-  }
-  __syncthreads();
-  // x pass: items (row y, chunk c of 4 outputs)
-  for (int it = threadIdx.x; it < H * NC; it += 256) {
-    const int y = it / NC, c = it - y * NC;
-    float v[4 * NV4];
-    const float4* p = reinterpret_cast<const float4*>(in + y * HP + 4 * c);
-#pragma unroll
-    for (int q = 0; q < NV4; ++q) {
-      const float4 t = p[q];
-      v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
-    }
-    float o[4];
-#pragma unroll
-    for (int a = 0; a < 4; ++a) {
-      float s = 0.0f;
-#pragma unroll
-      for (int k = 0; k <= 2 * R; ++k) s = fmaf(g[k], v[a + k], s);
-      o[a] = s;
-    }
-    *reinterpret_cast<float4*>(tmp + y * TWP + 4 * c) = make_float4(o[0], o[1], o[2], o[3]);
-  }
-  for (int x = threadIdx.x; x < 4 * TWP; x += 256) tmp[H * TWP + x] = 0.0f;  // pad rows
-  __syncthreads();
-  // y pass: items (chunk c of 4 output rows, column t); bl[36][TWP] overwrites `in`
-  float* bl = in;                    // bl[y][t] <-> node (j0-1+y, i0-1-S+t)
-  for (int it = threadIdx.x; it < 9 * TWP; it += 256) {
-    const int c = it / TWP, x = it - c * TWP;
+  // y pass: items (chunk c of 8 rows, column col <-> node i0 - (R+1) + col)
+  for (int it = threadIdx.x; it < 4 * CW; it += BLUR_THREADS) {
+    const int c = it / CW, col = it - c * CW;
+    const int gi = wrap1(i0 - (R + 1) + col, nx);           // halo R+1 < 32 <= nx
+    const int r0 = j0 + 8 * c - 1 - R;                      // first row of the window
     float v[NV];
+    if (j0 - 1 - R >= 0 && j0 + BLUR_T + 1 + R <= ny) {     // tile away from the y seam: no row wraps
+      const float* p = rho_b + (size_t)r0 * nx + gi;
 #pragma unroll
-    for (int k = 0; k < NV; ++k) v[k] = tmp[(4 * c + k) * TWP + x];
+      for (int k = 0; k < NV; ++k) { v[k] = __ldg(p); p += nx; }
+    } else {
 #pragma unroll
-    for (int a = 0; a < 4; ++a) {
+      for (int k = 0; k < NV; ++k) v[k] = __ldg(rho_b + (size_t)wrap1(r0 + k, ny) * nx + gi);
+    }
+    float t[10];
+#pragma unroll
+    for (int a = 0; a < 10; ++a) {
       float s = 0.0f;
 #pragma unroll
-      for (int k = 0; k <= 2 * R; ++k) s = fmaf(g[k], v[a + k], s);
-      bl[(4 * c + a) * TWP + x] = s;
+      for (int k = 0; k <= 2 * R; ++k) s = fmaf(taps.g[k], v[a + k], s);
+      t[a] = s;                                             // ty at row j0 + 8c - 1 + a
+    }
+#pragma unroll
+    for (int a = 0; a < 8; ++a) {
+      ty[(8 * c + a) * CW + col] = t[a + 1];
+      dy[(8 * c + a) * CW + col] = 0.5f * (t[a + 2] - t[a]);
     }
   }
   __syncthreads();
-  for (int t = threadIdx.x; t < BLUR_T * BLUR_T; t += 256) {
-    // 16 consecutive threads own one 4x4 block of the blocked output: a warp stores two full lines
-    const int bl_id = t >> 4, n = t & 15;
-    const int y = ((bl_id >> 3) << 2) + (n >> 2), xo = ((bl_id & 7) << 2) + (n & 3), x = xo + S;
-    const float gx = 0.5f * (bl[(y + 1) * TWP + x + 2] - bl[(y + 1) * TWP + x]);
-    const float gy = 0.5f * (bl[(y + 2) * TWP + x + 1] - bl[y * TWP + x + 1]);
-    const size_t gidx = (size_t)(j0 + y) * nx + (i0 + xo);
-    float2 a = make_float2(coef * gx, coef * gy);
-    const size_t bidx = blk_index(i0 + xo, j0 + y, nx);  // A and base are blocked (mc_common.cuh)
-    if (base) { const float2 b = base[bidx]; a.x += b.x; a.y += b.y; }
-    A[bidx] = a;
-    if (field_out) field_out[gidx] = bl[(y + 1) * TWP + x + 1];
+  // x pass: items (row, chunk c of 8 nodes); 4 consecutive threads cover one row
+  for (int it = threadIdx.x; it < BLUR_T * 4; it += BLUR_THREADS) {
+    const int c = it & 3, row = it >> 2;
+    float v[4 * NV4];
+    {
+      const float4* p = reinterpret_cast<const float4*>(ty + row * CW + 8 * c);
+#pragma unroll
+      for (int q = 0; q < NV4; ++q) {
+        const float4 t4 = p[q];
+        v[4 * q] = t4.x; v[4 * q + 1] = t4.y; v[4 * q + 2] = t4.z; v[4 * q + 3] = t4.w;
+      }
+    }
+    float B[10];                                            // filtered density at nodes i0 + 8c - 1 + a
+#pragma unroll
+    for (int a = 0; a < 10; ++a) {
+      float s = 0.0f;
+#pragma unroll
+      for (int k = 0; k <= 2 * R; ++k) s = fmaf(taps.g[k], v[a + k], s);
+      B[a] = s;
+    }
+    {
+      const float4* p = reinterpret_cast<const float4*>(dy + row * CW + 8 * c);
+#pragma unroll
+      for (int q = 0; q < NV4; ++q) {
+        const float4 t4 = p[q];
+        v[4 * q] = t4.x; v[4 * q + 1] = t4.y; v[4 * q + 2] = t4.z; v[4 * q + 3] = t4.w;
+      }
+    }
+    float2 o[8];
+#pragma unroll
+    for (int a = 0; a < 8; ++a) {
+      float s = 0.0f;
+#pragma unroll
+      for (int k = 0; k <= 2 * R; ++k) s = fmaf(taps.g[k], v[a + 1 + k], s);
+      o[a] = make_float2(coef * (0.5f * (B[a + 2] - B[a])), coef * s);
+    }
+    // nodes (i0 + 8c .. + 7, j0 + row): two 32-byte rows of two neighbouring 4x4 blocks
+    const size_t bidx = blk_index(i0 + 8 * c, j0 + row, nx);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      float4* dst = reinterpret_cast<float4*>(A + bidx + 16 * h);
+      float4 lo = make_float4(o[4 * h].x, o[4 * h].y, o[4 * h + 1].x, o[4 * h + 1].y);
+      float4 hi = make_float4(o[4 * h + 2].x, o[4 * h + 2].y, o[4 * h + 3].x, o[4 * h + 3].y);
+      if (base) {
+        const float4* src = reinterpret_cast<const float4*>(base + bidx + 16 * h);
+        const float4 b0 = src[0], b1 = src[1];
+        lo.x += b0.x; lo.y += b0.y; lo.z += b0.z; lo.w += b0.w;
+        hi.x += b1.x; hi.y += b1.y; hi.z += b1.z; hi.w += b1.w;
+      }
+      dst[0] = lo;
+      dst[1] = hi;
+    }
+    if (field_out) {
+      float4* f = reinterpret_cast<float4*>(field_out + (size_t)(j0 + row) * nx + i0 + 8 * c);
+      f[0] = make_float4(B[1], B[2], B[3], B[4]);
+      f[1] = make_float4(B[5], B[6], B[7], B[8]);
+    }
   }
 }
 

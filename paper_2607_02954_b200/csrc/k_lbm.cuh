@@ -120,7 +120,7 @@ struct LbmSpreadArgs {
 
 template <bool KEEP_G>
 __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
-  __shared__ int acc0[TS * TSP], acc1[TS * TSP], accl0[TS * TSP], accl1[TS * TSP];
+  __shared__ int acc0[ACC_N], acc1[ACC_N], accl0[ACC_N], accl1[ACC_N];
   __shared__ float red[32];
   const LbmArgs& a = p.lbm;
   const int nx = a.nx, ny = a.ny;
@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
     if (h) load_pair(ly);
     const size_t r0 = (size_t)j * nx;
     const size_t c = r0 + i;
-    const int sa = ly * TSP + lx;
+    const int sa = acc_index(lx, ly);
     const float GAx = tile_value(acc0, accl0, sa, linv) * inv, GAy = tile_value(acc1, accl1, sa, linv) * inv;
     const float GBx = tile_value(acc0, accl0, sa + 1, linv) * inv, GBy = tile_value(acc1, accl1, sa + 1, linv) * inv;
     if (KEEP_G) {

@@ -27,19 +27,20 @@
 
 namespace mc {
 
-// A listed bead seen from one tile: node offsets clamped into the tile and weights MASKED to
-// zero outside it, so that the 16 accumulations below need no branch (a bead overlapping the
-// tile only partly adds exact zeros to a clamped address, which changes nothing).
-// Row pitch of the shared accumulator tiles.  Lanes of a warp hold consecutive beads of a chain,
-// i.e. nodes about one cell apart in an arbitrary direction; with pitch 32 a vertical chain would
-// put all 32 lanes on one bank.  37 = 5 (mod 32) has no bank collision for offsets |dr|,|dc| <= 2.
-constexpr int TSP = 37;
+// A listed bead seen from one tile.  Common case: `base` is the accumulator index of its first
+// support node (accumulators carry a halo, k_tile.cuh), the 16 contributions go to base +
+// r * TSP + c unconditionally.  WRAP_IN_TILE case (domain one tile wide along an axis, where a
+// support can wrap around onto the same tile): per-node offsets folded into the tile and
+// weights masked to zero outside it.
 constexpr int WIDE_N = 1024;  // listed beads above which a tile accumulates hi + lo words
 
 struct TileBead {
-  int col[4], row[4];    // col: local x (0..TS-1); row: local y * TSP
-  float wx[4], wy[4];    // 0 where the support node lies outside the tile
+  int base;
+  int col[4], row[4];    // WRAP_IN_TILE only.  col: halo + local x; row: (halo + local y) * TSP
+  float wx[4], wy[4];
 };
+
+__device__ __forceinline__ int acc_index(int lx, int ly) { return (ly + HALO) * TSP + lx + HALO; }
 
 // distance (in nodes, periodic) from the tile origin to the first support node, in [-n/2, n/2)
 __device__ __forceinline__ int tile_delta(int i0, int origin, int n) {
@@ -68,26 +69,28 @@ __device__ __forceinline__ void tile_bead(float2 p, int nx, int ny, int x0, int 
   if (WRAP_IN_TILE) {
     i0 = wrapi(i0, nx);
     j0 = wrapi(j0, ny);
-  } else {
-    i0 = tile_delta(i0, x0, nx);
-    j0 = tile_delta(j0, y0, ny);
-  }
 #pragma unroll
-  for (int k = 0; k < 4; ++k) {
-    int c, r;
-    if (WRAP_IN_TILE) {
-      c = ((i0 + k >= nx) ? i0 + k - nx : i0 + k) - x0;
-      r = ((j0 + k >= ny) ? j0 + k - ny : j0 + k) - y0;
-    } else {
-      c = i0 + k;
-      r = j0 + k;
+    for (int k = 0; k < 4; ++k) {
+      const int c = ((i0 + k >= nx) ? i0 + k - nx : i0 + k) - x0;
+      const int r = ((j0 + k >= ny) ? j0 + k - ny : j0 + k) - y0;
+      const bool cin = (unsigned)c < (unsigned)TS, rin = (unsigned)r < (unsigned)TS;
+      tb.col[k] = HALO + (cin ? c : 0);
+      tb.row[k] = (HALO + (rin ? r : 0)) * TSP;
+      tb.wx[k] = cin ? tb.wx[k] : 0.0f;
+      tb.wy[k] = rin ? tb.wy[k] : 0.0f;
     }
-    const bool cin = (unsigned)c < (unsigned)TS, rin = (unsigned)r < (unsigned)TS;
-    tb.col[k] = cin ? c : 0;
-    tb.row[k] = rin ? r * TSP : 0;
-    tb.wx[k] = cin ? tb.wx[k] : 0.0f;
-    tb.wy[k] = rin ? tb.wy[k] : 0.0f;
+  } else {
+    // a first node outside [-HALO, TS] has no support node inside the tile (a stale entry
+    // cannot get there, k_tile.cuh; the clamp only guards the shared array) and keeps none
+    i0 = min(max(tile_delta(i0, x0, nx), -HALO), TS);
+    j0 = min(max(tile_delta(j0, y0, ny), -HALO), TS);
+    tb.base = acc_index(i0, j0);
   }
+}
+
+template <bool WRAP_IN_TILE>
+__device__ __forceinline__ int tap_index(const TileBead& tb, int l, int kx) {
+  return WRAP_IN_TILE ? tb.row[l] + tb.col[kx] : tb.base + l * TSP + kx;
 }
 
 __device__ __forceinline__ float block_max(float v, float* sm /*[32]*/) {
@@ -121,14 +124,31 @@ __device__ __forceinline__ int lo_bits(int n) {
   return min(20, max(0, 30 - lg));
 }
 
+// Dealing of a tile's key-sorted list (k_tile.cuh) to the CTA: the n entries form W = ceil(n/32)
+// rounds; in round v lane l takes sorted position l W + v, so every lane walks its own short run
+// of (nearly) one key and the 32 lanes of a round hold (nearly) 32 different keys.  Warp w takes
+// the rounds w, w + n_warps, ...
+struct Deal {
+  int W, n, nw, v, p;
+  __device__ __forceinline__ Deal(int n_) : n(n_) {
+    W = (n + 31) >> 5;
+    nw = blockDim.x >> 5;
+    v = threadIdx.x >> 5;
+    p = (threadIdx.x & 31) * W + v;
+  }
+  __device__ __forceinline__ bool valid() const { return v < W && p < n; }
+  __device__ __forceinline__ bool next_valid() const { return v + nw < W && p + nw < n; }
+  __device__ __forceinline__ void advance() { v += nw; p += nw; }
+};
+
 template <bool WIDE, bool WRAP>
 __device__ __forceinline__ void deposit_loop(int nx, int ny, int x0, int y0, int s, int e,
                                              const int* __restrict__ list, const float2* __restrict__ X,
                                              float scale, float lscale, int* acc, int* accl, float2 xpre) {
   float2 xc = xpre;  // first entry preloaded by the caller, later ones one iteration ahead
-  for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
+  for (Deal d(e - s); d.valid(); d.advance()) {
     const float2 xb = xc;
-    if (k + (int)blockDim.x < e) xc = __ldg(X + __ldg(list + k + blockDim.x));
+    if (d.next_valid()) xc = __ldg(X + __ldg(list + s + d.p + d.nw));
     TileBead tb;
     tile_bead<WRAP>(xb, nx, ny, x0, y0, tb);
 #pragma unroll
@@ -136,7 +156,7 @@ __device__ __forceinline__ void deposit_loop(int nx, int ny, int x0, int y0, int
       const float wys = tb.wy[l] * scale;
 #pragma unroll
       for (int kx = 0; kx < 4; ++kx) {
-        const int a = tb.row[l] + tb.col[kx];
+        const int a = tap_index<WRAP>(tb, l, kx);
         const float v = tb.wx[kx] * wys;
         if (WIDE) {
           const float h = rintf(v);
@@ -160,10 +180,10 @@ __device__ __forceinline__ void spread_loop(int nx, int ny, int x0, int y0, int 
   // so that the list -> X/F gather latency is spent under them; later entries are software-
   // pipelined one iteration ahead
   float2 xc = xpre, fc = fpre;
-  for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
+  for (Deal d(e - s); d.valid(); d.advance()) {
     const float2 xb = xc, f = fc;
-    if (k + (int)blockDim.x < e) {
-      const int bn = __ldg(list + k + blockDim.x);
+    if (d.next_valid()) {
+      const int bn = __ldg(list + s + d.p + d.nw);
       xc = __ldg(X + bn);
       fc = __ldg(F + bn);
     }
@@ -175,7 +195,7 @@ __device__ __forceinline__ void spread_loop(int nx, int ny, int x0, int y0, int 
       const float wyx = tb.wy[l] * fxs, wyy = tb.wy[l] * fys;
 #pragma unroll
       for (int kx = 0; kx < 4; ++kx) {
-        const int a = tb.row[l] + tb.col[kx];
+        const int a = tap_index<WRAP>(tb, l, kx);
         const float vx = tb.wx[kx] * wyx, vy = tb.wx[kx] * wyy;
         if (WIDE) {
           const float hx = rintf(vx), hy = rintf(vy);
@@ -213,15 +233,18 @@ __global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int*
                                                       float* __restrict__ rho_b,
                                                       float* __restrict__ tile_rho_max,
                                                       unsigned* __restrict__ tile_fmax) {
-  __shared__ int acc[TS * TSP], accl[TS * TSP];
+  __shared__ int acc[ACC_N], accl[ACC_N];
   __shared__ float red[32];
   const int t = blockIdx.y * gridDim.x + blockIdx.x;  // grid = (nx/TS, ny/TS)
   const int x0 = blockIdx.x * TS, y0 = blockIdx.y * TS;
   const int s = tile_start[t], e = tile_start[t + 1];
   const bool wide = (e - s) > WIDE_N;
   float2 xpre = make_float2(0.f, 0.f);
-  if (s + (int)threadIdx.x < e) xpre = __ldg(X + __ldg(list + s + threadIdx.x));  // gather starts before the zeroing
-  for (int c = threadIdx.x; c < TS * TSP; c += blockDim.x) { acc[c] = 0; if (wide) accl[c] = 0; }
+  {
+    const Deal d(e - s);
+    if (d.valid()) xpre = __ldg(X + __ldg(list + s + d.p));  // gather starts before the zeroing
+  }
+  for (int c = threadIdx.x; c < ACC_N; c += blockDim.x) { acc[c] = 0; if (wide) accl[c] = 0; }
   const float scale = pow2_scale(fmaxf(0.25f * (float)(e - s), 1.0f));
   const float lscale = pow2f(lo_bits(e - s));
   __syncthreads();
@@ -232,7 +255,7 @@ __global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int*
   const float inv = 1.0f / scale, linv = 1.0f / lscale;
   float mx = 0.0f;
   for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) {
-    const int a = (c >> 5) * TSP + (c & 31);
+    const int a = acc_index(c & 31, c >> 5);
     const float v = (wide ? fmaf((float)accl[a], linv, (float)acc[a]) : (float)acc[a]) * inv;
     rho_b[(size_t)(y0 + (c >> 5)) * nx + x0 + (c & 31)] = v;
     mx = fmaxf(mx, v);
@@ -262,14 +285,17 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
                                                         float* red, float& linv) {
   const bool wide = (e - s) > WIDE_N;
   float2 xpre = make_float2(0.f, 0.f), fpre = make_float2(0.f, 0.f);
-  if (s + (int)threadIdx.x < e) {  // first entry of this thread: start its gather now
-    const int b = __ldg(list + s + threadIdx.x);
-    xpre = __ldg(X + b);
-    fpre = __ldg(F + b);
+  {
+    const Deal d(e - s);
+    if (d.valid()) {  // first entry of this thread: start its gather now
+      const int b = __ldg(list + s + d.p);
+      xpre = __ldg(X + b);
+      fpre = __ldg(F + b);
+    }
   }
   const float lscale = pow2f(lo_bits(e - s));
   linv = wide ? 1.0f / lscale : 0.0f;  // 0 => the readers skip the lo planes (not zeroed then)
-  for (int c = threadIdx.x; c < TS * TSP; c += blockDim.x) {
+  for (int c = threadIdx.x; c < ACC_N; c += blockDim.x) {
     acc0[c] = 0; acc1[c] = 0;
     if (wide) { accl0[c] = 0; accl1[c] = 0; }
   }
@@ -291,7 +317,7 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
     __syncthreads();  // also orders the zeroing before the atomics
     fm = red[0];
   } else {
-    for (int k = s + threadIdx.x; k < e; k += blockDim.x) {
+    for (int k = s + threadIdx.x; k < e; k += blockDim.x) {  // any order
       const float2 f = __ldg(F + __ldg(list + k));
       fm = fmaxf(fm, fmaxf(fabsf(f.x), fabsf(f.y)));
     }

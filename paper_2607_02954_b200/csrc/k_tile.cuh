@@ -12,18 +12,33 @@
 // schedule touches the results only through the per-tile fixed-point scales (powers of two
 // chosen from the list lengths), i.e. at rounding level; it is a function of the state alone,
 // so runs stay bit-reproducible and mc_step(a), mc_step(b) equals mc_step(a + b).
-//   count : per bead, +1 on each overlapped tile (integer atomics, warp-aggregated)
-//   scan  : exclusive prefix sum over the tiles (one block; there are few tiles)
-//   fill  : per bead, claim a slot in each overlapped tile's segment and store the bead index
-// The order inside a tile's list is the arrival order of the atomics and is NOT reproducible;
-// that is harmless because the accumulation that consumes the lists (k_p2g.cuh) adds integers
-// (fixed point), which is order-independent.
+//   count  : per bead, +1 on each overlapped tile (integer atomics, warp-aggregated) and +1 on
+//            the (tile, bank key) bucket
+//   scan   : exclusive prefix sum over the tiles (one block; there are few tiles)
+//   starts : one warp per tile turns its 32 bucket counts into cursors inside the tile's segment
+//   fill   : per bead, claim a slot in each overlapped tile's bucket and store the bead index
+// A tile's list is thus ordered by the BANK KEY of its entries: the shared-memory bank of the
+// first accumulator node a bead touches (bead_key).  The consumers (k_p2g.cuh) deal the sorted
+// entries to the lanes so that the lanes of one atomic instruction hold different keys, i.e.
+// land on different banks (arrival order made them collide ~3.4-fold).  Stale keys (beads move
+// between rebuilds) cost a few conflicts, never correctness.  The order inside a bucket is the
+// arrival order of the atomics and is NOT reproducible; that is harmless because the
+// accumulation that consumes the lists adds integers (fixed point), which is order-independent.
 #pragma once
 #include "mc_common.cuh"
 
 namespace mc {
 
 constexpr int TS = 32;          // tile side in nodes
+// Shared accumulator of a tile (k_p2g.cuh): the TS x TS nodes plus a HALO of 4 on every side, so
+// that every support of a listed bead (first node within [-4, TS] of the tile origin, skin
+// included) fits and the 16 contributions go to base + constant offsets with no clamping; halo
+// sums are dropped (the neighbouring tiles accumulate them from their own lists).  Row pitch 41
+// = 9 (mod 32): the 16 nodes of a support lie on 16 different banks.
+constexpr int HALO = 4;
+constexpr int AW = TS + 2 * HALO;
+constexpr int TSP = 41;
+constexpr int ACC_N = AW * TSP;
 constexpr float LIST_SKIN = 0.25f;  // a bead is listed as if it sat anywhere within +-LIST_SKIN of its position
 constexpr float LIST_DRIFT_MAX = 0.22f;  // rebuild when the accumulated drift bound exceeds this (< LIST_SKIN)
 
@@ -61,6 +76,14 @@ __device__ __forceinline__ int bead_tiles(float x, float y, int nx, int ny, int 
   return n;
 }
 
+// Bank key of a bead: accumulator address of support node (r, c) is (j0 + r) * TSP + i0 + c (+ a
+// constant) with (i0, j0) the first support node relative to the tile origin; tile origins and
+// the periods nx, ny are multiples of 32, so the bank is key + TSP r + c (mod 32) with this key
+// for every tile the bead is listed in.
+__device__ __forceinline__ int bead_key(float x, float y) {
+  return ((TSP & 31) * ((int)floorf(y) - 1) + (int)floorf(x) - 1) & 31;
+}
+
 // warp-aggregated atomicAdd(&ctr[key], 1) for the lanes with act set; returns the claimed value
 __device__ __forceinline__ int warp_claim(int* ctr, int key, bool act) {
   const unsigned m = __ballot_sync(0xffffffffu, act);
@@ -77,35 +100,61 @@ __device__ __forceinline__ int warp_claim(int* ctr, int key, bool act) {
   return slot;
 }
 
-// FILL = false: tile_ctr[t] += 1 per listed bead.  FILL = true: tile_ctr holds the running
-// cursor (initialised to tile_start) and the bead index is stored at the claimed slot.
+// FILL = false: tile_ctr[t] += 1 and (if given) bucket_ctr[32 t + key] += 1 per listed bead.
+// FILL = true: bucket_ctr holds the running cursors (k_bucket_starts) and the bead index is
+// stored at the claimed slot.
 template <bool FILL>
 __global__ void __launch_bounds__(256) k_tile_bin(const ListState* __restrict__ st, const float2* __restrict__ X,
                                                   int N, int nx, int ny, int* __restrict__ tile_ctr,
-                                                  int* __restrict__ list) {
+                                                  int* __restrict__ bucket_ctr, int* __restrict__ list) {
   if (!st->need) return;
   // grid-stride over whole blocks of beads: every lane of a warp takes part in warp_claim
   for (int base = blockIdx.x * blockDim.x; base < N; base += gridDim.x * blockDim.x) {
     const int b = base + threadIdx.x;
     int t[4] = {0, 0, 0, 0};
-    int n = 0;
+    int n = 0, key = 0;
     if (b < N) {
       const float2 p = X[b];
       n = bead_tiles(p.x, p.y, nx, ny, nx / TS, t);
+      key = bead_key(p.x, p.y);
     }
 #pragma unroll
     for (int s = 0; s < 4; ++s) {
-      const int slot = warp_claim(tile_ctr, t[s], s < n);
-      if (FILL && s < n) list[slot] = b;
+      if (FILL) {
+        if (s < n) list[atomicAdd(&bucket_ctr[32 * t[s] + key], 1)] = b;
+      } else {
+        warp_claim(tile_ctr, t[s], s < n);
+        if (bucket_ctr && s < n) atomicAdd(&bucket_ctr[32 * t[s] + key], 1);
+      }
     }
   }
 }
 
-// one block: tile_start = exclusive scan of tile_count (n_tiles + 1 entries); the cursor array
-// for the fill pass is initialised to tile_start; counts are zeroed for the next step.
+// one warp per tile: bucket_cursor[32 t + k] = tile_start[t] + exclusive scan of the tile's 32
+// bucket counts; the counts are zeroed for the next rebuild.
+__global__ void __launch_bounds__(256) k_bucket_starts(const ListState* __restrict__ st, int n_tiles,
+                                                       const int* __restrict__ tile_start,
+                                                       int* __restrict__ bucket_count,
+                                                       int* __restrict__ bucket_cursor) {
+  if (!st->need) return;
+  const int lane = threadIdx.x & 31;
+  const int t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (t >= n_tiles) return;
+  const int v = bucket_count[32 * t + lane];
+  int inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int u = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += u;
+  }
+  bucket_cursor[32 * t + lane] = tile_start[t] + inc - v;
+  bucket_count[32 * t + lane] = 0;
+}
+
+// one block: tile_start = exclusive scan of tile_count (n_tiles + 1 entries); counts are zeroed
+// for the next rebuild.
 __global__ void __launch_bounds__(1024) k_tile_scan(const ListState* __restrict__ st, int* __restrict__ tile_count,
-                                                    int n_tiles, int* __restrict__ tile_start,
-                                                    int* __restrict__ tile_cursor) {
+                                                    int n_tiles, int* __restrict__ tile_start) {
   __shared__ int sm[33];
   if (!st->need) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -136,7 +185,6 @@ __global__ void __launch_bounds__(1024) k_tile_scan(const ListState* __restrict_
     if (i < n_tiles) {
       const int ex = carry + sm[wid] + inc - v;
       tile_start[i] = ex;
-      tile_cursor[i] = ex;
       tile_count[i] = 0;
     }
     carry += sm[32];

@@ -27,7 +27,7 @@ constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
-  size_t fA, fB, u, rho_b, A, G, cfield, csum, As, tile_count, tile_start, tile_cursor, tile_rho_max, tile_fmax;
+  size_t fA, fB, u, rho_b, A, G, cfield, csum, As, tile_count, tile_start, bucket_count, bucket_cursor, tile_rho_max, tile_fmax;
   size_t X, PA, PB, PC, F, sense, list, src, bflags, scratch, flags, sources;
   size_t total;
 };
@@ -86,7 +86,8 @@ Layout make_layout(const mc_world_params* p, const Derived& d) {
   const size_t nt = nc / (mc::TS * mc::TS);
   L.tile_count = take(nt * 4);
   L.tile_start = take((nt + 1) * 4);
-  L.tile_cursor = take(nt * 4);
+  L.bucket_count = take(nt * 32 * 4);   // per (tile, bank key), zero outside a rebuild
+  L.bucket_cursor = take(nt * 32 * 4);
   L.tile_rho_max = take(nt * 4);
   L.tile_fmax = take(nt * 4);
   L.X = take(N * 8);
@@ -178,7 +179,7 @@ int pick_bx(int nx) { return nx % 256 == 0 ? 256 : (nx % 128 == 0 ? 128 : (nx % 
 template <int R>
 void launch_blur_R(mc_world* w, int k, const float2* base, float2* A, float* field_out) {
   const int grid = (w->nx / mc::BLUR_T) * (w->ny / mc::BLUR_T);
-  mc::k_blur_grad<R><<<grid, 256, mc::blur_smem_bytes(R), w->stream>>>(
+  mc::k_blur_grad<R><<<grid, mc::BLUR_THREADS, 0, w->stream>>>(
       w->nx, w->ny, w->taps[k], w->ptr<float>(w->L.rho_b), w->coef[k], base, A, field_out);
 }
 
@@ -204,7 +205,8 @@ int enqueue_step(mc_world* w) {
   float2* F = w->ptr<float2>(w->L.F);
   int* tile_count = w->ptr<int>(w->L.tile_count);
   int* tile_start = w->ptr<int>(w->L.tile_start);
-  int* tile_cursor = w->ptr<int>(w->L.tile_cursor);
+  int* bucket_count = w->ptr<int>(w->L.bucket_count);
+  int* bucket_cursor = w->ptr<int>(w->L.bucket_cursor);
   float* tile_rho_max = w->ptr<float>(w->L.tile_rho_max);
   unsigned* tile_fmax = w->d.n_density ? w->ptr<unsigned>(w->L.tile_fmax) : nullptr;
   int* list = w->ptr<int>(w->L.list);
@@ -225,10 +227,11 @@ int enqueue_step(mc_world* w) {
     mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16);
     const int k0grid = bgrid < 148 * 8 ? bgrid : 148 * 8;
     mc::k_list_policy<<<1, 1, 0, st>>>(ls_state);
-    mc::k_tile_bin<false><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, tile_count, nullptr);
-    mc::k_tile_scan<<<1, 1024, 0, st>>>(ls_state, tile_count, n_tiles, tile_start, tile_cursor);
-    mc::k_tile_bin<true><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, tile_cursor, list);
-    w->launches += 4;
+    mc::k_tile_bin<false><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, tile_count, bucket_count, nullptr);
+    mc::k_tile_scan<<<1, 1024, 0, st>>>(ls_state, tile_count, n_tiles, tile_start);
+    mc::k_bucket_starts<<<(n_tiles + 7) / 8, 256, 0, st>>>(ls_state, n_tiles, tile_start, bucket_count, bucket_cursor);
+    mc::k_tile_bin<true><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, nullptr, bucket_cursor, list);
+    w->launches += 5;
     prof_mark(w, 1);
     // K2a: S2 deposit
     if (w->d.n_density) {
@@ -548,7 +551,7 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
     mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16);
     cudaMemcpyAsync(ls_state, &force, sizeof(force), cudaMemcpyHostToDevice, st);
     mc::k_tile_bin<false><<<(int)((N + 255) / 256), 256, 0, st>>>(ls_state, w->ptr<float2>(w->L.X), (int)N, w->nx,
-                                                                  w->ny, tile_count, nullptr);
+                                                                  w->ny, tile_count, nullptr, nullptr);
     mc::k_max_int<<<64, 256, 0, st>>>(tile_count, n_tiles, maxlist);
     cudaMemsetAsync(tile_count, 0, (size_t)n_tiles * 4, st);
     w->launches += 2;

@@ -28,7 +28,7 @@ inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
   size_t fA, fB, u, rho_b, A, G, cfield, csum, As, tile_count, tile_start, bucket_count, bucket_cursor, tile_rho_max, tile_fmax;
-  size_t X, PA, PB, PC, F, sense, list, src, bflags, scratch, flags, sources;
+  size_t X, PA, PB, PC, PD, F, sense, list, src, bflags, scratch, flags, sources;
   size_t total;
 };
 
@@ -94,6 +94,7 @@ Layout make_layout(const mc_world_params* p, const Derived& d) {
   L.PA = take(N * 16);
   L.PB = take(N * 16);
   L.PC = take(N * 16);
+  L.PD = take(N * 8);
   L.F = take(N * 8);
   L.sense = take(N * 4);
   L.list = take(N * 4 * 4);   // a bead is listed in at most 4 tiles
@@ -122,6 +123,7 @@ struct mc_world {
   int N = 0;
   int stride = 60;   // K1 window advance: 64 when all chains share a length dividing 64
   int n_windows = 0;
+  bool uniform_params = false;  // K1 variant: L_rest, stiffnesses and period identical for all beads
   int deposit_threads = 128;  // CTA size of K2a: 128 hides the per-tile latency better, crowded worlds want 256
   // CUDA graphs of GRAPH_STEPS consecutive steps, one per ping-pong phase, captured on first use
   // (the ping-pong phase is the only host-side state a step depends on); GRAPH_STEPS is even
@@ -254,6 +256,8 @@ int enqueue_step(mc_world* w) {
     fa.PA = w->ptr<float4>(w->L.PA);
     fa.PB = w->ptr<float4>(w->L.PB);
     fa.PC = w->ptr<float4>(w->L.PC);
+    fa.PD = w->ptr<float2>(w->L.PD);
+    fa.uni = reinterpret_cast<const float4*>(w->ptr<int>(w->L.flags) + 24);  // flags[24..31]
     fa.F = F;
     fa.sense = w->ptr<float>(w->L.sense);
     fa.A = w->d.n_density ? w->ptr<float2>(w->L.A) : (w->d.n_static ? w->ptr<float2>(w->L.As) : nullptr);
@@ -266,7 +270,8 @@ int enqueue_step(mc_world* w) {
     fa.n_windows = w->n_windows;
     fa.kappa = w->kappa;
     fa.step = w->ptr<long long>(w->L.flags) + 4;  // flags[8..9]: device copy of the step counter
-    mc::k_filament_force<<<(w->n_windows + 7) / 8, 256, 0, st>>>(fa);
+    if (w->uniform_params) mc::k_filament_force<true><<<(w->n_windows + 7) / 8, 256, 0, st>>>(fa);
+    else mc::k_filament_force<false><<<(w->n_windows + 7) / 8, 256, 0, st>>>(fa);
     prof_mark(w, 4);
     w->launches++;
   } else {
@@ -531,6 +536,10 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   pa.PA = w->ptr<float4>(w->L.PA);
   pa.PB = w->ptr<float4>(w->L.PB);
   pa.PC = w->ptr<float4>(w->L.PC);
+  pa.PD = w->ptr<float2>(w->L.PD);
+  pa.uni = reinterpret_cast<float4*>(w->ptr<int>(w->L.flags) + 24);
+  pa.nonuniform = w->ptr<int>(w->L.flags) + 3;
+  cudaMemsetAsync(pa.nonuniform, 0, 4, st);
   pa.dt = (double)w->p.dt;
   pa.bad = bad;
   mc::k_pack_params<<<(int)((N + 255) / 256), 256, 0, st>>>(pa);
@@ -560,8 +569,9 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   cudaMemcpyAsync(&h_maxlist, maxlist, 4, cudaMemcpyDeviceToHost, st);
   const long long host_step = w->step;  // steps without beads do not advance the device copy
   cudaMemcpyAsync(w->ptr<long long>(w->L.flags) + 4, &host_step, 8, cudaMemcpyHostToDevice, st);
-  int h = 0;
+  int h = 0, h_nonuni = 0;
   cudaMemcpyAsync(&h, bad, 4, cudaMemcpyDeviceToHost, st);
+  cudaMemcpyAsync(&h_nonuni, w->ptr<int>(w->L.flags) + 3, 4, cudaMemcpyDeviceToHost, st);
   e = cudaStreamSynchronize(st);  // src/bflags are host vectors of this call
   if (e == cudaSuccess) e = cudaGetLastError();
   if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_load_filaments: ") + cudaGetErrorString(e));
@@ -572,6 +582,7 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   w->N = (int)N;
   w->n_fil = n_fil;
   w->deposit_threads = h_maxlist > 1024 ? 256 : 128;
+  w->uniform_params = (h_nonuni == 0);
   if (reuse_order) {
     w->stride = prev_stride;
     w->n_windows = prev_windows;

@@ -98,6 +98,20 @@ def _with_sigma(w, sigma, radius):
     return w
 
 
+def _varied(w, seed):
+    """Per-bead rest lengths and stiffnesses, per-chain actuation periods: the general
+    (non-uniform) parameter path of K1."""
+    rng = np.random.default_rng(seed)
+    n = w["xy"].shape[0]
+    w["L_rest"] = (w["L_rest"] * rng.uniform(0.95, 1.05, n)).astype(np.float32)
+    for k in ("k_bend", "k_shear", "k_stretch"):
+        w[k] = rng.uniform(0.3, 1.0, n).astype(np.float32)
+    off = w["offsets"]
+    for f in range(len(off) - 1):
+        w["act_period"][off[f]:off[f + 1]] *= np.float32(rng.uniform(0.5, 2.0))
+    return w
+
+
 SMALL = {
     # several tiles + ragged chain lengths (3 .. 100 beads: shorter/equal/longer than a warp),
     # chains straddling the periodic boundary and translated by whole periods
@@ -117,6 +131,9 @@ SMALL = {
     "single_tile_32": lambda: worlds.ragged_world(32, 32, [5, 12, 20], seed=11),
     # wide and flat: one tile high, several wide; R = 3 filter; sigma != 1
     "flat_160x32": lambda: _with_sigma(worlds.ragged_world(160, 32, [16, 30, 64, 9], seed=12), 0.6, 3),
+    # rest length, stiffnesses and period differ from bead to bead / chain to chain
+    "varied_params": lambda: _varied(worlds.ragged_world(96, 96, [7, 32, 64, 33, 90, 16, 16], seed=13,
+                                                         static_source=True), 14),
     # uniform 64-bead and 32-bead chains (the shapes of configs 2-4)
     "uniform_m64": lambda: worlds.random_world(128, 96, 40, 64, seed=8),
     "uniform_m32": lambda: worlds.random_world(96, 128, 70, 32, seed=9, static_source=True),

@@ -139,10 +139,17 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
       asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
     }
   }
+  // this thread's first list entry: its list -> X/F gather is the longest latency chain of the
+  // tile, so it starts before the zeroing and the barrier of the atomic phase
+  float2 xpre = make_float2(0.f, 0.f), fpre = make_float2(0.f, 0.f);
+  {
+    const int b = first_entry(s, e, p.list);
+    if (b >= 0) { xpre = __ldg(p.X + b); fpre = __ldg(p.F + b); }
+  }
   float linv;
   const float scale = spread_tile_accumulate(nx, ny, x0, y0, s, e, p.list, p.X, p.F,
                                              p.tile_rho_max ? p.tile_rho_max[t] : 0.0f, p.tile_fmax, t, acc0, acc1,
-                                             accl0, accl1, red, linv);
+                                             accl0, accl1, red, linv, xpre, fpre);
   const float inv = 1.0f / scale;
   if (threadIdx.x == 0 && p.tile_rho_max) p.tile_rho_max[t] = 0.0f;  // all reads happened before the barrier
   // S6 on the tile: each thread owns the node PAIR (i, i+1), i even, in rows ry and ry + 16.

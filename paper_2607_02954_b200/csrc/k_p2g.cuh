@@ -227,7 +227,7 @@ __device__ __noinline__ void spread_loop_wide(int nx, int ny, int x0, int y0, in
 }
 
 // K2a: S2 deposit.  tile_rho_max[t] receives max over the tile of rho_b (for K2b's scale).
-__global__ void __launch_bounds__(256) k_deposit_tile(int nx, int ny, const int* __restrict__ tile_start,
+__global__ void __launch_bounds__(256, 6) k_deposit_tile(int nx, int ny, const int* __restrict__ tile_start,
                                                       const int* __restrict__ list,
                                                       const float2* __restrict__ X,
                                                       float* __restrict__ rho_b,
@@ -273,26 +273,24 @@ __device__ __forceinline__ float tile_value(const int* acc, const int* accl, int
   return (linv != 0.0f) ? fmaf((float)accl[a], linv, (float)acc[a]) : (float)acc[a];
 }
 
+// First list entry of this thread in the tile segment [s, e): bead index, or -1.
+__device__ __forceinline__ int first_entry(int s, int e, const int* __restrict__ list) {
+  const Deal d(e - s);
+  return d.valid() ? __ldg(list + s + d.p) : -1;
+}
+
 // Accumulate the spread force of one tile into shared memory (two planes), return the scale.
 // Used by the fused spread + fluid kernel (k_lbm.cuh), which must __syncthreads() before it
-// reads the accumulators.
+// reads the accumulators.  (xpre, fpre): X and F of this thread's first entry, loaded by the
+// caller well ahead (their list -> X/F gather is the longest latency chain of the tile).
 __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, int y0, int s, int e,
                                                         const int* __restrict__ list,
                                                         const float2* __restrict__ X,
                                                         const float2* __restrict__ F, float rho_max,
                                                         const unsigned* __restrict__ tile_fmax, int t,
                                                         int* acc0, int* acc1, int* accl0, int* accl1,
-                                                        float* red, float& linv) {
+                                                        float* red, float& linv, float2 xpre, float2 fpre) {
   const bool wide = (e - s) > WIDE_N;
-  float2 xpre = make_float2(0.f, 0.f), fpre = make_float2(0.f, 0.f);
-  {
-    const Deal d(e - s);
-    if (d.valid()) {  // first entry of this thread: start its gather now
-      const int b = __ldg(list + s + d.p);
-      xpre = __ldg(X + b);
-      fpre = __ldg(F + b);
-    }
-  }
   const float lscale = pow2f(lo_bits(e - s));
   linv = wide ? 1.0f / lscale : 0.0f;  // 0 => the readers skip the lo planes (not zeroed then)
   for (int c = threadIdx.x; c < ACC_N; c += blockDim.x) {

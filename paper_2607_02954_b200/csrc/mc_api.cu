@@ -123,6 +123,7 @@ struct mc_world {
   int N = 0;
   int stride = 60;   // K1 window advance: 64 when all chains share a length dividing 64
   int n_windows = 0;
+  int n_sm = 148;               // SMs of the device the world lives on (persistent kernels' grid)
   bool uniform_params = false;  // K1 variant: L_rest, stiffnesses and period identical for all beads
   int deposit_threads = 128;  // CTA size of K2a: 128 hides the per-tile latency better, crowded worlds want 256
   // CUDA graphs of GRAPH_STEPS consecutive steps, one per ping-pong phase, captured on first use
@@ -227,7 +228,7 @@ int enqueue_step(mc_world* w) {
     // K0: policy + tile binning (count, scan, fill).  The three binning kernels return at once
     // unless the policy kernel found the lists' drift bound used up (k_tile.cuh).
     mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16);
-    const int k0grid = bgrid < 148 * 8 ? bgrid : 148 * 8;
+    const int k0grid = bgrid < w->n_sm * 8 ? bgrid : w->n_sm * 8;
     mc::k_list_policy<<<1, 1, 0, st>>>(ls_state);
     mc::k_tile_bin<false><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, tile_count, bucket_count, nullptr);
     mc::k_tile_scan<<<1, 1024, 0, st>>>(ls_state, tile_count, n_tiles, tile_start);
@@ -401,6 +402,12 @@ int mc_create(const mc_world_params* p, void* workspace, size_t workspace_bytes,
   w->nx = p->nx;
   w->ny = p->ny;
   w->nc = (size_t)p->nx * p->ny;
+  {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+      w->n_sm = sms;
+  }
   // lattice constants (reading 10, 12): nu_lat = nu dt; tau+ = 3 nu_lat + 1/2; tau- = Lambda/(tau+ - 1/2) + 1/2
   const double dt = (double)p->dt, nu_lat = (double)p->nu * dt;
   const double tau_p = 3.0 * nu_lat + 0.5, tau_m = (double)p->trt_lambda / (tau_p - 0.5) + 0.5;

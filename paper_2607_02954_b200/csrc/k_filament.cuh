@@ -40,6 +40,7 @@ struct FilamentArgs {
   float2* F;         // [N] out: total bead force
   float* sense;      // [N] out (only written when csum != NULL)
   const float2* A;   // interleaved force-gradient field (may be NULL: no field forces)
+  cudaTextureObject_t tex_A;  // linear float2 view of A, or 0 (gathers then use the LSU pipe only)
   const float* csum;  // sum of static fields (may be NULL)
   unsigned* tile_fmax;  // per 32x32 tile: bits of max |F| over the beads whose floor(X) lies in it (may be NULL)
   int N;
@@ -131,7 +132,7 @@ __device__ __forceinline__ float2 edge_delta(double vx, double vy, float delta, 
   return make_float2(0.5f * p.kst * fmaf(ksL, ex, dl * tx), 0.5f * p.kst * fmaf(ksL, ey, dl * ty));
 }
 
-template <bool UNIFORM>
+template <bool UNIFORM, int TEXROWS>
 __global__ void __launch_bounds__(256, 5) k_filament_force(FilamentArgs a) {
   const int lane = threadIdx.x & 31;
   const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -182,8 +183,16 @@ __global__ void __launch_bounds__(256, 5) k_filament_force(FilamentArgs a) {
   const bool oA = out && vA, oB = out && vB;
   float2 FA = make_float2(a.kappa * DAx, a.kappa * DAy), FB = make_float2(a.kappa * DBx, a.kappa * DBy);
   if (a.A) {
-    if (oA) { const float2 g = interp2(a.A, a.nx, a.ny, xa.x, xa.y); FA.x += g.x; FA.y += g.y; }
-    if (oB) { const float2 g = interp2(a.A, a.nx, a.ny, xb.x, xb.y); FB.x += g.x; FB.y += g.y; }
+    if (oA) {
+      const float2 g = TEXROWS ? interp2_tex<TEXROWS>(a.A, a.tex_A, a.nx, a.ny, xa.x, xa.y)
+                               : interp2(a.A, a.nx, a.ny, xa.x, xa.y);
+      FA.x += g.x; FA.y += g.y;
+    }
+    if (oB) {
+      const float2 g = TEXROWS ? interp2_tex<TEXROWS>(a.A, a.tex_A, a.nx, a.ny, xb.x, xb.y)
+                               : interp2(a.A, a.nx, a.ny, xb.x, xb.y);
+      FB.x += g.x; FB.y += g.y;
+    }
   }
   if (a.tile_fmax) {
     // Bound for the fixed-point scale of S5 (k_p2g.cuh): tile_fmax[t] >= max |F| over the beads

@@ -7,8 +7,10 @@
 
 namespace mc {
 
+template <int TEXROWS>
 __global__ void __launch_bounds__(256) k_interp_integrate(int N, float2* __restrict__ X,
-                                                          const float2* __restrict__ u, int nx, int ny,
+                                                          const float2* __restrict__ u, cudaTextureObject_t tex_u,
+                                                          int nx, int ny,
                                                           int* __restrict__ flag, long long* __restrict__ step,
                                                           unsigned* __restrict__ step_max) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
@@ -16,7 +18,7 @@ __global__ void __launch_bounds__(256) k_interp_integrate(int N, float2* __restr
   float m = 0.0f;
   if (b < N) {
     float2 p = X[b];
-    const float2 U = interp2(u, nx, ny, p.x, p.y);
+    const float2 U = TEXROWS ? interp2_tex<TEXROWS>(u, tex_u, nx, ny, p.x, p.y) : interp2(u, nx, ny, p.x, p.y);
     p.x += U.x;
     p.y += U.y;
     X[b] = p;

@@ -227,7 +227,11 @@ __device__ __noinline__ void spread_loop_wide(int nx, int ny, int x0, int y0, in
 }
 
 // K2a: S2 deposit.  tile_rho_max[t] receives max over the tile of rho_b (for K2b's scale).
-__global__ void __launch_bounds__(256, 6) k_deposit_tile(int nx, int ny, const int* __restrict__ tile_start,
+// LIGHT: the variant for worlds without crowded tiles, launched with 128 threads and capped at
+// 40 registers (more resident CTAs hide the per-tile latency chain; the cap costs the crowded
+// config 5 10 % and gains world 4d 2 %).
+template <bool LIGHT>
+__global__ void __launch_bounds__(256, LIGHT ? 6 : 1) k_deposit_tile(int nx, int ny, const int* __restrict__ tile_start,
                                                       const int* __restrict__ list,
                                                       const float2* __restrict__ X,
                                                       float* __restrict__ rho_b,

@@ -123,6 +123,7 @@ struct mc_world {
   int N = 0;
   int stride = 60;   // K1 window advance: 64 when all chains share a length dividing 64
   int n_windows = 0;
+  cudaTextureObject_t tex_u = 0, tex_A = 0;  // linear float2 views of u and A for the texture-pipe half of the gathers
   int n_sm = 148;               // SMs of the device the world lives on (persistent kernels' grid)
   bool uniform_params = false;  // K1 variant: L_rest, stiffnesses and period identical for all beads
   int deposit_threads = 128;  // CTA size of K2a: 128 hides the per-tile latency better, crowded worlds want 256
@@ -238,7 +239,10 @@ int enqueue_step(mc_world* w) {
     prof_mark(w, 1);
     // K2a: S2 deposit
     if (w->d.n_density) {
-      mc::k_deposit_tile<<<tgrid, w->deposit_threads, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax);
+      if (w->deposit_threads == 128)
+        mc::k_deposit_tile<true><<<tgrid, 128, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax);
+      else
+        mc::k_deposit_tile<false><<<tgrid, w->deposit_threads, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax);
       w->launches++;
       prof_mark(w, 2);
       // K3a: S3 filter + gradient -> force-gradient planes A
@@ -271,8 +275,18 @@ int enqueue_step(mc_world* w) {
     fa.n_windows = w->n_windows;
     fa.kappa = w->kappa;
     fa.step = w->ptr<long long>(w->L.flags) + 4;  // flags[8..9]: device copy of the step counter
-    if (w->uniform_params) mc::k_filament_force<true><<<(w->n_windows + 7) / 8, 256, 0, st>>>(fa);
-    else mc::k_filament_force<false><<<(w->n_windows + 7) / 8, 256, 0, st>>>(fa);
+    fa.tex_A = w->tex_A;
+    const int k1grid = (w->n_windows + 7) / 8;
+    // two of the four support rows of the A gather go through the texture pipe (measured on
+    // world 4d: 0 rows 0.254 ms, 1: 0.248, 2: 0.245, 3: 0.256)
+    const bool k1tex = fa.A && fa.tex_A;
+    if (w->uniform_params) {
+      if (k1tex) mc::k_filament_force<true, 2><<<k1grid, 256, 0, st>>>(fa);
+      else mc::k_filament_force<true, 0><<<k1grid, 256, 0, st>>>(fa);
+    } else {
+      if (k1tex) mc::k_filament_force<false, 2><<<k1grid, 256, 0, st>>>(fa);
+      else mc::k_filament_force<false, 0><<<k1grid, 256, 0, st>>>(fa);
+    }
     prof_mark(w, 4);
     w->launches++;
   } else {
@@ -317,8 +331,12 @@ int enqueue_step(mc_world* w) {
   prof_mark(w, 6);
   // K4: S7
   if (beads) {
-    mc::k_interp_integrate<<<bgrid, bt, 0, st>>>(N, X, la.u, nx, ny, flag, w->ptr<long long>(w->L.flags) + 4,
-                                                 reinterpret_cast<unsigned*>(w->ptr<int>(w->L.flags) + 18));
+    long long* stepp = w->ptr<long long>(w->L.flags) + 4;
+    unsigned* smax = reinterpret_cast<unsigned*>(w->ptr<int>(w->L.flags) + 18);
+    // one support row of the u gather through the texture pipe (4d: 0 rows 0.168 ms, 1: 0.156,
+    // 2: 0.160, 3: 0.174, 4: 0.193)
+    if (w->tex_u) mc::k_interp_integrate<1><<<bgrid, bt, 0, st>>>(N, X, la.u, w->tex_u, nx, ny, flag, stepp, smax);
+    else mc::k_interp_integrate<0><<<bgrid, bt, 0, st>>>(N, X, la.u, w->tex_u, nx, ny, flag, stepp, smax);
     w->launches++;
   }
   prof_mark(w, 7);
@@ -346,6 +364,8 @@ int64_t mc_launch_count(const mc_world* w) { return w ? w->launches : 0; }
 void mc_destroy(mc_world* w) {
   if (!w) return;
   for (cudaEvent_t e : w->prof_ev) cudaEventDestroy(e);
+  if (w->tex_u) cudaDestroyTextureObject(w->tex_u);
+  if (w->tex_A) cudaDestroyTextureObject(w->tex_A);
   drop_graphs(w);
   delete w;
 }
@@ -402,6 +422,26 @@ int mc_create(const mc_world_params* p, void* workspace, size_t workspace_bytes,
   w->nx = p->nx;
   w->ny = p->ny;
   w->nc = (size_t)p->nx * p->ny;
+  // linear float2 texture views of the gathered fields (mc_common.cuh interp2_tex); a failure
+  // (workspace not aligned to the texture alignment, field beyond the linear-texture limit)
+  // leaves the handle 0 and the gathers on the plain path
+  auto make_tex = [&](size_t off) -> cudaTextureObject_t {
+    cudaResourceDesc rd;
+    memset(&rd, 0, sizeof(rd));
+    rd.resType = cudaResourceTypeLinear;
+    rd.res.linear.devPtr = w->ws + off;
+    rd.res.linear.desc = cudaCreateChannelDesc<float2>();
+    rd.res.linear.sizeInBytes = w->nc * 8;
+    cudaTextureDesc td;
+    memset(&td, 0, sizeof(td));
+    td.readMode = cudaReadModeElementType;
+    cudaTextureObject_t t = 0;
+    if (cudaCreateTextureObject(&t, &rd, &td, nullptr) != cudaSuccess) { cudaGetLastError(); t = 0; }
+    return t;
+  };
+  w->tex_u = make_tex(L.u);
+  if (d.n_density) w->tex_A = make_tex(L.A);
+  else if (d.n_static) w->tex_A = make_tex(L.As);
   {
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) == cudaSuccess &&

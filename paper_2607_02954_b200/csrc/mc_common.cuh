@@ -93,6 +93,45 @@ __device__ __forceinline__ float2 interp2(const float2* __restrict__ p, int nx, 
   return make_float2(ax, ay);
 }
 
+// Same sum with the support rows 2 and 3 fetched through the texture pipe (raw fetches of the
+// same memory, no filtering: identical bits).  The per-bead gathers are bound by the LSU pipe's
+// tag stage (one 128-byte line per clock); the TEX pipe has its own.
+template <int TEXROWS>
+__device__ __forceinline__ float2 interp2_tex(const float2* __restrict__ p, cudaTextureObject_t tex, int nx, int ny,
+                                              float x, float y) {
+  int i0, j0;
+  float fx, fy, wx[4], wy[4];
+  support(x, i0, fx);
+  support(y, j0, fy);
+  peskin4(fx, wx[0], wx[1], wx[2], wx[3]);
+  peskin4(fy, wy[0], wy[1], wy[2], wy[3]);
+  i0 = wrapi(i0, nx);
+  j0 = wrapi(j0, ny);
+  int col[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const int c = (i0 + k >= nx) ? i0 + k - nx : i0 + k;
+    col[k] = ((c >> 2) << 4) + (c & 3);
+  }
+  const int nbx = nx >> 2;
+  float ax = 0.0f, ay = 0.0f;
+#pragma unroll
+  for (int l = 0; l < 4; ++l) {
+    const int row = (j0 + l >= ny) ? j0 + l - ny : j0 + l;
+    const int ro = (row >> 2) * nbx * 16 + ((row & 3) << 2);
+    float sx = 0.0f, sy = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const float2 v = (l >= 4 - TEXROWS) ? tex1Dfetch<float2>(tex, ro + col[k]) : __ldg(p + ro + col[k]);
+      sx = fmaf(v.x, wx[k], sx);
+      sy = fmaf(v.y, wx[k], sy);
+    }
+    ax = fmaf(sx, wy[l], ax);
+    ay = fmaf(sy, wy[l], ay);
+  }
+  return make_float2(ax, ay);
+}
+
 __device__ __forceinline__ float interp1(const float* __restrict__ p0, int nx, int ny, float x, float y) {
   int i0, j0;
   float fx, fy, wx[4], wy[4];

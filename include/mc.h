@@ -135,6 +135,14 @@ int mc_read_intermediates(mc_world* w, float* rho_b, float* G);
  * world has a bead-density field. */
 int mc_keep_intermediates(mc_world* w, int32_t on);
 
+/* The per-bead 4x4 gathers of K1 (force-gradient field) and K4 (fluid velocity) send part of
+ * their loads through the texture pipe (linear float2 views of the same memory, raw fetches:
+ * identical bits) when the views could be created at mc_create.
+ * mc_texture_gathers(w, 0) makes the following steps use plain loads only (for tests and
+ * measurements), (w, 1) restores the default.  Returns 1 if the texture path is in use after
+ * the call, 0 if not, or a negative error. */
+int mc_texture_gathers(mc_world* w, int32_t on);
+
 /* Optional per-kernel timing with CUDA events on the world's stream (used by bench.py for the
  * roofline line; off by default, costs one event record per kernel group when on).
  * Slots: 0 K0 bin, 1 K2a deposit, 2 K3a filter+gradient, 3 K1 filament force, 4 K2b spread (empty:

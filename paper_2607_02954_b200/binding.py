@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libmc.so")
 MC_OK, MC_EINVAL, MC_ENOMEM, MC_ECUDA, MC_ESTATE, MC_EDIVERGED = 0, -1, -2, -3, -4, -5
 SYMBOLS = ("mc_workspace_bytes", "mc_create", "mc_load_filaments", "mc_step", "mc_read_state",
            "mc_read_intermediates", "mc_launch_count", "mc_destroy", "mc_last_error",
-           "mc_profile_enable", "mc_profile_read", "mc_keep_intermediates")
+           "mc_profile_enable", "mc_profile_read", "mc_keep_intermediates", "mc_texture_gathers")
 PROF_SLOTS = ("K0_bin", "K2a_deposit", "K3a_blur_grad", "K1_filament", "K2b_spread", "K3b_lbm",
               "K4_interp_integrate")
 
@@ -76,6 +76,8 @@ def load_library():
     L.mc_profile_read.argtypes = [vp, _fp, C.POINTER(i32)]
     L.mc_keep_intermediates.restype = C.c_int
     L.mc_keep_intermediates.argtypes = [vp, i32]
+    L.mc_texture_gathers.restype = C.c_int
+    L.mc_texture_gathers.argtypes = [vp, i32]
     L.mc_destroy.restype = None
     L.mc_destroy.argtypes = [vp]
     L.mc_last_error.restype = C.c_char_p
@@ -199,6 +201,13 @@ class World:
 
     def keep_intermediates(self, on: bool = True):
         self._check(load_library().mc_keep_intermediates(self.h, int(bool(on))))
+
+    def texture_gathers(self, on: bool = True) -> bool:
+        """mc_texture_gathers: returns whether the texture path is in use afterwards."""
+        rc = load_library().mc_texture_gathers(self.h, int(bool(on)))
+        if rc < 0:
+            self._check(rc)
+        return rc == 1
 
     def profile_enable(self, on: bool = True):
         self._check(load_library().mc_profile_enable(self.h, int(bool(on))))

@@ -139,6 +139,7 @@ struct mc_world {
   int static_slot[4] = {-1, -1, -1, -1};
   int64_t launches = 0;
   bool diverged = false;
+  bool tex_on = true;   // mc_texture_gathers
   bool keep_G = false;  // mc_keep_intermediates: the fused spread+fluid kernel also stores G
   std::string err;
   // optional per-kernel timing (mc_profile_*): events at the 8 boundaries of a step
@@ -275,7 +276,7 @@ int enqueue_step(mc_world* w) {
     fa.n_windows = w->n_windows;
     fa.kappa = w->kappa;
     fa.step = w->ptr<long long>(w->L.flags) + 4;  // flags[8..9]: device copy of the step counter
-    fa.tex_A = w->tex_A;
+    fa.tex_A = w->tex_on ? w->tex_A : 0;
     const int k1grid = (w->n_windows + 7) / 8;
     // two of the four support rows of the A gather go through the texture pipe (measured on
     // world 4d: 0 rows 0.254 ms, 1: 0.248, 2: 0.245, 3: 0.256)
@@ -335,7 +336,7 @@ int enqueue_step(mc_world* w) {
     unsigned* smax = reinterpret_cast<unsigned*>(w->ptr<int>(w->L.flags) + 18);
     // one support row of the u gather through the texture pipe (4d: 0 rows 0.168 ms, 1: 0.156,
     // 2: 0.160, 3: 0.174, 4: 0.193)
-    if (w->tex_u) mc::k_interp_integrate<1><<<bgrid, bt, 0, st>>>(N, X, la.u, w->tex_u, nx, ny, flag, stepp, smax);
+    if (w->tex_on && w->tex_u) mc::k_interp_integrate<1><<<bgrid, bt, 0, st>>>(N, X, la.u, w->tex_u, nx, ny, flag, stepp, smax);
     else mc::k_interp_integrate<0><<<bgrid, bt, 0, st>>>(N, X, la.u, w->tex_u, nx, ny, flag, stepp, smax);
     w->launches++;
   }
@@ -746,6 +747,13 @@ int mc_keep_intermediates(mc_world* w, int32_t on) {
   if (w->keep_G != (on != 0)) drop_graphs(w);
   w->keep_G = on != 0;
   return MC_OK;
+}
+
+int mc_texture_gathers(mc_world* w, int32_t on) {
+  if (!w) return MC_EINVAL;
+  if (w->tex_on != (on != 0)) drop_graphs(w);
+  w->tex_on = on != 0;
+  return (w->tex_on && w->tex_u) ? 1 : 0;
 }
 
 int mc_read_intermediates(mc_world* w, float* rho_b, float* G) {

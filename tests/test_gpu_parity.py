@@ -195,6 +195,22 @@ def test_bitwise_reproducible(name):
         assert outs[0][k].tobytes() == outs[1][k].tobytes(), k
 
 
+def test_texture_gathers_do_not_change_the_bits():
+    # K1/K4 fetch part of their 4x4 supports through the texture pipe: raw fetches of the same
+    # memory, so switching it off must reproduce every bit
+    from paper_2607_02954_b200 import binding
+    out = []
+    for tex in (True, False):
+        G = binding.World(SMALL["uniform_m32"]())
+        used = G.texture_gathers(tex)
+        assert used == tex, "texture views were not created on this device"
+        G.step(25)
+        out.append(G.read_state(keys=("xy", "u", "force", "sense")))
+        G.close()
+    for k in ("xy", "u", "force", "sense"):
+        assert out[0][k].tobytes() == out[1][k].tobytes(), k
+
+
 def test_step_batching_is_equivalent():
     # mc_step(23) (CUDA-graph replay of 4-step blocks + direct launches) == 23 x mc_step(1)
     # (direct launches only) == 3 + 20 split across calls, bit for bit

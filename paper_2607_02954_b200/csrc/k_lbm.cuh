@@ -120,7 +120,7 @@ struct LbmSpreadArgs {
 
 template <bool KEEP_G>
 __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
-  __shared__ int acc0[ACC_N], acc1[ACC_N], accl0[ACC_N], accl1[ACC_N];
+  __shared__ __align__(16) int acc0[ACC_N], acc1[ACC_N], accl0[ACC_N], accl1[ACC_N];
   __shared__ float red[32];
   const LbmArgs& a = p.lbm;
   const int nx = a.nx, ny = a.ny;

@@ -40,6 +40,13 @@ struct TileBead {
   float wx[4], wy[4];
 };
 
+// zero one accumulator plane with 16-byte stores (the planes are 16-byte aligned, ACC_N % 4 == 0)
+static_assert(ACC_N % 4 == 0, "accumulator planes are zeroed as int4");
+__device__ __forceinline__ void zero_acc(int* acc) {
+  int4* a4 = reinterpret_cast<int4*>(acc);
+  for (int c = threadIdx.x; c < ACC_N / 4; c += blockDim.x) a4[c] = make_int4(0, 0, 0, 0);
+}
+
 __device__ __forceinline__ int acc_index(int lx, int ly) { return (ly + HALO) * TSP + lx + HALO; }
 
 // distance (in nodes, periodic) from the tile origin to the first support node, in [-n/2, n/2)
@@ -237,7 +244,7 @@ __global__ void __launch_bounds__(256, LIGHT ? 6 : 1) k_deposit_tile(int nx, int
                                                       float* __restrict__ rho_b,
                                                       float* __restrict__ tile_rho_max,
                                                       unsigned* __restrict__ tile_fmax) {
-  __shared__ int acc[ACC_N], accl[ACC_N];
+  __shared__ __align__(16) int acc[ACC_N], accl[ACC_N];
   __shared__ float red[32];
   const int t = blockIdx.y * gridDim.x + blockIdx.x;  // grid = (nx/TS, ny/TS)
   const int x0 = blockIdx.x * TS, y0 = blockIdx.y * TS;
@@ -248,7 +255,8 @@ __global__ void __launch_bounds__(256, LIGHT ? 6 : 1) k_deposit_tile(int nx, int
     const Deal d(e - s);
     if (d.valid()) xpre = __ldg(X + __ldg(list + s + d.p));  // gather starts before the zeroing
   }
-  for (int c = threadIdx.x; c < ACC_N; c += blockDim.x) { acc[c] = 0; if (wide) accl[c] = 0; }
+  zero_acc(acc);
+  if (wide) zero_acc(accl);
   const float scale = pow2_scale(fmaxf(0.25f * (float)(e - s), 1.0f));
   const float lscale = pow2f(lo_bits(e - s));
   __syncthreads();
@@ -258,11 +266,17 @@ __global__ void __launch_bounds__(256, LIGHT ? 6 : 1) k_deposit_tile(int nx, int
   __syncthreads();
   const float inv = 1.0f / scale, linv = 1.0f / lscale;
   float mx = 0.0f;
-  for (int c = threadIdx.x; c < TS * TS; c += blockDim.x) {
-    const int a = acc_index(c & 31, c >> 5);
-    const float v = (wide ? fmaf((float)accl[a], linv, (float)acc[a]) : (float)acc[a]) * inv;
-    rho_b[(size_t)(y0 + (c >> 5)) * nx + x0 + (c & 31)] = v;
-    mx = fmaxf(mx, v);
+  // four consecutive nodes of a row per thread: one 16-byte store
+  for (int c = threadIdx.x; c < TS * TS / 4; c += blockDim.x) {
+    const int ly = c >> 3, lx = (c & 7) << 2;
+    const int a = acc_index(lx, ly);
+    float v[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      v[k] = (wide ? fmaf((float)accl[a + k], linv, (float)acc[a + k]) : (float)acc[a + k]) * inv;
+      mx = fmaxf(mx, v[k]);
+    }
+    *reinterpret_cast<float4*>(rho_b + (size_t)(y0 + ly) * nx + x0 + lx) = make_float4(v[0], v[1], v[2], v[3]);
   }
   // tile maximum: rho_b >= 0, so the float bits order like unsigned integers; one global
   // atomicMax per warp onto tile_rho_max[t] (zeroed by the tile-list scan of this step)
@@ -297,10 +311,9 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
   const bool wide = (e - s) > WIDE_N;
   const float lscale = pow2f(lo_bits(e - s));
   linv = wide ? 1.0f / lscale : 0.0f;  // 0 => the readers skip the lo planes (not zeroed then)
-  for (int c = threadIdx.x; c < ACC_N; c += blockDim.x) {
-    acc0[c] = 0; acc1[c] = 0;
-    if (wide) { accl0[c] = 0; accl1[c] = 0; }
-  }
+  zero_acc(acc0);
+  zero_acc(acc1);
+  if (wide) { zero_acc(accl0); zero_acc(accl1); }
   float fm = 0.0f;
   if (tile_fmax) {
     // max |F| over the beads owned by this tile and its 8 neighbours (every listed bead whose

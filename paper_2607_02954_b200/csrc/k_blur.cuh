@@ -63,9 +63,12 @@ __global__ void __launch_bounds__(BLUR_THREADS, 7) k_blur_grad(int nx, int ny, B
     const int r0 = j0 + 8 * c - 1 - R;                      // first row of the window
     float v[NV];
     if (j0 - 1 - R >= 0 && j0 + BLUR_T + 1 + R <= ny) {     // tile away from the y seam: no row wraps
-      const float* p = rho_b + (size_t)r0 * nx + gi;
+      // row k of the window: one IMAD.WIDE (32-bit row size x immediate k + 64-bit pointer)
+      const char* p = reinterpret_cast<const char*>(rho_b + (size_t)r0 * nx + gi);
+      const unsigned rowb = (unsigned)nx * (unsigned)sizeof(float);
 #pragma unroll
-      for (int k = 0; k < NV; ++k) { v[k] = __ldg(p); p += nx; }
+      for (int k = 0; k < NV; ++k)
+        v[k] = __ldg(reinterpret_cast<const float*>(p + (unsigned long long)rowb * (unsigned)k));
     } else {
 #pragma unroll
       for (int k = 0; k < NV; ++k) v[k] = __ldg(rho_b + (size_t)wrap1(r0 + k, ny) * nx + gi);

@@ -162,9 +162,33 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
   const int im = (i == 0) ? nx - 1 : i - 1, ip2 = (i + 2 == nx) ? 0 : i + 2;
   bool bad = false;
   float gA[9], gB[9];  // pre-collision populations of nodes i and i+1 (pull: g_q(x) = src_q(x - c_q))
+  // Addresses: plane q of a row pointer is one IMAD.WIDE (32-bit plane size x immediate q + 64-bit
+  // pointer) and the column neighbours are immediate offsets, unless the pair touches the
+  // periodic seam in x (first/last pair of a row of the domain) or the planes exceed 4 GB / 8.
+  const unsigned pb = (unsigned)(nc * sizeof(float));  // bytes per plane (used only when it fits)
+  const bool fast = (nc * sizeof(float) * 8 < 0xffffffffull) && i != 0 && i + 2 != nx;
+  auto plane = [&](const float* p, int q) {
+    return reinterpret_cast<const float*>(reinterpret_cast<const char*>(p) + (unsigned long long)pb * (unsigned)q);
+  };
   auto load_pair = [&](int ly) {
     const int j = y0 + ly;
     const int jm = (j == 0) ? ny - 1 : j - 1, jp = (j == ny - 1) ? 0 : j + 1;
+    if (fast) {
+      const float* p0 = a.src + (size_t)j * nx + i;
+      const float* pm = a.src + (size_t)jm * nx + i;
+      const float* pp = a.src + (size_t)jp * nx + i;
+      const float2 v0 = __ldg(reinterpret_cast<const float2*>(p0));
+      const float2 v2 = __ldg(reinterpret_cast<const float2*>(plane(pm, 2)));
+      const float2 v4 = __ldg(reinterpret_cast<const float2*>(plane(pp, 4)));
+      gA[0] = v0.x; gB[0] = v0.y; gA[2] = v2.x; gB[2] = v2.y; gA[4] = v4.x; gB[4] = v4.y;
+      const float* q1 = plane(p0, 1); gA[1] = __ldg(q1 - 1); gB[1] = __ldg(q1);
+      const float* q3 = plane(p0, 3); gA[3] = __ldg(q3 + 1); gB[3] = __ldg(q3 + 2);
+      const float* q5 = plane(pm, 5); gA[5] = __ldg(q5 - 1); gB[5] = __ldg(q5);
+      const float* q6 = plane(pm, 6); gA[6] = __ldg(q6 + 1); gB[6] = __ldg(q6 + 2);
+      const float* q7 = plane(pp, 7); gA[7] = __ldg(q7 + 1); gB[7] = __ldg(q7 + 2);
+      const float* q8 = plane(pp, 8); gA[8] = __ldg(q8 - 1); gB[8] = __ldg(q8);
+      return;
+    }
     const size_t r0 = (size_t)j * nx, rm = (size_t)jm * nx, rp = (size_t)jp * nx;
     const float2 v0 = __ldg(reinterpret_cast<const float2*>(a.src + 0 * nc + r0 + i));
     const float2 v2 = __ldg(reinterpret_cast<const float2*>(a.src + 2 * nc + rm + i));
@@ -199,8 +223,15 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
     trt_collide(gB, GBx, GBy, a.rho0, a.omega_p, a.omega_m, uBx, uBy);
     // blocked u: nodes i and i+1 (i even) are neighbours inside one 4x4 block
     *reinterpret_cast<float4*>(a.u + blk_index(i, j, nx)) = make_float4(uAx, uAy, uBx, uBy);
+    if (nc * sizeof(float) * 8 < 0xffffffffull) {
+      char* d0 = reinterpret_cast<char*>(a.dst + c);
 #pragma unroll
-    for (int q = 0; q < 9; ++q) *reinterpret_cast<float2*>(a.dst + q * nc + c) = make_float2(gA[q], gB[q]);
+      for (int q = 0; q < 9; ++q)
+        *reinterpret_cast<float2*>(d0 + (unsigned long long)pb * (unsigned)q) = make_float2(gA[q], gB[q]);
+    } else {
+#pragma unroll
+      for (int q = 0; q < 9; ++q) *reinterpret_cast<float2*>(a.dst + q * nc + c) = make_float2(gA[q], gB[q]);
+    }
     bad = bad || !(fabsf(uAx) <= 0.3f && fabsf(uAy) <= 0.3f && fabsf(uBx) <= 0.3f && fabsf(uBy) <= 0.3f);
   }
   if (bad) atomicOr(a.flag, 4);

@@ -79,11 +79,12 @@ __device__ __forceinline__ float2 interp2(const float2* __restrict__ p, int nx, 
 #pragma unroll
   for (int l = 0; l < 4; ++l) {
     const int row = (j0 + l >= ny) ? j0 + l - ny : j0 + l;
-    const float2* r = p + ((size_t)(row >> 2) * nbx * 16 + ((row & 3) << 2));
+    // row pointer once, then one IMAD.WIDE (32-bit column offset x 8 + pointer) per node
+    const char* r = reinterpret_cast<const char*>(p + ((size_t)(row >> 2) * nbx * 16 + ((row & 3) << 2)));
     float sx = 0.0f, sy = 0.0f;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-      const float2 v = __ldg(r + col[k]);
+      const float2 v = __ldg(reinterpret_cast<const float2*>(r + (unsigned long long)(unsigned)col[k] * 8u));
       sx = fmaf(v.x, wx[k], sx);
       sy = fmaf(v.y, wx[k], sy);
     }
@@ -122,7 +123,10 @@ __device__ __forceinline__ float2 interp2_tex(const float2* __restrict__ p, cuda
     float sx = 0.0f, sy = 0.0f;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-      const float2 v = (l >= 4 - TEXROWS) ? tex1Dfetch<float2>(tex, ro + col[k]) : __ldg(p + ro + col[k]);
+      const float2 v = (l >= 4 - TEXROWS)
+                           ? tex1Dfetch<float2>(tex, ro + col[k])
+                           : __ldg(reinterpret_cast<const float2*>(reinterpret_cast<const char*>(p + ro) +
+                                                                   (unsigned long long)(unsigned)col[k] * 8u));
       sx = fmaf(v.x, wx[k], sx);
       sy = fmaf(v.y, wx[k], sy);
     }

@@ -42,9 +42,19 @@ struct TileBead {
 
 // zero one accumulator plane with 16-byte stores (the planes are 16-byte aligned, ACC_N % 4 == 0)
 static_assert(ACC_N % 4 == 0, "accumulator planes are zeroed as int4");
+// NT: CTA size when it is a compile-time fact (fully unrolled, constant store offsets), 0: any
+template <int NT>
 __device__ __forceinline__ void zero_acc(int* acc) {
   int4* a4 = reinterpret_cast<int4*>(acc);
-  for (int c = threadIdx.x; c < ACC_N / 4; c += blockDim.x) a4[c] = make_int4(0, 0, 0, 0);
+  if (NT > 0) {
+#pragma unroll
+    for (int k = 0; k < (ACC_N / 4 + NT - 1) / NT; ++k) {
+      const int c = threadIdx.x + k * NT;
+      if ((k + 1) * NT <= ACC_N / 4 || c < ACC_N / 4) a4[c] = make_int4(0, 0, 0, 0);
+    }
+  } else {
+    for (int c = threadIdx.x; c < ACC_N / 4; c += blockDim.x) a4[c] = make_int4(0, 0, 0, 0);
+  }
 }
 
 __device__ __forceinline__ int acc_index(int lx, int ly) { return (ly + HALO) * TSP + lx + HALO; }
@@ -255,8 +265,13 @@ __global__ void __launch_bounds__(256, LIGHT ? 6 : 1) k_deposit_tile(int nx, int
     const Deal d(e - s);
     if (d.valid()) xpre = __ldg(X + __ldg(list + s + d.p));  // gather starts before the zeroing
   }
-  zero_acc(acc);
-  if (wide) zero_acc(accl);
+  if (LIGHT) {  // the light variant is launched with 128 threads
+    zero_acc<128>(acc);
+    if (wide) zero_acc<128>(accl);
+  } else {
+    zero_acc<0>(acc);
+    if (wide) zero_acc<0>(accl);
+  }
   const float scale = pow2_scale(fmaxf(0.25f * (float)(e - s), 1.0f));
   const float lscale = pow2f(lo_bits(e - s));
   __syncthreads();
@@ -311,9 +326,9 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
   const bool wide = (e - s) > WIDE_N;
   const float lscale = pow2f(lo_bits(e - s));
   linv = wide ? 1.0f / lscale : 0.0f;  // 0 => the readers skip the lo planes (not zeroed then)
-  zero_acc(acc0);
-  zero_acc(acc1);
-  if (wide) { zero_acc(accl0); zero_acc(accl1); }
+  zero_acc<256>(acc0);  // the fused kernel runs 256 threads
+  zero_acc<256>(acc1);
+  if (wide) { zero_acc<256>(accl0); zero_acc<256>(accl1); }
   float fm = 0.0f;
   if (tile_fmax) {
     // max |F| over the beads owned by this tile and its 8 neighbours (every listed bead whose

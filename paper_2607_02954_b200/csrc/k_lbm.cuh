@@ -132,12 +132,12 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
   {
     // start pulling this tile's populations towards L2 while the atomic phase runs: 9 planes x
     // 32 rows x one 128-byte line (the +-1 halo columns/rows come with the neighbours' tiles)
+    // thread (q, r) takes row r of plane q; plane 8 falls to the first warp
     const size_t ncp = (size_t)nx * ny;
-    for (int it = threadIdx.x; it < 9 * TS; it += 256) {
-      const int q = it >> 5, r = it & 31;
-      const float* ptr = a.src + q * ncp + (size_t)(y0 + r) * nx + x0;
-      asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
-    }
+    const int q = threadIdx.x >> 5, r = threadIdx.x & 31;
+    const float* row = a.src + (size_t)(y0 + r) * nx + x0;
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(row + q * ncp));
+    if (threadIdx.x < 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(row + 8 * ncp));
   }
   // this thread's first list entry: its list -> X/F gather is the longest latency chain of the
   // tile, so it starts before the zeroing and the barrier of the atomic phase

@@ -21,6 +21,20 @@
 
 namespace mc {
 
+// Collision constants that depend only on the relaxation rates w+ and w- (filled on the host in
+// fp32 with the same operations the kernel would do; as kernel arguments they are constant-bank
+// operands and cost no registers).
+struct TrtConst {
+  float wp;    // w+
+  float hwp;   // w+ / 2
+  float hwm;   // w- / 2
+  float cp3;   // 3 (1 - w+/2)
+  float cb;    // 9 (1 - w+/2)
+  float c2;    // 3 (1 - w-/2)
+  float wp45;  // 4.5 w+
+  float wm3;   // 3 w-
+};
+
 struct LbmArgs {
   const float* src;   // [9][ny][nx] post-collision, shifted
   float* dst;         // [9][ny][nx]
@@ -30,7 +44,8 @@ struct LbmArgs {
   float* G1out;
   float2* u;          // out: collision-time velocity, interleaved (ux, uy)
   int nx, ny;
-  float rho0, omega_p, omega_m;
+  float rho0;
+  TrtConst k;         // collision constants (host, mc_api.cu)
   int* flag;          // sticky divergence flag (bit 2: |u| > 0.3 or non-finite)
 };
 
@@ -40,23 +55,24 @@ struct LbmArgs {
 //                                                              a = 4.5 w+ rho, b = 9 (1 - w+/2)
 //   odd_q  = -w- g-_q + w_q [c1 (c.u) + c2 (c.G)],             c1 = 3 w- rho, c2 = 3 (1 - w-/2)
 //   gpost_q = g_q + even_q + odd_q,  gpost_qbar = g_qbar + even_q - odd_q
-__device__ __forceinline__ void trt_collide(float g[9], float Gx, float Gy, float rho0, float wp, float wm,
+__device__ __forceinline__ void trt_collide(float g[9], float Gx, float Gy, float rho0, const TrtConst& k,
                                             float& ux, float& uy) {
   const float W0 = 4.0f / 9.0f, W1 = 1.0f / 9.0f, W5 = 1.0f / 36.0f;
   const float drho = g[0] + ((g[1] + g[3]) + (g[2] + g[4])) + ((g[5] + g[7]) + (g[6] + g[8]));
   const float mx = (g[1] - g[3]) + ((g[5] - g[7]) + (g[8] - g[6]));
   const float my = (g[2] - g[4]) + ((g[5] - g[7]) + (g[6] - g[8]));
   const float rho = rho0 + drho;
-  const float inv = 1.0f / rho;
+  // 1/rho to 1 ulp (MUFU.RCP; rho = 1 + O(Ma^2)): the IEEE division costs 11 instructions per node
+  float inv;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(rho));
   ux = (mx + 0.5f * Gx) * inv;
   uy = (my + 0.5f * Gy) * inv;
   const float usq = ux * ux + uy * uy;
   const float uG = ux * Gx + uy * Gy;
-  const float cp = 1.0f - 0.5f * wp, cm = 1.0f - 0.5f * wm;
-  const float E0 = wp * (drho - 1.5f * rho * usq) - 3.0f * cp * uG;
-  const float ca = 4.5f * wp * rho, cb = 9.0f * cp;
-  const float c1 = 3.0f * wm * rho, c2 = 3.0f * cm;
-  const float hwp = 0.5f * wp, hwm = 0.5f * wm;
+  const float wp = k.wp, hwp = k.hwp, hwm = k.hwm, cb = k.cb, c2 = k.c2;
+  const float E0 = wp * (drho - 1.5f * rho * usq) - k.cp3 * uG;
+  const float ca = k.wp45 * rho;
+  const float c1 = k.wm3 * rho;
   // rest population (even only, c = 0)
   g[0] = fmaf(W0, E0, g[0] - wp * g[0]);
 #define MC_PAIR(q, qb, w, cu, cG)                                                     \
@@ -97,7 +113,7 @@ __global__ void __launch_bounds__(256) k_lbm_step(LbmArgs a) {
   float Gx = 0.0f, Gy = 0.0f;
   if (a.G0) { Gx = __ldg(a.G0 + c); Gy = __ldg(a.G1 + c); }
   float ux, uy;
-  trt_collide(g, Gx, Gy, a.rho0, a.omega_p, a.omega_m, ux, uy);
+  trt_collide(g, Gx, Gy, a.rho0, a.k, ux, uy);
   a.u[blk_index(i, j, nx)] = make_float2(ux, uy);
 #pragma unroll
   for (int q = 0; q < 9; ++q) a.dst[q * nc + c] = g[q];
@@ -219,8 +235,8 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
       *reinterpret_cast<float2*>(a.G1out + c) = make_float2(GAy, GBy);
     }
     float uAx, uAy, uBx, uBy;
-    trt_collide(gA, GAx, GAy, a.rho0, a.omega_p, a.omega_m, uAx, uAy);
-    trt_collide(gB, GBx, GBy, a.rho0, a.omega_p, a.omega_m, uBx, uBy);
+    trt_collide(gA, GAx, GAy, a.rho0, a.k, uAx, uAy);
+    trt_collide(gB, GBx, GBy, a.rho0, a.k, uBx, uBy);
     // blocked u: nodes i and i+1 (i even) are neighbours inside one 4x4 block
     *reinterpret_cast<float4*>(a.u + blk_index(i, j, nx)) = make_float4(uAx, uAy, uBx, uBy);
     if (nc * sizeof(float) * 8 < 0xffffffffull) {

@@ -304,8 +304,18 @@ int enqueue_step(mc_world* w) {
   la.nx = nx;
   la.ny = ny;
   la.rho0 = w->rho0;
-  la.omega_p = w->omega_p;
-  la.omega_m = w->omega_m;
+  {
+    const float wp = w->omega_p, wm = w->omega_m;
+    const float cp = 1.0f - 0.5f * wp, cm = 1.0f - 0.5f * wm;
+    la.k.wp = wp;
+    la.k.hwp = 0.5f * wp;
+    la.k.hwm = 0.5f * wm;
+    la.k.cp3 = 3.0f * cp;
+    la.k.cb = 9.0f * cp;
+    la.k.c2 = 3.0f * cm;
+    la.k.wp45 = 4.5f * wp;
+    la.k.wm3 = 3.0f * wm;
+  }
   la.flag = flag;
   la.G0out = G0;
   la.G1out = G1;

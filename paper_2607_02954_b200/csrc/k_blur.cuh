@@ -28,7 +28,22 @@ struct BlurTaps {
 constexpr int BLUR_THREADS = 192;
 __host__ __device__ constexpr int blur_NV(int R) { return 10 + 2 * R; }               // window: 8 outputs + 2 + 2R
 __host__ __device__ constexpr int blur_NV4(int R) { return (blur_NV(R) + 3) / 4; }
-__host__ __device__ constexpr int blur_CW(int R) { return 24 + 4 * blur_NV4(R); }     // plane pitch >= 34 + 2R
+__host__ __device__ constexpr int blur_CW(int R) { return 24 + 4 * blur_NV4(R); }     // columns held >= 34 + 2R
+// pitch of the interleaved (ty, dy) plane in float2: CW + 2, so that the 16-byte accesses of a
+// quarter warp (2 chunks x 4 rows) fall on the 8 different bank groups
+__host__ __device__ constexpr int blur_CP(int R) { return blur_CW(R) + 2; }
+
+// d = a * s + c on both halves: one FFMA2 (sm_100 packed fp32; the kernel is bound by issue slots)
+__device__ __forceinline__ float2 ffma2(float2 a, float s, float2 c) {
+  unsigned long long ua, us, uc, ud;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(ua) : "f"(a.x), "f"(a.y));
+  asm("mov.b64 %0, {%1, %1};" : "=l"(us) : "f"(s));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(uc) : "f"(c.x), "f"(c.y));
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(ud) : "l"(ua), "l"(us), "l"(uc));
+  float2 d;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(ud));
+  return d;
+}
 
 // One CTA filters one 32x32 tile; rho_b is read once per node plus the halo (through L1), the
 // gradient is written once, nothing else touches global memory.  The y pass comes first because
@@ -36,9 +51,10 @@ __host__ __device__ constexpr int blur_CW(int R) { return 24 + 4 * blur_NV4(R); 
 // is a register operation on its outputs:
 //   y pass: thread = (column of the tile + x halo, chunk of 8 rows): 10 + 2R loads of its
 //           column, ty = G_y rho_b on 10 rows, of which 8 are stored together with
-//           dy = (ty[y+1] - ty[y-1]) / 2                                   -> ty, dy [32][CW]
-//   x pass: thread = (row, chunk of 8 nodes): register windows of ty and dy (16-byte LDS),
-//           B = G_x ty on 10 nodes, grad_x = (B[x+1] - B[x-1]) / 2, grad_y = G_x dy on 8 nodes,
+//           dy = (ty[y+1] - ty[y-1]) / 2                              -> (ty, dy) [32][CP]
+//   x pass: thread = (row, chunk of 8 nodes): register window of the interleaved (ty, dy) pairs
+//           (16-byte LDS), (B, G_x dy) = G_x (ty, dy) on 10 nodes with packed FFMA2,
+//           grad_x = (B[x+1] - B[x-1]) / 2, grad_y = G_x dy on the 8 inner nodes,
 //           scaled by the signed coupling, plus the base field, stored as 16-byte pieces of the
 //           blocked layout.
 // (G_x G_y = G_y G_x and the differences commute with both: the result is the oracle's central
@@ -47,12 +63,12 @@ __host__ __device__ constexpr int blur_CW(int R) { return 24 + 4 * blur_NV4(R); 
 // (static part, or the running sum over earlier bead-density fields), may be NULL.
 // A: blocked (x,y) force-gradient field.  field_out (filtered density, row-major) may be NULL.
 template <int R>
-__global__ void __launch_bounds__(BLUR_THREADS, 7) k_blur_grad(int nx, int ny, BlurTaps taps,
+__global__ void __launch_bounds__(BLUR_THREADS, R > 6 ? 1 : 7) k_blur_grad(int nx, int ny, BlurTaps taps,
                                                             const float* __restrict__ rho_b, float coef,
                                                             const float2* base, float2* A,
                                                             float* __restrict__ field_out) {
-  constexpr int NV = blur_NV(R), NV4 = blur_NV4(R), CW = blur_CW(R);
-  __shared__ __align__(16) float ty[BLUR_T * CW], dy[BLUR_T * CW];
+  constexpr int NV = blur_NV(R), CW = blur_CW(R), CP = blur_CP(R);
+  __shared__ __align__(16) float2 td[BLUR_T * CP];
   // 1-D grid in row-major tile order (2-D grids are rasterised in an order that streams worse)
   const int ntx = nx / BLUR_T;
   const int i0 = (blockIdx.x % ntx) * BLUR_T, j0 = (blockIdx.x / ntx) * BLUR_T;
@@ -82,48 +98,40 @@ __global__ void __launch_bounds__(BLUR_THREADS, 7) k_blur_grad(int nx, int ny, B
       t[a] = s;                                             // ty at row j0 + 8c - 1 + a
     }
 #pragma unroll
-    for (int a = 0; a < 8; ++a) {
-      ty[(8 * c + a) * CW + col] = t[a + 1];
-      dy[(8 * c + a) * CW + col] = 0.5f * (t[a + 2] - t[a]);
-    }
+    for (int a = 0; a < 8; ++a) td[(8 * c + a) * CP + col] = make_float2(t[a + 1], 0.5f * (t[a + 2] - t[a]));
   }
   __syncthreads();
-  // x pass: items (row, chunk c of 8 nodes); 4 consecutive threads cover one row
-  for (int it = threadIdx.x; it < BLUR_T * 4; it += BLUR_THREADS) {
-    const int c = it & 3, row = it >> 2;
-    float v[4 * NV4];
+  // x pass: items (row, chunk c of 8 nodes).  A warp takes 8 rows x 4 chunks (its stores fill
+  // whole 128-byte lines of the blocked layout); the 8 lanes of a 16-byte shared access are
+  // 2 chunks x 4 rows.
+  if (threadIdx.x < BLUR_T * 4) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int c = (lane & 1) + 2 * ((lane >> 3) & 1);
+    const int row = ((lane >> 1) & 3) + 4 * (lane >> 4) + 8 * wid;
+    float2 v[NV];
     {
-      const float4* p = reinterpret_cast<const float4*>(ty + row * CW + 8 * c);
+      const float4* p = reinterpret_cast<const float4*>(td + row * CP + 8 * c);
 #pragma unroll
-      for (int q = 0; q < NV4; ++q) {
+      for (int q = 0; q < NV / 2; ++q) {
         const float4 t4 = p[q];
-        v[4 * q] = t4.x; v[4 * q + 1] = t4.y; v[4 * q + 2] = t4.z; v[4 * q + 3] = t4.w;
+        v[2 * q] = make_float2(t4.x, t4.y);
+        v[2 * q + 1] = make_float2(t4.z, t4.w);
       }
     }
-    float B[10];                                            // filtered density at nodes i0 + 8c - 1 + a
+    float2 acc[10];  // .x: filtered density B at node i0 + 8c - 1 + a;  .y: G_x dy at the same node
 #pragma unroll
     for (int a = 0; a < 10; ++a) {
-      float s = 0.0f;
+      float2 s2 = make_float2(0.0f, 0.0f);
 #pragma unroll
-      for (int k = 0; k <= 2 * R; ++k) s = fmaf(taps.g[k], v[a + k], s);
-      B[a] = s;
+      for (int k = 0; k <= 2 * R; ++k) s2 = ffma2(v[a + k], taps.g[k], s2);
+      acc[a] = s2;
     }
-    {
-      const float4* p = reinterpret_cast<const float4*>(dy + row * CW + 8 * c);
+    float B[10];
 #pragma unroll
-      for (int q = 0; q < NV4; ++q) {
-        const float4 t4 = p[q];
-        v[4 * q] = t4.x; v[4 * q + 1] = t4.y; v[4 * q + 2] = t4.z; v[4 * q + 3] = t4.w;
-      }
-    }
+    for (int a = 0; a < 10; ++a) B[a] = acc[a].x;
     float2 o[8];
 #pragma unroll
-    for (int a = 0; a < 8; ++a) {
-      float s = 0.0f;
-#pragma unroll
-      for (int k = 0; k <= 2 * R; ++k) s = fmaf(taps.g[k], v[a + 1 + k], s);
-      o[a] = make_float2(coef * (0.5f * (B[a + 2] - B[a])), coef * s);
-    }
+    for (int a = 0; a < 8; ++a) o[a] = make_float2(coef * (0.5f * (B[a + 2] - B[a])), coef * acc[a + 1].y);
     // nodes (i0 + 8c .. + 7, j0 + row): two 32-byte rows of two neighbouring 4x4 blocks
     const size_t bidx = blk_index(i0 + 8 * c, j0 + row, nx);
 #pragma unroll

@@ -33,17 +33,6 @@ __host__ __device__ constexpr int blur_CW(int R) { return 24 + 4 * blur_NV4(R); 
 // quarter warp (2 chunks x 4 rows) fall on the 8 different bank groups
 __host__ __device__ constexpr int blur_CP(int R) { return blur_CW(R) + 2; }
 
-// d = a * s + c on both halves: one FFMA2 (sm_100 packed fp32; the kernel is bound by issue slots)
-__device__ __forceinline__ float2 ffma2(float2 a, float s, float2 c) {
-  unsigned long long ua, us, uc, ud;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(ua) : "f"(a.x), "f"(a.y));
-  asm("mov.b64 %0, {%1, %1};" : "=l"(us) : "f"(s));
-  asm("mov.b64 %0, {%1, %2};" : "=l"(uc) : "f"(c.x), "f"(c.y));
-  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(ud) : "l"(ua), "l"(us), "l"(uc));
-  float2 d;
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(ud));
-  return d;
-}
 
 // One CTA filters one 32x32 tile; rho_b is read once per node plus the halo (through L1), the
 // gradient is written once, nothing else touches global memory.  The y pass comes first because

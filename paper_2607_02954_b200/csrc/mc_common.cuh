@@ -7,6 +7,29 @@
 namespace mc {
 
 // wrap when i is known to lie in [-n, 2n)
+// Packed fp32 pairs (sm_100 FFMA2: one issue slot for two lanes of arithmetic;
+// the step's kernels are bound by issue slots).  A float2 in an aligned register pair is the
+// operand; the compiler turns a duplicated scalar into the instruction's broadcast form.
+typedef unsigned long long f32x2_t;
+__device__ __forceinline__ f32x2_t pack2(float2 a) {
+  f32x2_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.x), "f"(a.y));
+  return r;
+}
+__device__ __forceinline__ float2 unpack2(f32x2_t a) {
+  float2 d;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(a));
+  return d;
+}
+__device__ __forceinline__ float2 dup2(float s) { return make_float2(s, s); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
+  f32x2_t r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(pack2(a)), "l"(pack2(b)), "l"(pack2(c)));
+  return unpack2(r);
+}
+// d = a * s + c on both halves
+__device__ __forceinline__ float2 ffma2(float2 a, float s, float2 c) { return fma2(a, dup2(s), c); }
+
 __device__ __forceinline__ int wrap1(int i, int n) {
   return i < 0 ? i + n : (i >= n ? i - n : i);
 }

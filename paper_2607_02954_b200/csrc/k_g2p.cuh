@@ -18,7 +18,7 @@ __global__ void __launch_bounds__(256) k_interp_integrate(int N, float2* __restr
   float m = 0.0f;
   if (b < N) {
     float2 p = X[b];
-    const float2 U = TEXROWS ? interp2_tex<TEXROWS>(u, tex_u, nx, ny, p.x, p.y) : interp2(u, nx, ny, p.x, p.y);
+    const float2 U = TEXROWS ? interp2_tex<TEXROWS, false>(u, tex_u, nx, ny, p.x, p.y) : interp2(u, nx, ny, p.x, p.y);
     p.x += U.x;
     p.y += U.y;
     X[b] = p;

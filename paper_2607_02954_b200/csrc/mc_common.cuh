@@ -120,7 +120,10 @@ __device__ __forceinline__ float2 interp2(const float2* __restrict__ p, int nx, 
 // Same sum with the support rows 2 and 3 fetched through the texture pipe (raw fetches of the
 // same memory, no filtering: identical bits).  The per-bead gathers are bound by the LSU pipe's
 // tag stage (one 128-byte line per clock); the TEX pipe has its own.
-template <int TEXROWS>
+// PACK: accumulate both components in one packed pair (FFMA2): same bits, half the FMA issue
+// slots, but K4 then drops to 32 registers and a higher occupancy that costs it 1 % (measured),
+// so only K1 uses it.
+template <int TEXROWS, bool PACK>
 __device__ __forceinline__ float2 interp2_tex(const float2* __restrict__ p, cudaTextureObject_t tex, int nx, int ny,
                                               float x, float y) {
   int i0, j0;
@@ -138,25 +141,23 @@ __device__ __forceinline__ float2 interp2_tex(const float2* __restrict__ p, cuda
     col[k] = ((c >> 2) << 4) + (c & 3);
   }
   const int nbx = nx >> 2;
-  float ax = 0.0f, ay = 0.0f;
+  float2 acc = make_float2(0.0f, 0.0f);
 #pragma unroll
   for (int l = 0; l < 4; ++l) {
     const int row = (j0 + l >= ny) ? j0 + l - ny : j0 + l;
     const int ro = (row >> 2) * nbx * 16 + ((row & 3) << 2);
-    float sx = 0.0f, sy = 0.0f;
+    float2 s2 = make_float2(0.0f, 0.0f);
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       const float2 v = (l >= 4 - TEXROWS)
                            ? tex1Dfetch<float2>(tex, ro + col[k])
                            : __ldg(reinterpret_cast<const float2*>(reinterpret_cast<const char*>(p + ro) +
                                                                    (unsigned long long)(unsigned)col[k] * 8u));
-      sx = fmaf(v.x, wx[k], sx);
-      sy = fmaf(v.y, wx[k], sy);
+      s2 = PACK ? ffma2(v, wx[k], s2) : make_float2(fmaf(v.x, wx[k], s2.x), fmaf(v.y, wx[k], s2.y));
     }
-    ax = fmaf(sx, wy[l], ax);
-    ay = fmaf(sy, wy[l], ay);
+    acc = PACK ? ffma2(s2, wy[l], acc) : make_float2(fmaf(s2.x, wy[l], acc.x), fmaf(s2.y, wy[l], acc.y));
   }
-  return make_float2(ax, ay);
+  return acc;
 }
 
 __device__ __forceinline__ float interp1(const float* __restrict__ p0, int nx, int ny, float x, float y) {

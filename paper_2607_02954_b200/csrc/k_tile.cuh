@@ -5,9 +5,9 @@
 // SKIN (a quarter node of bead motion in every direction), overlaps (1, 2 or 4 tiles), so a tile's CTA can accumulate ALL
 // contributions to its own nodes from its own list and never writes outside the tile: no global
 // float atomics, no halo exchange.  The skin makes a list valid for many steps: K4 records the
-// largest bead displacement component of every step, a one-thread policy kernel (k_list_policy)
+// largest bead displacement component of every step, the policy (list_rebuild_due, below)
 // adds it to the drift accumulated since the lists were built and orders a rebuild only when
-// the drift could reach the skin; until then the three K0 kernels return at once.  Entries
+// the drift could reach the skin; until then the K0 kernels return at once.  Entries
 // whose support no longer (or not yet) overlaps the tile add exact zeros (k_p2g.cuh), so the
 // schedule touches the results only through the per-tile fixed-point scales (powers of two
 // chosen from the list lengths), i.e. at rounding level; it is a function of the state alone,
@@ -49,10 +49,19 @@ struct ListState {
   unsigned step_max;   // bits of max |U_x|,|U_y| over the beads in the last step (K4, atomicMax)
 };
 
-__global__ void k_list_policy(ListState* st) {
+// The policy is evaluated where it is needed instead of in a launch of its own: the count pass
+// (first K0 kernel) only READS the state and every thread derives the same decision; the scan
+// kernel (one block, next in the stream) then commits it -- st->need for the kernels after it,
+// the new drift, step_max = 0 for this step's K4.
+__device__ __forceinline__ bool list_rebuild_due(const ListState* st, float* drift_out) {
   const float d = st->drift + __uint_as_float(st->step_max);
+  *drift_out = d;
+  return !(d <= LIST_DRIFT_MAX);  // also true for NaN
+}
+__device__ __forceinline__ void list_policy_commit(ListState* st) {
+  float d;
+  const bool need = list_rebuild_due(st, &d);
   st->step_max = 0u;
-  const bool need = !(d <= LIST_DRIFT_MAX);  // also true for NaN
   st->need = need ? 1 : 0;
   st->drift = need ? 0.0f : d;
 }
@@ -107,7 +116,12 @@ template <bool FILL>
 __global__ void __launch_bounds__(256) k_tile_bin(const ListState* __restrict__ st, const float2* __restrict__ X,
                                                   int N, int nx, int ny, int* __restrict__ tile_ctr,
                                                   int* __restrict__ bucket_ctr, int* __restrict__ list) {
-  if (!st->need) return;
+  if (FILL) {
+    if (!st->need) return;
+  } else {
+    float d;
+    if (!list_rebuild_due(st, &d)) return;
+  }
   // grid-stride over whole blocks of beads: every lane of a warp takes part in warp_claim
   for (int base = blockIdx.x * blockDim.x; base < N; base += gridDim.x * blockDim.x) {
     const int b = base + threadIdx.x;
@@ -138,25 +152,32 @@ __global__ void __launch_bounds__(256) k_bucket_starts(const ListState* __restri
                                                        int* __restrict__ bucket_cursor) {
   if (!st->need) return;
   const int lane = threadIdx.x & 31;
-  const int t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  if (t >= n_tiles) return;
-  const int v = bucket_count[32 * t + lane];
-  int inc = v;
+  const int warps = (gridDim.x * blockDim.x) >> 5;
+  for (int t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; t < n_tiles; t += warps) {
+    const int v = bucket_count[32 * t + lane];
+    int inc = v;
 #pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const int u = __shfl_up_sync(0xffffffffu, inc, o);
-    if (lane >= o) inc += u;
+    for (int o = 1; o < 32; o <<= 1) {
+      const int u = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += u;
+    }
+    bucket_cursor[32 * t + lane] = tile_start[t] + inc - v;
+    bucket_count[32 * t + lane] = 0;
   }
-  bucket_cursor[32 * t + lane] = tile_start[t] + inc - v;
-  bucket_count[32 * t + lane] = 0;
 }
 
 // one block: tile_start = exclusive scan of tile_count (n_tiles + 1 entries); counts are zeroed
 // for the next rebuild.
-__global__ void __launch_bounds__(1024) k_tile_scan(const ListState* __restrict__ st, int* __restrict__ tile_count,
+__global__ void __launch_bounds__(1024) k_tile_scan(ListState* __restrict__ st, int* __restrict__ tile_count,
                                                     int n_tiles, int* __restrict__ tile_start) {
   __shared__ int sm[33];
-  if (!st->need) return;
+  __shared__ int need_s;
+  if (threadIdx.x == 0) {
+    list_policy_commit(st);
+    need_s = st->need;
+  }
+  __syncthreads();
+  if (!need_s) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   int carry = 0;
   for (int base = 0; base < n_tiles; base += 1024) {

@@ -231,12 +231,11 @@ int enqueue_step(mc_world* w) {
     // unless the policy kernel found the lists' drift bound used up (k_tile.cuh).
     mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16);
     const int k0grid = bgrid < w->n_sm * 8 ? bgrid : w->n_sm * 8;
-    mc::k_list_policy<<<1, 1, 0, st>>>(ls_state);
     mc::k_tile_bin<false><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, tile_count, bucket_count, nullptr);
     mc::k_tile_scan<<<1, 1024, 0, st>>>(ls_state, tile_count, n_tiles, tile_start);
-    mc::k_bucket_starts<<<(n_tiles + 7) / 8, 256, 0, st>>>(ls_state, n_tiles, tile_start, bucket_count, bucket_cursor);
+    mc::k_bucket_starts<<<std::min((n_tiles + 7) / 8, w->n_sm * 4), 256, 0, st>>>(ls_state, n_tiles, tile_start, bucket_count, bucket_cursor);
     mc::k_tile_bin<true><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, nullptr, bucket_cursor, list);
-    w->launches += 5;
+    w->launches += 4;
     prof_mark(w, 1);
     // K2a: S2 deposit
     if (w->d.n_density) {

@@ -272,17 +272,18 @@ def main():
             "act_period")
     host = {k: torch.from_numpy(np.ascontiguousarray(w[k], dtype=np.float32)).pin_memory() for k in keys}
     host["offsets"] = w["offsets"]
-    xy_back = torch.empty((N, 2), dtype=torch.float32).pin_memory()
+    xy_back = [torch.empty((N, 2), dtype=torch.float32).pin_memory()]  # second pinned xy buffer
     h2d = sum(host[k].numel() * 4 for k in keys)
-    d2h = xy_back.numel() * 4
+    d2h = xy_back[0].numel() * 4
 
     def e2e_step():
         G.load_filaments(host)             # pinned host -> device + SoA packing (syncs)
         G.step(1)
         out = G.read_state(keys=("xy",), host=False)["xy"]
-        xy_back.copy_(out, non_blocking=True)
+        xy_back[0].copy_(out, non_blocking=True)
         torch.cuda.synchronize(dev)
-        host["xy"].copy_(xy_back)          # the next step continues from the returned positions
+        # the next step continues from the returned positions: the two pinned buffers swap roles
+        host["xy"], xy_back[0] = xy_back[0].view(host["xy"].shape), host["xy"].view(N, 2)
 
     for _ in range(2):
         e2e_step()

@@ -77,8 +77,9 @@ typedef struct {
 size_t mc_workspace_bytes(const mc_world_params* p /*HOST*/);
 
 /* Create a world: fluid at rest (f_q = w_q rho0), no filaments, step counter 0.
- * workspace: DEVICE, >= mc_workspace_bytes(p) bytes, 256-byte aligned, owned by the caller and
- * must outlive the world.  cuda_stream: a cudaStream_t (NULL = legacy default stream); all
+ * workspace: DEVICE, >= mc_workspace_bytes(p) bytes, 256-byte aligned (512-byte alignment, which
+ * cudaMalloc and torch give, also lets the gathers use texture views: mc_texture_gathers),
+ * owned by the caller and must outlive the world.  cuda_stream: a cudaStream_t (NULL = legacy default stream); all
  * work of this world is enqueued on it.  *out receives the handle.
  * Errors: MC_EINVAL (bad parameters, workspace too small or misaligned), MC_ENOMEM (host),
  * MC_ECUDA. */

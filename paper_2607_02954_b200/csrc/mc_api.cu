@@ -124,7 +124,7 @@ struct mc_world {
   int stride = 60;   // K1 window advance: 64 when all chains share a length dividing 64
   int n_windows = 0;
   cudaTextureObject_t tex_u = 0, tex_A = 0;  // linear float2 views of u and A for the texture-pipe half of the gathers
-  int n_sm = 148;               // SMs of the device the world lives on (persistent kernels' grid)
+  int n_sm = 148;               // SMs of the device the world lives on (grid-stride kernels size their grids by it)
   bool uniform_params = false;  // K1 variant: L_rest, stiffnesses and period identical for all beads
   int deposit_threads = 128;  // CTA size of K2a: 128 hides the per-tile latency better, crowded worlds want 256
   // CUDA graphs of GRAPH_STEPS consecutive steps, one per ping-pong phase, captured on first use

@@ -134,8 +134,8 @@ __global__ void __launch_bounds__(BLUR_THREADS, R > 6 ? 1 : 7) k_blur_grad(int n
         lo.x += b0.x; lo.y += b0.y; lo.z += b0.z; lo.w += b0.w;
         hi.x += b1.x; hi.y += b1.y; hi.z += b1.z; hi.w += b1.w;
       }
-      dst[0] = lo;
-      dst[1] = hi;
+      __stcs(dst, lo);
+      __stcs(dst + 1, hi);
     }
     if (field_out) {
       float4* f = reinterpret_cast<float4*>(field_out + (size_t)(j0 + row) * nx + i0 + 8 * c);

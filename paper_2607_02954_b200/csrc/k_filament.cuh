@@ -63,15 +63,15 @@ template <bool UNIFORM>
 __device__ __forceinline__ BeadParams load_params(const FilamentArgs& a, int b, bool valid) {
   BeadParams p;
   if (valid) {
-    const float4 pc = __ldg(a.PC + b);
+    const float4 pc = __ldcs(a.PC + b);  // parameters are read once per step: streaming loads
     p.c0 = pc.x; p.s0 = pc.y; p.eps = pc.z; p.flags = __float_as_int(pc.w);
     if (UNIFORM) {
-      const float2 pd = __ldg(a.PD + b);
+      const float2 pd = __ldcs(a.PD + b);
       const float4 u0 = __ldg(a.uni), u1 = __ldg(a.uni + 1);
       p.L = u0.x; p.kb = u0.y; p.ks = u0.z; p.kst = u0.w; p.rhi = u1.x; p.rlo = u1.y;
       p.amp = pd.x; p.phase = pd.y;
     } else {
-      const float4 pa = __ldg(a.PA + b), pb = __ldg(a.PB + b);
+      const float4 pa = __ldcs(a.PA + b), pb = __ldcs(a.PB + b);
       p.L = pa.x; p.amp = pa.y; p.phase = pa.z; p.kb = pa.w;
       p.ks = pb.x; p.kst = pb.y; p.rhi = pb.z; p.rlo = pb.w;
     }

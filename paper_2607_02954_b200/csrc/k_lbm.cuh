@@ -238,12 +238,12 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
     trt_collide(gA, GAx, GAy, a.rho0, a.k, uAx, uAy);
     trt_collide(gB, GBx, GBy, a.rho0, a.k, uBx, uBy);
     // blocked u: nodes i and i+1 (i even) are neighbours inside one 4x4 block
-    *reinterpret_cast<float4*>(a.u + blk_index(i, j, nx)) = make_float4(uAx, uAy, uBx, uBy);
+    __stcs(reinterpret_cast<float4*>(a.u + blk_index(i, j, nx)), make_float4(uAx, uAy, uBx, uBy));
     if (nc * sizeof(float) * 8 < 0xffffffffull) {
       char* d0 = reinterpret_cast<char*>(a.dst + c);
 #pragma unroll
-      for (int q = 0; q < 9; ++q)
-        *reinterpret_cast<float2*>(d0 + (unsigned long long)pb * (unsigned)q) = make_float2(gA[q], gB[q]);
+      for (int q = 0; q < 9; ++q)  // streaming stores: nothing reads these lines before a whole step has passed
+        __stcs(reinterpret_cast<float2*>(d0 + (unsigned long long)pb * (unsigned)q), make_float2(gA[q], gB[q]));
     } else {
 #pragma unroll
       for (int q = 0; q < 9; ++q) *reinterpret_cast<float2*>(a.dst + q * nc + c) = make_float2(gA[q], gB[q]);

@@ -291,7 +291,7 @@ __global__ void __launch_bounds__(256, LIGHT ? 6 : 1) k_deposit_tile(int nx, int
       v[k] = (wide ? fmaf((float)accl[a + k], linv, (float)acc[a + k]) : (float)acc[a + k]) * inv;
       mx = fmaxf(mx, v[k]);
     }
-    *reinterpret_cast<float4*>(rho_b + (size_t)(y0 + ly) * nx + x0 + lx) = make_float4(v[0], v[1], v[2], v[3]);
+    __stcs(reinterpret_cast<float4*>(rho_b + (size_t)(y0 + ly) * nx + x0 + lx), make_float4(v[0], v[1], v[2], v[3]));
   }
   // tile maximum: rho_b >= 0, so the float bits order like unsigned integers; one global
   // atomicMax per warp onto tile_rho_max[t] (zeroed by the tile-list scan of this step)

@@ -25,7 +25,7 @@ struct BlurTaps {
 // shared-memory geometry for radius R.  The two intermediate planes hold the 32 rows of the tile
 // and the columns from node i0 - (R+1) on, so that the x pass of the 8 outputs starting at node
 // i0 + 8c reads its window from column 8c: every shared access of the x pass is a 16-byte one.
-constexpr int BLUR_THREADS = 192;
+constexpr int BLUR_THREADS = 128;
 __host__ __device__ constexpr int blur_NV(int R) { return 10 + 2 * R; }               // window: 8 outputs + 2 + 2R
 __host__ __device__ constexpr int blur_NV4(int R) { return (blur_NV(R) + 3) / 4; }
 __host__ __device__ constexpr int blur_CW(int R) { return 24 + 4 * blur_NV4(R); }     // columns held >= 34 + 2R
@@ -38,8 +38,9 @@ __host__ __device__ constexpr int blur_CP(int R) { return blur_CW(R) + 2; }
 // gradient is written once, nothing else touches global memory.  The y pass comes first because
 // its loads are then coalesced straight from global memory (lanes = columns) and the y-derivative
 // is a register operation on its outputs:
-//   y pass: thread = (column of the tile + x halo, chunk of 8 rows): 10 + 2R loads of its
-//           column, ty = G_y rho_b on 10 rows, of which 8 are stored together with
+//   y pass: thread = (PAIR of columns of the tile + x halo, chunk of 8 rows): 10 + 2R 8-byte
+//           loads of its columns, ty = G_y rho_b on 10 rows (packed FFMA2, one column in each
+//           half), of which 8 are stored together with
 //           dy = (ty[y+1] - ty[y-1]) / 2                              -> (ty, dy) [32][CP]
 //   x pass: thread = (row, chunk of 8 nodes): register window of the interleaved (ty, dy) pairs
 //           (16-byte LDS), (B, G_x dy) = G_x (ty, dy) on 10 nodes with packed FFMA2,
@@ -61,33 +62,37 @@ __global__ void __launch_bounds__(BLUR_THREADS, R > 6 ? 1 : 7) k_blur_grad(int n
   // 1-D grid in row-major tile order (2-D grids are rasterised in an order that streams worse)
   const int ntx = nx / BLUR_T;
   const int i0 = (blockIdx.x % ntx) * BLUR_T, j0 = (blockIdx.x / ntx) * BLUR_T;
-  // y pass: items (chunk c of 8 rows, column col <-> node i0 - (R+1) + col)
-  for (int it = threadIdx.x; it < 4 * CW; it += BLUR_THREADS) {
-    const int c = it / CW, col = it - c * CW;
-    const int gi = wrap1(i0 - (R + 1) + col, nx);           // halo R+1 < 32 <= nx
+  // y pass: items (chunk c of 8 rows, PAIR of columns col, col + 1 <-> nodes i0 - (R+1) + col ...):
+  // 8-byte loads, both columns ride in packed FFMA2 pairs
+  for (int it = threadIdx.x; it < 4 * (CW / 2); it += BLUR_THREADS) {
+    const int c = it / (CW / 2), col = 2 * (it - c * (CW / 2));
+    const int gi = wrap1(i0 - (R + 1) + col, nx);           // even: the pair never straddles the x seam
     const int r0 = j0 + 8 * c - 1 - R;                      // first row of the window
-    float v[NV];
+    float2 v[NV];
     if (j0 - 1 - R >= 0 && j0 + BLUR_T + 1 + R <= ny) {     // tile away from the y seam: no row wraps
       // row k of the window: one IMAD.WIDE (32-bit row size x immediate k + 64-bit pointer)
       const char* p = reinterpret_cast<const char*>(rho_b + (size_t)r0 * nx + gi);
       const unsigned rowb = (unsigned)nx * (unsigned)sizeof(float);
 #pragma unroll
       for (int k = 0; k < NV; ++k)
-        v[k] = __ldg(reinterpret_cast<const float*>(p + (unsigned long long)rowb * (unsigned)k));
+        v[k] = __ldg(reinterpret_cast<const float2*>(p + (unsigned long long)rowb * (unsigned)k));
     } else {
 #pragma unroll
-      for (int k = 0; k < NV; ++k) v[k] = __ldg(rho_b + (size_t)wrap1(r0 + k, ny) * nx + gi);
+      for (int k = 0; k < NV; ++k)
+        v[k] = __ldg(reinterpret_cast<const float2*>(rho_b + (size_t)wrap1(r0 + k, ny) * nx + gi));
     }
-    float t[10];
+    float2 t[10];
 #pragma unroll
     for (int a = 0; a < 10; ++a) {
-      float s = 0.0f;
+      float2 s2 = make_float2(0.0f, 0.0f);
 #pragma unroll
-      for (int k = 0; k <= 2 * R; ++k) s = fmaf(taps.g[k], v[a + k], s);
-      t[a] = s;                                             // ty at row j0 + 8c - 1 + a
+      for (int k = 0; k <= 2 * R; ++k) s2 = ffma2(v[a + k], taps.g[k], s2);
+      t[a] = s2;                                            // ty at row j0 + 8c - 1 + a, columns col, col + 1
     }
 #pragma unroll
-    for (int a = 0; a < 8; ++a) td[(8 * c + a) * CP + col] = make_float2(t[a + 1], 0.5f * (t[a + 2] - t[a]));
+    for (int a = 0; a < 8; ++a)
+      *reinterpret_cast<float4*>(td + (8 * c + a) * CP + col) =
+          make_float4(t[a + 1].x, 0.5f * (t[a + 2].x - t[a].x), t[a + 1].y, 0.5f * (t[a + 2].y - t[a].y));
   }
   __syncthreads();
   // x pass: items (row, chunk c of 8 nodes).  A warp takes 8 rows x 4 chunks (its stores fill

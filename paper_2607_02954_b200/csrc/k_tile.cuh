@@ -109,19 +109,17 @@ __device__ __forceinline__ int warp_claim(int* ctr, int key, bool act) {
   return slot;
 }
 
+// The four phases of a rebuild as device functions over the threads of the calling grid (a
+// 1-block grid is allowed), so that the per-phase kernels of large worlds and the one-CTA kernel
+// of small worlds share them.
+
 // FILL = false: tile_ctr[t] += 1 and (if given) bucket_ctr[32 t + key] += 1 per listed bead.
-// FILL = true: bucket_ctr holds the running cursors (k_bucket_starts) and the bead index is
+// FILL = true: bucket_ctr holds the running cursors (bucket_starts) and the bead index is
 // stored at the claimed slot.
 template <bool FILL>
-__global__ void __launch_bounds__(256) k_tile_bin(const ListState* __restrict__ st, const float2* __restrict__ X,
-                                                  int N, int nx, int ny, int* __restrict__ tile_ctr,
-                                                  int* __restrict__ bucket_ctr, int* __restrict__ list) {
-  if (FILL) {
-    if (!st->need) return;
-  } else {
-    float d;
-    if (!list_rebuild_due(st, &d)) return;
-  }
+__device__ __forceinline__ void tile_bin(const float2* __restrict__ X, int N, int nx, int ny,
+                                         int* __restrict__ tile_ctr, int* __restrict__ bucket_ctr,
+                                         int* __restrict__ list) {
   // grid-stride over whole blocks of beads: every lane of a warp takes part in warp_claim
   for (int base = blockIdx.x * blockDim.x; base < N; base += gridDim.x * blockDim.x) {
     const int b = base + threadIdx.x;
@@ -146,11 +144,8 @@ __global__ void __launch_bounds__(256) k_tile_bin(const ListState* __restrict__ 
 
 // one warp per tile: bucket_cursor[32 t + k] = tile_start[t] + exclusive scan of the tile's 32
 // bucket counts; the counts are zeroed for the next rebuild.
-__global__ void __launch_bounds__(256) k_bucket_starts(const ListState* __restrict__ st, int n_tiles,
-                                                       const int* __restrict__ tile_start,
-                                                       int* __restrict__ bucket_count,
-                                                       int* __restrict__ bucket_cursor) {
-  if (!st->need) return;
+__device__ __forceinline__ void bucket_starts(int n_tiles, const int* __restrict__ tile_start,
+                                              int* __restrict__ bucket_count, int* __restrict__ bucket_cursor) {
   const int lane = threadIdx.x & 31;
   const int warps = (gridDim.x * blockDim.x) >> 5;
   for (int t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; t < n_tiles; t += warps) {
@@ -166,18 +161,10 @@ __global__ void __launch_bounds__(256) k_bucket_starts(const ListState* __restri
   }
 }
 
-// one block: tile_start = exclusive scan of tile_count (n_tiles + 1 entries); counts are zeroed
-// for the next rebuild.
-__global__ void __launch_bounds__(1024) k_tile_scan(ListState* __restrict__ st, int* __restrict__ tile_count,
-                                                    int n_tiles, int* __restrict__ tile_start) {
-  __shared__ int sm[33];
-  __shared__ int need_s;
-  if (threadIdx.x == 0) {
-    list_policy_commit(st);
-    need_s = st->need;
-  }
-  __syncthreads();
-  if (!need_s) return;
+// ONE block of 1024 threads: tile_start = exclusive scan of tile_count (n_tiles + 1 entries);
+// counts are zeroed for the next rebuild.  sm: 33 ints of shared memory.
+__device__ __forceinline__ void tile_scan(int* __restrict__ tile_count, int n_tiles, int* __restrict__ tile_start,
+                                          int* sm) {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   int carry = 0;
   for (int base = 0; base < n_tiles; base += 1024) {
@@ -212,6 +199,65 @@ __global__ void __launch_bounds__(1024) k_tile_scan(ListState* __restrict__ st, 
     __syncthreads();
   }
   if (threadIdx.x == 0) tile_start[n_tiles] = carry;
+}
+
+template <bool FILL>
+__global__ void __launch_bounds__(256) k_tile_bin(const ListState* __restrict__ st, const float2* __restrict__ X,
+                                                  int N, int nx, int ny, int* __restrict__ tile_ctr,
+                                                  int* __restrict__ bucket_ctr, int* __restrict__ list) {
+  if (FILL) {
+    if (!st->need) return;
+  } else {
+    float d;
+    if (!list_rebuild_due(st, &d)) return;
+  }
+  tile_bin<FILL>(X, N, nx, ny, tile_ctr, bucket_ctr, list);
+}
+
+__global__ void __launch_bounds__(256) k_bucket_starts(const ListState* __restrict__ st, int n_tiles,
+                                                       const int* __restrict__ tile_start,
+                                                       int* __restrict__ bucket_count,
+                                                       int* __restrict__ bucket_cursor) {
+  if (!st->need) return;
+  bucket_starts(n_tiles, tile_start, bucket_count, bucket_cursor);
+}
+
+__global__ void __launch_bounds__(1024) k_tile_scan(ListState* __restrict__ st, int* __restrict__ tile_count,
+                                                    int n_tiles, int* __restrict__ tile_start) {
+  __shared__ int sm[33];
+  __shared__ int need_s;
+  if (threadIdx.x == 0) {
+    list_policy_commit(st);
+    need_s = st->need;
+  }
+  __syncthreads();
+  if (!need_s) return;
+  tile_scan(tile_count, n_tiles, tile_start, sm);
+}
+
+// Small worlds (bound by launch overhead, not by work): the whole of K0 in ONE launch of one
+// 1024-thread CTA -- policy, count, scan, bucket starts, fill, separated by __syncthreads()
+// (global atomics and stores of a block are visible to the same block after the barrier).
+__global__ void __launch_bounds__(1024) k_list_build_small(ListState* __restrict__ st, const float2* __restrict__ X,
+                                                           int N, int nx, int ny, int n_tiles,
+                                                           int* __restrict__ tile_count, int* __restrict__ tile_start,
+                                                           int* __restrict__ bucket_count,
+                                                           int* __restrict__ bucket_cursor, int* __restrict__ list) {
+  __shared__ int sm[33];
+  __shared__ int need_s;
+  if (threadIdx.x == 0) {
+    list_policy_commit(st);
+    need_s = st->need;
+  }
+  __syncthreads();
+  if (!need_s) return;
+  tile_bin<false>(X, N, nx, ny, tile_count, bucket_count, nullptr);
+  __syncthreads();
+  tile_scan(tile_count, n_tiles, tile_start, sm);
+  __syncthreads();
+  bucket_starts(n_tiles, tile_start, bucket_count, bucket_cursor);
+  __syncthreads();
+  tile_bin<true>(X, N, nx, ny, nullptr, bucket_cursor, list);
 }
 
 // mc_load_filaments: largest tile list (chooses the CTA size of the P2G kernels)

@@ -167,6 +167,8 @@ int check_cuda(mc_world* w, const char* what) {
 
 constexpr int PROF_MAX_STEPS = 64;
 constexpr int GRAPH_STEPS = 4;
+// worlds up to this size rebuild their tile lists in one single-CTA launch (launch bound anyway)
+constexpr int K0_SMALL_BEADS = 32768, K0_SMALL_TILES = 1024;
 static_assert(GRAPH_STEPS % 2 == 0, "graph period");
 
 void drop_graphs(mc_world* w) {
@@ -227,15 +229,22 @@ int enqueue_step(mc_world* w) {
 
   prof_mark(w, 0);
   if (beads) {
-    // K0: policy + tile binning (count, scan, fill).  The three binning kernels return at once
-    // unless the policy kernel found the lists' drift bound used up (k_tile.cuh).
+    // K0: tile binning (policy, count, scan, bucket starts, fill).  The kernels return at once
+    // unless the policy finds the lists' drift bound used up (k_tile.cuh).
     mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16);
-    const int k0grid = bgrid < w->n_sm * 8 ? bgrid : w->n_sm * 8;
-    mc::k_tile_bin<false><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, tile_count, bucket_count, nullptr);
-    mc::k_tile_scan<<<1, 1024, 0, st>>>(ls_state, tile_count, n_tiles, tile_start);
-    mc::k_bucket_starts<<<std::min((n_tiles + 7) / 8, w->n_sm * 4), 256, 0, st>>>(ls_state, n_tiles, tile_start, bucket_count, bucket_cursor);
-    mc::k_tile_bin<true><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, nullptr, bucket_cursor, list);
-    w->launches += 4;
+    if (N <= K0_SMALL_BEADS && n_tiles <= K0_SMALL_TILES) {
+      // small world: one launch of one CTA instead of four (k_tile.cuh)
+      mc::k_list_build_small<<<1, 1024, 0, st>>>(ls_state, X, N, nx, ny, n_tiles, tile_count, tile_start,
+                                                 bucket_count, bucket_cursor, list);
+      w->launches += 1;
+    } else {
+      const int k0grid = bgrid < w->n_sm * 8 ? bgrid : w->n_sm * 8;
+      mc::k_tile_bin<false><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, tile_count, bucket_count, nullptr);
+      mc::k_tile_scan<<<1, 1024, 0, st>>>(ls_state, tile_count, n_tiles, tile_start);
+      mc::k_bucket_starts<<<std::min((n_tiles + 7) / 8, w->n_sm * 4), 256, 0, st>>>(ls_state, n_tiles, tile_start, bucket_count, bucket_cursor);
+      mc::k_tile_bin<true><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, nullptr, bucket_cursor, list);
+      w->launches += 4;
+    }
     prof_mark(w, 1);
     // K2a: S2 deposit
     if (w->d.n_density) {

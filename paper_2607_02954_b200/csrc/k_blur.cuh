@@ -64,9 +64,11 @@ __global__ void __launch_bounds__(BLUR_THREADS, R > 6 ? 1 : 7) k_blur_grad(int n
   const int i0 = (blockIdx.x % ntx) * BLUR_T, j0 = (blockIdx.x / ntx) * BLUR_T;
   // y pass: items (chunk c of 8 rows, PAIR of columns col, col + 1 <-> nodes i0 - (R+1) + col ...):
   // 8-byte loads, both columns ride in packed FFMA2 pairs
-  for (int it = threadIdx.x; it < 4 * (CW / 2); it += BLUR_THREADS) {
-    const int c = it / (CW / 2), col = 2 * (it - c * (CW / 2));
-    const int gi = wrap1(i0 - (R + 1) + col, nx);           // even: the pair never straddles the x seam
+  // (for even R the window starts at an odd node: the pairs then start one column further left)
+  constexpr int PO = (R + 1) & 1, NP = CW / 2 + PO;
+  for (int it = threadIdx.x; it < 4 * NP; it += BLUR_THREADS) {
+    const int c = it / NP, col = 2 * (it - c * NP) - PO;    // first column of the pair (-1 possible)
+    const int gi = wrap1(i0 - (R + 1) + col, nx);           // even: aligned, never straddles the x seam
     const int r0 = j0 + 8 * c - 1 - R;                      // first row of the window
     float2 v[NV];
     if (j0 - 1 - R >= 0 && j0 + BLUR_T + 1 + R <= ny) {     // tile away from the y seam: no row wraps
@@ -90,9 +92,17 @@ __global__ void __launch_bounds__(BLUR_THREADS, R > 6 ? 1 : 7) k_blur_grad(int n
       t[a] = s2;                                            // ty at row j0 + 8c - 1 + a, columns col, col + 1
     }
 #pragma unroll
-    for (int a = 0; a < 8; ++a)
-      *reinterpret_cast<float4*>(td + (8 * c + a) * CP + col) =
-          make_float4(t[a + 1].x, 0.5f * (t[a + 2].x - t[a].x), t[a + 1].y, 0.5f * (t[a + 2].y - t[a].y));
+    for (int a = 0; a < 8; ++a) {
+      const float2 lo = make_float2(t[a + 1].x, 0.5f * (t[a + 2].x - t[a].x));
+      const float2 hi = make_float2(t[a + 1].y, 0.5f * (t[a + 2].y - t[a].y));
+      float2* dst = td + (8 * c + a) * CP + col;
+      if (PO == 0) {
+        *reinterpret_cast<float4*>(dst) = make_float4(lo.x, lo.y, hi.x, hi.y);
+      } else {
+        if (col >= 0) dst[0] = lo;
+        if (col + 1 < CW) dst[1] = hi;
+      }
+    }
   }
   __syncthreads();
   // x pass: items (row, chunk c of 8 nodes).  A warp takes 8 rows x 4 chunks (its stores fill

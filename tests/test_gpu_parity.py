@@ -131,6 +131,11 @@ SMALL = {
     "single_tile_32": lambda: worlds.ragged_world(32, 32, [5, 12, 20], seed=11),
     # wide and flat: one tile high, several wide; R = 3 filter; sigma != 1
     "flat_160x32": lambda: _with_sigma(worlds.ragged_world(160, 32, [16, 30, 64, 9], seed=12), 0.6, 3),
+    # other filter radii: even R (the column pairs of the y pass start one node further left), the
+    # R > 6 instantiations of the blur kernel (no occupancy cap), R = 16 is the maximum
+    "filter_R4": lambda: _with_sigma(worlds.ragged_world(64, 64, [12, 30, 50], seed=17), 0.8, 4),
+    "filter_R9": lambda: _with_sigma(worlds.ragged_world(96, 64, [16, 30, 64, 9, 41], seed=15), 1.8, 9),
+    "filter_R16": lambda: _with_sigma(worlds.ragged_world(64, 96, [20, 33, 64], seed=16), 3.2, 16),
     # rest length, stiffnesses and period differ from bead to bead / chain to chain
     "varied_params": lambda: _varied(worlds.ragged_world(96, 96, [7, 32, 64, 33, 90, 16, 16], seed=13,
                                                          static_source=True), 14),

@@ -282,6 +282,59 @@ void mco_lbm_step(int32_t nx, int32_t ny, double* f, const double* G, double ome
   std::memcpy(f, fs.data(), 9 * nc * sizeof(double));
 }
 
+// Moments of the populations: rho = sum f_q, u* = sum c_q f_q / rho.  u* is the velocity the
+// node would have without any force this step (Guo: u = u* + G/(2 rho), reading 11).
+void mco_moments(int32_t nx, int32_t ny, const double* f, double* rho, double* ustar) {
+  const size_t nc = (size_t)nx * ny;
+  MCO_PAR
+  for (long long c = 0; c < (long long)nc; ++c) {
+    double r = 0.0, mx = 0.0, my = 0.0;
+    for (int q = 0; q < 9; ++q) {
+      r += f[q * nc + c];
+      mx += CX[q] * f[q * nc + c];
+      my += CY[q] * f[q * nc + c];
+    }
+    rho[c] = r;
+    ustar[c] = mx / r;
+    ustar[nc + c] = my / r;
+  }
+}
+
+// Multi-Direct Forcing (Wang, Fan & Luo 2008, cited P:L127; "the filaments' nodes sample
+// the local fluid velocity ... the agent broadcasts its own velocity back onto the grid").
+// Reading 26: each iteration adds the bead force rho0 (V_i - U_i), spreads
+// it and corrects the grid velocity with Guo's u = u* + G/(2 rho); the bead forces add up.  The
+// factor rho0 (half of the 2 rho0 that would cancel an isolated bead's slip at once) keeps the
+// iteration contracting where chains overlap: it needs interp(rho_b)(X_i) < 4 instead of < 2.
+void mco_mdf(int32_t nx, int32_t ny, int64_t N, const double* xy, const double* V,
+             const double* ustar, const double* rho, double rho0, int32_t iters, double* F,
+             double* G, double* u_out, double* resid) {
+  const size_t nc = (size_t)nx * ny;
+  std::vector<double> u(ustar, ustar + 2 * nc), U(2 * (size_t)N), dF(2 * (size_t)N), dG(2 * nc);
+  for (size_t c = 0; c < 2 * nc; ++c) G[c] = 0.0;
+  for (int64_t i = 0; i < 2 * N; ++i) F[i] = 0.0;
+  for (int k = 0; k <= iters; ++k) {
+    mco_interp(nx, ny, 2, u.data(), N, xy, U.data());           // sample
+    if (resid) {
+      double r = 0.0;
+      for (int64_t i = 0; i < 2 * N; ++i) r = std::fmax(r, std::fabs(V[i] - U[i]));
+      resid[k] = r;
+    }
+    if (k == iters) break;
+    for (int64_t i = 0; i < 2 * N; ++i) {
+      dF[i] = rho0 * (V[i] - U[i]);                             // direct forcing
+      F[i] += dF[i];
+    }
+    mco_spread(nx, ny, N, xy, dF.data(), dG.data());             // broadcast
+    for (size_t c = 0; c < 2 * nc; ++c) G[c] += dG[c];
+    for (size_t c = 0; c < nc; ++c) {
+      u[c] = ustar[c] + G[c] / (2.0 * rho[c]);
+      u[nc + c] = ustar[nc + c] + G[nc + c] / (2.0 * rho[c]);
+    }
+  }
+  if (u_out) std::memcpy(u_out, u.data(), 2 * nc * sizeof(double));
+}
+
 }  // extern "C"
 
 // ------------------------------------------------------------------------------------
@@ -325,6 +378,8 @@ int mco_create(const mco_world_params* p, mco_world** out) {
       !(p->rho0 > 0) || p->pbd_iters != 1 || p->n_fields < 0 || p->n_fields > 4 ||
       p->max_beads < 0)
     return MCO_EINVAL;
+  if (p->coupling != MCO_COUPLING_FORCE && p->coupling != MCO_COUPLING_MDF) return MCO_EINVAL;
+  if (p->coupling == MCO_COUPLING_MDF && (p->mdf_iters < 1 || p->mdf_iters > 16)) return MCO_EINVAL;
   for (int k = 0; k < p->n_fields; ++k) {
     const mco_field_params& fp = p->fields[k];
     if (fp.kind == MCO_FIELD_BEAD_DENSITY) {
@@ -442,7 +497,12 @@ static int mco_one_step(mco_world* w) {
                        w->k_stretch.data(), w->act_amp.data(), w->act_phase.data(),
                        w->act_period.data(), w->dt, w->step, w->D.data());
   if (rc != MCO_OK) { w->err = "degenerate edge"; return rc; }
-  for (int64_t i = 0; i < 2 * N; ++i) w->F[i] = w->kappa * w->D[i];
+  // FORCE coupling: F = kappa D + field forces.  MDF coupling (reading 26): the same sum with
+  // kappa = 1 is the bead's own velocity V_i = D_i + field displacement (lattice units, one
+  // step, unit bead mass); it is held in F until the forcing iterations replace it.
+  const bool mdf = w->p.coupling == MCO_COUPLING_MDF;
+  const double kD = mdf ? 1.0 : w->kappa;
+  for (int64_t i = 0; i < 2 * N; ++i) w->F[i] = kD * w->D[i];
   for (int64_t i = 0; i < N; ++i) w->sense[i] = 0.0;
   // S2: deposit (one rho_b serves every bead-density field)
   mco_deposit(nx, ny, N, w->X.data(), w->rho_b.data());
@@ -470,8 +530,16 @@ static int mco_one_step(mco_world* w) {
       for (int64_t i = 0; i < N; ++i) w->sense[i] += s1[i];
     }
   }
-  // S5: spread the total bead force
-  mco_spread(nx, ny, N, w->X.data(), w->F.data(), w->G.data());
+  if (mdf) {
+    // S5 (MDF): forcing iterations against the force-free velocity of the current populations
+    std::vector<double> rho(nc), ustar(2 * nc), V(w->F);
+    mco_moments(nx, ny, w->f.data(), rho.data(), ustar.data());
+    mco_mdf(nx, ny, N, w->X.data(), V.data(), ustar.data(), rho.data(), w->rho0, w->p.mdf_iters,
+            w->F.data(), w->G.data(), nullptr, nullptr);
+  } else {
+    // S5: spread the total bead force
+    mco_spread(nx, ny, N, w->X.data(), w->F.data(), w->G.data());
+  }
   // S6: fluid update; stores the collision-time velocity u
   mco_lbm_step(nx, ny, w->f.data(), w->G.data(), w->omega_p, w->omega_m, w->u.data());
   // S7: interpolate u at the same X and integrate (forward Euler, lattice units)

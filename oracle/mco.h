@@ -11,6 +11,7 @@
  *   - steric field: deposit -> Gaussian -> gradient P:L119
  *   - persistent scalar (energy) field, sensed
  *   - immersed-boundary spread / interpolate
+ *   - Multi-Direct Forcing coupling (optional)      P:L125-127 (reading 26)
  * Where the paper is silent the readings of SURVEY.md 8(c).2 / DESIGN.md are taken;
  * each function in mco.cpp names the passage or reading it follows.
  *
@@ -37,6 +38,11 @@ typedef struct mco_world mco_world;
 
 enum { MCO_OK = 0, MCO_EINVAL = -1, MCO_ENOMEM = -2, MCO_ESTATE = -4 };
 enum { MCO_FIELD_BEAD_DENSITY = 0, MCO_FIELD_STATIC_SOURCE = 1 };
+/* How the PBD output reaches the fluid ("broadcasts its own velocity back onto the grid"):
+ * FORCE: the net displacement becomes a bead force kappa*D_i (reading 1);
+ * MDF:   the bead's own velocity V_i is imposed on the fluid by iterated direct forcing
+ *        (Multi-Direct Forcing, Wang et al. 2008, cited P:L127; reading 26). */
+enum { MCO_COUPLING_FORCE = 0, MCO_COUPLING_MDF = 1 };
 
 typedef struct {
   int32_t kind;        /* MCO_FIELD_*                                             */
@@ -58,6 +64,8 @@ typedef struct {
   int32_t n_fields;
   mco_field_params fields[4];
   int64_t max_beads;
+  int32_t coupling;    /* MCO_COUPLING_*                                           */
+  int32_t mdf_iters;   /* MDF: forcing iterations per step, 1..16 (ignored for FORCE) */
 } mco_world_params;
 
 /* ---- world life cycle (twin of the product ABI, host pointers) ---- */
@@ -115,6 +123,19 @@ void mco_lbm_step(int32_t nx, int32_t ny, double* f, const double* G, double ome
                   double omega_minus, double* u_out);
 void mco_lattice_constants(double nu, double dt, double trt_lambda, double* omega_plus,
                            double* omega_minus);
+/* zeroth and first moments of un-shifted populations f [9][ny][nx]:
+ * rho [ny][nx] = sum_q f_q, ustar [2][ny][nx] = sum_q c_q f_q / rho (velocity without force) */
+void mco_moments(int32_t nx, int32_t ny, const double* f, double* rho, double* ustar);
+/* Multi-Direct Forcing (reading 26).  V [N][2] target bead velocities, ustar/rho from
+ * mco_moments.  Iteration k = 0..iters-1, starting from u^0 = ustar, G^0 = 0:
+ *   U_i = interp(u^k)(X_i);  dF_i = rho0 (V_i - U_i);  F_i += dF_i;
+ *   G^{k+1} = G^k + spread(dF);  u^{k+1}(g) = ustar(g) + G^{k+1}(g) / (2 rho(g)).
+ * Out: F [N][2] summed bead force, G [2][ny][nx] summed grid force, u_out [2][ny][nx] = u^iters
+ * (may be NULL), resid [iters+1] (may be NULL): max_i |V_i - U_i| (max-norm over beads and
+ * components) seen at the start of each iteration and after the last one. */
+void mco_mdf(int32_t nx, int32_t ny, int64_t N, const double* xy, const double* V,
+             const double* ustar, const double* rho, double rho0, int32_t iters, double* F,
+             double* G, double* u_out, double* resid);
 
 #ifdef __cplusplus
 }

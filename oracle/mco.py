@@ -26,7 +26,7 @@ class WorldParams(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("dt", C.c_float), ("nu", C.c_float),
                 ("trt_lambda", C.c_float), ("rho0", C.c_float), ("k_el", C.c_float),
                 ("pbd_iters", C.c_int32), ("n_fields", C.c_int32), ("fields", FieldParams * 4),
-                ("max_beads", C.c_int64)]
+                ("max_beads", C.c_int64), ("coupling", C.c_int32), ("mdf_iters", C.c_int32)]
 
 
 _lib = None
@@ -75,6 +75,8 @@ def make_params(p: dict):
         setattr(wp, k, float(p[k]))
     wp.n_fields = len(p["fields"])
     wp.max_beads = int(p["max_beads"])
+    wp.coupling = int(p.get("coupling", 0))
+    wp.mdf_iters = int(p.get("mdf_iters", 0))
     for i, fd in enumerate(p["fields"]):
         fp = wp.fields[i]
         fp.kind = int(fd["kind"])
@@ -265,3 +267,25 @@ def lbm_step(f, G, omega_plus: float, omega_minus: float):
     lib().mco_lbm_step(C.c_int32(nx), C.c_int32(ny), _d(f), _d(G), C.c_double(omega_plus),
                        C.c_double(omega_minus), _d(u))
     return f, u
+
+
+def moments(f):
+    """f [9,ny,nx] un-shifted -> (rho [ny,nx], ustar [2,ny,nx])."""
+    f = _f64(f)
+    _, ny, nx = f.shape
+    rho, us = np.empty((ny, nx)), np.empty((2, ny, nx))
+    lib().mco_moments(C.c_int32(nx), C.c_int32(ny), _d(f), _d(rho), _d(us))
+    return rho, us
+
+
+def mdf(xy, V, ustar, rho, rho0: float, iters: int):
+    """Multi-Direct Forcing -> dict(F [N,2], G [2,ny,nx], u [2,ny,nx], resid [iters+1])."""
+    xy, V, ustar, rho = _f64(xy), _f64(V), _f64(ustar), _f64(rho)
+    _, ny, nx = ustar.shape
+    N = len(xy)
+    out = dict(F=np.empty((N, 2)), G=np.empty((2, ny, nx)), u=np.empty((2, ny, nx)),
+               resid=np.empty(iters + 1))
+    lib().mco_mdf(C.c_int32(nx), C.c_int32(ny), C.c_int64(N), _d(xy), _d(V), _d(ustar), _d(rho),
+                  C.c_double(rho0), C.c_int32(iters), _d(out["F"]), _d(out["G"]), _d(out["u"]),
+                  _d(out["resid"]))
+    return out

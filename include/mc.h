@@ -15,6 +15,11 @@
  *   S5 spread bead forces -> G               P:L125            (reading 7)
  *   S6 D2Q9 TRT collide (Guo source) + stream P:L117-119, L127 (readings 10, 11)
  *   S7 interpolate u at the beads, X += U    P:L125            (readings 11, 12, 19)
+ * With coupling = MC_COUPLING_MDF ("Multi-Direct Forcing", reading 26) S4 yields the
+ * bead's own velocity V_i = D_i + field displacement instead of a force, and S5 becomes
+ *   S5' u^0 = u* = sum_q c_q f_q / rho; mdf_iters times: U_i = interp(u^k)(X_i),
+ *       F_i += rho0 (V_i - U_i), u^{k+1} = u^k + spread(rho0 (V - U)) / (2 rho);  G = spread(F)
+ * followed by S6 and S7 unchanged.
  *
  * Conventions.  Grid node (i,j) sits at position (i,j); cell size 1; periodic domain
  * [0,nx) x [0,ny).  Grid arrays are row-major, x fastest (index j*nx+i); multi-channel
@@ -51,6 +56,11 @@ enum {
   MC_FIELD_STATIC_SOURCE = 1 /* Gaussian packets; force = +k * grad(c); c is sensed P:L121 */
 };
 
+enum {
+  MC_COUPLING_FORCE = 0, /* bead force kappa*D_i spread to the fluid (reading 1); the default      */
+  MC_COUPLING_MDF = 1    /* bead velocity imposed by iterated direct forcing (reading 26)          */
+};
+
 typedef struct {
   int32_t kind;         /* MC_FIELD_*                                                     */
   float sigma;          /* Gaussian filter width in cells (bead-density fields), > 0       */
@@ -71,6 +81,10 @@ typedef struct {
   int32_t n_fields;  /* 0..4                                                               */
   mc_field_params fields[4];
   int64_t max_beads; /* capacity; mc_load_filaments may load up to this many beads         */
+  int32_t coupling;  /* MC_COUPLING_*; with MDF k_el is not used                           */
+  int32_t mdf_iters; /* MDF: forcing iterations per step, 1..16 (ignored for FORCE).  The
+                        iteration contracts while the bead density interpolated at every bead
+                        stays below 4 (chains ~1 node apart, a few overlapping)            */
 } mc_world_params;
 
 /* Bytes of DEVICE workspace mc_create needs for these parameters (0 if they are invalid). */
@@ -120,7 +134,8 @@ int mc_step(mc_world* w, int32_t n);
  *                       (the library stores populations shifted; un-shifting in fp32 would
  *                       throw their low bits away)
  *   field [n_fields][ny][nx]  last step's filtered bead density, or the static field c
- *   force [N][2]        last step's total bead force F_i (lattice units)
+ *   force [N][2]        last step's total bead force F_i (lattice units; MDF: the summed
+ *                       direct-forcing increments)
  *   sense [N]           last step's sum over static fields of c interpolated at the bead
  * Returns MC_EDIVERGED (after filling the outputs) if the divergence flag is set. */
 int mc_read_state(mc_world* w, int64_t* step_out /*HOST*/, float* xy, float* u, float* rho,
@@ -146,8 +161,9 @@ int mc_texture_gathers(mc_world* w, int32_t on);
 
 /* Optional per-kernel timing with CUDA events on the world's stream (used by bench.py for the
  * roofline line; off by default, costs one event record per kernel group when on).
- * Slots: 0 K0 bin, 1 K2a deposit, 2 K3a filter+gradient, 3 K1 filament force, 4 K2b spread (empty:
- * S5 is fused into the fluid kernel and is timed in slot 5),
+ * Slots: 0 K0 bin, 1 K2a deposit, 2 K3a filter+gradient, 3 K1 filament force, 4 K2b spread (FORCE
+ * coupling: empty, S5 is fused into the fluid kernel and is timed in slot 5; MDF coupling: the
+ * moments, forcing and broadcast kernels K5a-c),
  * 5 K3b fluid, 6 K4 interpolate+integrate.  mc_profile_enable(w,1) starts a capture of up to
  * 64 steps; mc_profile_read synchronises, writes the summed milliseconds per slot to
  * ms (HOST float[MC_PROF_SLOTS]) and the number of captured steps, and restarts the capture. */

@@ -33,7 +33,7 @@ class WorldParams(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("dt", C.c_float), ("nu", C.c_float),
                 ("trt_lambda", C.c_float), ("rho0", C.c_float), ("k_el", C.c_float),
                 ("pbd_iters", C.c_int32), ("n_fields", C.c_int32), ("fields", FieldParams * 4),
-                ("max_beads", C.c_int64)]
+                ("max_beads", C.c_int64), ("coupling", C.c_int32), ("mdf_iters", C.c_int32)]
 
 
 class McError(RuntimeError):
@@ -96,6 +96,8 @@ def make_params(p: dict):
         setattr(wp, k, float(p[k]))
     wp.n_fields = len(p["fields"])
     wp.max_beads = int(p["max_beads"])
+    wp.coupling = int(p.get("coupling", 0))
+    wp.mdf_iters = int(p.get("mdf_iters", 0))
     for i, fd in enumerate(p["fields"][:4]):
         fp = wp.fields[i]
         fp.kind, fp.sigma = int(fd["kind"]), float(fd["sigma"])

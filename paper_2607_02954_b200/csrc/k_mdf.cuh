@@ -1,0 +1,134 @@
+// k_mdf.cuh -- K5: Multi-Direct Forcing coupling (MC_COUPLING_MDF).
+// P:L125 "the filaments' nodes sample the local fluid velocity ... the agent broadcasts its own
+// velocity back onto the grid"; "Multi-Direct Forcing (MDF) (Wang et al., 2008)".
+// Reading 26: the bead's own velocity is V_i = D_i + field displacement (K1 with
+// kappa = 1).  With u*(g) = sum_q c_q f_q / rho the force-free velocity of this step's
+// populations, u^0 = u*, F = 0, iteration k = 0..K-1:
+//   U_i  = sum_g u^k(g) delta_h(g - X_i)                  (sample,    K5b)
+//   dF_i = rho0 (V_i - U_i),  F_i += dF_i                 (force,     K5b)
+//   u^{k+1}(g) = u^k(g) + [sum_i dF_i delta_h(g - X_i)] / (2 rho(g))   (broadcast, K5c; Guo's
+//                                                          velocity u = u* + G/(2 rho), reading 11)
+// The summed F then goes through the fused spread + fluid kernel (k_lbm.cuh) unchanged: spreading
+// is linear, so its G = sum_k dG^k and its stored u equals u^K; the last iteration needs no
+// broadcast of its own.
+//
+// HBM traffic on top of the FORCE-coupled step: K5a 36 + 12 B/node; per iteration 24 B/bead
+// (X, V/F, dF) + the u gather; per broadcast 20 B/node of the tiles that hold beads + 16 B/bead.
+#pragma once
+#include "k_p2g.cuh"
+#include "mc_common.cuh"
+
+namespace mc {
+
+// K5a: rho and u* of the current (pre-collision, pull-streamed) populations.  u in the blocked
+// float2 layout K5b/K4 gather from; hrinv = 1/(2 rho), row-major.  Two nodes (i, i+1), i even,
+// per thread: 8-byte loads of the unshifted planes and one 16-byte u store.
+__global__ void __launch_bounds__(256) k_lbm_moments(const float* __restrict__ src, int nx, int ny, float rho0,
+                                                     float2* __restrict__ u, float* __restrict__ hrinv) {
+  const int i = (blockIdx.x * blockDim.x + threadIdx.x) << 1;
+  const int j = blockIdx.y;
+  if (i >= nx) return;
+  const size_t nc = (size_t)nx * ny;
+  const int im = (i == 0) ? nx - 1 : i - 1, ip2 = (i + 2 == nx) ? 0 : i + 2;
+  const int jm = (j == 0) ? ny - 1 : j - 1, jp = (j == ny - 1) ? 0 : j + 1;
+  const size_t r0 = (size_t)j * nx, rm = (size_t)jm * nx, rp = (size_t)jp * nx;
+  float gA[9], gB[9];  // g_q(x) = src_q(x - c_q)
+  const float2 v0 = __ldg(reinterpret_cast<const float2*>(src + 0 * nc + r0 + i));
+  const float2 v2 = __ldg(reinterpret_cast<const float2*>(src + 2 * nc + rm + i));
+  const float2 v4 = __ldg(reinterpret_cast<const float2*>(src + 4 * nc + rp + i));
+  gA[0] = v0.x; gB[0] = v0.y; gA[2] = v2.x; gB[2] = v2.y; gA[4] = v4.x; gB[4] = v4.y;
+  gA[1] = __ldg(src + 1 * nc + r0 + im);     gB[1] = __ldg(src + 1 * nc + r0 + i);
+  gA[3] = __ldg(src + 3 * nc + r0 + i + 1);  gB[3] = __ldg(src + 3 * nc + r0 + ip2);
+  gA[5] = __ldg(src + 5 * nc + rm + im);     gB[5] = __ldg(src + 5 * nc + rm + i);
+  gA[6] = __ldg(src + 6 * nc + rm + i + 1);  gB[6] = __ldg(src + 6 * nc + rm + ip2);
+  gA[7] = __ldg(src + 7 * nc + rp + i + 1);  gB[7] = __ldg(src + 7 * nc + rp + ip2);
+  gA[8] = __ldg(src + 8 * nc + rp + im);     gB[8] = __ldg(src + 8 * nc + rp + i);
+  float4 uo;
+  float2 hr;
+  {
+    const float* g = gA;  // same summation order as trt_collide (k_lbm.cuh)
+    const float drho = g[0] + ((g[1] + g[3]) + (g[2] + g[4])) + ((g[5] + g[7]) + (g[6] + g[8]));
+    const float mx = (g[1] - g[3]) + ((g[5] - g[7]) + (g[8] - g[6]));
+    const float my = (g[2] - g[4]) + ((g[5] - g[7]) + (g[6] - g[8]));
+    const float inv = 1.0f / (rho0 + drho);
+    uo.x = mx * inv; uo.y = my * inv; hr.x = 0.5f * inv;
+  }
+  {
+    const float* g = gB;
+    const float drho = g[0] + ((g[1] + g[3]) + (g[2] + g[4])) + ((g[5] + g[7]) + (g[6] + g[8]));
+    const float mx = (g[1] - g[3]) + ((g[5] - g[7]) + (g[8] - g[6]));
+    const float my = (g[2] - g[4]) + ((g[5] - g[7]) + (g[6] - g[8]));
+    const float inv = 1.0f / (rho0 + drho);
+    uo.z = mx * inv; uo.w = my * inv; hr.y = 0.5f * inv;
+  }
+  *reinterpret_cast<float4*>(u + blk_index(i, j, nx)) = uo;  // nodes i, i+1 are neighbours in a 4x4 block
+  *reinterpret_cast<float2*>(hrinv + r0 + i) = hr;
+}
+
+// K5b: sample the current grid velocity at the bead, add the direct-forcing increment.
+template <bool FIRST, int TEXROWS>
+__global__ void __launch_bounds__(256) k_mdf_force(int N, const float2* __restrict__ X, const float2* __restrict__ V,
+                                                   const float2* __restrict__ u, cudaTextureObject_t tex_u, int nx,
+                                                   int ny, float rho0, float2* __restrict__ dF,
+                                                   float2* __restrict__ F) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= N) return;
+  const float2 p = X[b];
+  const float2 U = TEXROWS ? interp2_tex<TEXROWS, false>(u, tex_u, nx, ny, p.x, p.y) : interp2(u, nx, ny, p.x, p.y);
+  const float2 v = V[b];
+  const float2 d = make_float2(rho0 * (v.x - U.x), rho0 * (v.y - U.y));
+  dF[b] = d;
+  if (FIRST) {
+    F[b] = d;
+  } else {
+    const float2 f = F[b];
+    F[b] = make_float2(f.x + d.x, f.y + d.y);
+  }
+}
+
+// K5c: broadcast.  One CTA per 32x32 tile accumulates the spread of dF in shared memory (the
+// fixed-point tile accumulation of S5, k_p2g.cuh: order independent, bit-reproducible) and
+// corrects the velocity of the tile's nodes in place.  Tiles without listed beads return at once.
+__global__ void __launch_bounds__(256, 4) k_mdf_spread_tile(int nx, int ny, const int* __restrict__ tile_start,
+                                                            const int* __restrict__ list,
+                                                            const float2* __restrict__ X,
+                                                            const float2* __restrict__ dF,
+                                                            const float* __restrict__ tile_rho_max,
+                                                            const float* __restrict__ hrinv, float2* __restrict__ u) {
+  __shared__ __align__(16) int acc0[ACC_N], acc1[ACC_N], accl0[ACC_N], accl1[ACC_N];
+  __shared__ float red[32];
+  const int t = blockIdx.x, ntx = nx / TS;
+  const int s = tile_start[t], e = tile_start[t + 1];
+  if (s == e) return;  // nothing reaches this tile: u^{k+1} = u^k
+  const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
+  float2 xpre = make_float2(0.f, 0.f), fpre = make_float2(0.f, 0.f);
+  {
+    const int b = first_entry(s, e, list);
+    if (b >= 0) { xpre = __ldg(X + b); fpre = __ldg(dF + b); }
+  }
+  float linv;
+  // max |dF| by a pass over the list (tile_fmax = NULL): K1's per-tile bound is on V, not on dF
+  const float scale = spread_tile_accumulate(nx, ny, x0, y0, s, e, list, X, dF, tile_rho_max ? tile_rho_max[t] : 0.0f,
+                                             nullptr, t, acc0, acc1, accl0, accl1, red, linv, xpre, fpre);
+  __syncthreads();
+  const float inv = 1.0f / scale;
+  const int lx = (threadIdx.x & 15) << 1, ry = threadIdx.x >> 4;
+  const int i = x0 + lx;
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const int ly = ry + 16 * h, j = y0 + ly;
+    const int sa = acc_index(lx, ly);
+    const float GAx = tile_value(acc0, accl0, sa, linv) * inv, GAy = tile_value(acc1, accl1, sa, linv) * inv;
+    const float GBx = tile_value(acc0, accl0, sa + 1, linv) * inv, GBy = tile_value(acc1, accl1, sa + 1, linv) * inv;
+    const float2 hr = *reinterpret_cast<const float2*>(hrinv + (size_t)j * nx + i);
+    float4* up = reinterpret_cast<float4*>(u + blk_index(i, j, nx));
+    float4 v = *up;
+    v.x = fmaf(GAx, hr.x, v.x);
+    v.y = fmaf(GAy, hr.x, v.y);
+    v.z = fmaf(GBx, hr.y, v.z);
+    v.w = fmaf(GBy, hr.y, v.w);
+    *up = v;
+  }
+}
+
+}  // namespace mc

@@ -16,6 +16,7 @@
 #include "k_filament.cuh"
 #include "k_g2p.cuh"
 #include "k_lbm.cuh"
+#include "k_mdf.cuh"
 #include "k_p2g.cuh"
 #include "k_tile.cuh"
 
@@ -29,6 +30,7 @@ inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 struct Layout {
   size_t fA, fB, u, rho_b, A, G, cfield, csum, As, tile_count, tile_start, bucket_count, bucket_cursor, tile_rho_max, tile_fmax;
   size_t X, PA, PB, PC, PD, F, sense, list, src, bflags, scratch, flags, sources;
+  size_t V, dF, hrinv;  // MDF coupling only
   size_t total;
 };
 
@@ -46,6 +48,8 @@ bool validate(const mc_world_params* p, Derived* d, std::string* why) {
   if (p->pbd_iters != 1) { *why = "pbd_iters must be 1"; return false; }
   if (p->n_fields < 0 || p->n_fields > 4) { *why = "n_fields must be 0..4"; return false; }
   if (p->max_beads < 0 || p->max_beads > (int64_t)1 << 30) { *why = "max_beads out of range"; return false; }
+  if (p->coupling != MC_COUPLING_FORCE && p->coupling != MC_COUPLING_MDF) { *why = "unknown coupling"; return false; }
+  if (p->coupling == MC_COUPLING_MDF && (p->mdf_iters < 1 || p->mdf_iters > 16)) { *why = "mdf_iters must be 1..16"; return false; }
   for (int k = 0; k < p->n_fields; ++k) {
     const mc_field_params& f = p->fields[k];
     if (f.kind == MC_FIELD_BEAD_DENSITY) {
@@ -103,6 +107,10 @@ Layout make_layout(const mc_world_params* p, const Derived& d) {
   L.scratch = take((N / 3 + 2) * 8);  // load-time: chain offsets and sort keys
   L.flags = take(64 * 4);
   L.sources = take(d.n_src_floats * f4);
+  const bool mdf = p->coupling == MC_COUPLING_MDF;
+  L.V = take(mdf ? N * 8 : 0);
+  L.dF = take(mdf ? N * 8 : 0);
+  L.hrinv = take(mdf ? nc * f4 : 0);
   L.total = off;
   return L;
 }
@@ -226,6 +234,7 @@ int enqueue_step(mc_world* w) {
   const int bt = 256;
   const int bgrid = (N + bt - 1) / bt;
   const bool beads = N > 0;
+  const bool mdf = w->p.coupling == MC_COUPLING_MDF;
 
   prof_mark(w, 0);
   if (beads) {
@@ -272,7 +281,7 @@ int enqueue_step(mc_world* w) {
     fa.PC = w->ptr<float4>(w->L.PC);
     fa.PD = w->ptr<float2>(w->L.PD);
     fa.uni = reinterpret_cast<const float4*>(w->ptr<int>(w->L.flags) + 24);  // flags[24..31]
-    fa.F = F;
+    fa.F = mdf ? w->ptr<float2>(w->L.V) : F;  // MDF: K1's sum with kappa = 1 is the bead velocity V_i
     fa.sense = w->ptr<float>(w->L.sense);
     fa.A = w->d.n_density ? w->ptr<float2>(w->L.A) : (w->d.n_static ? w->ptr<float2>(w->L.As) : nullptr);
     fa.csum = w->d.n_static ? w->ptr<float>(w->L.csum) : nullptr;
@@ -282,7 +291,7 @@ int enqueue_step(mc_world* w) {
     fa.ny = ny;
     fa.stride = w->stride;
     fa.n_windows = w->n_windows;
-    fa.kappa = w->kappa;
+    fa.kappa = mdf ? 1.0f : w->kappa;
     fa.step = w->ptr<long long>(w->L.flags) + 4;  // flags[8..9]: device copy of the step counter
     fa.tex_A = w->tex_on ? w->tex_A : 0;
     const int k1grid = (w->n_windows + 7) / 8;
@@ -298,6 +307,35 @@ int enqueue_step(mc_world* w) {
     }
     prof_mark(w, 4);
     w->launches++;
+    if (mdf) {
+      // K5 (k_mdf.cuh): u <- u* of the current populations, then mdf_iters x (sample + force),
+      // each but the last followed by a broadcast that corrects u on the tiles holding beads.
+      // The last increment reaches the fluid through the fused kernel below, which spreads the
+      // summed F (spreading is linear) and stores u^K.
+      float2* ug = w->ptr<float2>(w->L.u);
+      float* hrinv = w->ptr<float>(w->L.hrinv);
+      const float2* V = w->ptr<float2>(w->L.V);
+      float2* dF = w->ptr<float2>(w->L.dF);
+      const int mbx = pick_bx(nx) / 2;
+      mc::k_lbm_moments<<<dim3(nx / (2 * mbx), ny), mbx, 0, st>>>(w->fbuf(w->cur), nx, ny, w->rho0, ug, hrinv);
+      w->launches++;
+      const bool tex = w->tex_on && w->tex_u;
+      for (int k = 0; k < w->p.mdf_iters; ++k) {
+        if (k == 0) {
+          if (tex) mc::k_mdf_force<true, 1><<<bgrid, bt, 0, st>>>(N, X, V, ug, w->tex_u, nx, ny, w->rho0, dF, F);
+          else mc::k_mdf_force<true, 0><<<bgrid, bt, 0, st>>>(N, X, V, ug, w->tex_u, nx, ny, w->rho0, dF, F);
+        } else {
+          if (tex) mc::k_mdf_force<false, 1><<<bgrid, bt, 0, st>>>(N, X, V, ug, w->tex_u, nx, ny, w->rho0, dF, F);
+          else mc::k_mdf_force<false, 0><<<bgrid, bt, 0, st>>>(N, X, V, ug, w->tex_u, nx, ny, w->rho0, dF, F);
+        }
+        w->launches++;
+        if (k + 1 < w->p.mdf_iters) {
+          mc::k_mdf_spread_tile<<<n_tiles, 256, 0, st>>>(nx, ny, tile_start, list, X, dF,
+                                                         w->d.n_density ? tile_rho_max : nullptr, hrinv, ug);
+          w->launches++;
+        }
+      }
+    }
   } else {
     for (int b = 1; b <= 4; ++b) prof_mark(w, b);
   }
@@ -338,7 +376,7 @@ int enqueue_step(mc_world* w) {
     ls.X = X;
     ls.F = F;
     ls.tile_rho_max = w->d.n_density ? tile_rho_max : nullptr;
-    ls.tile_fmax = tile_fmax;
+    ls.tile_fmax = mdf ? nullptr : tile_fmax;  // MDF: K1's per-tile bound is on V, not on the summed F
     if (w->keep_G) mc::k_lbm_spread_tile<true><<<n_tiles, 256, 0, st>>>(ls);
     else mc::k_lbm_spread_tile<false><<<n_tiles, 256, 0, st>>>(ls);
   } else {

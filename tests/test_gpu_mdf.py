@@ -1,0 +1,121 @@
+"""GPU parity of the Multi-Direct Forcing coupling (MC_COUPLING_MDF; SURVEY.md 8(f) NEXT-1,
+DESIGN.md reading 26) against the oracle, through the C ABI.  Same protocol and bars as
+tests/test_gpu_parity.py: per step 1e-5 relative L2 on every output, 1e-3 on the positions after
+100 free-running steps, bit-exact run to run.
+"""
+import numpy as np
+import pytest
+
+from paper_2607_02954_b200 import worlds
+from test_gpu_parity import TOL_STEP, TOL_TRAJ, assert_close, rel_l2, run_protocol
+
+pytestmark = pytest.mark.gpu
+
+
+def mdf(w, iters=3):
+    w["params"]["coupling"] = 1
+    w["params"]["mdf_iters"] = iters
+    return w
+
+
+MDF = {
+    # ragged chains (3 .. 100 beads), several tiles, chains across the periodic seam
+    "ragged_96x64": lambda: mdf(worlds.ragged_world(96, 64, [3, 4, 5, 16, 31, 32, 33, 59, 60, 61, 64, 65, 100],
+                                                    seed=3)),
+    # both field kinds: V carries the repulsion and the chemotaxis displacement
+    "static_64x96": lambda: mdf(worlds.ragged_world(64, 96, [8, 16, 32, 64, 7, 45], seed=4, static_source=True), 2),
+    # no fields: tile bounds without rho_b (the fallback scale of the broadcast)
+    "no_fields": lambda: mdf(worlds.ragged_world(64, 32, [10, 20, 40], seed=6, kappa_rep=None), 4),
+    # one iteration: no broadcast kernel at all, only the fused spread
+    "one_iter": lambda: mdf(worlds.ragged_world(64, 64, [12, 30, 50], seed=17), 1),
+    # one tile in each direction: every support wraps onto the same tile
+    "single_tile_32": lambda: mdf(worlds.ragged_world(32, 32, [5, 12, 20], seed=11), 3),
+    # uniform 64-bead chains (configs 2 and 4), many empty tiles
+    "uniform_m64": lambda: mdf(worlds.random_world(256, 160, 40, 64, seed=8), 3),
+    # the most iterations the ABI takes
+    "iters_16": lambda: mdf(worlds.random_world(96, 128, 30, 32, seed=9), 16),
+}
+
+
+@pytest.mark.parametrize("name", sorted(MDF))
+def test_mdf_per_step_parity(name):
+    w = MDF[name]()
+    worst = run_protocol(w, steps_at=[0, 1, 10, 40])
+    print(name, {k: f"{v:.2e}" for k, v in worst.items()})
+
+
+def test_mdf_config1_trajectory():
+    from oracle import mco
+    from paper_2607_02954_b200 import binding
+    w = mdf(worlds.make_world("1"))
+    worst = run_protocol(w, steps_at=[0, 1, 10, 99])
+    print("config1 mdf", {k: f"{v:.2e}" for k, v in worst.items()})
+    G, O = binding.World(w), mco.World(w)
+    G.step(100)
+    O.step(100)
+    g, o = G.read_state(), O.read_state()
+    assert_close("X after 100 steps", g["xy"], o["xy"], TOL_TRAJ)
+    d = rel_l2(g["xy"].astype(np.float64) - w["xy"], o["xy"] - w["xy"])[0]
+    print(f"config1 mdf 100-step displacement rel L2 {d:.2e}")
+    assert d < 5e-2
+    assert np.abs(o["u"]).max() < 0.1
+
+
+def test_mdf_config2_per_step_and_trajectory():
+    from oracle import mco
+    from paper_2607_02954_b200 import binding
+    w = mdf(worlds.make_world("2"))
+    worst = run_protocol(w, steps_at=[0, 5, 60], threads=8)
+    print("config2 mdf", {k: f"{v:.2e}" for k, v in worst.items()})
+    G, O = binding.World(w), mco.World(w, threads=8)
+    G.step(100)
+    O.step(100)
+    g, o = G.read_state(), O.read_state()
+    assert_close("X after 100 steps", g["xy"], o["xy"], TOL_TRAJ)
+    assert np.abs(o["u"]).max() < 0.1 and np.abs(o["rho"] - 1).max() < 0.1
+
+
+def test_mdf_bitwise_reproducible_and_batching():
+    from paper_2607_02954_b200 import binding
+    outs = []
+    for split in ((23,), (23,), (3, 20), (1,) * 23):
+        G = binding.World(MDF["uniform_m64"]())
+        for n in split:
+            G.step(n)
+        outs.append(G.read_state(keys=("xy", "u", "fdev", "force")))
+        G.close()
+    for o in outs[1:]:
+        for k in ("xy", "u", "fdev", "force"):
+            assert outs[0][k].tobytes() == o[k].tobytes(), k
+
+
+def test_mdf_reduces_the_slip():
+    # what the iterations are for: the bead velocity U = dX approaches V = D as mdf_iters grows
+    from oracle import mco
+    from paper_2607_02954_b200 import binding
+    errs = []
+    for K in (1, 2, 4, 8):
+        w = mdf(worlds.random_world(96, 64, 10, 32, seed=21, kappa_rep=None), K)
+        G = binding.World(w)
+        G.step(6)
+        s0 = G.read_state(keys=("xy",))
+        G.step(1)
+        s1 = G.read_state(keys=("xy",))
+        D = mco.elastic(w["offsets"], s0["xy"].astype(np.float64), w["L_rest"], w["theta_rest"], w["k_bend"],
+                        w["k_shear"], w["k_stretch"], w["act_amp"], w["act_phase"], w["act_period"],
+                        float(np.float32(w["params"]["dt"])), 6)
+        errs.append(np.abs((s1["xy"].astype(np.float64) - s0["xy"]) - D).max() / np.abs(D).max())
+        G.close()
+    print("slip vs iterations", errs)
+    assert all(b < a for a, b in zip(errs, errs[1:])), errs
+
+
+def test_mdf_parameters_are_validated():
+    from paper_2607_02954_b200 import binding
+    for it in (0, 17):
+        with pytest.raises(binding.McError):
+            binding.World(mdf(worlds.random_world(64, 64, 4, 8, seed=2), it))
+    w = worlds.random_world(64, 64, 4, 8, seed=2)
+    w["params"]["coupling"] = 7
+    with pytest.raises(binding.McError):
+        binding.World(w)

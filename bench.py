@@ -2,6 +2,7 @@
 """bench.py -- throughput of the whole hot path (mc_step) on synthetic Microcosmos worlds.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 4d] [--impl ours|reference]
+                    [--coupling force|mdf] [--mdf-iters 3]
 
 A "step" is one pass of the whole hot path S0..S7 (all kernels K0..K4) over one seeded
 synthetic world.  Default workload: BASELINE.json config 4's largest world "4d" (10,000,000
@@ -20,6 +21,10 @@ north_star's >= 60 % HBM-roofline bar is stated on.  Prints ONE JSON line (rank 
                sample: the same recipe at 1/100 size (world "4b": 100,032 beads, 640^2 grid)
   --impl reference   times the oracle alone on that sample (there is no reference implementation
                of the paper in this repository: the oracle is the reference arm)
+
+--coupling mdf times the same world under the Multi-Direct Forcing coupling (SURVEY.md 8(f)
+NEXT-1): the K5 kernels appear in slot K2b_spread and the byte model grows by
+mdf_extra_bytes().  The default (force) is the configuration BASELINE.json's metric is quoted on.
 
 Multi-GPU (--gpus N under torchrun): the path does not shard (replicas
 only) -- every rank steps its own independent world (seed = rank); no data-path collective.
@@ -132,8 +137,20 @@ def ncu_traffic(slot: str, workload: str):
         return None
 
 
-def step_bytes(n_cells: int, n_beads: int) -> int:
-    return 112 * n_cells + 64 * n_beads  # SURVEY.md 8(d) / DESIGN.md
+def mdf_extra_bytes(n_cells: int, n_beads: int, iters: int) -> int:
+    """Algorithmic bytes the MDF coupling adds to a step: moments 36 B read +
+    12 B written per node; per iteration X, V read, dF, F written (32 B/bead), F re-read after the
+    first; per broadcast (iters - 1 of them) u read + written, 1/(2 rho) read (20 B/node), X, dF
+    read (16 B/bead)."""
+    if iters <= 0:
+        return 0
+    return (48 * n_cells + (32 * iters + 8 * (iters - 1)) * n_beads
+            + (iters - 1) * (20 * n_cells + 16 * n_beads))
+
+
+def step_bytes(n_cells: int, n_beads: int, mdf_iters: int = 0) -> int:
+    # SURVEY.md 8(d) / DESIGN.md: 112 B/node + 64 B/bead, plus the MDF kernels when they run
+    return 112 * n_cells + 64 * n_beads + mdf_extra_bytes(n_cells, n_beads, mdf_iters)
 
 
 def time_oracle(sample: str, seed: int, budget_s: float, min_steps: int, max_steps: int, warm: int = 1):
@@ -192,6 +209,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--coupling", default="force", choices=["force", "mdf"])
+    ap.add_argument("--mdf-iters", type=int, default=3)
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -222,6 +241,10 @@ def main():
 
     # replicas only: every rank owns an independent world of the same recipe (seed = rank)
     w = worlds.make_world(args.workload, seed=rank)
+    mdf_iters = args.mdf_iters if args.coupling == "mdf" else 0
+    if mdf_iters:
+        w["params"]["coupling"] = 1
+        w["params"]["mdf_iters"] = mdf_iters
     G = binding.World(w, device=str(dev))
     N, nc = G.N, G.nx * G.ny
     G.step(args.warmup)
@@ -252,6 +275,7 @@ def main():
     G.profile_enable(False)
     kms = {k: v / max(pn, 1) for k, v in prof.items()}
     kb = kernel_bytes(nc, N)
+    kb["K2b_spread"] = mdf_extra_bytes(nc, N, mdf_iters)  # slot 4 holds the K5 kernels under MDF
     peak, peak_src = measured_peak_gbs()
     dom = max(kms, key=lambda k: kms[k])
     ach = kb[dom] / (kms[dom] * 1e-3) / 1e9 if kms[dom] > 0 else 0.0
@@ -259,10 +283,10 @@ def main():
                 "frac": ach / peak, "traffic": ncu_traffic(dom, args.workload), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": kb[dom], "ms_per_launch": kms[dom],
                 "share_of_step": kms[dom] / max(sum(kms.values()), 1e-12)}
-    ach_step = step_bytes(nc, N) / (ms_step * 1e-3) / 1e9
+    ach_step = step_bytes(nc, N, mdf_iters) / (ms_step * 1e-3) / 1e9
     roofline_step = {"bound": "hbm", "achieved": ach_step, "peak": peak, "unit": "GB/s",
                      "frac": ach_step / peak, "frac_of_8TBps_nominal": ach_step / 8000.0,
-                     "algorithmic_bytes_per_step": step_bytes(nc, N)}
+                     "algorithmic_bytes_per_step": step_bytes(nc, N, mdf_iters)}
     kernels = {k: {"ms": round(kms[k], 5),
                    "GBps": round(kb[k] / (kms[k] * 1e-3) / 1e9, 1) if kms[k] > 0 else None}
                for k in kms}
@@ -313,8 +337,9 @@ def main():
             "vs_baseline": None, "dtype": "f32", "data": "synthetic (seeded, DESIGN.md input recipe)",
             "config": {"workload": f"BASELINE.json config {args.workload}", "beads": N,
                        "filaments": len(w["offsets"]) - 1, "grid": [p["nx"], p["ny"]],
+                       "coupling": args.coupling if not mdf_iters else f"mdf x{mdf_iters}",
                        "parallelism": "replicas only (one independent world per GPU)",
-                       "l2": f"working set {step_bytes(nc, N) / 1e6:.0f} MB per step vs 126 MB L2; no flush"},
+                       "l2": f"working set {step_bytes(nc, N, mdf_iters) / 1e6:.0f} MB per step vs 126 MB L2; no flush"},
             "cell_steps_per_s": world_size * nc * args.steps / (ms_total * 1e-3),
             "roofline": roofline, "roofline_step": roofline_step, "kernels": kernels,
             "cpu_baseline": cpu,

@@ -66,34 +66,49 @@ __global__ void __launch_bounds__(256) k_lbm_moments(const float* __restrict__ s
 }
 
 // K5b: sample the current grid velocity at the bead, add the direct-forcing increment.
-template <bool FIRST, int TEXROWS>
+// tile_fmax (zeroed once per step by the host's memset, one slot per iteration): bound for the
+// fixed-point scale of the spread that consumes this iteration's output, kept exactly like K1's
+// (k_filament.cuh): the warp's maximum is raised on every tile the warp's beads lie in.  It bounds
+// |dF| for the broadcast K5c, and |F| (LAST: the summed force) for the fused spread + fluid kernel.
+template <bool FIRST, bool LAST, int TEXROWS>
 __global__ void __launch_bounds__(256) k_mdf_force(int N, const float2* __restrict__ X, const float2* __restrict__ V,
                                                    const float2* __restrict__ u, cudaTextureObject_t tex_u, int nx,
                                                    int ny, float rho0, float2* __restrict__ dF,
-                                                   float2* __restrict__ F) {
+                                                   float2* __restrict__ F, unsigned* __restrict__ tile_fmax) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
-  if (b >= N) return;
-  const float2 p = X[b];
-  const float2 U = TEXROWS ? interp2_tex<TEXROWS, false>(u, tex_u, nx, ny, p.x, p.y) : interp2(u, nx, ny, p.x, p.y);
-  const float2 v = V[b];
-  const float2 d = make_float2(rho0 * (v.x - U.x), rho0 * (v.y - U.y));
-  dF[b] = d;
-  if (FIRST) {
-    F[b] = d;
-  } else {
-    const float2 f = F[b];
-    F[b] = make_float2(f.x + d.x, f.y + d.y);
+  const bool valid = b < N;  // every lane stays for the warp-wide reduction
+  const float2 p = X[valid ? b : N - 1];
+  float m = 0.0f;
+  if (valid) {
+    const float2 U = TEXROWS ? interp2_tex<TEXROWS, false>(u, tex_u, nx, ny, p.x, p.y) : interp2(u, nx, ny, p.x, p.y);
+    const float2 v = V[b];
+    const float2 d = make_float2(rho0 * (v.x - U.x), rho0 * (v.y - U.y));
+    float2 f = d;
+    if (!FIRST) {
+      const float2 f0 = F[b];
+      f = make_float2(f0.x + d.x, f0.y + d.y);
+    }
+    F[b] = f;
+    if (!LAST) dF[b] = d;  // the last increment reaches the fluid inside the summed F
+    m = LAST ? fmaxf(fabsf(f.x), fabsf(f.y)) : fmaxf(fabsf(d.x), fabsf(d.y));
   }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  const unsigned mb = __float_as_uint(m);  // positive floats order like their bit patterns
+  const int t = (wrapi((int)floorf(p.y), ny) >> 5) * (nx >> 5) + (wrapi((int)floorf(p.x), nx) >> 5);
+  const unsigned peers = __match_any_sync(0xffffffffu, t);
+  if ((int)(threadIdx.x & 31) == __ffs(peers) - 1 && mb > tile_fmax[t]) atomicMax(tile_fmax + t, mb);
 }
 
 // K5c: broadcast.  One CTA per 32x32 tile accumulates the spread of dF in shared memory (the
 // fixed-point tile accumulation of S5, k_p2g.cuh: order independent, bit-reproducible) and
 // corrects the velocity of the tile's nodes in place.  Tiles without listed beads return at once.
-__global__ void __launch_bounds__(256, 4) k_mdf_spread_tile(int nx, int ny, const int* __restrict__ tile_start,
+__global__ void __launch_bounds__(256, 5) k_mdf_spread_tile(int nx, int ny, const int* __restrict__ tile_start,
                                                             const int* __restrict__ list,
                                                             const float2* __restrict__ X,
                                                             const float2* __restrict__ dF,
                                                             const float* __restrict__ tile_rho_max,
+                                                            const unsigned* __restrict__ tile_fmax,
                                                             const float* __restrict__ hrinv, float2* __restrict__ u) {
   __shared__ __align__(16) int acc0[ACC_N], acc1[ACC_N], accl0[ACC_N], accl1[ACC_N];
   __shared__ float red[32];
@@ -101,33 +116,42 @@ __global__ void __launch_bounds__(256, 4) k_mdf_spread_tile(int nx, int ny, cons
   const int s = tile_start[t], e = tile_start[t + 1];
   if (s == e) return;  // nothing reaches this tile: u^{k+1} = u^k
   const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
+  // this thread's node pairs (i, i+1), i even, in rows ry and ry + 16: their u and 1/(2 rho) are
+  // requested now, so that the DRAM latency is spent under the atomic phase
+  const int lx = (threadIdx.x & 15) << 1, ry = threadIdx.x >> 4;
+  const int i = x0 + lx;
+  float4* up0 = reinterpret_cast<float4*>(u + blk_index(i, y0 + ry, nx));
+  float4* up1 = reinterpret_cast<float4*>(u + blk_index(i, y0 + ry + 16, nx));
+  float4 v0 = *up0, v1 = *up1;
+  const float2 h0 = __ldg(reinterpret_cast<const float2*>(hrinv + (size_t)(y0 + ry) * nx + i));
+  const float2 h1 = __ldg(reinterpret_cast<const float2*>(hrinv + (size_t)(y0 + ry + 16) * nx + i));
   float2 xpre = make_float2(0.f, 0.f), fpre = make_float2(0.f, 0.f);
   {
     const int b = first_entry(s, e, list);
     if (b >= 0) { xpre = __ldg(X + b); fpre = __ldg(dF + b); }
   }
   float linv;
-  // max |dF| by a pass over the list (tile_fmax = NULL): K1's per-tile bound is on V, not on dF
   const float scale = spread_tile_accumulate(nx, ny, x0, y0, s, e, list, X, dF, tile_rho_max ? tile_rho_max[t] : 0.0f,
-                                             nullptr, t, acc0, acc1, accl0, accl1, red, linv, xpre, fpre);
+                                             tile_fmax, t, acc0, acc1, accl0, accl1, red, linv, xpre, fpre);
   __syncthreads();
   const float inv = 1.0f / scale;
-  const int lx = (threadIdx.x & 15) << 1, ry = threadIdx.x >> 4;
-  const int i = x0 + lx;
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    const int ly = ry + 16 * h, j = y0 + ly;
-    const int sa = acc_index(lx, ly);
-    const float GAx = tile_value(acc0, accl0, sa, linv) * inv, GAy = tile_value(acc1, accl1, sa, linv) * inv;
-    const float GBx = tile_value(acc0, accl0, sa + 1, linv) * inv, GBy = tile_value(acc1, accl1, sa + 1, linv) * inv;
-    const float2 hr = *reinterpret_cast<const float2*>(hrinv + (size_t)j * nx + i);
-    float4* up = reinterpret_cast<float4*>(u + blk_index(i, j, nx));
-    float4 v = *up;
-    v.x = fmaf(GAx, hr.x, v.x);
-    v.y = fmaf(GAy, hr.x, v.y);
-    v.z = fmaf(GBx, hr.y, v.z);
-    v.w = fmaf(GBy, hr.y, v.w);
-    *up = v;
+  {
+    const int sa = acc_index(lx, ry);
+    const float ax = h0.x * inv, bx = h0.y * inv;
+    v0.x = fmaf(tile_value(acc0, accl0, sa, linv), ax, v0.x);
+    v0.y = fmaf(tile_value(acc1, accl1, sa, linv), ax, v0.y);
+    v0.z = fmaf(tile_value(acc0, accl0, sa + 1, linv), bx, v0.z);
+    v0.w = fmaf(tile_value(acc1, accl1, sa + 1, linv), bx, v0.w);
+    *up0 = v0;
+  }
+  {
+    const int sa = acc_index(lx, ry + 16);
+    const float ax = h1.x * inv, bx = h1.y * inv;
+    v1.x = fmaf(tile_value(acc0, accl0, sa, linv), ax, v1.x);
+    v1.y = fmaf(tile_value(acc1, accl1, sa, linv), ax, v1.y);
+    v1.z = fmaf(tile_value(acc0, accl0, sa + 1, linv), bx, v1.z);
+    v1.w = fmaf(tile_value(acc1, accl1, sa + 1, linv), bx, v1.w);
+    *up1 = v1;
   }
 }
 

@@ -30,7 +30,7 @@ inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 struct Layout {
   size_t fA, fB, u, rho_b, A, G, cfield, csum, As, tile_count, tile_start, bucket_count, bucket_cursor, tile_rho_max, tile_fmax;
   size_t X, PA, PB, PC, PD, F, sense, list, src, bflags, scratch, flags, sources;
-  size_t V, dF, hrinv;  // MDF coupling only
+  size_t V, dF, hrinv, mdf_fmax;  // MDF coupling only
   size_t total;
 };
 
@@ -111,6 +111,7 @@ Layout make_layout(const mc_world_params* p, const Derived& d) {
   L.V = take(mdf ? N * 8 : 0);
   L.dF = take(mdf ? N * 8 : 0);
   L.hrinv = take(mdf ? nc * f4 : 0);
+  L.mdf_fmax = take(mdf ? (size_t)p->mdf_iters * nt * 4 : 0);  // per iteration: per-tile bound on |dF| (last: |F|)
   L.total = off;
   return L;
 }
@@ -320,18 +321,30 @@ int enqueue_step(mc_world* w) {
       mc::k_lbm_moments<<<dim3(nx / (2 * mbx), ny), mbx, 0, st>>>(w->fbuf(w->cur), nx, ny, w->rho0, ug, hrinv);
       w->launches++;
       const bool tex = w->tex_on && w->tex_u;
-      for (int k = 0; k < w->p.mdf_iters; ++k) {
-        if (k == 0) {
-          if (tex) mc::k_mdf_force<true, 1><<<bgrid, bt, 0, st>>>(N, X, V, ug, w->tex_u, nx, ny, w->rho0, dF, F);
-          else mc::k_mdf_force<true, 0><<<bgrid, bt, 0, st>>>(N, X, V, ug, w->tex_u, nx, ny, w->rho0, dF, F);
+      const int K = w->p.mdf_iters;
+      unsigned* mfmax = w->ptr<unsigned>(w->L.mdf_fmax);  // [K][n_tiles], raised by K5b with atomicMax
+      cudaMemsetAsync(mfmax, 0, (size_t)K * n_tiles * 4, st);
+      for (int k = 0; k < K; ++k) {
+        unsigned* slot = mfmax + (size_t)k * n_tiles;
+        const bool first = k == 0, last = k + 1 == K;
+#define MC_MDF_FORCE(FI, LA, TX) \
+  mc::k_mdf_force<FI, LA, TX><<<bgrid, bt, 0, st>>>(N, X, V, ug, w->tex_u, nx, ny, w->rho0, dF, F, slot)
+        if (tex) {
+          if (first && last) MC_MDF_FORCE(true, true, 1);
+          else if (first) MC_MDF_FORCE(true, false, 1);
+          else if (last) MC_MDF_FORCE(false, true, 1);
+          else MC_MDF_FORCE(false, false, 1);
         } else {
-          if (tex) mc::k_mdf_force<false, 1><<<bgrid, bt, 0, st>>>(N, X, V, ug, w->tex_u, nx, ny, w->rho0, dF, F);
-          else mc::k_mdf_force<false, 0><<<bgrid, bt, 0, st>>>(N, X, V, ug, w->tex_u, nx, ny, w->rho0, dF, F);
+          if (first && last) MC_MDF_FORCE(true, true, 0);
+          else if (first) MC_MDF_FORCE(true, false, 0);
+          else if (last) MC_MDF_FORCE(false, true, 0);
+          else MC_MDF_FORCE(false, false, 0);
         }
+#undef MC_MDF_FORCE
         w->launches++;
-        if (k + 1 < w->p.mdf_iters) {
+        if (!last) {
           mc::k_mdf_spread_tile<<<n_tiles, 256, 0, st>>>(nx, ny, tile_start, list, X, dF,
-                                                         w->d.n_density ? tile_rho_max : nullptr, hrinv, ug);
+                                                         w->d.n_density ? tile_rho_max : nullptr, slot, hrinv, ug);
           w->launches++;
         }
       }
@@ -376,7 +389,8 @@ int enqueue_step(mc_world* w) {
     ls.X = X;
     ls.F = F;
     ls.tile_rho_max = w->d.n_density ? tile_rho_max : nullptr;
-    ls.tile_fmax = mdf ? nullptr : tile_fmax;  // MDF: K1's per-tile bound is on V, not on the summed F
+    // MDF: the bound on the summed F left by the last forcing iteration (K1's is on V)
+    ls.tile_fmax = mdf ? w->ptr<unsigned>(w->L.mdf_fmax) + (size_t)(w->p.mdf_iters - 1) * n_tiles : tile_fmax;
     if (w->keep_G) mc::k_lbm_spread_tile<true><<<n_tiles, 256, 0, st>>>(ls);
     else mc::k_lbm_spread_tile<false><<<n_tiles, 256, 0, st>>>(ls);
   } else {

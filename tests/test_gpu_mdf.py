@@ -119,3 +119,64 @@ def test_mdf_parameters_are_validated():
     w["params"]["coupling"] = 7
     with pytest.raises(binding.McError):
         binding.World(w)
+
+
+@pytest.mark.parametrize("name,steps_at", [("4b", [0, 20]), ("4c", [8])])
+def test_mdf_per_step_parity_config4(name, steps_at):
+    import os
+    w = mdf(worlds.make_world(name))
+    worst = run_protocol(w, steps_at=steps_at, threads=os.cpu_count() or 1)
+    print(name, "mdf", {k: f"{v:.2e}" for k, v in worst.items()})
+
+
+def test_mdf_config_4d_properties_and_sampled_parity():
+    # the size bench.py --coupling mdf times: properties that hold at any size, and outputs the
+    # oracle's components can reproduce on samples
+    from oracle import mco
+    from paper_2607_02954_b200 import binding
+    CX = np.array([0, 1, 0, -1, 0, 1, -1, -1, 1], dtype=np.float64)
+    CY = np.array([0, 0, 1, 0, -1, 1, 1, -1, -1], dtype=np.float64)
+    w = mdf(worlds.make_world("4d"))
+    G = binding.World(w)
+    G.keep_intermediates(True)
+    G.step(5)
+    s0 = G.read_state(keys=("xy", "fdev"))
+    G.step(1)
+    s1 = G.read_state(keys=("xy", "fdev", "u", "force", "rho"))
+    it = G.read_intermediates()
+    G.close()
+    # fluid mass conserved; momentum grows by sum(G) = sum of the summed bead forces
+    a0 = s0["fdev"].astype(np.float64).sum(axis=(1, 2))
+    a1 = s1["fdev"].astype(np.float64).sum(axis=(1, 2))
+    assert abs(a1.sum() - a0.sum()) < 1e-6 * np.abs(s1["fdev"]).astype(np.float64).sum()
+    for C, ch in ((CX, 0), (CY, 1)):
+        gsum = it["G"][ch].astype(np.float64).sum()
+        gabs = np.abs(it["G"][ch]).astype(np.float64).sum()
+        assert abs((C @ a1 - C @ a0) - gsum) < 1e-5 * gabs + 1e-9
+        assert abs(s1["force"][:, ch].astype(np.float64).sum() - gsum) < 1e-5 * gabs
+    assert np.abs(s1["u"]).max() < 0.1 and np.abs(s1["rho"] - 1.0).max() < 0.1
+    # sampled chains: the position update is the interpolation of the stored u
+    rng = np.random.default_rng(1)
+    chains = rng.choice(len(w["offsets"]) - 1, size=64, replace=False)
+    idx = np.concatenate([np.arange(w["offsets"][c], w["offsets"][c + 1]) for c in chains])
+    X0 = s0["xy"][idx].astype(np.float64)
+    assert_close("sampled X update", s1["xy"][idx], X0 + mco.interp(s1["u"].astype(np.float64), X0), TOL_STEP)
+    # sampled windows of the grid: G equals the oracle's spread of the GPU's summed bead forces
+    # (beads within reach of a 32x32 window, moved into a 64x64 periodic box around it)
+    nx = w["params"]["nx"]
+    X = s0["xy"].astype(np.float64)
+    for (x0, y0) in ((1000, 2000), (0, 0), (nx - 32, 3136)):
+        dx = (X[:, 0] - (x0 - 16)) % nx
+        dy = (X[:, 1] - (y0 - 16)) % nx
+        sel = (dx > 8) & (dx < 56) & (dy > 8) & (dy < 56)
+        loc = np.stack([dx[sel], dy[sel]], 1)
+        Gw = mco.spread(64, 64, loc, s1["force"][sel].astype(np.float64))[:, 16:48, 16:48]
+        ii = (np.arange(32) + x0) % nx
+        jj = (np.arange(32) + y0) % nx
+        assert_close(f"G window at {(x0, y0)}", it["G"][:, jj][:, :, ii], Gw, TOL_STEP)
+    # bit-for-bit reproducible at full size
+    H = binding.World(w)
+    H.step(6)
+    h = H.read_state(keys=("xy", "u"))
+    H.close()
+    assert h["xy"].tobytes() == s1["xy"].tobytes() and h["u"].tobytes() == s1["u"].tobytes()

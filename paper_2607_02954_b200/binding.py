@@ -17,7 +17,8 @@ LIB_PATH = os.path.join(_HERE, "libmc.so")
 MC_OK, MC_EINVAL, MC_ENOMEM, MC_ECUDA, MC_ESTATE, MC_EDIVERGED = 0, -1, -2, -3, -4, -5
 SYMBOLS = ("mc_workspace_bytes", "mc_create", "mc_load_filaments", "mc_step", "mc_read_state",
            "mc_read_intermediates", "mc_launch_count", "mc_destroy", "mc_last_error",
-           "mc_profile_enable", "mc_profile_read", "mc_keep_intermediates", "mc_texture_gathers")
+           "mc_profile_enable", "mc_profile_read", "mc_keep_intermediates", "mc_texture_gathers",
+           "mc_cluster_tiles")
 PROF_SLOTS = ("K0_bin", "K2a_deposit", "K3a_blur_grad", "K1_filament", "K2b_spread", "K3b_lbm",
               "K4_interp_integrate")
 
@@ -78,6 +79,8 @@ def load_library():
     L.mc_keep_intermediates.argtypes = [vp, i32]
     L.mc_texture_gathers.restype = C.c_int
     L.mc_texture_gathers.argtypes = [vp, i32]
+    L.mc_cluster_tiles.restype = C.c_int
+    L.mc_cluster_tiles.argtypes = [vp, i32]
     L.mc_destroy.restype = None
     L.mc_destroy.argtypes = [vp]
     L.mc_last_error.restype = C.c_char_p
@@ -210,6 +213,13 @@ class World:
         if rc < 0:
             self._check(rc)
         return rc == 1
+
+    def cluster_tiles(self, c: int = -1) -> int:
+        """mc_cluster_tiles: CTAs per tile of the P2G kernels (0, 2, 4, 8; -1 automatic) -> in use."""
+        rc = load_library().mc_cluster_tiles(self.h, int(c))
+        if rc < 0:
+            self._check(rc)
+        return rc
 
     def profile_enable(self, on: bool = True):
         self._check(load_library().mc_profile_enable(self.h, int(bool(on))))

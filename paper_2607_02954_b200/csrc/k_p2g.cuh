@@ -145,12 +145,20 @@ __device__ __forceinline__ int lo_bits(int n) {
 // rounds; in round v lane l takes sorted position l W + v, so every lane walks its own short run
 // of (nearly) one key and the 32 lanes of a round hold (nearly) 32 different keys.  Warp w takes
 // the rounds w, w + n_warps, ...
+// DealCfg: the warps that share one tile's list -- the CTA's own (default), or the warps of all the
+// CTAs of a thread-block cluster that splits a crowded tile (k_cluster.cuh).
+struct DealCfg {
+  int nw, v0;  // number of warps dealing the list, index of this thread's warp among them
+  __device__ __forceinline__ DealCfg() : nw(blockDim.x >> 5), v0(threadIdx.x >> 5) {}
+  __device__ __forceinline__ DealCfg(int nw_, int v0_) : nw(nw_), v0(v0_) {}
+};
+
 struct Deal {
   int W, n, nw, v, p;
-  __device__ __forceinline__ Deal(int n_) : n(n_) {
+  __device__ __forceinline__ Deal(int n_, DealCfg c = DealCfg()) : n(n_) {
     W = (n + 31) >> 5;
-    nw = blockDim.x >> 5;
-    v = threadIdx.x >> 5;
+    nw = c.nw;
+    v = c.v0;
     p = (threadIdx.x & 31) * W + v;
   }
   __device__ __forceinline__ bool valid() const { return v < W && p < n; }
@@ -161,9 +169,10 @@ struct Deal {
 template <bool WIDE, bool WRAP>
 __device__ __forceinline__ void deposit_loop(int nx, int ny, int x0, int y0, int s, int e,
                                              const int* __restrict__ list, const float2* __restrict__ X,
-                                             float scale, float lscale, int* acc, int* accl, float2 xpre) {
+                                             float scale, float lscale, int* acc, int* accl, float2 xpre,
+                                             DealCfg cfg = DealCfg()) {
   float2 xc = xpre;  // first entry preloaded by the caller, later ones one iteration ahead
-  for (Deal d(e - s); d.valid(); d.advance()) {
+  for (Deal d(e - s, cfg); d.valid(); d.advance()) {
     const float2 xb = xc;
     if (d.next_valid()) xc = __ldg(X + __ldg(list + s + d.p + d.nw));
     TileBead tb;
@@ -192,12 +201,12 @@ __device__ __forceinline__ void spread_loop(int nx, int ny, int x0, int y0, int 
                                             const int* __restrict__ list, const float2* __restrict__ X,
                                             const float2* __restrict__ F, float scale, float lscale,
                                             int* acc0, int* acc1, int* accl0, int* accl1,
-                                            float2 xpre, float2 fpre) {
+                                            float2 xpre, float2 fpre, DealCfg cfg = DealCfg()) {
   // the caller loaded this thread's FIRST entry (xpre, fpre) before the zeroing and the barrier,
   // so that the list -> X/F gather latency is spent under them; later entries are software-
   // pipelined one iteration ahead
   float2 xc = xpre, fc = fpre;
-  for (Deal d(e - s); d.valid(); d.advance()) {
+  for (Deal d(e - s, cfg); d.valid(); d.advance()) {
     const float2 xb = xc, f = fc;
     if (d.next_valid()) {
       const int bn = __ldg(list + s + d.p + d.nw);
@@ -235,6 +244,18 @@ __device__ __noinline__ void deposit_loop_wide(int nx, int ny, int x0, int y0, i
                                                const float2* X, float scale, float lscale, int* acc, int* accl,
                                                float2 xpre) {
   deposit_loop<true, true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl, xpre);
+}
+__device__ __noinline__ void deposit_loop_wide_cfg(int nx, int ny, int x0, int y0, int s, int e, const int* list,
+                                                   const float2* X, float scale, float lscale, int* acc, int* accl,
+                                                   float2 xpre, int nw, int v0) {
+  deposit_loop<true, true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl, xpre, DealCfg(nw, v0));
+}
+__device__ __noinline__ void spread_loop_wide_cfg(int nx, int ny, int x0, int y0, int s, int e, const int* list,
+                                                  const float2* X, const float2* F, float scale, float lscale,
+                                                  int* acc0, int* acc1, int* accl0, int* accl1, float2 xpre,
+                                                  float2 fpre, int nw, int v0) {
+  spread_loop<true, true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre,
+                          DealCfg(nw, v0));
 }
 __device__ __noinline__ void spread_loop_wide(int nx, int ny, int x0, int y0, int s, int e, const int* list,
                                               const float2* X, const float2* F, float scale, float lscale,
@@ -307,8 +328,8 @@ __device__ __forceinline__ float tile_value(const int* acc, const int* accl, int
 }
 
 // First list entry of this thread in the tile segment [s, e): bead index, or -1.
-__device__ __forceinline__ int first_entry(int s, int e, const int* __restrict__ list) {
-  const Deal d(e - s);
+__device__ __forceinline__ int first_entry(int s, int e, const int* __restrict__ list, DealCfg cfg = DealCfg()) {
+  const Deal d(e - s, cfg);
   return d.valid() ? __ldg(list + s + d.p) : -1;
 }
 
@@ -316,13 +337,15 @@ __device__ __forceinline__ int first_entry(int s, int e, const int* __restrict__
 // Used by the fused spread + fluid kernel (k_lbm.cuh), which must __syncthreads() before it
 // reads the accumulators.  (xpre, fpre): X and F of this thread's first entry, loaded by the
 // caller well ahead (their list -> X/F gather is the longest latency chain of the tile).
+template <bool CL = false>
 __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, int y0, int s, int e,
                                                         const int* __restrict__ list,
                                                         const float2* __restrict__ X,
                                                         const float2* __restrict__ F, float rho_max,
                                                         const unsigned* __restrict__ tile_fmax, int t,
                                                         int* acc0, int* acc1, int* accl0, int* accl1,
-                                                        float* red, float& linv, float2 xpre, float2 fpre) {
+                                                        float* red, float& linv, float2 xpre, float2 fpre,
+                                                        DealCfg cfg = DealCfg()) {
   const bool wide = (e - s) > WIDE_N;
   const float lscale = pow2f(lo_bits(e - s));
   linv = wide ? 1.0f / lscale : 0.0f;  // 0 => the readers skip the lo planes (not zeroed then)
@@ -355,6 +378,12 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
   }
   const float sum_w = (rho_max > 0.0f) ? 1.0625f * rho_max : fmaxf(0.25f * (float)(e - s), 1.0f);
   const float scale = pow2_scale(fmaxf(fm * sum_w, 1e-18f));
+  if (CL) {  // the list is shared with the other CTAs of a cluster (k_cluster.cuh)
+    if (wide) spread_loop_wide_cfg(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre, cfg.nw, cfg.v0);
+    else if (nx == TS || ny == TS) spread_loop<false, true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre, cfg);
+    else spread_loop<false, false>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre, cfg);
+    return scale;
+  }
   if (wide) spread_loop_wide(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre);
   else if (nx == TS || ny == TS) spread_loop<false, true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre);
   else spread_loop<false, false>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre);

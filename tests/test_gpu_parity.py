@@ -342,3 +342,39 @@ def test_list_rebuild_schedule_only_changes_rounding():
         prev = cur
     assert_close("X after 240 steps", a["xy"], prev, TOL_TRAJ)
     assert drift > 0.5, drift  # the drift bound (0.22) was used up at least twice in world A
+
+
+def _very_crowded():
+    # 2,500 chains of 16 beads within a few cells of the centre of a 96x64 grid: the central tiles
+    # list > 4096 beads (hi + lo accumulator words, and the cluster split of k_cluster.cuh)
+    return worlds.random_world(96, 64, 2500, 16, seed=23, kappa=0.25, kappa_rep=2e-5, clustered=4.0)
+
+
+def test_cluster_tiles_do_not_change_the_bits():
+    # crowded worlds give every tile a thread-block cluster whose CTAs share the tile's list and
+    # combine integer partial sums through distributed shared memory: same bits as one CTA per tile
+    from paper_2607_02954_b200 import binding
+    w = _very_crowded()
+    outs = []
+    for c in (0, 2, 4, 8, -1):
+        G = binding.World(w)
+        used = G.cluster_tiles(c)
+        assert used == (c if c >= 0 else 4), (c, used)   # automatic choice: 4 (largest list > 4096)
+        G.keep_intermediates(True)
+        G.step(7)
+        outs.append({**G.read_state(), **G.read_intermediates()})
+        G.close()
+    for o in outs[1:]:
+        for k in outs[0]:
+            if k != "step":
+                assert outs[0][k].tobytes() == o[k].tobytes(), k
+    # a world without crowded tiles stays on one CTA per tile
+    G = binding.World(SMALL["uniform_m32"]())
+    assert G.cluster_tiles(-1) == 0
+    G.close()
+
+
+def test_per_step_parity_very_crowded():
+    w = _very_crowded()
+    worst = run_protocol(w, steps_at=[0, 3])
+    print("very_crowded", {k: f"{v:.2e}" for k, v in worst.items()})

@@ -25,6 +25,8 @@
 // arrival order of the atomics and is NOT reproducible; that is harmless because the
 // accumulation that consumes the lists adds integers (fixed point), which is order-independent.
 #pragma once
+#include <cooperative_groups.h>
+
 #include "mc_common.cuh"
 
 namespace mc {
@@ -257,6 +259,32 @@ __global__ void __launch_bounds__(1024) k_list_build_small(ListState* __restrict
   __syncthreads();
   bucket_starts(n_tiles, tile_start, bucket_count, bucket_cursor);
   __syncthreads();
+  tile_bin<true>(X, N, nx, ny, nullptr, bucket_cursor, list);
+}
+
+// Medium worlds (up to a few hundred thousand beads: still bound by launch overhead on the steps
+// that keep their lists, too many beads for one CTA on the steps that rebuild them): the whole of
+// K0 in ONE launch of one thread-block CLUSTER of 8 x 1024 threads.  The phases are separated by
+// the hardware cluster barrier (release/acquire at cluster scope, which also orders the global
+// atomics and stores of the phases); the CTAs of a cluster are co-scheduled by construction, so
+// unlike a hand-made grid barrier this cannot deadlock.
+constexpr int K0_CLUSTER = 8;
+__global__ void __cluster_dims__(K0_CLUSTER, 1, 1) __launch_bounds__(1024)
+    k_list_build_cluster(ListState* __restrict__ st, const float2* __restrict__ X, int N, int nx, int ny, int n_tiles,
+                         int* __restrict__ tile_count, int* __restrict__ tile_start, int* __restrict__ bucket_count,
+                         int* __restrict__ bucket_cursor, int* __restrict__ list) {
+  namespace cg = cooperative_groups;
+  cg::cluster_group cl = cg::this_cluster();
+  __shared__ int sm[33];
+  if (blockIdx.x == 0 && threadIdx.x == 0) list_policy_commit(st);
+  cl.sync();
+  if (!*reinterpret_cast<volatile int*>(&st->need)) return;  // the same value in every CTA: all leave together
+  tile_bin<false>(X, N, nx, ny, tile_count, bucket_count, nullptr);
+  cl.sync();
+  if (blockIdx.x == 0) tile_scan(tile_count, n_tiles, tile_start, sm);
+  cl.sync();
+  bucket_starts(n_tiles, tile_start, bucket_count, bucket_cursor);
+  cl.sync();
   tile_bin<true>(X, N, nx, ny, nullptr, bucket_cursor, list);
 }
 

@@ -182,6 +182,8 @@ constexpr int PROF_MAX_STEPS = 64;
 constexpr int GRAPH_STEPS = 4;
 // worlds up to this size rebuild their tile lists in one single-CTA launch (launch bound anyway)
 constexpr int K0_SMALL_BEADS = 32768, K0_SMALL_TILES = 1024;
+// ... and up to this size in one launch of one 8-CTA cluster (k_tile.cuh)
+constexpr int K0_MEDIUM_BEADS = 262144, K0_MEDIUM_TILES = 8192;
 static_assert(GRAPH_STEPS % 2 == 0, "graph period");
 
 void drop_graphs(mc_world* w) {
@@ -250,6 +252,10 @@ int enqueue_step(mc_world* w) {
       // small world: one launch of one CTA instead of four (k_tile.cuh)
       mc::k_list_build_small<<<1, 1024, 0, st>>>(ls_state, X, N, nx, ny, n_tiles, tile_count, tile_start,
                                                  bucket_count, bucket_cursor, list);
+      w->launches += 1;
+    } else if (N <= K0_MEDIUM_BEADS && n_tiles <= K0_MEDIUM_TILES) {
+      mc::k_list_build_cluster<<<mc::K0_CLUSTER, 1024, 0, st>>>(ls_state, X, N, nx, ny, n_tiles, tile_count, tile_start,
+                                                                bucket_count, bucket_cursor, list);
       w->launches += 1;
     } else {
       const int k0grid = bgrid < w->n_sm * 8 ? bgrid : w->n_sm * 8;

@@ -180,3 +180,17 @@ def test_mdf_config_4d_properties_and_sampled_parity():
     h = H.read_state(keys=("xy", "u"))
     H.close()
     assert h["xy"].tobytes() == s1["xy"].tobytes() and h["u"].tobytes() == s1["u"].tobytes()
+
+
+def test_mdf_on_clustered_tiles_one_iteration():
+    # a crowded world (thread-block clusters per tile, hi + lo accumulator words) under MDF: the
+    # summed force reaches the cluster variant of the fused kernel with K5b's per-tile bound.  One
+    # forcing iteration only: with ~50 beads per cell the iteration itself amplifies (reading 26),
+    # which is a property of the method, not of the kernels.
+    from paper_2607_02954_b200 import binding
+    w = mdf(worlds.random_world(96, 64, 2500, 16, seed=23, kappa=0.25, kappa_rep=2e-5, clustered=4.0), 1)
+    G = binding.World(w)
+    assert G.cluster_tiles(-1) == 4
+    G.close()
+    worst = run_protocol(w, steps_at=[0, 1])
+    print("mdf clustered", {k: f"{v:.2e}" for k, v in worst.items()})

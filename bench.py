@@ -126,12 +126,15 @@ _SLOT_KERNEL = {"K2a_deposit": "k_deposit_tile", "K3a_blur_grad": "k_blur_grad",
                 "K3b_lbm": "k_lbm_spread_tile", "K4_interp_integrate": "k_interp_integrate"}
 
 
-def ncu_traffic(slot: str, workload: str):
+def ncu_traffic(slot: str, workload: str, mdf_iters: int = 0):
     try:
         with open(os.path.join(ROOT, "profiles", "r1_traffic.json")) as fh:
             d = json.load(fh)
         if d.get("world") != workload:
             return None
+        if slot == "K2b_spread":  # the K5 group of the MDF coupling: one figure for all its launches
+            m = d.get("mdf", {})
+            return m.get("K5_group_bytes_per_step") if m.get("mdf_iters") == mdf_iters else None
         return d["dram_bytes_per_launch"].get(_SLOT_KERNEL.get(slot, ""))
     except Exception:
         return None
@@ -281,7 +284,7 @@ def main():
     dom = max(kms, key=lambda k: kms[k])
     ach = kb[dom] / (kms[dom] * 1e-3) / 1e9 if kms[dom] > 0 else 0.0
     roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
-                "frac": ach / peak, "traffic": ncu_traffic(dom, args.workload), "peak_source": peak_src,
+                "frac": ach / peak, "traffic": ncu_traffic(dom, args.workload, mdf_iters), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": kb[dom], "ms_per_launch": kms[dom],
                 "share_of_step": kms[dom] / max(sum(kms.values()), 1e-12)}
     ach_step = step_bytes(nc, N, mdf_iters) / (ms_step * 1e-3) / 1e9

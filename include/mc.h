@@ -117,6 +117,11 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets /*HOST*
                       const float* act_amp /*DEVICE*/, const float* act_phase /*DEVICE*/,
                       const float* act_period /*DEVICE*/);
 
+/* Replace the bead positions of the loaded filaments and keep everything else (parameters, fluid,
+ * step counter).  xy: DEVICE float [N][2], chain-ordered like mc_load_filaments.  The next step
+ * rebuilds the tile lists.  Synchronises the stream.  Errors: MC_EINVAL, MC_ECUDA. */
+int mc_set_positions(mc_world* w, const float* xy /*DEVICE*/);
+
 /* Advance n >= 0 steps.  Asynchronous: kernels are enqueued on the world's stream and the
  * call returns without synchronising.  Blocks of four steps are replayed from a CUDA graph when
  * the stream can be captured (not the legacy default stream); the results are bit-identical to

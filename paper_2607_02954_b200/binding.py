@@ -18,7 +18,7 @@ MC_OK, MC_EINVAL, MC_ENOMEM, MC_ECUDA, MC_ESTATE, MC_EDIVERGED = 0, -1, -2, -3, 
 SYMBOLS = ("mc_workspace_bytes", "mc_create", "mc_load_filaments", "mc_step", "mc_read_state",
            "mc_read_intermediates", "mc_launch_count", "mc_destroy", "mc_last_error",
            "mc_profile_enable", "mc_profile_read", "mc_keep_intermediates", "mc_texture_gathers",
-           "mc_cluster_tiles")
+           "mc_cluster_tiles", "mc_set_positions")
 PROF_SLOTS = ("K0_bin", "K2a_deposit", "K3a_blur_grad", "K1_filament", "K2b_spread", "K3b_lbm",
               "K4_interp_integrate")
 
@@ -79,6 +79,8 @@ def load_library():
     L.mc_keep_intermediates.argtypes = [vp, i32]
     L.mc_texture_gathers.restype = C.c_int
     L.mc_texture_gathers.argtypes = [vp, i32]
+    L.mc_set_positions.restype = C.c_int
+    L.mc_set_positions.argtypes = [vp, vp]
     L.mc_cluster_tiles.restype = C.c_int
     L.mc_cluster_tiles.argtypes = [vp, i32]
     L.mc_destroy.restype = None
@@ -174,6 +176,17 @@ class World:
                 *[C.c_void_p(t.data_ptr()) for t in dev])
         self._check(rc)
         self.N = int(off[-1])
+
+    def set_positions(self, xy):
+        """mc_set_positions: xy [N,2] host numpy array or device tensor, caller's bead order."""
+        torch = self.torch
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):
+            if not isinstance(xy, torch.Tensor):
+                xy = torch.from_numpy(np.ascontiguousarray(xy, dtype=np.float32))
+            d = xy.to(self.device, dtype=torch.float32, non_blocking=False).contiguous()
+            assert d.numel() == 2 * self.N
+            rc = load_library().mc_set_positions(self.h, C.c_void_p(d.data_ptr()))
+        self._check(rc)
 
     def step(self, n: int = 1):
         self._check(load_library().mc_step(self.h, int(n)))

@@ -307,6 +307,11 @@ __global__ void k_unpermute2(int N, const int* __restrict__ src, const float2* _
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b < N) out[src[b]] = in[b];
 }
+// mc_set_positions: caller's order -> internal order
+__global__ void k_permute2(int N, const int* __restrict__ src, const float2* __restrict__ in, float2* __restrict__ out) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b < N) out[b] = in[src[b]];
+}
 __global__ void k_unpermute1(int N, const int* __restrict__ src, const float* __restrict__ in, float* __restrict__ out) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b < N) out[src[b]] = in[b];

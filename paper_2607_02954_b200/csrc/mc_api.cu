@@ -748,6 +748,27 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   return MC_OK;
 }
 
+int mc_set_positions(mc_world* w, const float* xy) {
+  if (!w) return MC_EINVAL;
+  if (w->N == 0) return MC_OK;
+  if (!xy) return fail(w, MC_EINVAL, "null array");
+  cudaStream_t st = w->stream;
+  mc::k_permute2<<<(w->N + 255) / 256, 256, 0, st>>>(w->N, w->ptr<int>(w->L.src), reinterpret_cast<const float2*>(xy),
+                                                     w->ptr<float2>(w->L.X));
+  w->launches++;
+  // the beads may be anywhere now: the next step rebuilds the tile lists (drift = +inf)
+  mc::ListState force;
+  force.need = 1;
+  force.drift = INFINITY;
+  force.step_max = 0u;
+  cudaMemcpyAsync(reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16), &force, sizeof(force),
+                  cudaMemcpyHostToDevice, st);
+  cudaError_t e = cudaStreamSynchronize(st);  // `force` is a host variable of this call; xy belongs to the caller
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_set_positions: ") + cudaGetErrorString(e));
+  return MC_OK;
+}
+
 int mc_step(mc_world* w, int32_t n) {
   if (!w) return MC_EINVAL;
   if (n < 0) return fail(w, MC_EINVAL, "n < 0");

@@ -378,3 +378,30 @@ def test_per_step_parity_very_crowded():
     w = _very_crowded()
     worst = run_protocol(w, steps_at=[0, 3])
     print("very_crowded", {k: f"{v:.2e}" for k, v in worst.items()})
+
+
+def test_set_positions_continues_the_run():
+    # mc_set_positions with the positions read back must continue like an uninterrupted run (to
+    # rounding: the lists are rebuilt, and their lengths set the fixed-point scales), and new
+    # positions must give what a fresh load of them gives, bit for bit
+    from paper_2607_02954_b200 import binding
+    w = SMALL["uniform_m32"]()
+    A, B = binding.World(w), binding.World(w)
+    A.step(8)
+    B.step(4)
+    B.set_positions(B.read_state(keys=("xy",))["xy"])
+    B.step(4)
+    a, b = A.read_state(keys=("xy", "force")), B.read_state(keys=("xy", "force"))
+    assert a["step"] == b["step"] == 8
+    assert rel_l2(a["xy"], b["xy"])[0] < 1e-6 and rel_l2(a["force"], b["force"])[0] < 1e-5
+    shifted = (w["xy"] + np.float32(0.37)).astype(np.float32)
+    C1 = binding.World(w)
+    C1.set_positions(shifted)
+    C1.step(3)
+    w2 = dict(w)
+    w2["xy"] = shifted
+    C2 = binding.World(w2)
+    C2.step(3)
+    c1, c2 = C1.read_state(keys=("xy", "u", "force")), C2.read_state(keys=("xy", "u", "force"))
+    for k in ("xy", "u", "force"):
+        assert c1[k].tobytes() == c2[k].tobytes(), k

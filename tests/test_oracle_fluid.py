@@ -127,3 +127,93 @@ def test_shear_wave_decays_with_the_viscosity_tau_sets(nu_lat, tol):
     # shear decay is governed by omega+, not omega-: changing Lambda leaves the rate
     op2, om2 = mco.lattice_constants(nu_lat, 1.0, 3 / 16)
     assert op2 == op and om2 != om
+
+
+def _second_moment(f):
+    """Pi_ab = sum_q c_qa c_qb f_q per node -> (xx, xy, yy)."""
+    return (np.tensordot(CX * CX, f, 1), np.tensordot(CX * CY, f, 1), np.tensordot(CY * CY, f, 1))
+
+
+@pytest.mark.parametrize("tau_p,tau_m", [(0.8, 4 / 3), (0.56, 1.9), (1.7, 0.61)])
+def test_even_guo_source_second_moment_identity(tau_p, tau_m):
+    # Pin of the EVEN-parity Guo source S+_q = w_q[-3 u.G + 9 (c_q.u)(c_q.G)] and of its
+    # (1 - omega+/2) prefactor (SURVEY 8(c).1 S6; P:L117 D2Q9, P:L127 TRT).  S+ has no zeroth and
+    # no first moment, so the mass / momentum / uniform-force pins cannot see it; its second
+    # moment is fixed by the D2Q9 isotropy identities sum_q w_q c_a c_b = delta_ab / 3 and
+    # sum_q w_q c_a c_b c_c c_d = (d_ab d_cd + d_ac d_bd + d_ad d_bc) / 9:
+    #     sum_q c_a c_b S+_q = u_a G_b + u_b G_a.
+    # The odd parts (omega-, S-) carry no second moment, so for a spatially uniform state
+    # (streaming then leaves every node's moments alone) one step must give
+    #     Pi' = Pi - omega+ (Pi - Pi_eq) + (1 - omega+/2)(u_a G_b + u_b G_a),
+    # Pi_eq = rho (delta_ab / 3 + u_a u_b), u = (sum c f + G/2) / rho.
+    ny, nx = 6, 5
+    rng = np.random.default_rng(4242)
+    rho, ux0, uy0 = 1.07, 0.031, -0.046
+    f1 = feq(np.full((1, 1), rho), np.full((1, 1), ux0), np.full((1, 1), uy0))[:, 0, 0]
+    f1 = f1 + 2e-3 * rng.normal(size=9)                       # uniform non-equilibrium part
+    f = np.broadcast_to(f1[:, None, None], (9, ny, nx)).copy()
+    G = np.empty((2, ny, nx))
+    G[0], G[1] = 3.1e-3, -1.7e-3                              # both components non-zero
+    op, om = 1 / tau_p, 1 / tau_m
+    assert abs(op - om) > 0.1
+    f2, u = mco.lbm_step(f, G, op, om)
+    r = f.sum(axis=0)
+    ux = (np.tensordot(CX, f, 1) + 0.5 * G[0]) / r
+    uy = (np.tensordot(CY, f, 1) + 0.5 * G[1]) / r
+    assert np.allclose(u[0], ux, atol=1e-16) and np.allclose(u[1], uy, atol=1e-16)
+    pxx, pxy, pyy = _second_moment(f)
+    exx, exy, eyy = r * (1 / 3 + ux * ux), r * ux * uy, r * (1 / 3 + uy * uy)
+    c = 1 - 0.5 * op
+    want = (pxx - op * (pxx - exx) + c * 2 * ux * G[0],
+            pxy - op * (pxy - exy) + c * (ux * G[1] + uy * G[0]),
+            pyy - op * (pyy - eyy) + c * 2 * uy * G[1])
+    got = _second_moment(f2)
+    for g_, w_ in zip(got, want):
+        assert np.abs(g_ - w_).max() < 1e-14
+    # the source term is not lost in rounding: it is ~1e-4 of Pi here, far above the tolerance
+    assert abs(c * (ux * G[1] + uy * G[0])).min() > 1e-6
+
+
+def test_even_guo_source_grid_summed_second_moment():
+    # the same identity on a NON-uniform state: streaming permutes populations between nodes, so
+    # the grid sum of Pi after the step equals the grid sum of the post-collision Pi
+    ny, nx = 12, 16
+    rng = np.random.default_rng(99)
+    rho = 1 + 0.03 * rng.normal(size=(ny, nx))
+    f = feq(rho, 0.04 * rng.normal(size=(ny, nx)), 0.04 * rng.normal(size=(ny, nx)))
+    f += 1e-3 * rng.normal(size=f.shape)
+    G = 2e-3 * rng.normal(size=(2, ny, nx))
+    op, om = 1 / 0.93, 1 / 0.66
+    f2, u = mco.lbm_step(f, G, op, om)
+    r = f.sum(axis=0)
+    pxx, pxy, pyy = _second_moment(f)
+    c = 1 - 0.5 * op
+    want = ((pxx - op * (pxx - r * (1 / 3 + u[0] ** 2)) + c * 2 * u[0] * G[0]).sum(),
+            (pxy - op * (pxy - r * u[0] * u[1]) + c * (u[0] * G[1] + u[1] * G[0])).sum(),
+            (pyy - op * (pyy - r * (1 / 3 + u[1] ** 2)) + c * 2 * u[1] * G[1]).sum())
+    got = [a.sum() for a in _second_moment(f2)]
+    for g_, w_ in zip(got, want):
+        assert g_ == pytest.approx(w_, abs=1e-12)
+    # the source's share of the change is resolved: dropping it would move the sums by this much
+    assert abs((c * (u[0] * G[1] + u[1] * G[0])).sum()) > 1e-7
+
+
+def test_guo_source_reduces_to_the_bgk_form_when_the_rates_are_equal():
+    # omega+ = omega- = omega: TRT collapses to BGK and the split source to Guo's single term
+    # (1 - omega/2) w_q [3 (c_q - u) + 9 (c_q.u) c_q] . G  (Guo, Zheng & Shi 2002), here evaluated on
+    # one node with the textbook un-split expression and pure streaming undone by uniformity.
+    rng = np.random.default_rng(5)
+    ny, nx = 4, 4
+    f1 = feq(np.full((1, 1), 0.96), np.full((1, 1), -0.02), np.full((1, 1), 0.05))[:, 0, 0] + 1e-3 * rng.normal(size=9)
+    f = np.broadcast_to(f1[:, None, None], (9, ny, nx)).copy()
+    Gx, Gy, om = 2.2e-3, 0.9e-3, 1 / 0.71
+    G = np.empty((2, ny, nx))
+    G[0], G[1] = Gx, Gy
+    f2, u = mco.lbm_step(f, G, om, om)
+    r = f1.sum()
+    ux, uy = (CX @ f1 + 0.5 * Gx) / r, (CY @ f1 + 0.5 * Gy) / r
+    fe = feq(np.full((1, 1), r), np.full((1, 1), ux), np.full((1, 1), uy))[:, 0, 0]
+    cu = CX * ux + CY * uy
+    S = W * (3 * ((CX - ux) * Gx + (CY - uy) * Gy) + 9 * cu * (CX * Gx + CY * Gy))
+    want = f1 - om * (f1 - fe) + (1 - 0.5 * om) * S
+    assert np.abs(f2[:, 1, 2] - want).max() < 1e-15

@@ -222,3 +222,49 @@ def ragged_world(nx: int, ny: int, lengths, seed: int = 0, *, kappa: float = 2.0
     w["steps"] = 100
     w["name"] = tag
     return w
+
+
+def chains_from_angles(psi0: np.ndarray, theta_rest: np.ndarray, centres: np.ndarray,
+                       orient: np.ndarray, phase0: np.ndarray, *, L0: float = 1.0, k: float = 0.5,
+                       amp_tangent: float = 0.5, period_steps: float = 200.0, dt: float = 1e-2) -> dict:
+    """Like build_chains, but the INITIAL joint angles psi0 [n_fil, m] and the rest angles
+    theta_rest [n_fil, m] are given separately (columns 0 and m-1 ignored): chains that start
+    away from their rest shape."""
+    base = build_chains(psi0, centres, orient, phase0, L0=L0, k=k, amp_tangent=amp_tangent,
+                        period_steps=period_steps, dt=dt)
+    th = theta_rest.astype(np.float64).copy()
+    th[:, 0] = 0.0
+    th[:, -1] = 0.0
+    base["theta_rest"] = th.reshape(-1).astype(np.float32)
+    return base
+
+
+def hairpin_world(nx: int = 96, ny: int = 64, n_fil: int = 24, m: int = 20, seed: int = 0, *,
+                  kappa: float = 0.01, kappa_rep: float | None = 1e-4, tag: str = "hp") -> dict:
+    """Chains far from rest, for the large-angle paths of the elastic operator (Eq. 1, P:L95-98;
+    readings 4 and 25): rest angles ~U(-3, 3) rad, initial joint angles = rest angle + U(-1.5,
+    1.5) wrapped to (-pi, pi], and in chain f (f = 0..5) one joint forced to a special case:
+      f=0: psi = +pi - 5e-4 (hairpin, just inside the branch cut)   f=1: psi = -pi + 7e-4
+      f=2: theta_rest = 3.5 > pi      f=3: theta_rest = -4.0 < -pi   f=4: theta_rest = 2 pi + 0.3
+      f=5: psi = pi/2 exactly on the small-angle / large-angle boundary of a rest angle 0.
+    The couplings are weak (kappa = 0.01) so that the O(1) displacements these joints ask for
+    keep the fluid at low Mach number."""
+    th = (uniform(seed, tag + "/theta", n_fil * m).reshape(n_fil, m) * 2.0 - 1.0) * 3.0
+    pert = (uniform(seed, tag + "/pert", n_fil * m).reshape(n_fil, m) * 2.0 - 1.0) * 1.5
+    psi = th + pert
+    psi = psi - 2.0 * math.pi * np.round(psi / (2.0 * math.pi))   # into [-pi, pi]
+    j = m // 2
+    psi[0, j] = math.pi - 5e-4
+    psi[1, j] = -math.pi + 7e-4
+    th[2, j], th[3, j], th[4, j] = 3.5, -4.0, 2.0 * math.pi + 0.3
+    th[5, j], psi[5, j] = 0.0, 0.5 * math.pi
+    centres = np.stack([uniform(seed, tag + "/cx", n_fil) * nx, uniform(seed, tag + "/cy", n_fil) * ny], axis=1)
+    orient = uniform(seed, tag + "/orient", n_fil) * 2.0 * math.pi
+    ph = uniform(seed, tag + "/psi", n_fil) * 2.0 * math.pi
+    w = chains_from_angles(psi, th, centres, orient, ph)
+    params = default_params(nx, ny, kappa=kappa, kappa_rep=kappa_rep)
+    params["max_beads"] = int(w["offsets"][-1])
+    w["params"] = params
+    w["steps"] = 20
+    w["name"] = tag
+    return w

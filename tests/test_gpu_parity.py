@@ -17,6 +17,12 @@ pytestmark = pytest.mark.gpu
 
 TOL_STEP = 1e-5   # BASELINE.json north_star: per-step relative L2 on fp32 fields and positions
 TOL_TRAJ = 1e-3   # ... and on bead positions after 100 steps
+# Companion of the L2 bar: no single element may be off by more than
+# TOL_MAX x the largest oracle magnitude of its array.  A whole-array L2 of 1e-5 lets one node of a
+# 4 M-node field be wrong by 2 %; this does not.  Calibrated on the B200 runs of round 2 (worst
+# observed ratio 2.6e-6, on `force` of the hairpin world) and set 4x above it.
+TOL_MAX = 1e-5
+WORST = {}        # name -> (worst rel L2, worst max-abs ratio) seen in this session (printed by the tests)
 
 
 def rel_l2(a, b):
@@ -28,13 +34,50 @@ def rel_l2(a, b):
     return float(np.linalg.norm(a - b) / nb), False
 
 
-def assert_close(name, gpu, orc, tol=TOL_STEP):
+def max_ratio(a, b):
+    """max |a - b| / max |b| (0 when both vanish)."""
+    a = np.asarray(a, dtype=np.float64).ravel()
+    b = np.asarray(b, dtype=np.float64).ravel()
+    if a.size == 0:
+        return 0.0
+    d, m = float(np.abs(a - b).max()), float(np.abs(b).max())
+    return d / m if m > 0 else (0.0 if d <= 1e-7 else np.inf)
+
+
+def assert_close(name, gpu, orc, tol=TOL_STEP, tol_max=None):
     err, absolute = rel_l2(gpu, orc)
     if absolute:
         assert err <= 1e-7, f"{name}: abs L2 {err:.3e} (oracle is zero)"
     else:
         assert err <= tol, f"{name}: rel L2 {err:.3e} > {tol}"
+    # element-wise companion: scaled with the L2 tolerance the caller asks for
+    mr = max_ratio(gpu, orc)
+    lim = tol_max if tol_max is not None else TOL_MAX * (tol / TOL_STEP)
+    assert mr <= lim, f"{name}: max |gpu - orc| = {mr:.3e} x max |orc| > {lim:.1e}"
+    w = WORST.get(name, (0.0, 0.0))
+    WORST[name] = (max(w[0], err), max(w[1], mr))
     return err
+
+
+def assert_displacement(name, x0_f32, x1_gpu_f32, dX_ref, rel=TOL_STEP):
+    """Gate of S7 / K4 ("nodes sample the local fluid velocity"): the bead displacement of
+    ONE step, element by element.  X is fp32 and |X| ~ 100 while |dX| ~ 1e-3, so X itself cannot
+    see a wrong U; the displacement can, up to the rounding of the stored position:
+        |dX_gpu - dX_ref| <= ulp32(|X1|)/2 [storing X1] + rel * (|dX_ref| of the bead + 0.05 max |dX_ref|)
+    (the second term: U mixes 16 nodes whose velocities may exceed the bead's own near a
+    stagnation point).  Returns the worst error in units of that bound."""
+    x0 = np.asarray(x0_f32, dtype=np.float32)
+    x1 = np.asarray(x1_gpu_f32, dtype=np.float32)
+    d_gpu = x1.astype(np.float64) - x0.astype(np.float64)
+    d_ref = np.asarray(dX_ref, dtype=np.float64)
+    if d_ref.size == 0:
+        return 0.0
+    half_ulp = 0.5 * np.spacing(np.maximum(np.abs(x1), np.abs(x0) + np.abs(d_ref).astype(np.float32)))
+    bead = np.linalg.norm(d_ref, axis=1, keepdims=True)
+    bound = half_ulp.astype(np.float64) * 1.0001 + rel * (bead + 0.05 * np.abs(d_ref).max()) + 1e-12
+    ratio = float((np.abs(d_gpu - d_ref) / bound).max())
+    assert ratio <= 1.0, f"{name}: bead displacement off by {ratio:.2f} x (ulp/2 + {rel:g} |dX|)"
+    return ratio
 
 
 def has_density(w):
@@ -62,14 +105,19 @@ def step_parity(G, w, threads=0, check=True):
         pairs.append(("sense", g["sense"], o["sense"]))
     if has_density(w):
         pairs.append(("rho_b", gi["rho_b"], oi["rho_b"]))
-    # bead displacement of this step (a much harder test than X itself: X is O(100))
-    pairs.append(("dX", g["xy"].astype(np.float64) - s0["xy"], o["xy"] - s0["xy"].astype(np.float64)))
     for name, a, b in pairs:
-        if name == "dX":
-            # dX = U is O(1e-3) while X is O(100): fp32 X cannot hold dX to 1e-5; the bar is on X
-            errs[name] = rel_l2(a, b)[0]
-            continue
         errs[name] = assert_close(name, a, b) if check else rel_l2(a, b)[0]
+    # S7 / K4 gated on its own output, the displacement of this step (X is O(100), dX O(1e-3): a
+    # 40 % error in U passes the 1e-5 bar on X).  Twice: against the oracle's displacement, and
+    # against the oracle's interpolation of the GPU's OWN velocity field at the pre-step positions
+    # (K4 alone: its gather, weights and the update).
+    x0 = s0["xy"]
+    dX_orc = o["xy"] - x0.astype(np.float64)
+    U_own = mco.interp(g["u"].astype(np.float64), x0.astype(np.float64))
+    if check:
+        errs["dX/bound"] = assert_displacement("dX vs oracle", x0, g["xy"], dX_orc)
+        errs["dX_own_u/bound"] = assert_displacement("dX vs interp(own u)", x0, g["xy"], U_own, rel=2e-6)
+    errs["dX"] = rel_l2(g["xy"].astype(np.float64) - x0.astype(np.float64), dX_orc)[0]
     return errs
 
 
@@ -150,6 +198,20 @@ def test_per_step_parity_small(name):
     w = SMALL[name]()
     worst = run_protocol(w, steps_at=[0, 1, 10, 40])
     print(name, {k: f"{v:.2e}" for k, v in worst.items()})
+
+
+def test_per_step_parity_hairpin_world():
+    # K1's rare paths (k_filament.cuh): atan2f fallback beyond 0.46 rad of the rest angle, the
+    # restored (-pi, pi] branch for joints bent beyond 90 degrees, hairpins within 1e-3 of +-pi,
+    # sinf fallback of the director rotation, rest angles outside (-pi, pi] (reading 25).
+    # tests/test_worlds.py checks that the world really holds those joints.  (Eq. 1.)
+    w = worlds.hairpin_world()
+    worst = run_protocol(w, steps_at=[0, 1, 5, 12])
+    print("hairpin", {k: f"{v:.2e}" for k, v in worst.items()})
+    # the same chains with non-uniform parameters (the general K1 variant) and longer than a window
+    w2 = _varied(worlds.hairpin_world(128, 96, 9, 75, seed=3, tag="hp2"), 5)
+    worst = run_protocol(w2, steps_at=[0, 3])
+    print("hairpin varied", {k: f"{v:.2e}" for k, v in worst.items()})
 
 
 def test_config1_per_step_and_trajectory():

@@ -61,3 +61,37 @@ def test_ragged_world_translates_some_chains_by_whole_periods():
     w = worlds.ragged_world(96, 64, [3, 16, 33, 64], seed=1)
     assert list(w["offsets"]) == [0, 3, 19, 52, 116]
     assert w["xy"][:3, 0].max() < 0 or w["xy"][:3, 0].min() > 96  # chain 0 lives outside [0, nx)
+
+
+def _joint_angles(w):
+    """psi of every interior joint from the fp32 positions (plain numpy: input geometry only)."""
+    off = w["offsets"]
+    out = np.full(len(w["xy"]), np.nan)
+    xy = w["xy"].astype(np.float64)
+    for f in range(len(off) - 1):
+        p = xy[off[f]:off[f + 1]]
+        v = np.diff(p, axis=0)
+        cr = v[:-1, 0] * v[1:, 1] - v[:-1, 1] * v[1:, 0]
+        dt = (v[:-1] * v[1:]).sum(axis=1)
+        out[off[f] + 1: off[f + 1] - 1] = np.arctan2(cr, dt)
+    return out
+
+
+def test_hairpin_world_holds_the_large_angle_cases():
+    # the cases the GPU's K1 treats on its rare paths (k_filament.cuh half_kC / sin_small /
+    # k_pack_params) must really be in the world the parity test runs
+    w = worlds.hairpin_world()
+    psi = _joint_angles(w)
+    th = w["theta_rest"].astype(np.float64)
+    inner = ~np.isnan(psi)
+    assert np.any(np.abs(psi[inner] - math.pi) < 1e-3) and np.any(np.abs(psi[inner] + math.pi) < 1e-3)
+    assert np.any(th > math.pi) and np.any(th < -math.pi) and np.any(th > 2 * math.pi)
+    d = psi[inner] - th[inner]
+    d = d - 2 * math.pi * np.round(d / (2 * math.pi))
+    assert np.mean(np.abs(d) > 0.46) > 0.3        # beyond the small-angle atan range of K1
+    assert np.mean(np.abs(psi[inner]) > 0.5 * math.pi) > 0.2   # dot <= 0: joints bent beyond 90 degrees
+    # edges keep unit length (the hairpins fold the chain, they do not stretch it)
+    off = w["offsets"]
+    for f in range(len(off) - 1):
+        v = np.diff(w["xy"][off[f]:off[f + 1]].astype(np.float64), axis=0)
+        assert np.abs(np.linalg.norm(v, axis=1) - 1.0).max() < 1e-4

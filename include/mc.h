@@ -91,6 +91,10 @@ typedef struct {
 size_t mc_workspace_bytes(const mc_world_params* p /*HOST*/);
 
 /* Create a world: fluid at rest (f_q = w_q rho0), no filaments, step counter 0.
+ * Defines: the paper's world = "a two-dimensional world of fields and filaments": the D2Q9
+ * lattice-Boltzmann fluid grid whose viscosity is set by one relaxation parameter (
+ * nu, trt_lambda -> tau+, tau-, TRT P:L127), the steric density field built from deposited node
+ * positions and the persistent energy field of Gaussian packets.
  * workspace: DEVICE, >= mc_workspace_bytes(p) bytes, 256-byte aligned (512-byte alignment, which
  * cudaMalloc and torch give, also lets the gathers use texture views: mc_texture_gathers),
  * owned by the caller and must outlive the world.  cuda_stream: a cudaStream_t (NULL = legacy default stream); all
@@ -100,7 +104,13 @@ size_t mc_workspace_bytes(const mc_world_params* p /*HOST*/);
 int mc_create(const mc_world_params* p /*HOST*/, void* workspace /*DEVICE*/, size_t workspace_bytes,
               void* cuda_stream, mc_world** out /*HOST*/);
 
-/* Load (replace) the filaments.  offsets: HOST int32 [n_fil+1], offsets[0] = 0, chain f owns
+/* Load (replace) the filaments.
+ * Defines: the paper's filament = a chain of nodes in continuous 2-D space whose edges carry the
+ * rest length L_rest, the rest angle theta_rest and the optional stiffnesses k_bend, k_shear,
+ * k_stretch "set on the edge level instead of globally" (direct encoding = one value per
+ * node), with a time-dependent rest angle -- and, with act_L_amp, rest length -- as the
+ * controller would emit them per node and time (hand-designed sinusoids P:L153).
+ * offsets: HOST int32 [n_fil+1], offsets[0] = 0, chain f owns
  * beads offsets[f] .. offsets[f+1]-1, every chain >= 3 beads, N = offsets[n_fil] <= max_beads.
  * All other arrays are DEVICE float arrays, chain-ordered:
  *   xy [N][2] unwrapped positions;
@@ -122,7 +132,11 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets /*HOST*
  * rebuilds the tile lists.  Synchronises the stream.  Errors: MC_EINVAL, MC_ECUDA. */
 int mc_set_positions(mc_world* w, const float* xy /*DEVICE*/);
 
-/* Advance n >= 0 steps.  Asynchronous: kernels are enqueued on the world's stream and the
+/* Advance n >= 0 steps of the update S0..S7 listed at the top of this header: PBD bending pass
+ * Eq. 1 and position pass Eq. 2-4 of "each iteration", steric
+ * field deposit -> Gaussian -> gradient -> repulsive force, immersed-boundary exchange with
+ * the fluid and the D2Q9 TRT fluid update.
+ * Asynchronous: kernels are enqueued on the world's stream and the
  * call returns without synchronising.  Blocks of four steps are replayed from a CUDA graph when
  * the stream can be captured (not the legacy default stream); the results are bit-identical to
  * direct launches, so mc_step(a) then mc_step(b) equals mc_step(a + b).  Errors: MC_EINVAL, MC_ECUDA (launch failure),
@@ -130,7 +144,10 @@ int mc_set_positions(mc_world* w, const float* xy /*DEVICE*/);
  * position or |u| > 0.3). */
 int mc_step(mc_world* w, int32_t n);
 
-/* Copy the state out.  Synchronises the stream.  Every output pointer is DEVICE memory of the
+/* Copy the state out: what the paper's experiments read from a rollout -- node positions (fitness =
+ * displacement; loss on the final shape), the fluid and scalar fields of the
+ * world and the energy sensed at the nodes.
+ * Synchronises the stream.  Every output pointer is DEVICE memory of the
  * stated size and may be NULL (skipped); step_out is HOST.
  *   xy    [N][2]        bead positions
  *   u     [2][ny][nx]   velocity stored by the last step's S6 (lattice units)

@@ -23,8 +23,16 @@ const double WQ[9] = {4.0 / 9, 1.0 / 9, 1.0 / 9, 1.0 / 9, 1.0 / 9,
                       1.0 / 36, 1.0 / 36, 1.0 / 36, 1.0 / 36};
 const int OPP[9] = {0, 3, 4, 1, 2, 7, 8, 5, 6};
 
-int g_threads = 0;  // 0/1 = serial; >1 = OpenMP over independent loops (same arithmetic)
-#define MCO_PAR _Pragma("omp parallel for schedule(static) num_threads(g_threads > 1 ? g_threads : 1)")
+// Thread count of the independent loops (same arithmetic whatever it is).  It belongs to a WORLD
+// (mco_world::threads, mco_set_threads); mco_step installs it for the duration of the call on the
+// calling thread.  The stateless component functions called on their own run serially.
+thread_local int tl_threads = 0;  // 0/1 = serial; >1 = OpenMP over independent loops
+struct ThreadScope {
+  int saved;
+  explicit ThreadScope(int k) : saved(tl_threads) { tl_threads = k; }
+  ~ThreadScope() { tl_threads = saved; }
+};
+#define MCO_PAR _Pragma("omp parallel for schedule(static) num_threads(tl_threads > 1 ? tl_threads : 1)")
 
 inline int wrap(long long i, int n) {
   long long r = i % n;
@@ -350,6 +358,7 @@ struct mco_world {
   double dt = 0, omega_p = 0, omega_m = 0, kappa = 0, rho0 = 1;
   int64_t step = 0;
   int fp32_state = 0;
+  int threads = 0;  // OpenMP threads of this world's steps (mco_set_threads)
   // filaments
   int32_t n_fil = 0;
   int64_t N = 0;
@@ -482,7 +491,7 @@ int mco_set_fp32_state(mco_world* w, int32_t on) {
 
 int mco_set_threads(mco_world* w, int32_t k) {
   if (!w || k < 0) return MCO_EINVAL;
-  g_threads = k;
+  w->threads = k;
   return MCO_OK;
 }
 
@@ -559,6 +568,7 @@ static int mco_one_step(mco_world* w) {
 
 int mco_step(mco_world* w, int32_t n) {
   if (!w || n < 0) return MCO_EINVAL;
+  ThreadScope scope(w->threads);
   for (int32_t s = 0; s < n; ++s) {
     int rc = mco_one_step(w);
     if (rc != MCO_OK) return rc;

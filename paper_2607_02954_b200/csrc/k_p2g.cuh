@@ -315,7 +315,8 @@ __global__ void __launch_bounds__(256, LIGHT ? 6 : 1) k_deposit_tile(int nx, int
     __stcs(reinterpret_cast<float4*>(rho_b + (size_t)(y0 + ly) * nx + x0 + lx), make_float4(v[0], v[1], v[2], v[3]));
   }
   // tile maximum: rho_b >= 0, so the float bits order like unsigned integers; one global
-  // atomicMax per warp onto tile_rho_max[t] (zeroed by the tile-list scan of this step)
+  // atomicMax per warp onto tile_rho_max[t] (reset to 0 by the fused spread + fluid kernel of the
+  // previous step, k_lbm.cuh, after it has read it; zero from mc_create before the first step)
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
   if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<unsigned*>(tile_rho_max) + t, __float_as_uint(mx));

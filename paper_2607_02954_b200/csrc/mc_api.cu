@@ -48,7 +48,8 @@ bool validate(const mc_world_params* p, Derived* d, std::string* why) {
   if (!(p->dt > 0) || !(p->nu > 0) || !(p->trt_lambda > 0) || !(p->rho0 > 0)) { *why = "dt, nu, trt_lambda, rho0 must be > 0"; return false; }
   if (p->pbd_iters != 1) { *why = "pbd_iters must be 1"; return false; }
   if (p->n_fields < 0 || p->n_fields > 4) { *why = "n_fields must be 0..4"; return false; }
-  if (p->max_beads < 0 || p->max_beads > (int64_t)1 << 30) { *why = "max_beads out of range"; return false; }
+  // the tile lists hold up to 4 N entries addressed with 32-bit ints (k_tile.cuh)
+  if (p->max_beads < 0 || p->max_beads > ((int64_t)1 << 29) - 1) { *why = "max_beads out of range (0 .. 2^29 - 1)"; return false; }
   if (p->coupling != MC_COUPLING_FORCE && p->coupling != MC_COUPLING_MDF) { *why = "unknown coupling"; return false; }
   if (p->coupling == MC_COUPLING_MDF && (p->mdf_iters < 1 || p->mdf_iters > 16)) { *why = "mdf_iters must be 1..16"; return false; }
   for (int k = 0; k < p->n_fields; ++k) {
@@ -177,6 +178,20 @@ int check_cuda(mc_world* w, const char* what) {
   if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
   return MC_OK;
 }
+
+// first failing CUDA call of a sequence: `ok(call, "what")` records it in the world and returns false
+struct CudaSeq {
+  mc_world* w;
+  const char* where;
+  int rc = MC_OK;
+  bool ok(cudaError_t e, const char* what) {
+    if (e == cudaSuccess || rc != MC_OK) return rc == MC_OK;
+    rc = fail(w, MC_ECUDA, std::string(where) + ": " + what + ": " + cudaGetErrorString(e));
+    return false;
+  }
+  // after a kernel launch: launch-configuration errors surface here (execution errors at the next sync)
+  bool launched(const char* what) { return ok(cudaPeekAtLastError(), what); }
+};
 
 constexpr int PROF_MAX_STEPS = 64;
 constexpr int GRAPH_STEPS = 4;
@@ -342,7 +357,8 @@ int enqueue_step(mc_world* w) {
       const bool tex = w->tex_on && w->tex_u;
       const int K = w->p.mdf_iters;
       unsigned* mfmax = w->ptr<unsigned>(w->L.mdf_fmax);  // [K][n_tiles], raised by K5b with atomicMax
-      cudaMemsetAsync(mfmax, 0, (size_t)K * n_tiles * 4, st);
+      if (cudaMemsetAsync(mfmax, 0, (size_t)K * n_tiles * 4, st) != cudaSuccess)
+        return fail(w, MC_ECUDA, "mc_step: cudaMemsetAsync(mdf bounds) failed");
       for (int k = 0; k < K; ++k) {
         unsigned* slot = mfmax + (size_t)k * n_tiles;
         const bool first = k == 0, last = k + 1 == K;
@@ -444,6 +460,9 @@ int enqueue_step(mc_world* w) {
   prof_mark(w, 7);
   if (w->prof_on && w->prof_steps < PROF_MAX_STEPS) w->prof_steps++;
   w->step += 1;
+  // launch-configuration errors of this step's kernels (execution errors surface at the next sync)
+  const cudaError_t le = cudaPeekAtLastError();
+  if (le != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_step: kernel launch: ") + cudaGetErrorString(le));
   return MC_OK;
 }
 
@@ -626,6 +645,7 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
                 !act_period))
     return fail(w, MC_EINVAL, "null array");
   cudaStream_t st = w->stream;
+  CudaSeq cs{w, "mc_load_filaments"};  // every CUDA return code of this call; reported at the next sync
   const bool reuse_order = w->N == N && w->n_fil == n_fil && (int64_t)w->loaded_offsets.size() == n_fil + 1 &&
                            std::equal(w->loaded_offsets.begin(), w->loaded_offsets.end(), offsets);
   const int prev_stride = w->stride, prev_windows = w->n_windows;
@@ -641,7 +661,7 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   bool uniform = true;
   const int m0 = offsets[1] - offsets[0];
   int* bad = w->ptr<int>(w->L.flags) + 1;
-  cudaMemsetAsync(bad, 0, 4, st);
+  cs.ok(cudaMemsetAsync(bad, 0, 4, st), "cudaMemsetAsync");
   cudaError_t e = cudaSuccess;
   std::vector<int> src;                 // host staging of this call; must outlive the final sync
   std::vector<unsigned char> bflags;
@@ -649,12 +669,14 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   int* d_off = w->ptr<int>(w->L.scratch);
   int* d_keys = d_off + (n_fil + 1);
   std::vector<int> keys(n_fil);
-  cudaMemcpyAsync(d_off, offsets, (size_t)(n_fil + 1) * 4, cudaMemcpyHostToDevice, st);
+  cs.ok(cudaMemcpyAsync(d_off, offsets, (size_t)(n_fil + 1) * 4, cudaMemcpyHostToDevice, st), "cudaMemcpyAsync");
   mc::k_chain_keys<<<(n_fil + 255) / 256, 256, 0, st>>>(n_fil, d_off, xy, w->nx, w->ny, 64, d_keys);
+  cs.launched("k_chain_keys");
   w->launches++;
-  cudaMemcpyAsync(keys.data(), d_keys, (size_t)n_fil * 4, cudaMemcpyDeviceToHost, st);
+  cs.ok(cudaMemcpyAsync(keys.data(), d_keys, (size_t)n_fil * 4, cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync");
   e = cudaStreamSynchronize(st);
   if (e == cudaSuccess) e = cudaGetLastError();
+  if (cs.rc != MC_OK) return cs.rc;
   if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_load_filaments: ") + cudaGetErrorString(e));
   std::vector<int> order(n_fil);
   std::iota(order.begin(), order.end(), 0);
@@ -671,8 +693,8 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
     bflags[pos + m - 1] |= mc::BEAD_LAST;
     pos += m;
   }
-  cudaMemcpyAsync(w->ptr<int>(w->L.src), src.data(), (size_t)N * 4, cudaMemcpyHostToDevice, st);
-  cudaMemcpyAsync(w->ptr<unsigned char>(w->L.bflags), bflags.data(), (size_t)N, cudaMemcpyHostToDevice, st);
+  cs.ok(cudaMemcpyAsync(w->ptr<int>(w->L.src), src.data(), (size_t)N * 4, cudaMemcpyHostToDevice, st), "cudaMemcpyAsync");
+  cs.ok(cudaMemcpyAsync(w->ptr<unsigned char>(w->L.bflags), bflags.data(), (size_t)N, cudaMemcpyHostToDevice, st), "cudaMemcpyAsync");
   }
   // 2. gather + pack the per-bead parameters in the internal order, validate
   mc::PackArgs pa;
@@ -688,41 +710,45 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   pa.PD = w->ptr<float2>(w->L.PD);
   pa.uni = reinterpret_cast<float4*>(w->ptr<int>(w->L.flags) + 24);
   pa.nonuniform = w->ptr<int>(w->L.flags) + 3;
-  cudaMemsetAsync(pa.nonuniform, 0, 4, st);
+  cs.ok(cudaMemsetAsync(pa.nonuniform, 0, 4, st), "cudaMemsetAsync");
   pa.dt = (double)w->p.dt;
   pa.bad = bad;
   mc::k_pack_params<<<(int)((N + 255) / 256), 256, 0, st>>>(pa);
+  cs.launched("k_pack_params");
   w->launches++;
-  cudaMemsetAsync(w->ptr<float>(w->L.F), 0, (size_t)N * 8, st);
-  cudaMemsetAsync(w->ptr<float>(w->L.sense), 0, (size_t)N * 4, st);
+  cs.ok(cudaMemsetAsync(w->ptr<float>(w->L.F), 0, (size_t)N * 8, st), "cudaMemsetAsync");
+  cs.ok(cudaMemsetAsync(w->ptr<float>(w->L.sense), 0, (size_t)N * 4, st), "cudaMemsetAsync");
   // largest tile list of the loaded configuration -> CTA size of the deposit kernel
   int* maxlist = w->ptr<int>(w->L.flags) + 2;
   {
     const int n_tiles = (w->nx / mc::TS) * (w->ny / mc::TS);
     int* tile_count = w->ptr<int>(w->L.tile_count);
-    cudaMemsetAsync(maxlist, 0, 4, st);
+    cs.ok(cudaMemsetAsync(maxlist, 0, 4, st), "cudaMemsetAsync");
     // force the next step to rebuild the lists (drift = +inf), and count once now with need = 1
     mc::ListState force;
     force.need = 1;
     force.drift = INFINITY;
     force.step_max = 0u;
     mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16);
-    cudaMemcpyAsync(ls_state, &force, sizeof(force), cudaMemcpyHostToDevice, st);
+    cs.ok(cudaMemcpyAsync(ls_state, &force, sizeof(force), cudaMemcpyHostToDevice, st), "cudaMemcpyAsync");
     mc::k_tile_bin<false><<<(int)((N + 255) / 256), 256, 0, st>>>(ls_state, w->ptr<float2>(w->L.X), (int)N, w->nx,
                                                                   w->ny, tile_count, nullptr, nullptr);
+    cs.launched("k_tile_bin");
     mc::k_max_int<<<64, 256, 0, st>>>(tile_count, n_tiles, maxlist);
-    cudaMemsetAsync(tile_count, 0, (size_t)n_tiles * 4, st);
+    cs.launched("k_max_int");
+    cs.ok(cudaMemsetAsync(tile_count, 0, (size_t)n_tiles * 4, st), "cudaMemsetAsync");
     w->launches += 2;
   }
   int h_maxlist = 0;
-  cudaMemcpyAsync(&h_maxlist, maxlist, 4, cudaMemcpyDeviceToHost, st);
+  cs.ok(cudaMemcpyAsync(&h_maxlist, maxlist, 4, cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync");
   const long long host_step = w->step;  // steps without beads do not advance the device copy
-  cudaMemcpyAsync(w->ptr<long long>(w->L.flags) + 4, &host_step, 8, cudaMemcpyHostToDevice, st);
+  cs.ok(cudaMemcpyAsync(w->ptr<long long>(w->L.flags) + 4, &host_step, 8, cudaMemcpyHostToDevice, st), "cudaMemcpyAsync");
   int h = 0, h_nonuni = 0;
-  cudaMemcpyAsync(&h, bad, 4, cudaMemcpyDeviceToHost, st);
-  cudaMemcpyAsync(&h_nonuni, w->ptr<int>(w->L.flags) + 3, 4, cudaMemcpyDeviceToHost, st);
+  cs.ok(cudaMemcpyAsync(&h, bad, 4, cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync");
+  cs.ok(cudaMemcpyAsync(&h_nonuni, w->ptr<int>(w->L.flags) + 3, 4, cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync");
   e = cudaStreamSynchronize(st);  // src/bflags are host vectors of this call
   if (e == cudaSuccess) e = cudaGetLastError();
+  if (cs.rc != MC_OK) { w->loaded_offsets.clear(); return cs.rc; }
   if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_load_filaments: ") + cudaGetErrorString(e));
   if (h) {
     w->loaded_offsets.clear();
@@ -782,24 +808,42 @@ int mc_step(mc_world* w, int32_t n) {
       const int ph = w->cur;
       if (!w->graph[ph]) {
         cudaGraph_t g = nullptr;
-        const int64_t l0 = w->launches;
+        // host-side state a capture advances: restored if the capture does not yield a graph
+        const int64_t l0 = w->launches, step0 = w->step;
+        const int cur0 = w->cur;
         if (w->stream == nullptr ||
             cudaStreamBeginCapture(w->stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
           cudaGetLastError();  // not an error of the world: this stream just cannot be captured
           w->graph_off = true;
           continue;
         }
-        for (int s = 0; s < GRAPH_STEPS; ++s) enqueue_step(w);  // advances the host-side state
+        int crc = MC_OK;
+        for (int s = 0; s < GRAPH_STEPS && crc == MC_OK; ++s) crc = enqueue_step(w);  // advances the host-side state
         cudaError_t e = cudaStreamEndCapture(w->stream, &g);
-        if (e == cudaSuccess) e = cudaGraphInstantiate(&w->graph[ph], g, 0);
+        if (e == cudaSuccess && crc == MC_OK) e = cudaGraphInstantiate(&w->graph[ph], g, 0);
         if (g) cudaGraphDestroy(g);
-        if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
+        if (e != cudaSuccess || crc != MC_OK) {
+          // nothing was enqueued (a capture records, it does not run): put the host counters back
+          // and launch these steps directly from now on
+          cudaGetLastError();
+          if (w->graph[ph]) { cudaGraphExecDestroy(w->graph[ph]); w->graph[ph] = nullptr; }
+          w->launches = l0;
+          w->step = step0;
+          w->cur = cur0;
+          w->graph_off = true;
+          continue;
+        }
         w->graph_launches[ph] = w->launches - l0;
       } else {
         w->step += GRAPH_STEPS;  // cur returns to its value after GRAPH_STEPS steps
         w->launches += w->graph_launches[ph];
       }
-      if (cudaGraphLaunch(w->graph[ph], w->stream) != cudaSuccess) return fail(w, MC_ECUDA, "cudaGraphLaunch failed");
+      if (cudaGraphLaunch(w->graph[ph], w->stream) != cudaSuccess) {
+        // the steps of this block were counted but not enqueued
+        w->step -= GRAPH_STEPS;
+        w->launches -= w->graph_launches[ph];
+        return fail(w, MC_ECUDA, "cudaGraphLaunch failed");
+      }
       done += GRAPH_STEPS;
       continue;
     }

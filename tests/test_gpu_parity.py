@@ -19,9 +19,10 @@ TOL_STEP = 1e-5   # BASELINE.json north_star: per-step relative L2 on fp32 field
 TOL_TRAJ = 1e-3   # ... and on bead positions after 100 steps
 # Companion of the L2 bar: no single element may be off by more than
 # TOL_MAX x the largest oracle magnitude of its array.  A whole-array L2 of 1e-5 lets one node of a
-# 4 M-node field be wrong by 2 %; this does not.  Calibrated on the B200 runs of round 2 (worst
-# observed ratio 2.6e-6, on `force` of the hairpin world) and set 4x above it.
-TOL_MAX = 1e-5
+# 4 M-node field be wrong by 2 %; this does not.  Calibrated on the B200 run of round 2 over all
+# worlds of the GPU suite (worst per-step ratios: G 9.9e-7, force 7.9e-7, u 6.4e-7, fdev 4.5e-7,
+# rho_b 4.0e-7; gpurun_out/parity_worst.json is rewritten by every GPU session) and set 5x above.
+TOL_MAX = 5e-6
 WORST = {}        # name -> (worst rel L2, worst max-abs ratio) seen in this session (printed by the tests)
 
 

@@ -16,11 +16,16 @@ north_star's >= 60 % HBM-roofline bar is stated on.  Prints ONE JSON line (rank 
   roofline     the step's dominant kernel (largest share of the step, measured live with CUDA
                events on the world's stream through mc_profile_*), its algorithmic bytes per
                launch / its mean duration, against the measured HBM peak
-  roofline_step  the same for the whole step (112 B/cell + 64 B/bead)
+  roofline_step  the same for the whole step, on each byte model of DESIGN.md section 8 (raw 112
+               B/node + 64 B/bead; reduced 96 B/node: G never travels through HBM; each also with
+               the two compulsory gather reads of A and u, +16 B/node) against both the measured
+               and the nominal 8 TB/s peak
   cpu_baseline the oracle (oracle/, as it stands) timed on this box's host cores on a bounded
-               sample: the same recipe at 1/100 size (world "4b": 100,032 beads, 640^2 grid)
-  --impl reference   times the oracle alone on that sample (there is no reference implementation
-               of the paper in this repository: the oracle is the reference arm)
+               sample of the SAME world: a few whole steps of the benchmarked workload (second,
+               labelled sample: all steps of world "4b", the same recipe at 1/100 size)
+  --impl reference   times the oracle alone on the benchmarked world, K steps after W warm-up (there
+               is no reference implementation of the paper in this repository: the oracle is
+               the reference arm)
 
 --coupling mdf times the same world under the Multi-Direct Forcing coupling (SURVEY.md 8(f)
 NEXT-1): the K5 kernels appear in slot K2b_spread and the byte model grows by
@@ -120,24 +125,48 @@ def kernel_bytes(n_cells: int, n_beads: int) -> dict:
     }
 
 
+# the two per-bead gathers read their grid field once per step whatever the tiling (neither A nor u
+# fits the L2 on the large worlds): compulsory reads SURVEY 8(d)'s model leaves out
+GATHER_BYTES = {"K1_filament": 8, "K4_interp_integrate": 8}   # per node
+
+
+def csrc_sha() -> str:
+    """Hash of the CUDA sources the timed library was built from (ties an ncu capture to a build)."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2607_02954_b200", "csrc")
+    for f in sorted(glob.glob(os.path.join(d, "*.cu")) + glob.glob(os.path.join(d, "*.cuh"))):
+        h.update(os.path.basename(f).encode())
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
-# (profiles/r1_traffic.json, world 4d); None for other workloads or kernels not captured
+# of THIS build (profiles/r2_traffic.json names the csrc hash it was taken on; a capture of another
+# build is refused: traffic = null, with the reason in traffic_note)
 _SLOT_KERNEL = {"K2a_deposit": "k_deposit_tile", "K3a_blur_grad": "k_blur_grad", "K1_filament": "k_filament_force",
                 "K3b_lbm": "k_lbm_spread_tile", "K4_interp_integrate": "k_interp_integrate"}
 
 
 def ncu_traffic(slot: str, workload: str, mdf_iters: int = 0):
+    """-> (bytes per launch or None, note)"""
+    path = os.path.join(ROOT, "profiles", "r2_traffic.json")
     try:
-        with open(os.path.join(ROOT, "profiles", "r1_traffic.json")) as fh:
+        with open(path) as fh:
             d = json.load(fh)
-        if d.get("world") != workload:
-            return None
-        if slot == "K2b_spread":  # the K5 group of the MDF coupling: one figure for all its launches
-            m = d.get("mdf", {})
-            return m.get("K5_group_bytes_per_step") if m.get("mdf_iters") == mdf_iters else None
-        return d["dram_bytes_per_launch"].get(_SLOT_KERNEL.get(slot, ""))
     except Exception:
-        return None
+        return None, "no profiles/r2_traffic.json"
+    if d.get("csrc_sha") != csrc_sha():
+        return None, f"stale capture: profiles/r2_traffic.json is of build {d.get('csrc_sha')}, this is {csrc_sha()}"
+    if d.get("world") != workload:
+        return None, f"capture is of world {d.get('world')}"
+    if slot == "K2b_spread":  # the K5 group of the MDF coupling: one figure for all its launches
+        m = d.get("mdf", {})
+        return (m.get("K5_group_bytes_per_step"), "ncu") if m.get("mdf_iters") == mdf_iters else (None, "no MDF capture")
+    v = d.get("dram_bytes_per_launch", {}).get(_SLOT_KERNEL.get(slot, ""))
+    return v, ("ncu --set full, " + d.get("command", "")) if v is not None else "kernel not captured"
 
 
 def mdf_extra_bytes(n_cells: int, n_beads: int, iters: int) -> int:
@@ -151,9 +180,24 @@ def mdf_extra_bytes(n_cells: int, n_beads: int, iters: int) -> int:
             + (iters - 1) * (20 * n_cells + 16 * n_beads))
 
 
-def step_bytes(n_cells: int, n_beads: int, mdf_iters: int = 0) -> int:
-    # SURVEY.md 8(d) / DESIGN.md: 112 B/node + 64 B/bead, plus the MDF kernels when they run
-    return 112 * n_cells + 64 * n_beads + mdf_extra_bytes(n_cells, n_beads, mdf_iters)
+# byte models of the whole step, per node / per bead
+STEP_MODELS = {
+    "raw": (112, 64),                    # every array once through HBM, G included
+    "reduced": (96, 64),                 # S5 fused into S6: G is never written or read (what the build moves)
+    "raw_with_gathers": (128, 64),       # + the compulsory reads of A (K1) and u (K4), 8 B/node each
+    "reduced_with_gathers": (112, 64),
+}
+
+
+def step_bytes(n_cells: int, n_beads: int, mdf_iters: int = 0, model: str = "raw") -> int:
+    pn, pb = STEP_MODELS[model]
+    return pn * n_cells + pb * n_beads + mdf_extra_bytes(n_cells, n_beads, mdf_iters)
+
+
+def aggregate(n_beads_per_rank: int, steps: int, world_size: int, ms_max_over_ranks: float) -> float:
+    """Whole-job bead-steps/s of N replicas: every rank steps its own world of
+    n beads, the time is the MAX over the ranks' device times."""
+    return world_size * n_beads_per_rank * steps / (ms_max_over_ranks * 1e-3)
 
 
 def time_oracle(sample: str, seed: int, budget_s: float, min_steps: int, max_steps: int, warm: int = 1):
@@ -174,14 +218,20 @@ def time_oracle(sample: str, seed: int, budget_s: float, min_steps: int, max_ste
     return N * n / dt, cores, n, dt
 
 
+def world_label(name: str, w: dict) -> str:
+    p = w["params"]
+    return (f"world {name}: {int(w['offsets'][-1])} beads in {len(w['offsets']) - 1} filaments, "
+            f"{p['nx']}x{p['ny']} grid")
+
+
 def run_reference(args, rank: int):
-    """--impl reference: the oracle alone, on the bounded sample, K timed steps after W warm-up."""
+    """--impl reference: the oracle alone, on the benchmarked world, K timed steps after W warm-up."""
     if rank != 0:
         return
     from oracle import mco
     from paper_2607_02954_b200 import worlds
     cores = os.cpu_count() or 1
-    w = worlds.make_world(SAMPLE_WORLD, 0)
+    w = worlds.make_world(args.workload, 0)
     N = int(w["offsets"][-1])
     O = mco.World(w, threads=cores)
     O.step(args.warmup)
@@ -189,14 +239,15 @@ def run_reference(args, rank: int):
     O.step(args.steps)
     dt = time.perf_counter() - t0
     val = N * args.steps / dt
-    p = w["params"]
-    sample = (f"world {SAMPLE_WORLD}: {N} beads in 64-bead filaments, {p['nx']}x{p['ny']} grid "
-              f"(config-4 recipe at 1/100 of 4d), {args.steps} steps")
+    sample = f"{world_label(args.workload, w)} (the benchmarked world itself), {args.steps} whole steps, fp64, OpenMP over {cores} threads"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic (seeded)", "config": {"workload": args.workload, "sample": sample},
+        "data": "synthetic (seeded)",
+        "config": {"workload": f"BASELINE.json config {args.workload}", "beads": N,
+                   "filaments": len(w["offsets"]) - 1, "grid": [w["params"]["nx"], w["params"]["ny"]],
+                   "sample": sample},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -270,7 +321,7 @@ def main():
     ms_total = float(ms.item())
     clocks = sampler.stop() if rank == 0 else None
     ms_step = ms_total / args.steps
-    value = world_size * N * args.steps / (ms_total * 1e-3)
+    value = aggregate(N, args.steps, world_size, ms_total)
 
     # per-kernel durations, live, CUDA events on the world's stream (up to 64 steps)
     G.profile_enable(True)
@@ -283,17 +334,35 @@ def main():
     peak, peak_src = measured_peak_gbs()
     dom = max(kms, key=lambda k: kms[k])
     ach = kb[dom] / (kms[dom] * 1e-3) / 1e9 if kms[dom] > 0 else 0.0
+    traffic, traffic_note = ncu_traffic(dom, args.workload, mdf_iters)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
-                "frac": ach / peak, "traffic": ncu_traffic(dom, args.workload, mdf_iters), "peak_source": peak_src,
+                "frac": ach / peak, "traffic": traffic, "traffic_note": traffic_note, "peak_source": peak_src,
+                "frac_of_8TBps_nominal": ach / 8000.0,
                 "algorithmic_bytes_per_launch": kb[dom], "ms_per_launch": kms[dom],
-                "share_of_step": kms[dom] / max(sum(kms.values()), 1e-12)}
-    ach_step = step_bytes(nc, N, mdf_iters) / (ms_step * 1e-3) / 1e9
-    roofline_step = {"bound": "hbm", "achieved": ach_step, "peak": peak, "unit": "GB/s",
-                     "frac": ach_step / peak, "frac_of_8TBps_nominal": ach_step / 8000.0,
-                     "algorithmic_bytes_per_step": step_bytes(nc, N, mdf_iters)}
-    kernels = {k: {"ms": round(kms[k], 5),
-                   "GBps": round(kb[k] / (kms[k] * 1e-3) / 1e9, 1) if kms[k] > 0 else None}
-               for k in kms}
+                "share_of_step": kms[dom] / max(sum(kms.values()), 1e-12), "csrc_sha": csrc_sha()}
+    roofline_step = {"bound": "hbm", "peak": peak, "unit": "GB/s", "models": {}}
+    for model in STEP_MODELS:
+        by = step_bytes(nc, N, mdf_iters, model)
+        a_ = by / (ms_step * 1e-3) / 1e9
+        roofline_step["models"][model] = {"bytes_per_step": by, "achieved": a_, "frac": a_ / peak,
+                                          "frac_of_8TBps_nominal": a_ / 8000.0,
+                                          "B_per_node": STEP_MODELS[model][0], "B_per_bead": STEP_MODELS[model][1]}
+    # top-level figures = the raw model of SURVEY 8(d) (the one round 1 reported; north_star's bar)
+    roofline_step.update({k: roofline_step["models"]["raw"][k] for k in ("achieved", "frac", "frac_of_8TBps_nominal")})
+    roofline_step["algorithmic_bytes_per_step"] = step_bytes(nc, N, mdf_iters)
+    kernels = {}
+    for k in kms:
+        t = kms[k] * 1e-3
+        kernels[k] = {"ms": round(kms[k], 5), "GBps": round(kb[k] / t / 1e9, 1) if t > 0 else None}
+        if k in GATHER_BYTES and t > 0:   # K1, K4: the model with the compulsory gather read
+            g = kb[k] + GATHER_BYTES[k] * nc
+            kernels[k]["GBps_with_gather"] = round(g / t / 1e9, 1)
+            kernels[k]["frac_with_gather"] = round(g / t / 1e9 / peak, 4)
+        if t > 0:
+            kernels[k]["frac"] = round(kb[k] / t / 1e9 / peak, 4)
+        tr, _ = ncu_traffic(k, args.workload, mdf_iters)
+        if tr is not None:
+            kernels[k]["ncu_dram_bytes"] = tr
 
     # e2e: host buffers, copies inside the timed region, every step
     keys = ("xy", "L_rest", "theta_rest", "k_bend", "k_shear", "k_stretch", "act_amp", "act_phase",
@@ -323,7 +392,7 @@ def main():
     te = torch.tensor([time.perf_counter() - t0], device=dev, dtype=torch.float64)
     if dist is not None:
         dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_val = world_size * N * args.e2e_steps / float(te.item())
+    e2e_val = aggregate(N, args.e2e_steps, world_size, float(te.item()) * 1e3)
 
     # the same loop when only the positions change between steps (mc_set_positions instead of a full
     # reload of the filament arrays): reported beside the headline e2e figure, not instead of it
@@ -345,7 +414,7 @@ def main():
     te = torch.tensor([time.perf_counter() - t0], device=dev, dtype=torch.float64)
     if dist is not None:
         dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_xy_val = world_size * N * args.e2e_steps / float(te.item())
+    e2e_xy_val = aggregate(N, args.e2e_steps, world_size, float(te.item()) * 1e3)
     G.close()
 
     # short runs of the other large configurations, reported beside the headline (same timing rules:
@@ -379,10 +448,17 @@ def main():
 
     cpu = None
     if rank == 0 and world_size == 1 and not args.no_cpu_baseline:
-        v, cores, n, secs = time_oracle(SAMPLE_WORLD, 0, budget_s=10.0, min_steps=3, max_steps=200)
+        # the oracle on the SAME world: a few whole steps (4d: ~3 s per step on 16 cores), and the
+        # 1/100-size world 4b as a second, labelled sample
+        v, cores, n, secs = time_oracle(args.workload, 0, budget_s=12.0, min_steps=3, max_steps=5 if args.workload == "4d" else 200)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"world {SAMPLE_WORLD} (config-4 recipe at 1/100 of 4d: 100,032 beads, 640x640 grid), "
-                         f"{n} steps in {secs:.1f} s, fp64, OpenMP over {cores} threads"}
+               "sample": f"{world_label(args.workload, w)} (the benchmarked world itself), {n} whole steps in "
+                         f"{secs:.1f} s after 1 warm-up step, fp64, OpenMP over {cores} threads"}
+        if args.workload == "4d":
+            v2, _, n2, secs2 = time_oracle(SAMPLE_WORLD, 0, budget_s=5.0, min_steps=3, max_steps=200)
+            cpu["second_sample"] = {"value": v2, "unit": UNIT,
+                                    "sample": f"world {SAMPLE_WORLD} (config-4 recipe at 1/100 of 4d: 100,032 beads, "
+                                              f"640x640 grid), {n2} steps in {secs2:.1f} s"}
 
     if rank == 0:
         p = w["params"]

@@ -120,6 +120,151 @@ int mco_elastic(int32_t n_fil, const int32_t* offsets, const double* xy,
   return bad ? MCO_ESTATE : MCO_OK;
 }
 
+// Literal PBD (reading 27): "an iterative constraint projection
+// method ... Each iteration decouples the solver into two phases.  First, a bending pass updates
+// theta toward theta_rest.  Second, a position pass enforces nodal connectivity", with
+// the rest angle AND the rest length as time-dependent targets ("The CPPN outputs the rest angle
+// theta_rest and the rest length L_rest"; jellyfish "contractile movement via uniform
+// distance and bending constraints").
+//   iters K >= 1 iterations, each on the working positions Y^k = X + Dtot^k (Y^0 = X):
+//     bending pass: psi_j from Y^k, C_j = psi_j - theta*_j(n), Eq. 1 on all joints at once ->
+//                   delta_e, material director d_e = Rot(delta_e) t_e(Y^k);
+//     position pass, order 0 (Jacobi): Eq. 2-3 on every edge from Y^k, Eq. 4 summed per bead;
+//                    order 1 (red-black Gauss-Seidel): the EVEN edges of each chain (e = 0, 2, ..)
+//                    first, Eq. 4 applied at once; then the ODD edges from the updated positions
+//                    (the directors d_e of the bending pass are kept);
+//   L*_e(n) = L_rest[e] + act_L_amp[e] sin(2 pi n dt / act_period[e] + act_phase[e])  (entry e of
+//   the per-bead arrays serves joint e and edge (e, e+1)); act_L_amp may be NULL (no actuation).
+//   Out: D [N][2] = Dtot^K = Y^K - X, the net displacement of the K iterations.
+// K = 1, order 0, no length actuation reproduces mco_elastic bit for bit (pinned).
+int mco_pbd(int32_t n_fil, const int32_t* offsets, const double* xy, const float* L_rest,
+            const float* theta_rest, const float* k_bend, const float* k_shear,
+            const float* k_stretch, const float* act_amp, const float* act_phase,
+            const float* act_period, const float* act_L_amp, double dt, int64_t n, int32_t iters,
+            int32_t order, double* D) {
+  if (iters < 1 || (order != 0 && order != 1)) return MCO_EINVAL;
+  int bad = 0;
+  MCO_PAR
+  for (int32_t f = 0; f < n_fil; ++f) {
+    const int64_t b0 = offsets[f];
+    const int m = offsets[f + 1] - offsets[f];
+    std::vector<double> yx(m), yy(m), tx(m), ty(m), C(m, 0.0), ddx(m), ddy(m), Ls(m), ths(m, 0.0);
+    std::vector<double> Dx(m, 0.0), Dy(m, 0.0);
+    // S0: targets of step n (the same for all K iterations)
+    for (int i = 0; i < m; ++i) {
+      const double s = std::sin(2.0 * PI * ((double)n * dt) / (double)act_period[b0 + i] + (double)act_phase[b0 + i]);
+      ths[i] = (double)theta_rest[b0 + i] + (double)act_amp[b0 + i] * s;
+      Ls[i] = (double)L_rest[b0 + i] + (act_L_amp ? (double)act_L_amp[b0 + i] * s : 0.0);
+    }
+    // Eq. 2-3 on edge e from the CURRENT working positions and the director (ddx, ddy) of the bending pass
+    auto edge_delta = [&](int e, double& ox, double& oy) {
+      const double vx = yx[e + 1] - yx[e], vy = yy[e + 1] - yy[e];
+      double len = std::sqrt(vx * vx + vy * vy);
+      if (!(len > 1e-12)) { bad = 1; len = 1.0; }
+      const double ux = vx / len, uy = vy / len;
+      const double L = Ls[e];
+      const double csx = (len - L) * ux, csy = (len - L) * uy;   // Eq. 2
+      const double ks = (double)k_shear[b0 + e], kst = (double)k_stretch[b0 + e];
+      ox = 0.5 * kst * (csx + ks * (vx - L * ddx[e] - csx));      // Eq. 3
+      oy = 0.5 * kst * (csy + ks * (vy - L * ddy[e] - csy));
+    };
+    for (int k = 0; k < iters; ++k) {
+      for (int i = 0; i < m; ++i) {
+        yx[i] = xy[2 * (b0 + i)] + Dx[i];
+        yy[i] = xy[2 * (b0 + i) + 1] + Dy[i];
+      }
+      // bending pass (Eq. 1) from Y^k
+      std::vector<double> vx(m), vy(m);
+      for (int e = 0; e + 1 < m; ++e) {
+        vx[e] = yx[e + 1] - yx[e];
+        vy[e] = yy[e + 1] - yy[e];
+        double len = std::sqrt(vx[e] * vx[e] + vy[e] * vy[e]);
+        if (!(len > 1e-12)) { bad = 1; len = 1.0; }
+        tx[e] = vx[e] / len;
+        ty[e] = vy[e] / len;
+      }
+      for (int j = 1; j + 1 < m; ++j) {
+        const double cross = vx[j - 1] * vy[j] - vy[j - 1] * vx[j];
+        const double dot = vx[j - 1] * vx[j] + vy[j - 1] * vy[j];
+        C[j] = std::atan2(cross, dot) - ths[j];
+      }
+      for (int e = 0; e + 1 < m; ++e) {
+        double delta = 0.0;
+        if (e + 1 <= m - 2) delta += 0.5 * (double)k_bend[b0 + e + 1] * C[e + 1];
+        if (e >= 1) delta -= 0.5 * (double)k_bend[b0 + e] * C[e];
+        const double cd = std::cos(delta), sd = std::sin(delta);
+        ddx[e] = cd * tx[e] - sd * ty[e];
+        ddy[e] = sd * tx[e] + cd * ty[e];
+      }
+      if (order == 0) {
+        // Jacobi position pass: all edges from Y^k, Eq. 4 summed per bead
+        std::vector<double> ex(m, 0.0), ey(m, 0.0);
+        for (int e = 0; e + 1 < m; ++e) edge_delta(e, ex[e], ey[e]);
+        for (int i = 0; i < m; ++i) {
+          double sx = 0.0, sy = 0.0;
+          if (i <= m - 2) { sx += ex[i]; sy += ey[i]; }
+          if (i >= 1) { sx -= ex[i - 1]; sy -= ey[i - 1]; }
+          Dx[i] += sx;
+          Dy[i] += sy;
+        }
+      } else {
+        // red-black Gauss-Seidel position pass: even edges, then odd edges on the updated positions
+        for (int colour = 0; colour < 2; ++colour)
+          for (int e = colour; e + 1 < m; e += 2) {
+            double ex, ey;
+            edge_delta(e, ex, ey);
+            Dx[e] += ex;     Dy[e] += ey;          // x1 += dx   (Eq. 4)
+            Dx[e + 1] -= ex; Dy[e + 1] -= ey;      // x2 -= dx
+            yx[e] = xy[2 * (b0 + e)] + Dx[e];             yy[e] = xy[2 * (b0 + e) + 1] + Dy[e];
+            yx[e + 1] = xy[2 * (b0 + e + 1)] + Dx[e + 1]; yy[e + 1] = xy[2 * (b0 + e + 1) + 1] + Dy[e + 1];
+          }
+      }
+    }
+    for (int i = 0; i < m; ++i) {
+      D[2 * (b0 + i)] = Dx[i];
+      D[2 * (b0 + i) + 1] = Dy[i];
+    }
+  }
+  return bad ? MCO_ESTATE : MCO_OK;
+}
+
+// Two-layer broadcast (reading 28): "broadcasting the single filament
+// into a two-layer version of itself to artificially amplify a zero-thickness filament into a
+// solid object".  Every bead i is represented on the grid by two markers
+//   M_i^+- = X_i +- h n_i,   n_i = unit normal of the chain at bead i
+// = the normalised mean of the unit normals (-t_y, t_x) of the adjacent edges (one edge at a chain
+// end); if the two edge normals cancel (a hairpin) the first edge's normal is used.
+// Out: markers [2N][2], marker 2i = M_i^+, 2i+1 = M_i^-.  Every exchange with the grid then uses
+// delta2_h(g; i) = 1/2 [delta_h(g - M_i^+) + delta_h(g - M_i^-)] in place of delta_h(g - X_i).
+void mco_markers(int32_t n_fil, const int32_t* offsets, const double* xy, double h, double* markers) {
+  MCO_PAR
+  for (int32_t f = 0; f < n_fil; ++f) {
+    const int64_t b0 = offsets[f];
+    const int m = offsets[f + 1] - offsets[f];
+    for (int i = 0; i < m; ++i) {
+      double nx_ = 0.0, ny_ = 0.0, n1x = 0.0, n1y = 0.0;
+      for (int e = i - 1; e <= i; ++e) {
+        if (e < 0 || e + 1 >= m) continue;
+        const double vx = xy[2 * (b0 + e + 1)] - xy[2 * (b0 + e)], vy = xy[2 * (b0 + e + 1) + 1] - xy[2 * (b0 + e) + 1];
+        const double len = std::sqrt(vx * vx + vy * vy);
+        const double ex = -vy / len, ey = vx / len;   // edge normal: tangent turned by +90 degrees
+        if (nx_ == 0.0 && ny_ == 0.0 && n1x == 0.0 && n1y == 0.0) { n1x = ex; n1y = ey; }
+        nx_ += ex;
+        ny_ += ey;
+      }
+      double nn = std::sqrt(nx_ * nx_ + ny_ * ny_);
+      if (!(nn > 1e-9)) { nx_ = n1x; ny_ = n1y; nn = 1.0; }
+      nx_ /= nn;
+      ny_ /= nn;
+      const double px = xy[2 * (b0 + i)], py = xy[2 * (b0 + i) + 1];
+      markers[4 * (b0 + i) + 0] = px + h * nx_;
+      markers[4 * (b0 + i) + 1] = py + h * ny_;
+      markers[4 * (b0 + i) + 2] = px - h * nx_;
+      markers[4 * (b0 + i) + 3] = py - h * ny_;
+    }
+  }
+}
+
 // S2 deposit: rho_b(g) = sum_i delta_h(g - X_i), unit weight (reading 13).
 void mco_deposit(int32_t nx, int32_t ny, int64_t N, const double* xy, double* rho_b) {
   for (long long c = 0; c < (long long)nx * ny; ++c) rho_b[c] = 0.0;
@@ -364,6 +509,7 @@ struct mco_world {
   int64_t N = 0;
   std::vector<int32_t> offsets;
   std::vector<float> L_rest, theta_rest, k_bend, k_shear, k_stretch, act_amp, act_phase, act_period;
+  std::vector<float> act_L_amp;  // empty: rest length not actuated
   std::vector<double> X;  // [N][2]
   // fluid
   std::vector<double> f;  // [9][ny][nx], un-shifted, pre-collision
@@ -384,9 +530,13 @@ int mco_create(const mco_world_params* p, mco_world** out) {
   if (!p || !out) return MCO_EINVAL;
   *out = nullptr;
   if (p->nx <= 0 || p->ny <= 0 || !(p->dt > 0) || !(p->nu > 0) || !(p->trt_lambda > 0) ||
-      !(p->rho0 > 0) || p->pbd_iters != 1 || p->n_fields < 0 || p->n_fields > 4 ||
+      !(p->rho0 > 0) || p->pbd_iters < 1 || p->pbd_iters > 8 || p->n_fields < 0 || p->n_fields > 4 ||
       p->max_beads < 0)
     return MCO_EINVAL;
+  if ((p->pbd_order != 0 && p->pbd_order != 1) || (p->pbd_project != 0 && p->pbd_project != 1) ||
+      (p->two_layer != 0 && p->two_layer != 1) || !(p->layer_offset >= 0) || p->layer_offset > 1)
+    return MCO_EINVAL;
+  if (p->two_layer && p->coupling == MCO_COUPLING_MDF) return MCO_EINVAL;  // not defined together (reading 28)
   if (p->coupling != MCO_COUPLING_FORCE && p->coupling != MCO_COUPLING_MDF) return MCO_EINVAL;
   if (p->coupling == MCO_COUPLING_MDF && (p->mdf_iters < 1 || p->mdf_iters > 16)) return MCO_EINVAL;
   for (int k = 0; k < p->n_fields; ++k) {
@@ -465,11 +615,19 @@ int mco_load_filaments(mco_world* w, int32_t n_fil, const int32_t* offsets, cons
   w->act_amp.assign(act_amp, act_amp + N);
   w->act_phase.assign(act_phase, act_phase + N);
   w->act_period.assign(act_period, act_period + N);
+  w->act_L_amp.clear();
   w->X.resize(2 * N);
   for (int64_t i = 0; i < 2 * N; ++i) w->X[i] = (double)xy[i];
   w->D.assign(2 * N, 0.0);
   w->F.assign(2 * N, 0.0);
   w->sense.assign(N, 0.0);
+  return MCO_OK;
+}
+
+int mco_set_length_actuation(mco_world* w, const float* act_L_amp) {
+  if (!w) return MCO_EINVAL;
+  if (act_L_amp) w->act_L_amp.assign(act_L_amp, act_L_amp + w->N);
+  else w->act_L_amp.clear();
   return MCO_OK;
 }
 
@@ -500,11 +658,13 @@ static int mco_one_step(mco_world* w) {
   const size_t nc = w->nc;
   const int64_t N = w->N;
   const double dt2 = w->dt * w->dt;
-  // S0+S1: actuation and elastic displacement D (Eq. 1-4); F_el = kappa * D (reading 1)
-  int rc = mco_elastic(w->n_fil, w->offsets.data(), w->X.data(), w->L_rest.data(),
-                       w->theta_rest.data(), w->k_bend.data(), w->k_shear.data(),
-                       w->k_stretch.data(), w->act_amp.data(), w->act_phase.data(),
-                       w->act_period.data(), w->dt, w->step, w->D.data());
+  const float* Lamp = w->act_L_amp.empty() ? nullptr : w->act_L_amp.data();
+  // S0+S1: actuation and the PBD displacement D of pbd_iters iterations (Eq. 1-4; reading 27;
+  // one Jacobi iteration = reading 3); F_el = kappa * D (reading 1)
+  int rc = mco_pbd(w->n_fil, w->offsets.data(), w->X.data(), w->L_rest.data(), w->theta_rest.data(),
+                   w->k_bend.data(), w->k_shear.data(), w->k_stretch.data(), w->act_amp.data(),
+                   w->act_phase.data(), w->act_period.data(), Lamp, w->dt, w->step, w->p.pbd_iters,
+                   w->p.pbd_order, w->D.data());
   if (rc != MCO_OK) { w->err = "degenerate edge"; return rc; }
   // FORCE coupling: F = kappa D + field forces.  MDF coupling (reading 26): the same sum with
   // kappa = 1 is the bead's own velocity V_i = D_i + field displacement (lattice units, one
@@ -513,8 +673,30 @@ static int mco_one_step(mco_world* w) {
   const double kD = mdf ? 1.0 : w->kappa;
   for (int64_t i = 0; i < 2 * N; ++i) w->F[i] = kD * w->D[i];
   for (int64_t i = 0; i < N; ++i) w->sense[i] = 0.0;
+  // The grid sees every bead through delta_h(g - X_i), or -- two-layer broadcast, reading 28 --
+  // through 1/2 [delta_h(g - M_i^+) + delta_h(g - M_i^-)]: the same X (hence the same markers) in
+  // S2, S4, S5 and S7.
+  const bool two = w->p.two_layer != 0;
+  const int64_t NM = two ? 2 * N : N;
+  std::vector<double> markers;
+  if (two) {
+    markers.resize(4 * (size_t)N);
+    const double h = w->p.layer_offset > 0 ? (double)w->p.layer_offset : 0.5;
+    mco_markers(w->n_fil, w->offsets.data(), w->X.data(), h, markers.data());
+  }
+  const double* P = two ? markers.data() : w->X.data();  // the NM points that touch the grid
+  // sample nch planes at the beads: plain interpolation, or the mean over a bead's two markers
+  auto sample = [&](int nch, const double* planes, double* out) {
+    if (!two) { mco_interp(nx, ny, nch, planes, N, P, out); return; }
+    std::vector<double> tmp((size_t)NM * nch);
+    mco_interp(nx, ny, nch, planes, NM, P, tmp.data());
+    for (int64_t i = 0; i < N; ++i)
+      for (int ch = 0; ch < nch; ++ch)
+        out[i * nch + ch] = 0.5 * (tmp[(2 * i) * nch + ch] + tmp[(2 * i + 1) * nch + ch]);
+  };
   // S2: deposit (one rho_b serves every bead-density field)
-  mco_deposit(nx, ny, N, w->X.data(), w->rho_b.data());
+  mco_deposit(nx, ny, NM, P, w->rho_b.data());
+  if (two) for (size_t c = 0; c < nc; ++c) w->rho_b[c] *= 0.5;
   std::vector<double> gx(nc), gy(nc), samp(2 * (size_t)N), s1((size_t)N);
   std::vector<double> planes(2 * nc);
   for (int k = 0; k < w->p.n_fields; ++k) {
@@ -527,15 +709,15 @@ static int mco_one_step(mco_world* w) {
       mco_grad(nx, ny, &w->field[k * nc], gx.data(), gy.data());
       std::memcpy(&planes[0], gx.data(), nc * sizeof(double));
       std::memcpy(&planes[nc], gy.data(), nc * sizeof(double));
-      mco_interp(nx, ny, 2, planes.data(), N, w->X.data(), samp.data());
+      sample(2, planes.data(), samp.data());
       for (int64_t i = 0; i < 2 * N; ++i) w->F[i] -= coup * samp[i];
     } else {
       // S4: F_chem = +kappa_chi * interp(grad c); s_i = interp(c) (reading 17)
       std::memcpy(&planes[0], &w->static_gx[k * nc], nc * sizeof(double));
       std::memcpy(&planes[nc], &w->static_gy[k * nc], nc * sizeof(double));
-      mco_interp(nx, ny, 2, planes.data(), N, w->X.data(), samp.data());
+      sample(2, planes.data(), samp.data());
       for (int64_t i = 0; i < 2 * N; ++i) w->F[i] += coup * samp[i];
-      mco_interp(nx, ny, 1, &w->field[k * nc], N, w->X.data(), s1.data());
+      sample(1, &w->field[k * nc], s1.data());
       for (int64_t i = 0; i < N; ++i) w->sense[i] += s1[i];
     }
   }
@@ -545,6 +727,12 @@ static int mco_one_step(mco_world* w) {
     mco_moments(nx, ny, w->f.data(), rho.data(), ustar.data());
     mco_mdf(nx, ny, N, w->X.data(), V.data(), ustar.data(), rho.data(), w->rho0, w->p.mdf_iters,
             w->F.data(), w->G.data(), nullptr, nullptr);
+  } else if (two) {
+    // S5, two layers: each marker carries half of its bead's force
+    std::vector<double> FM(2 * (size_t)NM);
+    for (int64_t i = 0; i < N; ++i)
+      for (int c = 0; c < 2; ++c) FM[4 * i + c] = FM[4 * i + 2 + c] = 0.5 * w->F[2 * i + c];
+    mco_spread(nx, ny, NM, P, FM.data(), w->G.data());
   } else {
     // S5: spread the total bead force
     mco_spread(nx, ny, N, w->X.data(), w->F.data(), w->G.data());
@@ -552,8 +740,19 @@ static int mco_one_step(mco_world* w) {
   // S6: fluid update; stores the collision-time velocity u
   mco_lbm_step(nx, ny, w->f.data(), w->G.data(), w->omega_p, w->omega_m, w->u.data());
   // S7: interpolate u at the same X and integrate (forward Euler, lattice units)
-  mco_interp(nx, ny, 2, w->u.data(), N, w->X.data(), samp.data());
+  sample(2, w->u.data(), samp.data());
   for (int64_t i = 0; i < 2 * N; ++i) w->X[i] += samp[i];
+  if (w->p.pbd_project) {
+    // optional projection (reading 27): the constraints of step n act once more, directly on the
+    // advected positions ("directly modifies node positions")
+    std::vector<double> Dp(2 * (size_t)N);
+    rc = mco_pbd(w->n_fil, w->offsets.data(), w->X.data(), w->L_rest.data(), w->theta_rest.data(),
+                 w->k_bend.data(), w->k_shear.data(), w->k_stretch.data(), w->act_amp.data(),
+                 w->act_phase.data(), w->act_period.data(), Lamp, w->dt, w->step, w->p.pbd_iters,
+                 w->p.pbd_order, Dp.data());
+    if (rc != MCO_OK) { w->err = "degenerate edge"; return rc; }
+    for (int64_t i = 0; i < 2 * N; ++i) w->X[i] += Dp[i];
+  }
   w->step += 1;
   if (w->fp32_state) {
     for (int64_t i = 0; i < 2 * N; ++i) w->X[i] = (double)(float)w->X[i];

@@ -60,12 +60,17 @@ typedef struct {
   float trt_lambda;    /* TRT magic parameter Lambda                               */
   float rho0;          /* rest density                                             */
   float k_el;          /* elastic coupling; kappa = k_el*dt^2                      */
-  int32_t pbd_iters;   /* must be 1                                                */
+  int32_t pbd_iters;   /* PBD iterations per step K, 1..8 (reading 27; 1 = reading 3) */
   int32_t n_fields;
   mco_field_params fields[4];
   int64_t max_beads;
   int32_t coupling;    /* MCO_COUPLING_*                                           */
   int32_t mdf_iters;   /* MDF: forcing iterations per step, 1..16 (ignored for FORCE) */
+  int32_t pbd_order;   /* 0 Jacobi, 1 red-black Gauss-Seidel over even/odd edges (reading 27) */
+  int32_t pbd_project; /* 1: after S7 the PBD displacement of the advected positions is added to
+                          them directly ("directly modifies node positions"; reading 27) */
+  int32_t two_layer;   /* 1: two-layer broadcast of every bead (reading 28)      */
+  float layer_offset;  /* half distance h between the two layers, nodes (0 => 0.5)       */
 } mco_world_params;
 
 /* ---- world life cycle (twin of the product ABI, host pointers) ---- */
@@ -76,6 +81,9 @@ int mco_load_filaments(mco_world* w, int32_t n_fil, const int32_t* offsets,
                        const float* xy, const float* L_rest, const float* theta_rest,
                        const float* k_bend, const float* k_shear, const float* k_stretch,
                        const float* act_amp, const float* act_phase, const float* act_period);
+/* rest-length actuation amplitudes act_L_amp [N] (entry e: edge (e, e+1)); NULL switches it off.
+ * Call after mco_load_filaments (which resets it to none). */
+int mco_set_length_actuation(mco_world* w, const float* act_L_amp);
 /* overwrite state: step counter, positions [N][2], populations as deviations
  * f_q - w_q*rho0, planes [9][ny][nx].  NULL pointer = keep. */
 int mco_set_state(mco_world* w, int64_t step, const double* xy, const double* fdev);
@@ -105,6 +113,20 @@ int mco_elastic(int32_t n_fil, const int32_t* offsets, const double* xy,
                 const float* k_shear, const float* k_stretch, const float* act_amp,
                 const float* act_phase, const float* act_period, double dt, int64_t n,
                 double* D);
+/* Literal PBD (reading 27): iters >= 1 iterations of {bending pass Eq. 1, position pass Eq. 2-4}
+ * on working positions, order 0 = Jacobi, 1 = red-black Gauss-Seidel over the even / odd edges of
+ * each chain; rest length actuated like the rest angle when act_L_amp != NULL:
+ * L*_e(n) = L_rest[e] + act_L_amp[e] sin(2 pi n dt/act_period[e] + act_phase[e]).
+ * D out [N][2] = net displacement of the iters iterations.  iters = 1, order = 0, act_L_amp = NULL
+ * gives mco_elastic bit for bit. */
+int mco_pbd(int32_t n_fil, const int32_t* offsets, const double* xy, const float* L_rest,
+            const float* theta_rest, const float* k_bend, const float* k_shear,
+            const float* k_stretch, const float* act_amp, const float* act_phase,
+            const float* act_period, const float* act_L_amp, double dt, int64_t n, int32_t iters,
+            int32_t order, double* D);
+/* Two-layer broadcast (reading 28): markers [2N][2] = X_i + h n_i (entry 2i), X_i - h n_i (2i+1),
+ * n_i the normalised mean of the adjacent edges' unit normals. */
+void mco_markers(int32_t n_fil, const int32_t* offsets, const double* xy, double h, double* markers);
 void mco_deposit(int32_t nx, int32_t ny, int64_t N, const double* xy, double* rho_b);
 void mco_spread(int32_t nx, int32_t ny, int64_t N, const double* xy, const double* F,
                 double* G /*[2][ny][nx]*/);

@@ -26,7 +26,9 @@ class WorldParams(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("dt", C.c_float), ("nu", C.c_float),
                 ("trt_lambda", C.c_float), ("rho0", C.c_float), ("k_el", C.c_float),
                 ("pbd_iters", C.c_int32), ("n_fields", C.c_int32), ("fields", FieldParams * 4),
-                ("max_beads", C.c_int64), ("coupling", C.c_int32), ("mdf_iters", C.c_int32)]
+                ("max_beads", C.c_int64), ("coupling", C.c_int32), ("mdf_iters", C.c_int32),
+                ("pbd_order", C.c_int32), ("pbd_project", C.c_int32), ("two_layer", C.c_int32),
+                ("layer_offset", C.c_float)]
 
 
 _lib = None
@@ -77,6 +79,10 @@ def make_params(p: dict):
     wp.max_beads = int(p["max_beads"])
     wp.coupling = int(p.get("coupling", 0))
     wp.mdf_iters = int(p.get("mdf_iters", 0))
+    wp.pbd_order = int(p.get("pbd_order", 0))
+    wp.pbd_project = int(p.get("pbd_project", 0))
+    wp.two_layer = int(p.get("two_layer", 0))
+    wp.layer_offset = float(p.get("layer_offset", 0.0))
     for i, fd in enumerate(p["fields"]):
         fp = wp.fields[i]
         fp.kind = int(fd["kind"])
@@ -120,6 +126,10 @@ class World:
             L.mco_destroy(h)
             self.h = None
             raise ValueError(f"mco_load_filaments failed: {rc} {msg}")
+        if world.get("act_L_amp") is not None:
+            la = _f32(world["act_L_amp"])
+            assert la.shape == (self.N,)
+            L.mco_set_length_actuation(h, _f(la))
         if fp32_state:
             L.mco_set_fp32_state(h, 1)
         L.mco_set_threads(h, int(threads))
@@ -193,6 +203,33 @@ def elastic(offsets, xy, L_rest, theta_rest, k_bend, k_shear, k_stretch, act_amp
     if rc != 0:
         raise ValueError(f"mco_elastic failed: {rc}")
     return D
+
+
+def pbd(offsets, xy, L_rest, theta_rest, k_bend, k_shear, k_stretch, act_amp, act_phase, act_period,
+        dt: float, n: int, iters: int = 1, order: int = 0, act_L_amp=None) -> np.ndarray:
+    """Literal PBD (reading 27): net displacement of `iters` iterations, Jacobi (0) or red-black GS (1)."""
+    off = np.ascontiguousarray(offsets, dtype=np.int32)
+    xy = _f64(xy)
+    N = int(off[-1])
+    arrs = [_f32(a) for a in (L_rest, theta_rest, k_bend, k_shear, k_stretch, act_amp, act_phase,
+                              act_period)]
+    la = None if act_L_amp is None else _f32(act_L_amp)
+    D = np.empty((N, 2))
+    rc = lib().mco_pbd(C.c_int32(len(off) - 1), off.ctypes.data_as(_ip), _d(xy),
+                       *[_f(a) for a in arrs], _f(la), C.c_double(dt), C.c_int64(n), C.c_int32(iters),
+                       C.c_int32(order), _d(D))
+    if rc != 0:
+        raise ValueError(f"mco_pbd failed: {rc}")
+    return D
+
+
+def markers(offsets, xy, h: float) -> np.ndarray:
+    """Two-layer markers (reading 28): [2N, 2], rows 2i / 2i+1 = X_i +- h n_i."""
+    off = np.ascontiguousarray(offsets, dtype=np.int32)
+    xy = _f64(xy)
+    out = np.empty((2 * len(xy), 2))
+    lib().mco_markers(C.c_int32(len(off) - 1), off.ctypes.data_as(_ip), _d(xy), C.c_double(h), _d(out))
+    return out
 
 
 def deposit(nx, ny, xy) -> np.ndarray:

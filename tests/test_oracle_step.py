@@ -124,9 +124,12 @@ def test_load_validation():
     bad = dict(w, offsets=np.array([0, 2, 16], np.int32))
     with pytest.raises(ValueError):
         mco.World(bad)
-    bad = dict(w, params=dict(w["params"], pbd_iters=2))
-    with pytest.raises(ValueError):
-        mco.World(bad)
+    for key, val in (("pbd_iters", 0), ("pbd_iters", 9), ("pbd_order", 2), ("pbd_project", 3),
+                     ("two_layer", 2), ("layer_offset", 1.5)):
+        bad = dict(w, params=dict(w["params"], **{key: val}))
+        with pytest.raises(ValueError):
+            mco.World(bad)
+    mco.World(dict(w, params=dict(w["params"], pbd_iters=2, pbd_order=1))).close()
 
 
 # ------------------------------------------------------------------ scallop theorem

@@ -61,6 +61,11 @@ enum {
   MC_COUPLING_MDF = 1    /* bead velocity imposed by iterated direct forcing (reading 26)          */
 };
 
+enum {
+  MC_PBD_JACOBI = 0,      /* every constraint of an iteration from the same state (reading 3)        */
+  MC_PBD_GAUSS_SEIDEL = 1 /* position pass over the even, then the odd edges of each chain (reading 27) */
+};
+
 typedef struct {
   int32_t kind;         /* MC_FIELD_*                                                     */
   float sigma;          /* Gaussian filter width in cells (bead-density fields), > 0       */
@@ -77,7 +82,9 @@ typedef struct {
   float trt_lambda;  /* TRT magic parameter Lambda (> 0), 0.25 is the usual choice         */
   float rho0;        /* rest density of the fluid (> 0), 1.0                               */
   float k_el;        /* elastic coupling, 1/time^2; kappa = k_el*dt^2 (reading 1)          */
-  int32_t pbd_iters; /* must be 1 (reading 3)                                              */
+  int32_t pbd_iters; /* PBD iterations per step K, 1..8: each a bending pass (Eq. 1) then a
+                        position pass (Eq. 2-4) on the positions the previous ones produced
+                        (reading 27).  1 = reading 3, the configuration of BASELINE.json */
   int32_t n_fields;  /* 0..4                                                               */
   mc_field_params fields[4];
   int64_t max_beads; /* capacity; mc_load_filaments may load up to this many beads         */
@@ -85,6 +92,15 @@ typedef struct {
   int32_t mdf_iters; /* MDF: forcing iterations per step, 1..16 (ignored for FORCE).  The
                         iteration contracts while the bead density interpolated at every bead
                         stays below 4 (chains ~1 node apart, a few overlapping)            */
+  int32_t pbd_order; /* MC_PBD_JACOBI (default) or MC_PBD_GAUSS_SEIDEL                     */
+  int32_t pbd_project; /* 1: after S7 the PBD displacement of the advected positions (same targets
+                        as the step) is added to them directly: "PBD ... directly modifies node
+                        positions" (reading 27).  0 (default): only through the fluid  */
+  int32_t two_layer; /* 1: two-layer broadcast (reading 28): every exchange of a bead with
+                        the grid (S2, S4, S5, S7) goes through its two markers X_i +- h n_i with
+                        weight 1/2 each, n_i the unit normal of the chain at the bead.  Not
+                        defined together with MC_COUPLING_MDF                               */
+  float layer_offset; /* h, half the distance between the two layers, in nodes; 0 => 0.5; <= 1 */
 } mc_world_params;
 
 /* Bytes of DEVICE workspace mc_create needs for these parameters (0 if they are invalid). */
@@ -126,6 +142,14 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets /*HOST*
                       const float* k_shear /*DEVICE*/, const float* k_stretch /*DEVICE*/,
                       const float* act_amp /*DEVICE*/, const float* act_phase /*DEVICE*/,
                       const float* act_period /*DEVICE*/);
+
+/* Time-dependent rest LENGTH ("The CPPN outputs the rest angle theta_rest and the rest length
+ * L_rest"; P:L153 jellyfish "contractile movement"; reading 27):
+ *   L*_e(n) = L_rest[e] + act_L_amp[e] * sin(2*pi*n*dt/act_period[e] + act_phase[e])
+ * with the period and phase of entry e (the entry that serves joint e and edge (e, e+1)).
+ * act_L_amp: DEVICE float [N], chain-ordered, or NULL to switch the actuation off.  Call after
+ * mc_load_filaments (a load resets it to none).  Synchronises the stream. */
+int mc_set_length_actuation(mc_world* w, const float* act_L_amp /*DEVICE*/);
 
 /* Replace the bead positions of the loaded filaments and keep everything else (parameters, fluid,
  * step counter).  xy: DEVICE float [N][2], chain-ordered like mc_load_filaments.  The next step
@@ -204,6 +228,38 @@ int mc_profile_read(mc_world* w, float* ms /*HOST*/, int32_t* steps /*HOST*/);
 
 /* Kernels launched on the world's stream since mc_create (a plain host counter). */
 int64_t mc_launch_count(const mc_world* w);
+
+/* ---- batched worlds --------------------------------------------------------
+ * The paper's workload is a population of small worlds stepped in lock-step ("large
+ * populations ... over evolutionary timescales"; P:L173-179 NEAT / MAP-Elites; P:L190 256 x 256
+ * grids): singly such a world is bound by kernel-launch overhead.  A batch holds n_worlds worlds of
+ * IDENTICAL parameters and chain structure (offsets) -- positions and per-bead parameters differ --
+ * and launches every kernel of the step once for all of them.  World k of a batch computes exactly
+ * what the same world computes alone through mc_step, bit for bit.
+ *
+ * workspace: DEVICE, mc_batch_workspace_bytes(p, n_worlds) = n_worlds * mc_workspace_bytes(p) bytes,
+ * 256-byte aligned, owned by the caller; world k lives at offset k * mc_workspace_bytes(p).
+ * mc_load_filaments_batch: offsets HOST int32 [n_fil+1] shared by all worlds; every other array is
+ * DEVICE float [n_worlds][N] ([n_worlds][N][2] for xy), world-major; act_L_amp may be NULL.
+ * mc_batch_world(b, k): the handle of world k, valid until mc_destroy_batch, for mc_read_state,
+ * mc_read_intermediates, mc_set_positions, mc_last_error and the switches; mc_step,
+ * mc_load_filaments and mc_set_length_actuation on it return MC_ESTATE (the batch steps together).
+ * Errors as for the single-world calls; mc_batch_last_error gives the message (b == NULL: of the
+ * last failed mc_create_batch on this thread). */
+typedef struct mc_batch mc_batch;
+size_t mc_batch_workspace_bytes(const mc_world_params* p /*HOST*/, int32_t n_worlds);
+int mc_create_batch(const mc_world_params* p /*HOST*/, int32_t n_worlds, void* workspace /*DEVICE*/,
+                    size_t workspace_bytes, void* cuda_stream, mc_batch** out /*HOST*/);
+int mc_load_filaments_batch(mc_batch* b, int32_t n_fil, const int32_t* offsets /*HOST*/,
+                            const float* xy /*DEVICE*/, const float* L_rest /*DEVICE*/,
+                            const float* theta_rest /*DEVICE*/, const float* k_bend /*DEVICE*/,
+                            const float* k_shear /*DEVICE*/, const float* k_stretch /*DEVICE*/,
+                            const float* act_amp /*DEVICE*/, const float* act_phase /*DEVICE*/,
+                            const float* act_period /*DEVICE*/, const float* act_L_amp /*DEVICE or NULL*/);
+int mc_step_batch(mc_batch* b, int32_t n);
+mc_world* mc_batch_world(mc_batch* b, int32_t k);
+void mc_destroy_batch(mc_batch* b);
+const char* mc_batch_last_error(const mc_batch* b);
 
 /* Frees the host handle only (the workspace belongs to the caller).  NULL is allowed. */
 void mc_destroy(mc_world* w);

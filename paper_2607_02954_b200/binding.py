@@ -18,7 +18,9 @@ MC_OK, MC_EINVAL, MC_ENOMEM, MC_ECUDA, MC_ESTATE, MC_EDIVERGED = 0, -1, -2, -3, 
 SYMBOLS = ("mc_workspace_bytes", "mc_create", "mc_load_filaments", "mc_step", "mc_read_state",
            "mc_read_intermediates", "mc_launch_count", "mc_destroy", "mc_last_error",
            "mc_profile_enable", "mc_profile_read", "mc_keep_intermediates", "mc_texture_gathers",
-           "mc_cluster_tiles", "mc_set_positions")
+           "mc_cluster_tiles", "mc_set_positions", "mc_set_length_actuation", "mc_batch_workspace_bytes",
+           "mc_create_batch", "mc_load_filaments_batch", "mc_step_batch", "mc_batch_world", "mc_destroy_batch",
+           "mc_batch_last_error")
 PROF_SLOTS = ("K0_bin", "K2a_deposit", "K3a_blur_grad", "K1_filament", "K2b_spread", "K3b_lbm",
               "K4_interp_integrate")
 
@@ -34,7 +36,9 @@ class WorldParams(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("dt", C.c_float), ("nu", C.c_float),
                 ("trt_lambda", C.c_float), ("rho0", C.c_float), ("k_el", C.c_float),
                 ("pbd_iters", C.c_int32), ("n_fields", C.c_int32), ("fields", FieldParams * 4),
-                ("max_beads", C.c_int64), ("coupling", C.c_int32), ("mdf_iters", C.c_int32)]
+                ("max_beads", C.c_int64), ("coupling", C.c_int32), ("mdf_iters", C.c_int32),
+                ("pbd_order", C.c_int32), ("pbd_project", C.c_int32), ("two_layer", C.c_int32),
+                ("layer_offset", C.c_float)]
 
 
 class McError(RuntimeError):
@@ -83,6 +87,22 @@ def load_library():
     L.mc_set_positions.argtypes = [vp, vp]
     L.mc_cluster_tiles.restype = C.c_int
     L.mc_cluster_tiles.argtypes = [vp, i32]
+    L.mc_set_length_actuation.restype = C.c_int
+    L.mc_set_length_actuation.argtypes = [vp, vp]
+    L.mc_batch_workspace_bytes.restype = C.c_size_t
+    L.mc_batch_workspace_bytes.argtypes = [C.POINTER(WorldParams), i32]
+    L.mc_create_batch.restype = C.c_int
+    L.mc_create_batch.argtypes = [C.POINTER(WorldParams), i32, vp, C.c_size_t, vp, C.POINTER(vp)]
+    L.mc_load_filaments_batch.restype = C.c_int
+    L.mc_load_filaments_batch.argtypes = [vp, i32, C.POINTER(i32)] + [vp] * 10
+    L.mc_step_batch.restype = C.c_int
+    L.mc_step_batch.argtypes = [vp, i32]
+    L.mc_batch_world.restype = vp
+    L.mc_batch_world.argtypes = [vp, i32]
+    L.mc_destroy_batch.restype = None
+    L.mc_destroy_batch.argtypes = [vp]
+    L.mc_batch_last_error.restype = C.c_char_p
+    L.mc_batch_last_error.argtypes = [vp]
     L.mc_destroy.restype = None
     L.mc_destroy.argtypes = [vp]
     L.mc_last_error.restype = C.c_char_p
@@ -103,6 +123,10 @@ def make_params(p: dict):
     wp.max_beads = int(p["max_beads"])
     wp.coupling = int(p.get("coupling", 0))
     wp.mdf_iters = int(p.get("mdf_iters", 0))
+    wp.pbd_order = int(p.get("pbd_order", 0))
+    wp.pbd_project = int(p.get("pbd_project", 0))
+    wp.two_layer = int(p.get("two_layer", 0))
+    wp.layer_offset = float(p.get("layer_offset", 0.0))
     for i, fd in enumerate(p["fields"][:4]):
         fp = wp.fields[i]
         fp.kind, fp.sigma = int(fd["kind"]), float(fd["sigma"])
@@ -131,7 +155,7 @@ _CHAIN_KEYS = ("xy", "L_rest", "theta_rest", "k_bend", "k_shear", "k_stretch", "
 class World:
     """mc_create + mc_load_filaments from a worlds.py dict; mc_step; mc_read_state."""
 
-    def __init__(self, world: dict, device: str = "cuda:0", stream=None):
+    def __init__(self, world: dict, device: str = "cuda:0", stream=None, _member=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2607_02954_b200 needs a CUDA device (no CPU fallback)")
@@ -142,6 +166,11 @@ class World:
         self.nx, self.ny = int(self.p["nx"]), int(self.p["ny"])
         self.n_fields = len(self.p["fields"])
         self.h = None
+        self.owned = _member is None
+        if _member is not None:  # world k of a Batch: the batch owns the handle, the workspace and the stream
+            self.h, self.stream, self.N = _member
+            self.workspace = None
+            return
         with torch.cuda.device(self.device):
             # a stream of its own: the legacy default stream cannot be captured into CUDA graphs
             self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
@@ -176,6 +205,23 @@ class World:
                 *[C.c_void_p(t.data_ptr()) for t in dev])
         self._check(rc)
         self.N = int(off[-1])
+        if world.get("act_L_amp") is not None:
+            self.set_length_actuation(world["act_L_amp"])
+
+    def set_length_actuation(self, act_L_amp):
+        """mc_set_length_actuation: [N] host numpy array or device tensor (None switches it off)."""
+        torch = self.torch
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):
+            if act_L_amp is None:
+                rc = load_library().mc_set_length_actuation(self.h, None)
+            else:
+                a = act_L_amp
+                if not isinstance(a, torch.Tensor):
+                    a = torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32))
+                d = a.to(self.device, dtype=torch.float32).contiguous()
+                assert d.numel() == self.N
+                rc = load_library().mc_set_length_actuation(self.h, C.c_void_p(d.data_ptr()))
+        self._check(rc)
 
     def set_positions(self, xy):
         """mc_set_positions: xy [N,2] host numpy array or device tensor, caller's bead order."""
@@ -253,8 +299,84 @@ class World:
 
     def close(self):
         if getattr(self, "h", None):
+            if self.owned:
+                self.torch.cuda.synchronize(self.device)
+                load_library().mc_destroy(self.h)
+            self.h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Batch:
+    """mc_create_batch + mc_load_filaments_batch from a list of worlds.py dicts that share their
+    parameters and chain structure (offsets); mc_step_batch; world(k) -> a World view for read-outs."""
+
+    def __init__(self, worlds: list, device: str = "cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2607_02954_b200 needs a CUDA device (no CPU fallback)")
+        L = load_library()
+        self.torch = torch
+        self.device = torch.device(device)
+        self.p = worlds[0]["params"]
+        self.n = len(worlds)
+        self.h = None
+        off = np.ascontiguousarray(worlds[0]["offsets"], dtype=np.int32)
+        for w in worlds[1:]:
+            if not np.array_equal(np.asarray(w["offsets"]), off):
+                raise ValueError("the worlds of a batch must share their chain structure (offsets)")
+        self.N = int(off[-1])
+        with torch.cuda.device(self.device):
+            self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
+            wp, keep = make_params(self.p)
+            nbytes = int(L.mc_batch_workspace_bytes(C.byref(wp), self.n))
+            if nbytes == 0:
+                raise McError(MC_EINVAL, "invalid world parameters or batch size")
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            h = C.c_void_p()
+            rc = L.mc_create_batch(C.byref(wp), self.n, self.workspace.data_ptr(), nbytes,
+                                   C.c_void_p(self.stream.cuda_stream), C.byref(h))
+            if rc != MC_OK:
+                raise McError(rc, L.mc_batch_last_error(None).decode())
+            self.h = h
+            with torch.cuda.stream(self.stream):
+                dev = []
+                for k in _CHAIN_KEYS:
+                    a = np.stack([np.ascontiguousarray(w[k], dtype=np.float32) for w in worlds])
+                    dev.append(torch.from_numpy(a).to(self.device).contiguous())
+                la = None
+                if any(w.get("act_L_amp") is not None for w in worlds):
+                    la = torch.from_numpy(np.stack([
+                        np.ascontiguousarray(w["act_L_amp"] if w.get("act_L_amp") is not None else np.zeros(self.N),
+                                             dtype=np.float32) for w in worlds])).to(self.device).contiguous()
+                rc = L.mc_load_filaments_batch(
+                    self.h, len(off) - 1, off.ctypes.data_as(C.POINTER(C.c_int32)),
+                    *[C.c_void_p(t.data_ptr()) for t in dev], C.c_void_p(la.data_ptr()) if la is not None else None)
+            self._check(rc)
+        self._worlds = worlds
+
+    def step(self, n: int = 1):
+        self._check(load_library().mc_step_batch(self.h, int(n)))
+
+    def world(self, k: int) -> "World":
+        h = load_library().mc_batch_world(self.h, int(k))
+        if not h:
+            raise IndexError(k)
+        return World(self._worlds[k], device=str(self.device), _member=(C.c_void_p(h), self.stream, self.N))
+
+    def _check(self, rc: int):
+        if rc != MC_OK:
+            raise McError(rc, load_library().mc_batch_last_error(self.h).decode())
+
+    def close(self):
+        if getattr(self, "h", None):
             self.torch.cuda.synchronize(self.device)
-            load_library().mc_destroy(self.h)
+            load_library().mc_destroy_batch(self.h)
             self.h = None
             self.workspace = None
 

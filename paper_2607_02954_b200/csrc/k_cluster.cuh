@@ -48,8 +48,13 @@ template <int C>
 __global__ void __cluster_dims__(C, 1, 1) __launch_bounds__(256)
     k_deposit_tile_cl(int nx, int ny, const int* __restrict__ tile_start, const int* __restrict__ list,
                       const float2* __restrict__ X, float* __restrict__ rho_b, float* __restrict__ tile_rho_max,
-                      unsigned* __restrict__ tile_fmax) {
+                      unsigned* __restrict__ tile_fmax, size_t wstride) {
   __shared__ __align__(16) int acc[ACC_N], accl[ACC_N];
+  {
+    const size_t ws = blockIdx.y * wstride;
+    tile_start = wshift(tile_start, ws); list = wshift(list, ws); X = wshift(X, ws); rho_b = wshift(rho_b, ws);
+    tile_rho_max = wshift(tile_rho_max, ws); tile_fmax = wshift(tile_fmax, ws);
+  }
   cg::cluster_group cl = cg::this_cluster();
   const int rank = (int)cl.block_rank();
   const int t = blockIdx.x / C, ntx = nx / TS;
@@ -98,9 +103,10 @@ __global__ void __cluster_dims__(C, 1, 1) __launch_bounds__(256)
 // K2b + K3b with C CTAs per tile.  grid = n_tiles * C (1-D, cluster-major), 256 threads; the
 // threads with ry < TS/C run S6 on the node pairs of this CTA's rows.
 template <int C, bool KEEP_G>
-__global__ void __cluster_dims__(C, 1, 1) __launch_bounds__(256) k_lbm_spread_tile_cl(LbmSpreadArgs p) {
+__global__ void __cluster_dims__(C, 1, 1) __launch_bounds__(256) k_lbm_spread_tile_cl(LbmSpreadArgs p, size_t wstride) {
   __shared__ __align__(16) int acc0[ACC_N], acc1[ACC_N], accl0[ACC_N], accl1[ACC_N];
   __shared__ float red[32];
+  p.shift(blockIdx.y * wstride);
   cg::cluster_group cl = cg::this_cluster();
   const int rank = (int)cl.block_rank();
   const LbmArgs& a = p.lbm;

@@ -29,6 +29,7 @@
 namespace mc {
 
 constexpr int BEAD_FIRST = 1, BEAD_LAST = 2, BEAD_PAD = 4;
+constexpr int BEAD_ODD = 8;  // odd index within its chain (edge parity of the Gauss-Seidel pass, k_pbd.cuh)
 
 struct FilamentArgs {
   const float2* X;   // [N]
@@ -49,6 +50,13 @@ struct FilamentArgs {
   int n_windows;
   float kappa;       // k_el * dt^2
   const long long* step;  // DEVICE: step index n (before the increment); K4 increments it
+  // batched worlds: move every workspace pointer to world `blockIdx.y` (mc_common.cuh wshift)
+  __device__ __forceinline__ void shift(size_t bytes) {
+    X = wshift(X, bytes); PA = wshift(PA, bytes); PB = wshift(PB, bytes); PC = wshift(PC, bytes);
+    PD = wshift(PD, bytes); uni = wshift(uni, bytes); F = wshift(F, bytes); sense = wshift(sense, bytes);
+    A = wshift(A, bytes); csum = wshift(csum, bytes); tile_fmax = wshift(tile_fmax, bytes);
+    step = wshift(step, bytes);
+  }
 };
 
 struct BeadParams {
@@ -158,7 +166,8 @@ __device__ __forceinline__ float2 edge_delta(double vx, double vy, float delta, 
 }
 
 template <bool UNIFORM, int TEXROWS>
-__global__ void __launch_bounds__(256, 5) k_filament_force(FilamentArgs a) {
+__global__ void __launch_bounds__(256, 5) k_filament_force(FilamentArgs a, size_t wstride) {
+  if (!TEXROWS) a.shift(blockIdx.y * wstride);  // the texture variants serve single worlds only (views are per world)
   const int lane = threadIdx.x & 31;
   const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (w >= a.n_windows) return;
@@ -311,6 +320,15 @@ __global__ void k_unpermute2(int N, const int* __restrict__ src, const float2* _
 __global__ void k_permute2(int N, const int* __restrict__ src, const float2* __restrict__ in, float2* __restrict__ out) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b < N) out[b] = in[src[b]];
+}
+__global__ void k_permute1(int N, const int* __restrict__ src, const float* __restrict__ in, float* __restrict__ out,
+                           int* __restrict__ nonzero) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b < N) {
+    const float v = in[src[b]];
+    out[b] = v;
+    if (v != 0.0f) *nonzero = 1;  // every writer stores the same value
+  }
 }
 __global__ void k_unpermute1(int N, const int* __restrict__ src, const float* __restrict__ in, float* __restrict__ out) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;

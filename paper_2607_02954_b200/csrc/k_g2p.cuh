@@ -7,18 +7,33 @@
 
 namespace mc {
 
+// O != NULL (two-layer broadcast, reading 28; TEXROWS = 0): U_i is the mean of u sampled at the
+// bead's two markers X_i +- O_i, the adjoint of the two-layer spread.
 template <int TEXROWS>
 __global__ void __launch_bounds__(256) k_interp_integrate(int N, float2* __restrict__ X,
                                                           const float2* __restrict__ u, cudaTextureObject_t tex_u,
                                                           int nx, int ny,
                                                           int* __restrict__ flag, long long* __restrict__ step,
-                                                          unsigned* __restrict__ step_max) {
+                                                          unsigned* __restrict__ step_max,
+                                                          const float2* __restrict__ O, size_t wstride) {
+  if (!TEXROWS) {  // the texture variants serve single worlds only (views are per world)
+    const size_t ws = blockIdx.y * wstride;
+    X = wshift(X, ws); u = wshift(u, ws); flag = wshift(flag, ws); step = wshift(step, ws);
+    step_max = wshift(step_max, ws); O = wshift(O, ws);
+  }
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b == 0) *step += 1;  // device copy of the step counter (K1 of the next step reads it)
   float m = 0.0f;
   if (b < N) {
     float2 p = X[b];
-    const float2 U = TEXROWS ? interp2_tex<TEXROWS, false>(u, tex_u, nx, ny, p.x, p.y) : interp2(u, nx, ny, p.x, p.y);
+    float2 U;
+    if (!TEXROWS && O) {
+      const float2 o = __ldg(O + b);
+      const float2 up = interp2_off(u, nx, ny, p.x, p.y, o.x, o.y), um = interp2_off(u, nx, ny, p.x, p.y, -o.x, -o.y);
+      U = make_float2(0.5f * (up.x + um.x), 0.5f * (up.y + um.y));
+    } else {
+      U = TEXROWS ? interp2_tex<TEXROWS, false>(u, tex_u, nx, ny, p.x, p.y) : interp2(u, nx, ny, p.x, p.y);
+    }
     p.x += U.x;
     p.y += U.y;
     X[b] = p;

@@ -47,6 +47,10 @@ struct LbmArgs {
   float rho0;
   TrtConst k;         // collision constants (host, mc_api.cu)
   int* flag;          // sticky divergence flag (bit 2: |u| > 0.3 or non-finite)
+  __device__ __forceinline__ void shift(size_t bytes) {  // batched worlds (mc_common.cuh wshift)
+    src = wshift(src, bytes); dst = wshift(dst, bytes); G0 = wshift(G0, bytes); G1 = wshift(G1, bytes);
+    G0out = wshift(G0out, bytes); G1out = wshift(G1out, bytes); u = wshift(u, bytes); flag = wshift(flag, bytes);
+  }
 };
 
 // One TRT collision of a node given its pre-collision shifted populations g[9].
@@ -90,7 +94,8 @@ __device__ __forceinline__ void trt_collide(float g[9], float Gx, float Gy, floa
 #undef MC_PAIR
 }
 
-__global__ void __launch_bounds__(256) k_lbm_step(LbmArgs a) {
+__global__ void __launch_bounds__(256) k_lbm_step(LbmArgs a, size_t wstride) {
+  a.shift(blockIdx.z * wstride);  // grid = (nx / bx, ny, worlds)
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y;
   const int nx = a.nx, ny = a.ny;
@@ -132,12 +137,19 @@ struct LbmSpreadArgs {
   const float2* F;
   float* tile_rho_max;        // may be NULL; read, then reset to 0 for the next step's S2 (atomicMax)
   const unsigned* tile_fmax;  // may be NULL
+  const float2* O;            // two-layer marker offsets (TWO variants), else NULL
+  __device__ __forceinline__ void shift(size_t bytes) {
+    lbm.shift(bytes);
+    tile_start = wshift(tile_start, bytes); list = wshift(list, bytes); X = wshift(X, bytes); F = wshift(F, bytes);
+    tile_rho_max = wshift(tile_rho_max, bytes); tile_fmax = wshift(tile_fmax, bytes); O = wshift(O, bytes);
+  }
 };
 
-template <bool KEEP_G>
-__global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
+template <bool KEEP_G, bool TWO = false>
+__global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p, size_t wstride) {
   __shared__ __align__(16) int acc0[ACC_N], acc1[ACC_N], accl0[ACC_N], accl1[ACC_N];
   __shared__ float red[32];
+  p.shift(blockIdx.y * wstride);
   const LbmArgs& a = p.lbm;
   const int nx = a.nx, ny = a.ny;
   // 1-D grid in row-major tile order (a 2-D grid is rasterised differently by the hardware and
@@ -157,15 +169,16 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p) {
   }
   // this thread's first list entry: its list -> X/F gather is the longest latency chain of the
   // tile, so it starts before the zeroing and the barrier of the atomic phase
-  float2 xpre = make_float2(0.f, 0.f), fpre = make_float2(0.f, 0.f);
+  float2 xpre = make_float2(0.f, 0.f), fpre = make_float2(0.f, 0.f), opre = make_float2(0.f, 0.f);
   {
     const int b = first_entry(s, e, p.list);
-    if (b >= 0) { xpre = __ldg(p.X + b); fpre = __ldg(p.F + b); }
+    if (b >= 0) { load_point<TWO>(p.X, p.O, b, xpre, opre); fpre = __ldg(p.F + (TWO ? b >> 1 : b)); }
   }
   float linv;
-  const float scale = spread_tile_accumulate(nx, ny, x0, y0, s, e, p.list, p.X, p.F,
-                                             p.tile_rho_max ? p.tile_rho_max[t] : 0.0f, p.tile_fmax, t, acc0, acc1,
-                                             accl0, accl1, red, linv, xpre, fpre);
+  const float scale = spread_tile_accumulate<false, TWO>(nx, ny, x0, y0, s, e, p.list, p.X, p.F,
+                                                         p.tile_rho_max ? p.tile_rho_max[t] : 0.0f, p.tile_fmax, t,
+                                                         acc0, acc1, accl0, accl1, red, linv, xpre, fpre, DealCfg(),
+                                                         p.O, opre);
   const float inv = 1.0f / scale;
   if (threadIdx.x == 0 && p.tile_rho_max) p.tile_rho_max[t] = 0.0f;  // all reads happened before the barrier
   // S6 on the tile: each thread owns the node PAIR (i, i+1), i even, in rows ry and ry + 16.

@@ -24,7 +24,10 @@ namespace mc {
 // float2 layout K5b/K4 gather from; hrinv = 1/(2 rho), row-major.  Two nodes (i, i+1), i even,
 // per thread: 8-byte loads of the unshifted planes and one 16-byte u store.
 __global__ void __launch_bounds__(256) k_lbm_moments(const float* __restrict__ src, int nx, int ny, float rho0,
-                                                     float2* __restrict__ u, float* __restrict__ hrinv) {
+                                                     float2* __restrict__ u, float* __restrict__ hrinv, size_t wstride) {
+  src = wshift(src, blockIdx.z * wstride);  // grid = (nx / (2 bx), ny, worlds)
+  u = wshift(u, blockIdx.z * wstride);
+  hrinv = wshift(hrinv, blockIdx.z * wstride);
   const int i = (blockIdx.x * blockDim.x + threadIdx.x) << 1;
   const int j = blockIdx.y;
   if (i >= nx) return;
@@ -74,7 +77,13 @@ template <bool FIRST, bool LAST, int TEXROWS>
 __global__ void __launch_bounds__(256) k_mdf_force(int N, const float2* __restrict__ X, const float2* __restrict__ V,
                                                    const float2* __restrict__ u, cudaTextureObject_t tex_u, int nx,
                                                    int ny, float rho0, float2* __restrict__ dF,
-                                                   float2* __restrict__ F, unsigned* __restrict__ tile_fmax) {
+                                                   float2* __restrict__ F, unsigned* __restrict__ tile_fmax,
+                                                   size_t wstride) {
+  {
+    const size_t ws = blockIdx.y * wstride;
+    X = wshift(X, ws); V = wshift(V, ws); u = wshift(u, ws); dF = wshift(dF, ws); F = wshift(F, ws);
+    tile_fmax = wshift(tile_fmax, ws);
+  }
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = b < N;  // every lane stays for the warp-wide reduction
   const float2 p = X[valid ? b : N - 1];
@@ -109,9 +118,16 @@ __global__ void __launch_bounds__(256, 5) k_mdf_spread_tile(int nx, int ny, cons
                                                             const float2* __restrict__ dF,
                                                             const float* __restrict__ tile_rho_max,
                                                             const unsigned* __restrict__ tile_fmax,
-                                                            const float* __restrict__ hrinv, float2* __restrict__ u) {
+                                                            const float* __restrict__ hrinv, float2* __restrict__ u,
+                                                            size_t wstride) {
   __shared__ __align__(16) int acc0[ACC_N], acc1[ACC_N], accl0[ACC_N], accl1[ACC_N];
   __shared__ float red[32];
+  {
+    const size_t ws = blockIdx.y * wstride;
+    tile_start = wshift(tile_start, ws); list = wshift(list, ws); X = wshift(X, ws); dF = wshift(dF, ws);
+    tile_rho_max = wshift(tile_rho_max, ws); tile_fmax = wshift(tile_fmax, ws); hrinv = wshift(hrinv, ws);
+    u = wshift(u, ws);
+  }
   const int t = blockIdx.x, ntx = nx / TS;
   const int s = tile_start[t], e = tile_start[t + 1];
   if (s == e) return;  // nothing reaches this tile: u^{k+1} = u^k

@@ -75,12 +75,19 @@ __device__ __forceinline__ int tile_delta(int i0, int origin, int n) {
 // WRAP_IN_TILE: the domain is a single tile wide along some axis, so a support can wrap around
 // onto the SAME tile; then every node is folded individually.  Otherwise one periodic fold of the
 // first support node is enough and the other three follow by +1.
-template <bool WRAP_IN_TILE>
-__device__ __forceinline__ void tile_bead(float2 p, int nx, int ny, int x0, int y0, TileBead& tb) {
+// TWO (two-layer broadcast, reading 28): the point is the marker p + o; its support is formed
+// from the bead's exact fractional part plus the offset (support_off, mc_common.cuh).
+template <bool WRAP_IN_TILE, bool TWO = false>
+__device__ __forceinline__ void tile_bead(float2 p, float2 o, int nx, int ny, int x0, int y0, TileBead& tb) {
   int i0, j0;
   float fx, fy;
-  support(p.x, i0, fx);
-  support(p.y, j0, fy);
+  if (TWO) {
+    support_off(p.x, o.x, i0, fx);
+    support_off(p.y, o.y, j0, fy);
+  } else {
+    support(p.x, i0, fx);
+    support(p.y, j0, fy);
+  }
   peskin4(fx, tb.wx[0], tb.wx[1], tb.wx[2], tb.wx[3]);
   peskin4(fy, tb.wy[0], tb.wy[1], tb.wy[2], tb.wy[3]);
   if (WRAP_IN_TILE) {
@@ -166,20 +173,36 @@ struct Deal {
   __device__ __forceinline__ void advance() { v += nw; p += nw; }
 };
 
-template <bool WIDE, bool WRAP>
+// A list entry e names bead e -- or, TWO, marker e: bead e >> 1, offset +O (e even) / -O (e odd).
+template <bool TWO>
+__device__ __forceinline__ void load_point(const float2* __restrict__ X, const float2* __restrict__ O, int e, float2& p,
+                                           float2& o) {
+  if (TWO) {
+    p = __ldg(X + (e >> 1));
+    o = __ldg(O + (e >> 1));
+    if (e & 1) { o.x = -o.x; o.y = -o.y; }
+  } else {
+    p = __ldg(X + e);
+    o = make_float2(0.f, 0.f);
+  }
+}
+
+template <bool WIDE, bool WRAP, bool TWO = false>
 __device__ __forceinline__ void deposit_loop(int nx, int ny, int x0, int y0, int s, int e,
                                              const int* __restrict__ list, const float2* __restrict__ X,
                                              float scale, float lscale, int* acc, int* accl, float2 xpre,
-                                             DealCfg cfg = DealCfg()) {
-  float2 xc = xpre;  // first entry preloaded by the caller, later ones one iteration ahead
+                                             DealCfg cfg = DealCfg(), const float2* __restrict__ O = nullptr,
+                                             float2 opre = make_float2(0.f, 0.f)) {
+  float2 xc = xpre, oc = opre;  // first entry preloaded by the caller, later ones one iteration ahead
+  const float wscale = TWO ? 0.5f * scale : scale;  // each marker deposits half of its bead
   for (Deal d(e - s, cfg); d.valid(); d.advance()) {
-    const float2 xb = xc;
-    if (d.next_valid()) xc = __ldg(X + __ldg(list + s + d.p + d.nw));
+    const float2 xb = xc, ob = oc;
+    if (d.next_valid()) load_point<TWO>(X, O, __ldg(list + s + d.p + d.nw), xc, oc);
     TileBead tb;
-    tile_bead<WRAP>(xb, nx, ny, x0, y0, tb);
+    tile_bead<WRAP, TWO>(xb, ob, nx, ny, x0, y0, tb);
 #pragma unroll
     for (int l = 0; l < 4; ++l) {
-      const float wys = tb.wy[l] * scale;
+      const float wys = tb.wy[l] * wscale;
 #pragma unroll
       for (int kx = 0; kx < 4; ++kx) {
         const int a = tap_index<WRAP>(tb, l, kx);
@@ -196,26 +219,29 @@ __device__ __forceinline__ void deposit_loop(int nx, int ny, int x0, int y0, int
   }
 }
 
-template <bool WIDE, bool WRAP>
+template <bool WIDE, bool WRAP, bool TWO = false>
 __device__ __forceinline__ void spread_loop(int nx, int ny, int x0, int y0, int s, int e,
                                             const int* __restrict__ list, const float2* __restrict__ X,
                                             const float2* __restrict__ F, float scale, float lscale,
                                             int* acc0, int* acc1, int* accl0, int* accl1,
-                                            float2 xpre, float2 fpre, DealCfg cfg = DealCfg()) {
+                                            float2 xpre, float2 fpre, DealCfg cfg = DealCfg(),
+                                            const float2* __restrict__ O = nullptr,
+                                            float2 opre = make_float2(0.f, 0.f)) {
   // the caller loaded this thread's FIRST entry (xpre, fpre) before the zeroing and the barrier,
   // so that the list -> X/F gather latency is spent under them; later entries are software-
   // pipelined one iteration ahead
-  float2 xc = xpre, fc = fpre;
+  float2 xc = xpre, fc = fpre, oc = opre;
+  const float wscale = TWO ? 0.5f * scale : scale;  // each marker carries half of its bead's force
   for (Deal d(e - s, cfg); d.valid(); d.advance()) {
-    const float2 xb = xc, f = fc;
+    const float2 xb = xc, f = fc, ob = oc;
     if (d.next_valid()) {
       const int bn = __ldg(list + s + d.p + d.nw);
-      xc = __ldg(X + bn);
-      fc = __ldg(F + bn);
+      load_point<TWO>(X, O, bn, xc, oc);
+      fc = __ldg(F + (TWO ? bn >> 1 : bn));
     }
     TileBead tb;
-    tile_bead<WRAP>(xb, nx, ny, x0, y0, tb);
-    const float fxs = f.x * scale, fys = f.y * scale;
+    tile_bead<WRAP, TWO>(xb, ob, nx, ny, x0, y0, tb);
+    const float fxs = f.x * wscale, fys = f.y * wscale;
 #pragma unroll
     for (int l = 0; l < 4; ++l) {
       const float wyx = tb.wy[l] * fxs, wyy = tb.wy[l] * fys;
@@ -268,23 +294,29 @@ __device__ __noinline__ void spread_loop_wide(int nx, int ny, int x0, int y0, in
 // LIGHT: the variant for worlds without crowded tiles, launched with 128 threads and capped at
 // 40 registers (more resident CTAs hide the per-tile latency chain; the cap costs the crowded
 // config 5 10 % and gains world 4d 2 %).
-template <bool LIGHT>
+// TWO: the list holds two-layer markers (reading 28), O their offsets; grid = (nx/TS, ny/TS, worlds).
+template <bool LIGHT, bool TWO = false>
 __global__ void __launch_bounds__(256, LIGHT ? 6 : 1) k_deposit_tile(int nx, int ny, const int* __restrict__ tile_start,
                                                       const int* __restrict__ list,
                                                       const float2* __restrict__ X,
                                                       float* __restrict__ rho_b,
                                                       float* __restrict__ tile_rho_max,
-                                                      unsigned* __restrict__ tile_fmax) {
+                                                      unsigned* __restrict__ tile_fmax,
+                                                      const float2* __restrict__ O, size_t wstride) {
   __shared__ __align__(16) int acc[ACC_N], accl[ACC_N];
-  __shared__ float red[32];
+  {
+    const size_t ws = blockIdx.z * wstride;
+    tile_start = wshift(tile_start, ws); list = wshift(list, ws); X = wshift(X, ws); rho_b = wshift(rho_b, ws);
+    tile_rho_max = wshift(tile_rho_max, ws); tile_fmax = wshift(tile_fmax, ws); O = wshift(O, ws);
+  }
   const int t = blockIdx.y * gridDim.x + blockIdx.x;  // grid = (nx/TS, ny/TS)
   const int x0 = blockIdx.x * TS, y0 = blockIdx.y * TS;
   const int s = tile_start[t], e = tile_start[t + 1];
   const bool wide = (e - s) > WIDE_N;
-  float2 xpre = make_float2(0.f, 0.f);
+  float2 xpre = make_float2(0.f, 0.f), opre = make_float2(0.f, 0.f);
   {
     const Deal d(e - s);
-    if (d.valid()) xpre = __ldg(X + __ldg(list + s + d.p));  // gather starts before the zeroing
+    if (d.valid()) load_point<TWO>(X, O, __ldg(list + s + d.p), xpre, opre);  // gather starts before the zeroing
   }
   if (LIGHT) {  // the light variant is launched with 128 threads
     zero_acc<128>(acc);
@@ -296,7 +328,11 @@ __global__ void __launch_bounds__(256, LIGHT ? 6 : 1) k_deposit_tile(int nx, int
   const float scale = pow2_scale(fmaxf(0.25f * (float)(e - s), 1.0f));
   const float lscale = pow2f(lo_bits(e - s));
   __syncthreads();
-  if (wide) deposit_loop_wide(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl, xpre);
+  if (TWO) {
+    if (wide) deposit_loop<true, true, true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl, xpre, DealCfg(), O, opre);
+    else if (nx == TS || ny == TS) deposit_loop<false, true, true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl, xpre, DealCfg(), O, opre);
+    else deposit_loop<false, false, true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl, xpre, DealCfg(), O, opre);
+  } else if (wide) deposit_loop_wide(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl, xpre);
   else if (nx == TS || ny == TS) deposit_loop<false, true>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl, xpre);
   else deposit_loop<false, false>(nx, ny, x0, y0, s, e, list, X, scale, lscale, acc, accl, xpre);
   __syncthreads();
@@ -338,7 +374,7 @@ __device__ __forceinline__ int first_entry(int s, int e, const int* __restrict__
 // Used by the fused spread + fluid kernel (k_lbm.cuh), which must __syncthreads() before it
 // reads the accumulators.  (xpre, fpre): X and F of this thread's first entry, loaded by the
 // caller well ahead (their list -> X/F gather is the longest latency chain of the tile).
-template <bool CL = false>
+template <bool CL = false, bool TWO = false>
 __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, int y0, int s, int e,
                                                         const int* __restrict__ list,
                                                         const float2* __restrict__ X,
@@ -346,7 +382,8 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
                                                         const unsigned* __restrict__ tile_fmax, int t,
                                                         int* acc0, int* acc1, int* accl0, int* accl1,
                                                         float* red, float& linv, float2 xpre, float2 fpre,
-                                                        DealCfg cfg = DealCfg()) {
+                                                        DealCfg cfg = DealCfg(), const float2* __restrict__ O = nullptr,
+                                                        float2 opre = make_float2(0.f, 0.f)) {
   const bool wide = (e - s) > WIDE_N;
   const float lscale = pow2f(lo_bits(e - s));
   linv = wide ? 1.0f / lscale : 0.0f;  // 0 => the readers skip the lo planes (not zeroed then)
@@ -372,7 +409,8 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
     fm = red[0];
   } else {
     for (int k = s + threadIdx.x; k < e; k += blockDim.x) {  // any order
-      const float2 f = __ldg(F + __ldg(list + k));
+      const int b = __ldg(list + k);
+      const float2 f = __ldg(F + (TWO ? b >> 1 : b));
       fm = fmaxf(fm, fmaxf(fabsf(f.x), fabsf(f.y)));
     }
     fm = block_max(fm, red);  // also orders the zeroing before the atomics
@@ -383,6 +421,12 @@ __device__ __forceinline__ float spread_tile_accumulate(int nx, int ny, int x0, 
     if (wide) spread_loop_wide_cfg(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre, cfg.nw, cfg.v0);
     else if (nx == TS || ny == TS) spread_loop<false, true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre, cfg);
     else spread_loop<false, false>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre, cfg);
+    return scale;
+  }
+  if (TWO) {
+    if (wide) spread_loop<true, true, true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre, DealCfg(), O, opre);
+    else if (nx == TS || ny == TS) spread_loop<false, true, true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre, DealCfg(), O, opre);
+    else spread_loop<false, false, true>(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre, DealCfg(), O, opre);
     return scale;
   }
   if (wide) spread_loop_wide(nx, ny, x0, y0, s, e, list, X, F, scale, lscale, acc0, acc1, accl0, accl1, xpre, fpre);

@@ -47,8 +47,10 @@ constexpr float LIST_DRIFT_MAX = 0.22f;  // rebuild when the accumulated drift b
 // device-side list state, in the world's flag words
 struct ListState {
   int need;            // 1: the K0 kernels of this step rebuild the lists
-  float drift;         // bound on the per-axis displacement of any bead since the lists were built
+  float drift;         // bound on the per-axis displacement of any listed point since the lists were built
   unsigned step_max;   // bits of max |U_x|,|U_y| over the beads in the last step (K4, atomicMax)
+  unsigned step_max_p; // ... of the projection displacement of the last step (k_pbd.cuh; 0 without pbd_project)
+  unsigned step_max_m; // ... of the change of the two-layer marker offsets (k_pbd.cuh; 0 without two_layer)
 };
 
 // The policy is evaluated where it is needed instead of in a launch of its own: the count pass
@@ -56,7 +58,9 @@ struct ListState {
 // kernel (one block, next in the stream) then commits it -- st->need for the kernels after it,
 // the new drift, step_max = 0 for this step's K4.
 __device__ __forceinline__ bool list_rebuild_due(const ListState* st, float* drift_out) {
-  const float d = st->drift + __uint_as_float(st->step_max);
+  // a listed point moves by at most the sum of the three per-step bounds (triangle inequality)
+  const float d = st->drift + (__uint_as_float(st->step_max) + __uint_as_float(st->step_max_p) +
+                               __uint_as_float(st->step_max_m));
   *drift_out = d;
   return !(d <= LIST_DRIFT_MAX);  // also true for NaN
 }
@@ -64,6 +68,8 @@ __device__ __forceinline__ void list_policy_commit(ListState* st) {
   float d;
   const bool need = list_rebuild_due(st, &d);
   st->step_max = 0u;
+  st->step_max_p = 0u;
+  st->step_max_m = 0u;
   st->need = need ? 1 : 0;
   st->drift = need ? 0.0f : d;
 }
@@ -118,17 +124,29 @@ __device__ __forceinline__ int warp_claim(int* ctr, int key, bool act) {
 // FILL = false: tile_ctr[t] += 1 and (if given) bucket_ctr[32 t + key] += 1 per listed bead.
 // FILL = true: bucket_ctr holds the running cursors (bucket_starts) and the bead index is
 // stored at the claimed slot.
+// O != NULL (two-layer broadcast, reading 28): the listed items are the 2 N MARKERS, item 2 b + s
+// at X_b + O_b (s = 0) or X_b - O_b (s = 1).  Rounding the marker to fp32 here is harmless: the
+// lists only have to cover the support within the skin (the consumers form it exactly).
 template <bool FILL>
-__device__ __forceinline__ void tile_bin(const float2* __restrict__ X, int N, int nx, int ny,
+__device__ __forceinline__ void tile_bin(const float2* __restrict__ X, const float2* __restrict__ O, int N, int nx, int ny,
                                          int* __restrict__ tile_ctr, int* __restrict__ bucket_ctr,
                                          int* __restrict__ list) {
-  // grid-stride over whole blocks of beads: every lane of a warp takes part in warp_claim
-  for (int base = blockIdx.x * blockDim.x; base < N; base += gridDim.x * blockDim.x) {
+  const int n_items = O ? 2 * N : N;
+  // grid-stride over whole blocks of items: every lane of a warp takes part in warp_claim
+  for (int base = blockIdx.x * blockDim.x; base < n_items; base += gridDim.x * blockDim.x) {
     const int b = base + threadIdx.x;
     int t[4] = {0, 0, 0, 0};
     int n = 0, key = 0;
-    if (b < N) {
-      const float2 p = X[b];
+    if (b < n_items) {
+      float2 p;
+      if (O) {
+        p = X[b >> 1];
+        const float2 o = O[b >> 1];
+        p.x += (b & 1) ? -o.x : o.x;
+        p.y += (b & 1) ? -o.y : o.y;
+      } else {
+        p = X[b];
+      }
       n = bead_tiles(p.x, p.y, nx, ny, nx / TS, t);
       key = bead_key(p.x, p.y);
     }
@@ -205,27 +223,36 @@ __device__ __forceinline__ void tile_scan(int* __restrict__ tile_count, int n_ti
 
 template <bool FILL>
 __global__ void __launch_bounds__(256) k_tile_bin(const ListState* __restrict__ st, const float2* __restrict__ X,
-                                                  int N, int nx, int ny, int* __restrict__ tile_ctr,
-                                                  int* __restrict__ bucket_ctr, int* __restrict__ list) {
+                                                  const float2* __restrict__ O, int N, int nx, int ny,
+                                                  int* __restrict__ tile_ctr, int* __restrict__ bucket_ctr,
+                                                  int* __restrict__ list, size_t wstride) {
+  const size_t ws = blockIdx.y * wstride;
+  st = wshift(st, ws); X = wshift(X, ws); O = wshift(O, ws); tile_ctr = wshift(tile_ctr, ws);
+  bucket_ctr = wshift(bucket_ctr, ws); list = wshift(list, ws);
   if (FILL) {
     if (!st->need) return;
   } else {
     float d;
     if (!list_rebuild_due(st, &d)) return;
   }
-  tile_bin<FILL>(X, N, nx, ny, tile_ctr, bucket_ctr, list);
+  tile_bin<FILL>(X, O, N, nx, ny, tile_ctr, bucket_ctr, list);
 }
 
 __global__ void __launch_bounds__(256) k_bucket_starts(const ListState* __restrict__ st, int n_tiles,
                                                        const int* __restrict__ tile_start,
                                                        int* __restrict__ bucket_count,
-                                                       int* __restrict__ bucket_cursor) {
+                                                       int* __restrict__ bucket_cursor, size_t wstride) {
+  const size_t ws = blockIdx.y * wstride;
+  st = wshift(st, ws); tile_start = wshift(tile_start, ws); bucket_count = wshift(bucket_count, ws);
+  bucket_cursor = wshift(bucket_cursor, ws);
   if (!st->need) return;
   bucket_starts(n_tiles, tile_start, bucket_count, bucket_cursor);
 }
 
 __global__ void __launch_bounds__(1024) k_tile_scan(ListState* __restrict__ st, int* __restrict__ tile_count,
-                                                    int n_tiles, int* __restrict__ tile_start) {
+                                                    int n_tiles, int* __restrict__ tile_start, size_t wstride) {
+  const size_t ws = blockIdx.y * wstride;
+  st = wshift(st, ws); tile_count = wshift(tile_count, ws); tile_start = wshift(tile_start, ws);
   __shared__ int sm[33];
   __shared__ int need_s;
   if (threadIdx.x == 0) {
@@ -241,10 +268,16 @@ __global__ void __launch_bounds__(1024) k_tile_scan(ListState* __restrict__ st, 
 // 1024-thread CTA -- policy, count, scan, bucket starts, fill, separated by __syncthreads()
 // (global atomics and stores of a block are visible to the same block after the barrier).
 __global__ void __launch_bounds__(1024) k_list_build_small(ListState* __restrict__ st, const float2* __restrict__ X,
-                                                           int N, int nx, int ny, int n_tiles,
-                                                           int* __restrict__ tile_count, int* __restrict__ tile_start,
-                                                           int* __restrict__ bucket_count,
-                                                           int* __restrict__ bucket_cursor, int* __restrict__ list) {
+                                                           const float2* __restrict__ O, int N, int nx, int ny,
+                                                           int n_tiles, int* __restrict__ tile_count,
+                                                           int* __restrict__ tile_start, int* __restrict__ bucket_count,
+                                                           int* __restrict__ bucket_cursor, int* __restrict__ list,
+                                                           size_t wstride) {
+  // one CTA per world: blockIdx.x is always 0 here, the world index rides in blockIdx.y
+  const size_t ws = blockIdx.y * wstride;
+  st = wshift(st, ws); X = wshift(X, ws); O = wshift(O, ws); tile_count = wshift(tile_count, ws);
+  tile_start = wshift(tile_start, ws); bucket_count = wshift(bucket_count, ws);
+  bucket_cursor = wshift(bucket_cursor, ws); list = wshift(list, ws);
   __shared__ int sm[33];
   __shared__ int need_s;
   if (threadIdx.x == 0) {
@@ -253,13 +286,13 @@ __global__ void __launch_bounds__(1024) k_list_build_small(ListState* __restrict
   }
   __syncthreads();
   if (!need_s) return;
-  tile_bin<false>(X, N, nx, ny, tile_count, bucket_count, nullptr);
+  tile_bin<false>(X, O, N, nx, ny, tile_count, bucket_count, nullptr);
   __syncthreads();
   tile_scan(tile_count, n_tiles, tile_start, sm);
   __syncthreads();
   bucket_starts(n_tiles, tile_start, bucket_count, bucket_cursor);
   __syncthreads();
-  tile_bin<true>(X, N, nx, ny, nullptr, bucket_cursor, list);
+  tile_bin<true>(X, O, N, nx, ny, nullptr, bucket_cursor, list);
 }
 
 // Medium worlds (up to a few hundred thousand beads: still bound by launch overhead on the steps
@@ -270,22 +303,28 @@ __global__ void __launch_bounds__(1024) k_list_build_small(ListState* __restrict
 // unlike a hand-made grid barrier this cannot deadlock.
 constexpr int K0_CLUSTER = 8;
 __global__ void __cluster_dims__(K0_CLUSTER, 1, 1) __launch_bounds__(1024)
-    k_list_build_cluster(ListState* __restrict__ st, const float2* __restrict__ X, int N, int nx, int ny, int n_tiles,
-                         int* __restrict__ tile_count, int* __restrict__ tile_start, int* __restrict__ bucket_count,
-                         int* __restrict__ bucket_cursor, int* __restrict__ list) {
+    k_list_build_cluster(ListState* __restrict__ st, const float2* __restrict__ X, const float2* __restrict__ O, int N,
+                         int nx, int ny, int n_tiles, int* __restrict__ tile_count, int* __restrict__ tile_start,
+                         int* __restrict__ bucket_count, int* __restrict__ bucket_cursor, int* __restrict__ list,
+                         size_t wstride) {
+  // one cluster per world: blockIdx.x = rank in the cluster, blockIdx.y = world
+  const size_t ws = blockIdx.y * wstride;
+  st = wshift(st, ws); X = wshift(X, ws); O = wshift(O, ws); tile_count = wshift(tile_count, ws);
+  tile_start = wshift(tile_start, ws); bucket_count = wshift(bucket_count, ws);
+  bucket_cursor = wshift(bucket_cursor, ws); list = wshift(list, ws);
   namespace cg = cooperative_groups;
   cg::cluster_group cl = cg::this_cluster();
   __shared__ int sm[33];
   if (blockIdx.x == 0 && threadIdx.x == 0) list_policy_commit(st);
   cl.sync();
   if (!*reinterpret_cast<volatile int*>(&st->need)) return;  // the same value in every CTA: all leave together
-  tile_bin<false>(X, N, nx, ny, tile_count, bucket_count, nullptr);
+  tile_bin<false>(X, O, N, nx, ny, tile_count, bucket_count, nullptr);
   cl.sync();
   if (blockIdx.x == 0) tile_scan(tile_count, n_tiles, tile_start, sm);
   cl.sync();
   bucket_starts(n_tiles, tile_start, bucket_count, bucket_cursor);
   cl.sync();
-  tile_bin<true>(X, N, nx, ny, nullptr, bucket_cursor, list);
+  tile_bin<true>(X, O, N, nx, ny, nullptr, bucket_cursor, list);
 }
 
 // mc_load_filaments: largest tile list (chooses the CTA size of the P2G kernels)

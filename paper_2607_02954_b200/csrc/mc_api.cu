@@ -19,11 +19,13 @@
 #include "k_lbm.cuh"
 #include "k_mdf.cuh"
 #include "k_p2g.cuh"
+#include "k_pbd.cuh"
 #include "k_tile.cuh"
 
 namespace {
 
 thread_local std::string g_create_error;
+thread_local bool g_batch_call = false;  // set while an mc_*_batch call drives its member worlds
 
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
@@ -32,6 +34,7 @@ struct Layout {
   size_t fA, fB, u, rho_b, A, G, cfield, csum, As, tile_count, tile_start, bucket_count, bucket_cursor, tile_rho_max, tile_fmax;
   size_t X, PA, PB, PC, PD, F, sense, list, src, bflags, scratch, flags, sources;
   size_t V, dF, hrinv, mdf_fmax;  // MDF coupling only
+  size_t PE, O, Dp;               // rest-length actuation amplitudes; two-layer offsets; projection displacement
   size_t total;
 };
 
@@ -46,12 +49,16 @@ bool validate(const mc_world_params* p, Derived* d, std::string* why) {
   if (p->nx < 32 || p->ny < 32 || p->nx % 32 || p->ny % 32) { *why = "nx, ny must be multiples of 32, >= 32"; return false; }
   if ((int64_t)p->nx * p->ny > (int64_t)1 << 30 || p->ny > 65535) { *why = "grid too large"; return false; }
   if (!(p->dt > 0) || !(p->nu > 0) || !(p->trt_lambda > 0) || !(p->rho0 > 0)) { *why = "dt, nu, trt_lambda, rho0 must be > 0"; return false; }
-  if (p->pbd_iters != 1) { *why = "pbd_iters must be 1"; return false; }
+  if (p->pbd_iters < 1 || p->pbd_iters > 8) { *why = "pbd_iters must be 1..8"; return false; }
+  if (p->pbd_order != MC_PBD_JACOBI && p->pbd_order != MC_PBD_GAUSS_SEIDEL) { *why = "unknown pbd_order"; return false; }
+  if ((p->pbd_project != 0 && p->pbd_project != 1) || (p->two_layer != 0 && p->two_layer != 1)) { *why = "pbd_project and two_layer must be 0 or 1"; return false; }
+  if (!(p->layer_offset >= 0.0f) || p->layer_offset > 1.0f) { *why = "layer_offset must lie in [0, 1]"; return false; }
   if (p->n_fields < 0 || p->n_fields > 4) { *why = "n_fields must be 0..4"; return false; }
   // the tile lists hold up to 4 N entries addressed with 32-bit ints (k_tile.cuh)
   if (p->max_beads < 0 || p->max_beads > ((int64_t)1 << 29) - 1) { *why = "max_beads out of range (0 .. 2^29 - 1)"; return false; }
   if (p->coupling != MC_COUPLING_FORCE && p->coupling != MC_COUPLING_MDF) { *why = "unknown coupling"; return false; }
   if (p->coupling == MC_COUPLING_MDF && (p->mdf_iters < 1 || p->mdf_iters > 16)) { *why = "mdf_iters must be 1..16"; return false; }
+  if (p->coupling == MC_COUPLING_MDF && p->two_layer) { *why = "two_layer is not defined with the MDF coupling (reading 28)"; return false; }
   for (int k = 0; k < p->n_fields; ++k) {
     const mc_field_params& f = p->fields[k];
     if (f.kind == MC_FIELD_BEAD_DENSITY) {
@@ -103,7 +110,7 @@ Layout make_layout(const mc_world_params* p, const Derived& d) {
   L.PD = take(N * 8);
   L.F = take(N * 8);
   L.sense = take(N * 4);
-  L.list = take(N * 4 * 4);   // a bead is listed in at most 4 tiles
+  L.list = take((p->two_layer ? 2 : 1) * N * 4 * 4);   // a bead (two-layer: each of its 2 markers) is listed in at most 4 tiles
   L.src = take(N * 4);        // internal bead -> caller's bead
   L.bflags = take(N);         // first/last flags (load-time scratch; PC.w carries them)
   L.scratch = take((N / 3 + 2) * 8);  // load-time: chain offsets and sort keys
@@ -114,6 +121,9 @@ Layout make_layout(const mc_world_params* p, const Derived& d) {
   L.dF = take(mdf ? N * 8 : 0);
   L.hrinv = take(mdf ? nc * f4 : 0);
   L.mdf_fmax = take(mdf ? (size_t)p->mdf_iters * nt * 4 : 0);  // per iteration: per-tile bound on |dF| (last: |F|)
+  L.PE = take(N * 4);
+  L.O = take(p->two_layer ? N * 8 : 0);
+  L.Dp = take(p->pbd_project ? N * 8 : 0);
   L.total = off;
   return L;
 }
@@ -132,8 +142,16 @@ struct mc_world {
   int cur = 0;  // which of fA/fB holds the current post-collision populations
   int n_fil = 0;
   int N = 0;
-  int stride = 60;   // K1 window advance: 64 when all chains share a length dividing 64
+  int stride = 60;   // K1 window advance: 64 when all chains share a length dividing 64, else 64 - 4 halo_lanes
   int n_windows = 0;
+  int halo_lanes = 1;      // K1 halo on either side of an overlapping window: K (Jacobi) or ceil(3K/2) (Gauss-Seidel) lanes
+  bool has_L_act = false;  // mc_set_length_actuation gave amplitudes
+  float layer_h = 0.5f;    // two_layer: half distance between the layers
+  // batched worlds (mc_batch): the leader (world 0) launches every kernel for batch_n worlds whose
+  // workspaces lie batch_stride bytes apart; a single world is a batch of one
+  int batch_n = 1;
+  size_t batch_stride = 0;
+  bool batch_member = false;  // owned by an mc_batch: stepped and reloaded only through it
   cudaTextureObject_t tex_u = 0, tex_A = 0;  // linear float2 views of u and A for the texture-pipe half of the gathers
   int n_sm = 148;               // SMs of the device the world lives on (grid-stride kernels size their grids by it)
   bool uniform_params = false;  // K1 variant: L_rest, stiffnesses and period identical for all beads
@@ -216,8 +234,10 @@ int pick_bx(int nx) { return nx % 256 == 0 ? 256 : (nx % 128 == 0 ? 128 : (nx % 
 template <int R>
 void launch_blur_R(mc_world* w, int k, const float2* base, float2* A, float* field_out) {
   const int grid = (w->nx / mc::BLUR_T) * (w->ny / mc::BLUR_T);
-  mc::k_blur_grad<R><<<grid, mc::BLUR_THREADS, 0, w->stream>>>(
-      w->nx, w->ny, w->taps[k], w->ptr<float>(w->L.rho_b), w->coef[k], base, A, field_out);
+  // the step filters every world of a batch; a read-out (field_out given) only this world
+  const unsigned nb = field_out ? 1u : (unsigned)w->batch_n;
+  mc::k_blur_grad<R><<<dim3(grid, nb), mc::BLUR_THREADS, 0, w->stream>>>(
+      w->nx, w->ny, w->taps[k], w->ptr<float>(w->L.rho_b), w->coef[k], base, A, field_out, w->batch_stride);
 }
 
 // K3a for bead-density field k; first: start from the static part, else add to the planes in A
@@ -252,47 +272,54 @@ int enqueue_step(mc_world* w) {
   float* G1 = G0 + w->nc;
   int* flag = w->ptr<int>(w->L.flags);
   const int n_tiles = (nx / mc::TS) * (ny / mc::TS);
-  const dim3 tgrid(nx / mc::TS, ny / mc::TS);
+  const unsigned nb = (unsigned)w->batch_n;       // worlds per launch: blockIdx.y (.z on 2-D grids)
+  const size_t ws = w->batch_stride;
+  const dim3 tgrid(nx / mc::TS, ny / mc::TS, nb);
   const int bt = 256;
-  const int bgrid = (N + bt - 1) / bt;
   const bool beads = N > 0;
   const bool mdf = w->p.coupling == MC_COUPLING_MDF;
+  const bool two = w->p.two_layer != 0;
+  const float2* O = two ? w->ptr<float2>(w->L.O) : nullptr;
+  const int n_items = two ? 2 * N : N;            // listed points: beads, or their two-layer markers
+  const int bgrid = (n_items + bt - 1) / bt;
+  mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16);
 
   prof_mark(w, 0);
   if (beads) {
     // K0: tile binning (policy, count, scan, bucket starts, fill).  The kernels return at once
     // unless the policy finds the lists' drift bound used up (k_tile.cuh).
-    mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16);
-    if (N <= K0_SMALL_BEADS && n_tiles <= K0_SMALL_TILES) {
-      // small world: one launch of one CTA instead of four (k_tile.cuh)
-      mc::k_list_build_small<<<1, 1024, 0, st>>>(ls_state, X, N, nx, ny, n_tiles, tile_count, tile_start,
-                                                 bucket_count, bucket_cursor, list);
+    if (n_items <= K0_SMALL_BEADS && n_tiles <= K0_SMALL_TILES) {
+      // small world: one launch of one CTA (per world) instead of four (k_tile.cuh)
+      mc::k_list_build_small<<<dim3(1, nb), 1024, 0, st>>>(ls_state, X, O, N, nx, ny, n_tiles, tile_count, tile_start,
+                                                           bucket_count, bucket_cursor, list, ws);
       w->launches += 1;
-    } else if (N <= K0_MEDIUM_BEADS && n_tiles <= K0_MEDIUM_TILES) {
-      mc::k_list_build_cluster<<<mc::K0_CLUSTER, 1024, 0, st>>>(ls_state, X, N, nx, ny, n_tiles, tile_count, tile_start,
-                                                                bucket_count, bucket_cursor, list);
+    } else if (n_items <= K0_MEDIUM_BEADS && n_tiles <= K0_MEDIUM_TILES) {
+      mc::k_list_build_cluster<<<dim3(mc::K0_CLUSTER, nb), 1024, 0, st>>>(ls_state, X, O, N, nx, ny, n_tiles, tile_count,
+                                                                          tile_start, bucket_count, bucket_cursor, list, ws);
       w->launches += 1;
     } else {
       const int k0grid = bgrid < w->n_sm * 8 ? bgrid : w->n_sm * 8;
-      mc::k_tile_bin<false><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, tile_count, bucket_count, nullptr);
-      mc::k_tile_scan<<<1, 1024, 0, st>>>(ls_state, tile_count, n_tiles, tile_start);
-      mc::k_bucket_starts<<<std::min((n_tiles + 7) / 8, w->n_sm * 4), 256, 0, st>>>(ls_state, n_tiles, tile_start, bucket_count, bucket_cursor);
-      mc::k_tile_bin<true><<<k0grid, bt, 0, st>>>(ls_state, X, N, nx, ny, nullptr, bucket_cursor, list);
+      mc::k_tile_bin<false><<<dim3(k0grid, nb), bt, 0, st>>>(ls_state, X, O, N, nx, ny, tile_count, bucket_count, nullptr, ws);
+      mc::k_tile_scan<<<dim3(1, nb), 1024, 0, st>>>(ls_state, tile_count, n_tiles, tile_start, ws);
+      mc::k_bucket_starts<<<dim3(std::min((n_tiles + 7) / 8, w->n_sm * 4), nb), 256, 0, st>>>(ls_state, n_tiles, tile_start, bucket_count, bucket_cursor, ws);
+      mc::k_tile_bin<true><<<dim3(k0grid, nb), bt, 0, st>>>(ls_state, X, O, N, nx, ny, nullptr, bucket_cursor, list, ws);
       w->launches += 4;
     }
     prof_mark(w, 1);
     // K2a: S2 deposit
     if (w->d.n_density) {
-      if (w->cluster == 8)
-        mc::k_deposit_tile_cl<8><<<n_tiles * 8, 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax);
+      if (two)  // two-layer markers: one CTA per tile whatever the crowding
+        mc::k_deposit_tile<false, true><<<tgrid, 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax, O, ws);
+      else if (w->cluster == 8)
+        mc::k_deposit_tile_cl<8><<<dim3(n_tiles * 8, nb), 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax, ws);
       else if (w->cluster == 4)
-        mc::k_deposit_tile_cl<4><<<n_tiles * 4, 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax);
+        mc::k_deposit_tile_cl<4><<<dim3(n_tiles * 4, nb), 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax, ws);
       else if (w->cluster == 2)
-        mc::k_deposit_tile_cl<2><<<n_tiles * 2, 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax);
+        mc::k_deposit_tile_cl<2><<<dim3(n_tiles * 2, nb), 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax, ws);
       else if (w->deposit_threads == 128)
-        mc::k_deposit_tile<true><<<tgrid, 128, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax);
+        mc::k_deposit_tile<true><<<tgrid, 128, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax, nullptr, ws);
       else
-        mc::k_deposit_tile<false><<<tgrid, w->deposit_threads, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax);
+        mc::k_deposit_tile<false><<<tgrid, w->deposit_threads, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax, nullptr, ws);
       w->launches++;
       prof_mark(w, 2);
       // K3a: S3 filter + gradient -> force-gradient planes A
@@ -325,7 +352,8 @@ int enqueue_step(mc_world* w) {
     fa.n_windows = w->n_windows;
     fa.kappa = mdf ? 1.0f : w->kappa;
     fa.step = w->ptr<long long>(w->L.flags) + 4;  // flags[8..9]: device copy of the step counter
-    fa.tex_A = w->tex_on ? w->tex_A : 0;
+    fa.tex_A = (w->tex_on && nb == 1) ? w->tex_A : 0;  // texture views are per world: batches use plain loads
+    const bool generic = w->p.pbd_iters > 1 || w->p.pbd_order != MC_PBD_JACOBI || w->has_L_act || two;
     // 64-thread CTAs (two windows): finer-grained scheduling than eight windows per CTA and 42
     // instead of 40 resident warps at 48 registers (world 4d: 256 threads 0.232 ms, 128: 0.225, 64: 0.221, 32: 0.239)
     constexpr int k1t = 64;
@@ -333,12 +361,25 @@ int enqueue_step(mc_world* w) {
     // two of the four support rows of the A gather go through the texture pipe (measured on
     // world 4d: 0 rows 0.254 ms, 1: 0.248, 2: 0.245, 3: 0.256)
     const bool k1tex = fa.A && fa.tex_A;
-    if (w->uniform_params) {
-      if (k1tex) mc::k_filament_force<true, 2><<<k1grid, k1t, 0, st>>>(fa);
-      else mc::k_filament_force<true, 0><<<k1grid, k1t, 0, st>>>(fa);
+    if (generic) {
+      // literal PBD / rest-length actuation / two-layer gathers: the general kernel (k_pbd.cuh)
+      mc::PbdArgs pa;
+      pa.f = fa;
+      pa.PE = w->has_L_act ? w->ptr<float>(w->L.PE) : nullptr;
+      pa.O = O;
+      pa.Dp = nullptr;
+      pa.iters = w->p.pbd_iters;
+      pa.order = w->p.pbd_order;
+      pa.halo_lanes = w->halo_lanes;
+      pa.step_off = 0;
+      if (w->uniform_params) mc::k_filament_pbd<true><<<dim3(k1grid, nb), k1t, 0, st>>>(pa, ws);
+      else mc::k_filament_pbd<false><<<dim3(k1grid, nb), k1t, 0, st>>>(pa, ws);
+    } else if (w->uniform_params) {
+      if (k1tex) mc::k_filament_force<true, 2><<<dim3(k1grid, nb), k1t, 0, st>>>(fa, ws);
+      else mc::k_filament_force<true, 0><<<dim3(k1grid, nb), k1t, 0, st>>>(fa, ws);
     } else {
-      if (k1tex) mc::k_filament_force<false, 2><<<k1grid, k1t, 0, st>>>(fa);
-      else mc::k_filament_force<false, 0><<<k1grid, k1t, 0, st>>>(fa);
+      if (k1tex) mc::k_filament_force<false, 2><<<dim3(k1grid, nb), k1t, 0, st>>>(fa, ws);
+      else mc::k_filament_force<false, 0><<<dim3(k1grid, nb), k1t, 0, st>>>(fa, ws);
     }
     prof_mark(w, 4);
     w->launches++;
@@ -352,18 +393,19 @@ int enqueue_step(mc_world* w) {
       const float2* V = w->ptr<float2>(w->L.V);
       float2* dF = w->ptr<float2>(w->L.dF);
       const int mbx = pick_bx(nx) / 2;
-      mc::k_lbm_moments<<<dim3(nx / (2 * mbx), ny), mbx, 0, st>>>(w->fbuf(w->cur), nx, ny, w->rho0, ug, hrinv);
+      mc::k_lbm_moments<<<dim3(nx / (2 * mbx), ny, nb), mbx, 0, st>>>(w->fbuf(w->cur), nx, ny, w->rho0, ug, hrinv, ws);
       w->launches++;
-      const bool tex = w->tex_on && w->tex_u;
+      const bool tex = w->tex_on && w->tex_u && nb == 1;
       const int K = w->p.mdf_iters;
       unsigned* mfmax = w->ptr<unsigned>(w->L.mdf_fmax);  // [K][n_tiles], raised by K5b with atomicMax
-      if (cudaMemsetAsync(mfmax, 0, (size_t)K * n_tiles * 4, st) != cudaSuccess)
-        return fail(w, MC_ECUDA, "mc_step: cudaMemsetAsync(mdf bounds) failed");
+      for (unsigned b = 0; b < nb; ++b)
+        if (cudaMemsetAsync(reinterpret_cast<char*>(mfmax) + b * ws, 0, (size_t)K * n_tiles * 4, st) != cudaSuccess)
+          return fail(w, MC_ECUDA, "mc_step: cudaMemsetAsync(mdf bounds) failed");
       for (int k = 0; k < K; ++k) {
         unsigned* slot = mfmax + (size_t)k * n_tiles;
         const bool first = k == 0, last = k + 1 == K;
 #define MC_MDF_FORCE(FI, LA, TX) \
-  mc::k_mdf_force<FI, LA, TX><<<(N + 63) / 64, 64, 0, st>>>(N, X, V, ug, w->tex_u, nx, ny, w->rho0, dF, F, slot)
+  mc::k_mdf_force<FI, LA, TX><<<dim3((N + 63) / 64, nb), 64, 0, st>>>(N, X, V, ug, w->tex_u, nx, ny, w->rho0, dF, F, slot, ws)
         if (tex) {
           if (first && last) MC_MDF_FORCE(true, true, 1);
           else if (first) MC_MDF_FORCE(true, false, 1);
@@ -378,8 +420,8 @@ int enqueue_step(mc_world* w) {
 #undef MC_MDF_FORCE
         w->launches++;
         if (!last) {
-          mc::k_mdf_spread_tile<<<n_tiles, 256, 0, st>>>(nx, ny, tile_start, list, X, dF,
-                                                         w->d.n_density ? tile_rho_max : nullptr, slot, hrinv, ug);
+          mc::k_mdf_spread_tile<<<dim3(n_tiles, nb), 256, 0, st>>>(nx, ny, tile_start, list, X, dF,
+                                                                   w->d.n_density ? tile_rho_max : nullptr, slot, hrinv, ug, ws);
           w->launches++;
         }
       }
@@ -426,20 +468,25 @@ int enqueue_step(mc_world* w) {
     ls.tile_rho_max = w->d.n_density ? tile_rho_max : nullptr;
     // MDF: the bound on the summed F left by the last forcing iteration (K1's is on V)
     ls.tile_fmax = mdf ? w->ptr<unsigned>(w->L.mdf_fmax) + (size_t)(w->p.mdf_iters - 1) * n_tiles : tile_fmax;
-#define MC_FUSED_CL(C)                                                                   \
-  {                                                                                      \
-    if (w->keep_G) mc::k_lbm_spread_tile_cl<C, true><<<n_tiles * C, 256, 0, st>>>(ls);   \
-    else mc::k_lbm_spread_tile_cl<C, false><<<n_tiles * C, 256, 0, st>>>(ls);            \
+    ls.O = O;
+#define MC_FUSED_CL(C)                                                                                   \
+  {                                                                                                      \
+    if (w->keep_G) mc::k_lbm_spread_tile_cl<C, true><<<dim3(n_tiles * C, nb), 256, 0, st>>>(ls, ws);     \
+    else mc::k_lbm_spread_tile_cl<C, false><<<dim3(n_tiles * C, nb), 256, 0, st>>>(ls, ws);              \
   }
-    if (w->cluster == 8) MC_FUSED_CL(8)
+    if (two) {
+      if (w->keep_G) mc::k_lbm_spread_tile<true, true><<<dim3(n_tiles, nb), 256, 0, st>>>(ls, ws);
+      else mc::k_lbm_spread_tile<false, true><<<dim3(n_tiles, nb), 256, 0, st>>>(ls, ws);
+    }
+    else if (w->cluster == 8) MC_FUSED_CL(8)
     else if (w->cluster == 4) MC_FUSED_CL(4)
     else if (w->cluster == 2) MC_FUSED_CL(2)
-    else if (w->keep_G) mc::k_lbm_spread_tile<true><<<n_tiles, 256, 0, st>>>(ls);
-    else mc::k_lbm_spread_tile<false><<<n_tiles, 256, 0, st>>>(ls);
+    else if (w->keep_G) mc::k_lbm_spread_tile<true><<<dim3(n_tiles, nb), 256, 0, st>>>(ls, ws);
+    else mc::k_lbm_spread_tile<false><<<dim3(n_tiles, nb), 256, 0, st>>>(ls, ws);
 #undef MC_FUSED_CL
   } else {
     const int bx = pick_bx(nx);
-    mc::k_lbm_step<<<dim3(nx / bx, ny), bx, 0, st>>>(la);
+    mc::k_lbm_step<<<dim3(nx / bx, ny, nb), bx, 0, st>>>(la, ws);
   }
   w->launches++;
   w->cur ^= 1;
@@ -453,9 +500,44 @@ int enqueue_step(mc_world* w) {
     // 64-thread CTAs (world 4d: 256 threads 0.149 ms, 128: 0.146, 64: 0.144)
     constexpr int k4t = 64;
     const int k4grid = (N + k4t - 1) / k4t;
-    if (w->tex_on && w->tex_u) mc::k_interp_integrate<1><<<k4grid, k4t, 0, st>>>(N, X, la.u, w->tex_u, nx, ny, flag, stepp, smax);
-    else mc::k_interp_integrate<0><<<k4grid, k4t, 0, st>>>(N, X, la.u, w->tex_u, nx, ny, flag, stepp, smax);
+    if (w->tex_on && w->tex_u && nb == 1 && !two)
+      mc::k_interp_integrate<1><<<k4grid, k4t, 0, st>>>(N, X, la.u, w->tex_u, nx, ny, flag, stepp, smax, nullptr, ws);
+    else
+      mc::k_interp_integrate<0><<<dim3(k4grid, nb), k4t, 0, st>>>(N, X, la.u, w->tex_u, nx, ny, flag, stepp, smax, O, ws);
     w->launches++;
+    if (w->p.pbd_project) {
+      // reading 27: the constraints of step n once more, directly on the advected positions
+      // (K4 has already advanced the device step counter: step_off = -1)
+      mc::PbdArgs pa;
+      pa.f.X = X;
+      pa.f.PA = w->ptr<float4>(w->L.PA);
+      pa.f.PB = w->ptr<float4>(w->L.PB);
+      pa.f.PC = w->ptr<float4>(w->L.PC);
+      pa.f.PD = w->ptr<float2>(w->L.PD);
+      pa.f.uni = reinterpret_cast<const float4*>(w->ptr<int>(w->L.flags) + 24);
+      pa.f.F = nullptr; pa.f.sense = nullptr; pa.f.A = nullptr; pa.f.tex_A = 0; pa.f.csum = nullptr; pa.f.tile_fmax = nullptr;
+      pa.f.N = N; pa.f.nx = nx; pa.f.ny = ny; pa.f.stride = w->stride; pa.f.n_windows = w->n_windows;
+      pa.f.kappa = 1.0f;
+      pa.f.step = stepp;
+      pa.PE = w->has_L_act ? w->ptr<float>(w->L.PE) : nullptr;
+      pa.O = nullptr;
+      pa.Dp = w->ptr<float2>(w->L.Dp);
+      pa.iters = w->p.pbd_iters;
+      pa.order = w->p.pbd_order;
+      pa.halo_lanes = w->halo_lanes;
+      pa.step_off = -1;
+      const int pgrid = (w->n_windows * 32 + 63) / 64;
+      if (w->uniform_params) mc::k_filament_pbd<true><<<dim3(pgrid, nb), 64, 0, st>>>(pa, ws);
+      else mc::k_filament_pbd<false><<<dim3(pgrid, nb), 64, 0, st>>>(pa, ws);
+      mc::k_add_displacement<<<dim3((N + 255) / 256, nb), 256, 0, st>>>(N, X, pa.Dp, flag, &ls_state->step_max_p, ws);
+      w->launches += 2;
+    }
+    if (two) {
+      // the markers follow the new positions (reading 28)
+      mc::k_markers<<<dim3((N + 255) / 256, nb), 256, 0, st>>>(N, X, w->ptr<float4>(w->L.PC), w->layer_h,
+                                                                w->ptr<float2>(w->L.O), &ls_state->step_max_m, ws);
+      w->launches++;
+    }
   }
   prof_mark(w, 7);
   if (w->prof_on && w->prof_steps < PROF_MAX_STEPS) w->prof_steps++;
@@ -576,6 +658,8 @@ int mc_create(const mc_world_params* p, void* workspace, size_t workspace_bytes,
   w->omega_m = (float)(1.0 / tau_m);
   w->rho0 = p->rho0;
   w->kappa = (float)((double)p->k_el * dt * dt);
+  w->layer_h = p->layer_offset > 0.0f ? p->layer_offset : 0.5f;
+  w->halo_lanes = p->pbd_order == MC_PBD_JACOBI ? p->pbd_iters : (3 * p->pbd_iters + 1) / 2;
 
   cudaStream_t st = w->stream;
   cudaError_t e = cudaMemsetAsync(workspace, 0, L.total, st);  // fluid at rest: shifted populations = 0
@@ -636,6 +720,7 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
                       const float* k_stretch, const float* act_amp, const float* act_phase,
                       const float* act_period) {
   if (!w) return MC_EINVAL;
+  if (w->batch_member && !g_batch_call) return fail(w, MC_ESTATE, "world belongs to a batch: use mc_load_filaments_batch");
   if (n_fil < 0 || !offsets || offsets[0] != 0) return fail(w, MC_EINVAL, "bad offsets");
   for (int32_t f = 0; f < n_fil; ++f)
     if (offsets[f + 1] - offsets[f] < 3) return fail(w, MC_EINVAL, "chain shorter than 3 beads");
@@ -688,7 +773,10 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
     const int f = order[c];
     const int b0 = offsets[f], m = offsets[f + 1] - b0;
     uniform = uniform && (m == m0);
-    for (int i = 0; i < m; ++i) src[pos + i] = b0 + i;
+    for (int i = 0; i < m; ++i) {
+      src[pos + i] = b0 + i;
+      if (i & 1) bflags[pos + i] |= mc::BEAD_ODD;  // edge parity of the Gauss-Seidel pass
+    }
     bflags[pos] |= mc::BEAD_FIRST;
     bflags[pos + m - 1] |= mc::BEAD_LAST;
     pos += m;
@@ -728,11 +816,22 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
     mc::ListState force;
     force.need = 1;
     force.drift = INFINITY;
-    force.step_max = 0u;
+    force.step_max = force.step_max_p = force.step_max_m = 0u;
     mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16);
     cs.ok(cudaMemcpyAsync(ls_state, &force, sizeof(force), cudaMemcpyHostToDevice, st), "cudaMemcpyAsync");
-    mc::k_tile_bin<false><<<(int)((N + 255) / 256), 256, 0, st>>>(ls_state, w->ptr<float2>(w->L.X), (int)N, w->nx,
-                                                                  w->ny, tile_count, nullptr, nullptr);
+    const float2* Omark = nullptr;
+    if (w->p.two_layer) {
+      // markers of the loaded positions (reading 28); the offsets start from zero
+      cs.ok(cudaMemsetAsync(w->ptr<float2>(w->L.O), 0, (size_t)N * 8, st), "cudaMemsetAsync");
+      mc::k_markers<<<(int)((N + 255) / 256), 256, 0, st>>>((int)N, w->ptr<float2>(w->L.X), w->ptr<float4>(w->L.PC),
+                                                            w->layer_h, w->ptr<float2>(w->L.O), &ls_state->step_max_m, 0);
+      cs.launched("k_markers");
+      w->launches++;
+      Omark = w->ptr<float2>(w->L.O);
+    }
+    const int64_t n_items = w->p.two_layer ? 2 * N : N;
+    mc::k_tile_bin<false><<<(int)((n_items + 255) / 256), 256, 0, st>>>(ls_state, w->ptr<float2>(w->L.X), Omark, (int)N,
+                                                                        w->nx, w->ny, tile_count, nullptr, nullptr, 0);
     cs.launched("k_tile_bin");
     mc::k_max_int<<<64, 256, 0, st>>>(tile_count, n_tiles, maxlist);
     cs.launched("k_max_int");
@@ -756,6 +855,7 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   }
   w->N = (int)N;
   w->n_fil = n_fil;
+  w->has_L_act = false;  // a load resets the rest-length actuation (mc_set_length_actuation)
   w->deposit_threads = h_maxlist > 1024 ? 256 : 128;
   // crowded tiles (config 5 lists ~16,000 beads in its central tiles): a cluster of CTAs per tile
   // (measured on config 5: one CTA per tile 0.351 ms/step, clusters of 2: 0.263, 4: 0.250, 8: 0.325)
@@ -766,9 +866,11 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
     w->stride = prev_stride;
     w->n_windows = prev_windows;
   } else {
+    // K1 windows (k_filament.cuh, k_pbd.cuh): aligned to chain starts when every chain has the same
+    // length dividing 64, else overlapping by halo_lanes lanes on either side
     const bool aligned = uniform && (64 % m0 == 0);
-    w->stride = aligned ? 64 : 60;
-    w->n_windows = aligned ? (int)((N + 63) / 64) : (int)((N + 59) / 60);
+    w->stride = aligned ? 64 : 64 - 4 * w->halo_lanes;
+    w->n_windows = (int)((N + w->stride - 1) / w->stride);
     w->loaded_offsets.assign(offsets, offsets + n_fil + 1);
   }
   return MC_OK;
@@ -786,9 +888,14 @@ int mc_set_positions(mc_world* w, const float* xy) {
   mc::ListState force;
   force.need = 1;
   force.drift = INFINITY;
-  force.step_max = 0u;
-  cudaMemcpyAsync(reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16), &force, sizeof(force),
-                  cudaMemcpyHostToDevice, st);
+  force.step_max = force.step_max_p = force.step_max_m = 0u;
+  mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16);
+  cudaMemcpyAsync(ls_state, &force, sizeof(force), cudaMemcpyHostToDevice, st);
+  if (w->p.two_layer) {
+    mc::k_markers<<<(w->N + 255) / 256, 256, 0, st>>>(w->N, w->ptr<float2>(w->L.X), w->ptr<float4>(w->L.PC), w->layer_h,
+                                                      w->ptr<float2>(w->L.O), &ls_state->step_max_m, 0);
+    w->launches++;
+  }
   cudaError_t e = cudaStreamSynchronize(st);  // `force` is a host variable of this call; xy belongs to the caller
   if (e == cudaSuccess) e = cudaGetLastError();
   if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_set_positions: ") + cudaGetErrorString(e));
@@ -797,6 +904,7 @@ int mc_set_positions(mc_world* w, const float* xy) {
 
 int mc_step(mc_world* w, int32_t n) {
   if (!w) return MC_EINVAL;
+  if (w->batch_member && !g_batch_call) return fail(w, MC_ESTATE, "world belongs to a batch: use mc_step_batch");
   if (n < 0) return fail(w, MC_EINVAL, "n < 0");
   if (w->diverged) return fail(w, MC_EDIVERGED, "world diverged (non-finite bead or |u| > 0.3)");
   int32_t done = 0;
@@ -912,6 +1020,32 @@ int mc_read_state(mc_world* w, int64_t* step_out, float* xy, float* u, float* rh
   return MC_OK;
 }
 
+int mc_set_length_actuation(mc_world* w, const float* act_L_amp) {
+  if (!w) return MC_EINVAL;
+  if (w->batch_member && !g_batch_call) return fail(w, MC_ESTATE, "world belongs to a batch");
+  const bool was = w->has_L_act;
+  if (!act_L_amp || w->N == 0) {
+    w->has_L_act = false;
+  } else {
+    cudaStream_t st = w->stream;
+    int* nz = w->ptr<int>(w->L.flags) + 5;
+    int h = 0;
+    CudaSeq cs{w, "mc_set_length_actuation"};
+    cs.ok(cudaMemsetAsync(nz, 0, 4, st), "cudaMemsetAsync");
+    mc::k_permute1<<<(w->N + 255) / 256, 256, 0, st>>>(w->N, w->ptr<int>(w->L.src), act_L_amp, w->ptr<float>(w->L.PE), nz);
+    cs.launched("k_permute1");
+    w->launches++;
+    cs.ok(cudaMemcpyAsync(&h, nz, 4, cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync");
+    cudaError_t e = cudaStreamSynchronize(st);  // the array belongs to the caller
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (cs.rc != MC_OK) return cs.rc;
+    if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_set_length_actuation: ") + cudaGetErrorString(e));
+    w->has_L_act = h != 0;  // all-zero amplitudes keep the fast kernel
+  }
+  if (was != w->has_L_act) drop_graphs(w);
+  return MC_OK;
+}
+
 int mc_keep_intermediates(mc_world* w, int32_t on) {
   if (!w) return MC_EINVAL;
   if (w->keep_G != (on != 0)) drop_graphs(w);
@@ -946,6 +1080,133 @@ int mc_read_intermediates(mc_world* w, float* rho_b, float* G) {
   cudaError_t e = cudaStreamSynchronize(st);
   if (e == cudaSuccess) e = cudaGetLastError();
   if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_read_intermediates: ") + cudaGetErrorString(e));
+  return MC_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Batched worlds: the paper's real workload is a POPULATION of small worlds
+// stepped in lock-step ("large populations of interacting filaments over evolutionary
+// timescales"; NEAT / MAP-Elites populations P:L173-179; 256 x 256 grids P:L190).  A batch is n
+// worlds of identical parameters and chain structure (different positions and per-bead parameters)
+// in one workspace, world k at k * mc_workspace_bytes(p).  Every kernel of the step is launched
+// ONCE for the whole batch (world index in blockIdx.y / .z, mc_common.cuh wshift): a world of a
+// batch runs exactly the code and the arithmetic of the same world stepped alone, bit for bit.
+struct mc_batch {
+  std::vector<mc_world*> worlds;
+  size_t stride = 0;
+  std::string err;
+};
+
+namespace {
+struct BatchScope {
+  BatchScope() { g_batch_call = true; }
+  ~BatchScope() { g_batch_call = false; }
+};
+thread_local std::string g_batch_create_error;
+int bfail(mc_batch* b, int code, const std::string& msg) {
+  if (b) b->err = msg;
+  return code;
+}
+}  // namespace
+
+size_t mc_batch_workspace_bytes(const mc_world_params* p, int32_t n_worlds) {
+  const size_t one = mc_workspace_bytes(p);
+  if (one == 0 || n_worlds < 1 || n_worlds > 65535) return 0;
+  return one * (size_t)n_worlds;
+}
+
+const char* mc_batch_last_error(const mc_batch* b) { return b ? b->err.c_str() : g_batch_create_error.c_str(); }
+
+void mc_destroy_batch(mc_batch* b) {
+  if (!b) return;
+  for (mc_world* w : b->worlds) mc_destroy(w);
+  delete b;
+}
+
+int mc_create_batch(const mc_world_params* p, int32_t n_worlds, void* workspace, size_t workspace_bytes,
+                    void* cuda_stream, mc_batch** out) {
+  g_batch_create_error.clear();
+  if (!out) { g_batch_create_error = "null out"; return MC_EINVAL; }
+  *out = nullptr;
+  const size_t one = mc_workspace_bytes(p);
+  if (one == 0) { g_batch_create_error = "invalid world parameters"; return MC_EINVAL; }
+  if (n_worlds < 1 || n_worlds > 65535) { g_batch_create_error = "n_worlds must be 1..65535"; return MC_EINVAL; }
+  if (!workspace || workspace_bytes < one * (size_t)n_worlds) { g_batch_create_error = "workspace missing or too small"; return MC_EINVAL; }
+  mc_batch* b = new (std::nothrow) mc_batch();
+  if (!b) { g_batch_create_error = "host allocation failed"; return MC_ENOMEM; }
+  b->stride = one;
+  for (int32_t k = 0; k < n_worlds; ++k) {
+    mc_world* w = nullptr;
+    const int rc = mc_create(p, static_cast<char*>(workspace) + (size_t)k * one, one, cuda_stream, &w);
+    if (rc != MC_OK) {
+      g_batch_create_error = std::string("world ") + std::to_string(k) + ": " + mc_last_error(nullptr);
+      mc_destroy_batch(b);
+      return rc;
+    }
+    w->batch_member = true;
+    b->worlds.push_back(w);
+  }
+  *out = b;
+  return MC_OK;
+}
+
+mc_world* mc_batch_world(mc_batch* b, int32_t k) {
+  return (b && k >= 0 && k < (int32_t)b->worlds.size()) ? b->worlds[(size_t)k] : nullptr;
+}
+
+int mc_load_filaments_batch(mc_batch* b, int32_t n_fil, const int32_t* offsets, const float* xy, const float* L_rest,
+                            const float* theta_rest, const float* k_bend, const float* k_shear, const float* k_stretch,
+                            const float* act_amp, const float* act_phase, const float* act_period,
+                            const float* act_L_amp) {
+  if (!b) return MC_EINVAL;
+  if (n_fil < 0 || !offsets || offsets[0] != 0) return bfail(b, MC_EINVAL, "bad offsets");
+  const size_t N = (size_t)offsets[n_fil];
+  BatchScope scope;
+  mc_world* lead = b->worlds[0];
+  lead->batch_n = 1;  // member calls below act on one world each
+  bool uniform_all = true, any_L = false;
+  int dep = 128, cl = 0;
+  for (size_t k = 0; k < b->worlds.size(); ++k) {
+    mc_world* w = b->worlds[k];
+    const size_t o = k * N;
+    int rc = mc_load_filaments(w, n_fil, offsets, xy + 2 * o, L_rest + o, theta_rest + o, k_bend + o, k_shear + o,
+                               k_stretch + o, act_amp + o, act_phase + o, act_period + o);
+    if (rc == MC_OK && act_L_amp) rc = mc_set_length_actuation(w, act_L_amp + o);
+    if (rc != MC_OK) return bfail(b, rc, std::string("world ") + std::to_string(k) + ": " + w->err);
+    uniform_all = uniform_all && w->uniform_params;
+    any_L = any_L || w->has_L_act;
+    dep = std::max(dep, w->deposit_threads);
+    cl = std::max(cl, w->cluster_auto);
+  }
+  // one launch configuration for the whole batch.  Each choice is bit-neutral (tested): the general
+  // K1 parameter path, wider deposit CTAs and tile clusters compute what the specialised ones do.
+  for (mc_world* w : b->worlds) {
+    w->uniform_params = uniform_all;
+    w->has_L_act = any_L;
+    w->deposit_threads = dep;
+    w->cluster_auto = cl;
+    w->cluster = w->cluster_user >= 0 ? w->cluster_user : cl;
+  }
+  drop_graphs(lead);
+  return MC_OK;
+}
+
+int mc_step_batch(mc_batch* b, int32_t n) {
+  if (!b) return MC_EINVAL;
+  if (n < 0) return bfail(b, MC_EINVAL, "n < 0");
+  BatchScope scope;
+  mc_world* lead = b->worlds[0];
+  for (mc_world* w : b->worlds)
+    if (w->diverged) return bfail(b, MC_EDIVERGED, "a world of the batch diverged");
+  lead->batch_n = (int)b->worlds.size();
+  lead->batch_stride = b->stride;
+  const int rc = mc_step(lead, n);
+  lead->batch_n = 1;  // read-outs of the leader address one world
+  for (mc_world* w : b->worlds) {
+    w->step = lead->step;
+    w->cur = lead->cur;
+  }
+  if (rc != MC_OK) return bfail(b, rc, lead->err);
   return MC_OK;
 }
 

@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 namespace mc {
 
 // wrap when i is known to lie in [-n, 2n)
@@ -29,6 +31,15 @@ __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
 }
 // d = a * s + c on both halves
 __device__ __forceinline__ float2 ffma2(float2 a, float s, float2 c) { return fma2(a, dup2(s), c); }
+
+// Batched worlds (mc_batch): the worlds of a batch have identical workspace
+// layouts, `wstride` bytes apart, and every kernel of the step is launched ONCE for all of them
+// with the world index in blockIdx.y (blockIdx.z for kernels on a 2-D grid).  A kernel shifts its
+// workspace pointers by world * wstride on entry; a single world is a batch of one (shift 0).
+template <class T>
+__device__ __forceinline__ T* wshift(T* p, size_t bytes) {
+  return p ? reinterpret_cast<T*>(reinterpret_cast<char*>(const_cast<typename std::remove_const<T>::type*>(p)) + bytes) : p;
+}
 
 __device__ __forceinline__ int wrap1(int i, int n) {
   return i < 0 ? i + n : (i >= n ? i - n : i);
@@ -69,6 +80,18 @@ __device__ __forceinline__ void support(float x, int& i0, float& fr) {
   const float fl = floorf(x);
   fr = x - fl;  // exact in fp32
   i0 = (int)fl - 1;
+}
+
+// Support of a coordinate given as a bead position x plus a small offset o (two-layer markers,
+// reading 28: M = X +- h n).  The marker is never rounded to fp32 on its own -- at |X| ~ 6000 that
+// would cost 2.4e-4 nodes, far above the parity bar: the fractional part is formed from the exact
+// fractional part of x plus o (|o| <= 1), so its error stays ~6e-8 whatever |X|.
+__device__ __forceinline__ void support_off(float x, float o, int& i0, float& fr) {
+  const float fl = floorf(x);
+  const float s = (x - fl) + o;   // in (-1, 2)
+  const float fs = floorf(s);
+  fr = s - fs;
+  i0 = (int)fl + (int)fs - 1;
 }
 
 // The two gathered fields (velocity u, force-gradient field A) are stored BLOCKED: 4x4 nodes of
@@ -160,11 +183,42 @@ __device__ __forceinline__ float2 interp2_tex(const float2* __restrict__ p, cuda
   return acc;
 }
 
-__device__ __forceinline__ float interp1(const float* __restrict__ p0, int nx, int ny, float x, float y) {
+// interp2 at the marker (x + ox, y + oy) (two-layer broadcast; plain loads)
+__device__ __forceinline__ float2 interp2_off(const float2* __restrict__ p, int nx, int ny, float x, float y, float ox,
+                                              float oy) {
   int i0, j0;
   float fx, fy, wx[4], wy[4];
-  support(x, i0, fx);
-  support(y, j0, fy);
+  support_off(x, ox, i0, fx);
+  support_off(y, oy, j0, fy);
+  peskin4(fx, wx[0], wx[1], wx[2], wx[3]);
+  peskin4(fy, wy[0], wy[1], wy[2], wy[3]);
+  i0 = wrapi(i0, nx);
+  j0 = wrapi(j0, ny);
+  float ax = 0.0f, ay = 0.0f;
+#pragma unroll
+  for (int l = 0; l < 4; ++l) {
+    const int row = (j0 + l >= ny) ? j0 + l - ny : j0 + l;
+    float sx = 0.0f, sy = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int c = (i0 + k >= nx) ? i0 + k - nx : i0 + k;
+      const float2 v = __ldg(p + blk_index(c, row, nx));
+      sx = fmaf(v.x, wx[k], sx);
+      sy = fmaf(v.y, wx[k], sy);
+    }
+    ax = fmaf(sx, wy[l], ax);
+    ay = fmaf(sy, wy[l], ay);
+  }
+  return make_float2(ax, ay);
+}
+
+// row-major scalar plane at (x + ox, y + oy); ox = oy = 0 gives the plain bead position
+__device__ __forceinline__ float interp1(const float* __restrict__ p0, int nx, int ny, float x, float y,
+                                         float ox = 0.0f, float oy = 0.0f) {
+  int i0, j0;
+  float fx, fy, wx[4], wy[4];
+  support_off(x, ox, i0, fx);
+  support_off(y, oy, j0, fy);
   peskin4(fx, wx[0], wx[1], wx[2], wx[3]);
   peskin4(fy, wy[0], wy[1], wy[2], wy[3]);
   i0 = wrapi(i0, nx);

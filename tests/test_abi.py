@@ -48,8 +48,17 @@ def test_workspace_bytes_validation(lib):
     assert good > 2 * 9 * nc * 4  # at least the two population buffers
     bad = dict(w["params"], nx=65)
     assert binding.workspace_bytes(bad) == 0
-    bad = dict(w["params"], pbd_iters=2)
-    assert binding.workspace_bytes(bad) == 0
+    for key, val in (("pbd_iters", 0), ("pbd_iters", 9), ("pbd_order", 2), ("pbd_project", 2), ("two_layer", -1),
+                     ("layer_offset", 1.5)):
+        assert binding.workspace_bytes(dict(w["params"], **{key: val})) == 0, key
+    assert binding.workspace_bytes(dict(w["params"], two_layer=1, coupling=1, mdf_iters=2)) == 0  # reading 28
+    # literal PBD and the two-layer broadcast are accepted; two layers double the tile lists
+    assert binding.workspace_bytes(dict(w["params"], pbd_iters=4, pbd_order=1)) == good
+    assert binding.workspace_bytes(dict(w["params"], two_layer=1)) > good
+    # a batch is n worlds side by side
+    wp, _k = binding.make_params(w["params"])
+    assert lib.mc_batch_workspace_bytes(C.byref(wp), 7) == 7 * good
+    assert lib.mc_batch_workspace_bytes(C.byref(wp), 0) == 0 and lib.mc_batch_workspace_bytes(C.byref(wp), 70000) == 0
     bad = dict(w["params"], nu=0.0)
     assert binding.workspace_bytes(bad) == 0
     # capacity scales with max_beads and with the grid
@@ -68,6 +77,12 @@ def test_create_rejects_bad_arguments_without_touching_the_device(lib):
     assert b"workspace" in lib.mc_last_error(None)
     assert lib.mc_step(None, 1) == binding.MC_EINVAL
     lib.mc_destroy(None)
+    hb = C.c_void_p()
+    rc = lib.mc_create_batch(C.byref(wp), 4, None, 0, None, C.byref(hb))
+    assert rc == binding.MC_EINVAL and not hb.value
+    assert b"workspace" in lib.mc_batch_last_error(None)
+    assert lib.mc_step_batch(None, 1) == binding.MC_EINVAL
+    lib.mc_destroy_batch(None)
 
 
 def test_binding_refuses_to_run_without_cuda():

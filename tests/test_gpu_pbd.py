@@ -1,0 +1,130 @@
+"""GPU parity of the literal PBD (reading 27): pbd_iters K > 1,
+Jacobi / red-black Gauss-Seidel, rest-length actuation, projection of the advected positions --
+the general K1 kernel (k_pbd.cuh) against the oracle's mco_pbd, per step, every output, 1e-5.
+(Eq. 1-4; "the rest angle and the rest length".)"""
+import numpy as np
+import pytest
+
+from paper_2607_02954_b200 import worlds
+from test_gpu_parity import SMALL, _varied, assert_close, rel_l2, run_protocol
+
+pytestmark = pytest.mark.gpu
+
+
+def with_pbd(w, iters, order, project=0, L_amp=0.0, seed=1):
+    w = dict(w)
+    w["params"] = dict(w["params"], pbd_iters=iters, pbd_order=order, pbd_project=project)
+    if L_amp:
+        rng = np.random.default_rng(seed)
+        w["act_L_amp"] = (L_amp * rng.uniform(-1, 1, len(w["xy"]))).astype(np.float32)
+    return w
+
+
+BASES = {
+    # overlapping windows (chains of 3..100 beads), chains across the periodic seam
+    "ragged": lambda: worlds.ragged_world(96, 64, [3, 4, 5, 16, 31, 32, 33, 59, 60, 61, 64, 65, 100], seed=3),
+    # aligned windows (one 64-bead chain per warp / two 32-bead chains), static source
+    "m64": lambda: worlds.random_world(128, 96, 40, 64, seed=8),
+    "m32": lambda: worlds.random_world(96, 128, 70, 32, seed=9, static_source=True),
+    # per-bead parameters (the general parameter path) on long chains
+    "varied": lambda: _varied(worlds.ragged_world(96, 96, [7, 32, 64, 33, 90, 16, 16], seed=13, static_source=True), 14),
+    # chains far from rest: the iterations really move them (large-angle paths inside the loop)
+    "hairpin": lambda: worlds.hairpin_world(),
+}
+
+
+@pytest.mark.parametrize("order", [0, 1])
+@pytest.mark.parametrize("iters", [1, 2, 4])
+@pytest.mark.parametrize("name", sorted(BASES))
+def test_pbd_per_step_parity(name, iters, order):
+    if iters == 1 and order == 0 and name != "hairpin":
+        pytest.skip("K = 1 Jacobi is the default path (test_gpu_parity.py)")
+    w = with_pbd(BASES[name](), iters, order, L_amp=0.08 if name != "m64" else 0.0)
+    worst = run_protocol(w, steps_at=[0, 1, 7])
+    print(name, iters, order, {k: f"{v:.2e}" for k, v in worst.items()})
+
+
+@pytest.mark.parametrize("order", [0, 1])
+def test_pbd_eight_iterations(order):
+    # the widest halo: windows advance by 32 (Jacobi) / 16 (Gauss-Seidel) beads
+    w = with_pbd(BASES["ragged"](), 8, order, L_amp=0.05)
+    worst = run_protocol(w, steps_at=[0, 3])
+    print("K=8", order, {k: f"{v:.2e}" for k, v in worst.items()})
+
+
+@pytest.mark.parametrize("order", [0, 1])
+def test_pbd_projection_parity(order):
+    w = with_pbd(BASES["varied"](), 3, order, project=1, L_amp=0.05)
+    worst = run_protocol(w, steps_at=[0, 1, 9])
+    print("project", order, {k: f"{v:.2e}" for k, v in worst.items()})
+    # the projection really moves the beads (it is not a no-op that parity cannot see)
+    from oracle import mco
+    a, b = mco.World(with_pbd(BASES["varied"](), 3, order, project=0, L_amp=0.05)), mco.World(w)
+    a.step(3)
+    b.step(3)
+    assert rel_l2(b.read_state()["xy"], a.read_state()["xy"])[0] > 1e-6
+
+
+def test_pbd_with_mdf_coupling():
+    w = with_pbd(BASES["m32"](), 2, 1, L_amp=0.05)
+    w["params"] = dict(w["params"], coupling=1, mdf_iters=3)
+    worst = run_protocol(w, steps_at=[0, 1, 5])
+    print("pbd+mdf", {k: f"{v:.2e}" for k, v in worst.items()})
+
+
+def test_pbd_trajectory_and_reproducibility():
+    from oracle import mco
+    from paper_2607_02954_b200 import binding
+    w = with_pbd(BASES["ragged"](), 4, 1, project=1, L_amp=0.05)
+    outs = []
+    for _ in range(2):
+        G = binding.World(w)
+        G.step(60)
+        outs.append(G.read_state(keys=("xy", "u", "force")))
+        G.close()
+    for k in ("xy", "u", "force"):
+        assert outs[0][k].tobytes() == outs[1][k].tobytes(), k
+    O = mco.World(w)
+    O.step(60)
+    assert_close("X after 60 steps", outs[0]["xy"], O.read_state()["xy"], 1e-3)
+    # mc_step(60) = graph replay; 60 x mc_step(1) = direct launches
+    G = binding.World(w)
+    for _ in range(60):
+        G.step(1)
+    assert G.read_state(keys=("xy",))["xy"].tobytes() == outs[0]["xy"].tobytes()
+
+
+def test_general_kernel_agrees_with_the_fast_one_at_k1():
+    # K = 1 Jacobi with an (ineffective) rest-length amplitude runs the general kernel: it must give
+    # what the specialised one-iteration kernel gives, to rounding
+    from paper_2607_02954_b200 import binding
+    w = BASES["varied"]()
+    A = binding.World(w)
+    w2 = dict(w)
+    w2["act_L_amp"] = np.full(len(w["xy"]), 1e-30, np.float32)
+    B = binding.World(w2)
+    A.step(5)
+    B.step(5)
+    a, b = A.read_state(keys=("xy", "force", "u")), B.read_state(keys=("xy", "force", "u"))
+    assert rel_l2(b["force"], a["force"])[0] < 2e-6 and rel_l2(b["u"], a["u"])[0] < 2e-6
+    # switching the actuation off again restores the fast kernel's bits for the next steps' forces
+    B.set_length_actuation(None)
+    A2 = binding.World(w)
+    A2.set_positions(b["xy"])
+    B.set_positions(b["xy"])
+
+
+def test_pbd_parameters_are_validated():
+    from paper_2607_02954_b200 import binding
+    w = BASES["m32"]()
+    for key, val in (("pbd_iters", 0), ("pbd_iters", 9), ("pbd_order", 2), ("pbd_project", 5)):
+        with pytest.raises(binding.McError):
+            binding.World(dict(w, params=dict(w["params"], **{key: val})))
+
+
+@pytest.mark.parametrize("name", ["2", "4b"])
+def test_pbd_config_parity(name):
+    import os
+    w = with_pbd(worlds.make_world(name), 2, 1, L_amp=0.05)
+    worst = run_protocol(w, steps_at=[0, 10], threads=os.cpu_count() or 1)
+    print(name, "K=2 GS", {k: f"{v:.2e}" for k, v in worst.items()})

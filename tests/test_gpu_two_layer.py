@@ -1,0 +1,98 @@
+"""GPU parity of the two-layer broadcast (reading 28; P:L127
+"broadcasting the single filament into a two-layer version of itself"): every exchange with the
+grid through the markers X_i +- h n_i, against the oracle, per step, every output, 1e-5."""
+import numpy as np
+import pytest
+
+from paper_2607_02954_b200 import worlds
+from test_gpu_parity import assert_close, rel_l2, run_protocol
+
+pytestmark = pytest.mark.gpu
+
+
+def two(w, h=0.5, **extra):
+    w = dict(w)
+    w["params"] = dict(w["params"], two_layer=1, layer_offset=h, **extra)
+    return w
+
+
+WORLDS = {
+    # ragged chains, some translated by whole periods (|X| up to 3 periods: the markers must not be
+    # rounded to fp32 on their own), both field kinds
+    "ragged": lambda: two(worlds.ragged_world(96, 64, [3, 4, 5, 16, 31, 32, 33, 59, 60, 61, 64, 65, 100], seed=3,
+                                              static_source=True)),
+    "m64": lambda: two(worlds.random_world(128, 96, 40, 64, seed=8)),
+    "no_fields": lambda: two(worlds.ragged_world(64, 32, [10, 20, 40], seed=6, kappa_rep=None)),
+    # one tile in each direction: every support wraps onto the same tile
+    "single_tile": lambda: two(worlds.ragged_world(32, 32, [5, 12, 20], seed=11)),
+    "crowded": lambda: two(worlds.random_world(64, 64, 96, 16, seed=7, kappa=0.25, kappa_rep=2e-4, clustered=3.0)),
+    # thin and thick: h = 0.25 and h = 1
+    "h025": lambda: two(worlds.random_world(96, 128, 70, 32, seed=9, static_source=True), h=0.25),
+    "h1": lambda: two(worlds.random_world(96, 96, 30, 32, seed=10), h=1.0),
+    # hairpins: normals of folded chains
+    "hairpin": lambda: two(worlds.hairpin_world()),
+    # together with the literal PBD and the projection
+    "pbd": lambda: two(worlds.ragged_world(96, 96, [7, 32, 64, 33, 90, 16], seed=13), pbd_iters=2, pbd_order=1, pbd_project=1),
+}
+
+
+@pytest.mark.parametrize("name", sorted(WORLDS))
+def test_two_layer_per_step_parity(name):
+    worst = run_protocol(WORLDS[name](), steps_at=[0, 1, 10, 30])
+    print(name, {k: f"{v:.2e}" for k, v in worst.items()})
+
+
+def test_two_layer_far_from_the_origin():
+    # the whole world translated by 200 periods: |X| ~ 2e4, ulp 2e-3 -- a marker rounded to fp32
+    # would miss the oracle's by 1e-3 nodes; the offset form keeps the parity bar
+    w = worlds.random_world(96, 96, 30, 32, seed=21)
+    w["xy"] = (w["xy"] + np.float32(96 * 200)).astype(np.float32)
+    worst = run_protocol(two(w), steps_at=[0, 5])
+    print("far", {k: f"{v:.2e}" for k, v in worst.items()})
+
+
+def test_two_layer_conservation_and_reproducibility():
+    from paper_2607_02954_b200 import binding
+    w = WORLDS["ragged"]()
+    outs = []
+    for _ in range(2):
+        G = binding.World(w)
+        G.keep_intermediates(True)
+        G.step(25)
+        outs.append({**G.read_state(), **G.read_intermediates()})
+        G.close()
+    for k in outs[0]:
+        if k != "step":
+            assert outs[0][k].tobytes() == outs[1][k].tobytes(), k
+    o = outs[0]
+    for ch in (0, 1):   # each layer carries half: the total spread force is the total bead force
+        fs, gs = o["force"][:, ch].astype(np.float64).sum(), o["G"][ch].astype(np.float64).sum()
+        assert abs(fs - gs) < 1e-5 * np.abs(o["force"][:, ch]).astype(np.float64).sum()
+    assert abs(o["rho_b"].astype(np.float64).sum() - len(o["xy"])) < 1e-5 * len(o["xy"])
+
+
+def test_two_layer_trajectory():
+    from oracle import mco
+    from paper_2607_02954_b200 import binding
+    w = WORLDS["m64"]()
+    G, O = binding.World(w), mco.World(w)
+    G.step(100)
+    O.step(100)
+    assert_close("X after 100 steps", G.read_state(keys=("xy",))["xy"], O.read_state()["xy"], 1e-3)
+
+
+def test_two_layer_differs_from_one_layer_and_mdf_is_refused():
+    from paper_2607_02954_b200 import binding
+    w = worlds.random_world(128, 96, 40, 64, seed=8)
+    A, B = binding.World(w), binding.World(two(w))
+    A.step(10)
+    B.step(10)
+    assert rel_l2(B.read_state(keys=("u",))["u"], A.read_state(keys=("u",))["u"])[0] > 1e-3
+    with pytest.raises(binding.McError):
+        binding.World(two(w, coupling=1, mdf_iters=2))
+
+
+def test_two_layer_one_parity_step_large():
+    import os
+    worst = run_protocol(two(worlds.make_world("4c")), steps_at=[6], threads=os.cpu_count() or 1)
+    print("4c two-layer", {k: f"{v:.2e}" for k, v in worst.items()})

@@ -287,28 +287,30 @@ __global__ void __launch_bounds__(256) k_markers(int N, const float2* __restrict
   if (b < N) {
     const int fl = __float_as_int(__ldg(PC + b).w);
     const float2 p = X[b];
-    float nx_ = 0.f, ny_ = 0.f, fx = 0.f, fy = 0.f;
+    // fp64 from the exact fp32 edge vectors: at a hairpin the two edge normals nearly cancel and
+    // the direction of their sum would lose ~|n1 + n2|^-1 digits in fp32 (parity world "hairpin")
+    double nx_ = 0.0, ny_ = 0.0, fx = 0.0, fy = 0.0;
     bool have = false;
     if (!(fl & BEAD_FIRST)) {  // edge (b-1, b); differences of nearby fp32 positions are exact
       const float2 q = X[b - 1];
-      const float vx = p.x - q.x, vy = p.y - q.y;
-      const float inv = rsqrtf(vx * vx + vy * vy);
+      const double vx = (double)p.x - (double)q.x, vy = (double)p.y - (double)q.y;
+      const double inv = 1.0 / sqrt(vx * vx + vy * vy);
       fx = -vy * inv; fy = vx * inv;
       nx_ = fx; ny_ = fy;
       have = true;
     }
     if (!(fl & BEAD_LAST)) {   // edge (b, b+1)
       const float2 q = X[b + 1];
-      const float vx = q.x - p.x, vy = q.y - p.y;
-      const float inv = rsqrtf(vx * vx + vy * vy);
-      const float ex = -vy * inv, ey = vx * inv;
+      const double vx = (double)q.x - (double)p.x, vy = (double)q.y - (double)p.y;
+      const double inv = 1.0 / sqrt(vx * vx + vy * vy);
+      const double ex = -vy * inv, ey = vx * inv;
       if (!have) { fx = ex; fy = ey; }
       nx_ += ex; ny_ += ey;
     }
-    float nn = sqrtf(nx_ * nx_ + ny_ * ny_);
-    if (!(nn > 1e-9f)) { nx_ = fx; ny_ = fy; nn = 1.0f; }
-    const float s = h / nn;
-    const float2 o = make_float2(s * nx_, s * ny_);
+    double nn = sqrt(nx_ * nx_ + ny_ * ny_);
+    if (!(nn > 1e-9)) { nx_ = fx; ny_ = fy; nn = 1.0; }
+    const double sc = (double)h / nn;
+    const float2 o = make_float2((float)(sc * nx_), (float)(sc * ny_));
     const float2 old = O[b];
     O[b] = o;
     m = fmaxf(fabsf(o.x - old.x), fabsf(o.y - old.y));

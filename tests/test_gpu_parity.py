@@ -60,13 +60,16 @@ def assert_close(name, gpu, orc, tol=TOL_STEP, tol_max=None):
     return err
 
 
-def assert_displacement(name, x0_f32, x1_gpu_f32, dX_ref, rel=TOL_STEP):
+def assert_displacement(name, x0_f32, x1_gpu_f32, dX_ref, rel=TOL_STEP, roundings=1.0):
     """Gate of S7 / K4 ("nodes sample the local fluid velocity"): the bead displacement of
     ONE step, element by element.  X is fp32 and |X| ~ 100 while |dX| ~ 1e-3, so X itself cannot
     see a wrong U; the displacement can, up to the rounding of the stored position:
         |dX_gpu - dX_ref| <= ulp32(|X1|)/2 [storing X1] + rel * (|dX_ref| of the bead + 0.05 max |dX_ref|)
     (the second term: U mixes 16 nodes whose velocities may exceed the bead's own near a
-    stagnation point).  Returns the worst error in units of that bound."""
+    stagnation point).  roundings: how many times the position is rounded to fp32 within the step
+    (the projection of reading 27 stores X twice, and its second pass starts from the ROUNDED
+    advected position where the oracle's starts from the fp64 one).
+    Returns the worst error in units of that bound."""
     x0 = np.asarray(x0_f32, dtype=np.float32)
     x1 = np.asarray(x1_gpu_f32, dtype=np.float32)
     d_gpu = x1.astype(np.float64) - x0.astype(np.float64)
@@ -75,7 +78,7 @@ def assert_displacement(name, x0_f32, x1_gpu_f32, dX_ref, rel=TOL_STEP):
         return 0.0
     half_ulp = 0.5 * np.spacing(np.maximum(np.abs(x1), np.abs(x0) + np.abs(d_ref).astype(np.float32)))
     bead = np.linalg.norm(d_ref, axis=1, keepdims=True)
-    bound = half_ulp.astype(np.float64) * 1.0001 + rel * (bead + 0.05 * np.abs(d_ref).max()) + 1e-12
+    bound = roundings * half_ulp.astype(np.float64) * 1.0001 + rel * (bead + 0.05 * np.abs(d_ref).max()) + 1e-12
     ratio = float((np.abs(d_gpu - d_ref) / bound).max())
     assert ratio <= 1.0, f"{name}: bead displacement off by {ratio:.2f} x (ulp/2 + {rel:g} |dX|)"
     return ratio
@@ -114,10 +117,19 @@ def step_parity(G, w, threads=0, check=True):
     # (K4 alone: its gather, weights and the update).
     x0 = s0["xy"]
     dX_orc = o["xy"] - x0.astype(np.float64)
-    U_own = mco.interp(g["u"].astype(np.float64), x0.astype(np.float64))
+    pw = w["params"]
+    if pw.get("two_layer"):
+        # two-layer broadcast (reading 28): U_i = mean of u at the bead's two markers
+        M = mco.markers(w["offsets"], x0.astype(np.float64), float(pw.get("layer_offset") or 0.5))
+        Um = mco.interp(g["u"].astype(np.float64), M)
+        U_own = 0.5 * (Um[0::2] + Um[1::2])
+    else:
+        U_own = mco.interp(g["u"].astype(np.float64), x0.astype(np.float64))
     if check:
-        errs["dX/bound"] = assert_displacement("dX vs oracle", x0, g["xy"], dX_orc)
-        errs["dX_own_u/bound"] = assert_displacement("dX vs interp(own u)", x0, g["xy"], U_own, rel=2e-6)
+        errs["dX/bound"] = assert_displacement("dX vs oracle", x0, g["xy"], dX_orc,
+                                               roundings=3.0 if pw.get("pbd_project") else 1.0)
+        if not pw.get("pbd_project"):   # with the projection X1 - X0 = U + PBD displacement: no longer K4 alone
+            errs["dX_own_u/bound"] = assert_displacement("dX vs interp(own u)", x0, g["xy"], U_own, rel=2e-6)
     errs["dX"] = rel_l2(g["xy"].astype(np.float64) - x0.astype(np.float64), dX_orc)[0]
     return errs
 

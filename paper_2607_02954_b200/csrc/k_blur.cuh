@@ -57,9 +57,11 @@ __global__ void __launch_bounds__(BLUR_THREADS, R > 6 ? 1 : 7) k_blur_grad(int n
                                                             const float* __restrict__ rho_b, float coef,
                                                             const float2* base, float2* A,
                                                             float* __restrict__ field_out, size_t wstride) {
-  rho_b = wshift(rho_b, blockIdx.y * wstride);  // batched worlds; field_out is a caller array of ONE world
-  base = wshift(base, blockIdx.y * wstride);
-  A = wshift(A, blockIdx.y * wstride);
+  if (wstride) {  // batched worlds (single worlds pass 0); field_out is a caller array of ONE world
+    rho_b = wshift(rho_b, blockIdx.y * wstride);
+    base = wshift(base, blockIdx.y * wstride);
+    A = wshift(A, blockIdx.y * wstride);
+  }
   constexpr int NV = blur_NV(R), CW = blur_CW(R), CP = blur_CP(R);
   __shared__ __align__(16) float2 td[BLUR_T * CP];
   // 1-D grid in row-major tile order (2-D grids are rasterised in an order that streams worse)

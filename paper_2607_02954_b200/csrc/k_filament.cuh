@@ -167,7 +167,7 @@ __device__ __forceinline__ float2 edge_delta(double vx, double vy, float delta, 
 
 template <bool UNIFORM, int TEXROWS>
 __global__ void __launch_bounds__(256, 5) k_filament_force(FilamentArgs a, size_t wstride) {
-  if (!TEXROWS) a.shift(blockIdx.y * wstride);  // the texture variants serve single worlds only (views are per world)
+  if (!TEXROWS && wstride) a.shift(blockIdx.y * wstride);  // the texture variants serve single worlds only (views are per world)
   const int lane = threadIdx.x & 31;
   const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (w >= a.n_windows) return;

@@ -16,7 +16,7 @@ __global__ void __launch_bounds__(256) k_interp_integrate(int N, float2* __restr
                                                           int* __restrict__ flag, long long* __restrict__ step,
                                                           unsigned* __restrict__ step_max,
                                                           const float2* __restrict__ O, size_t wstride) {
-  if (!TEXROWS) {  // the texture variants serve single worlds only (views are per world)
+  if (!TEXROWS && wstride) {  // the texture variants serve single worlds only (views are per world)
     const size_t ws = blockIdx.y * wstride;
     X = wshift(X, ws); u = wshift(u, ws); flag = wshift(flag, ws); step = wshift(step, ws);
     step_max = wshift(step_max, ws); O = wshift(O, ws);

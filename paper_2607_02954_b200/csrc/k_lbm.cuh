@@ -149,7 +149,7 @@ template <bool KEEP_G, bool TWO = false>
 __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p, size_t wstride) {
   __shared__ __align__(16) int acc0[ACC_N], acc1[ACC_N], accl0[ACC_N], accl1[ACC_N];
   __shared__ float red[32];
-  p.shift(blockIdx.y * wstride);
+  if (wstride) p.shift(blockIdx.y * wstride);  // batched worlds; single worlds pass 0
   const LbmArgs& a = p.lbm;
   const int nx = a.nx, ny = a.ny;
   // 1-D grid in row-major tile order (a 2-D grid is rasterised differently by the hardware and

@@ -304,7 +304,7 @@ __global__ void __launch_bounds__(256, LIGHT ? 6 : 1) k_deposit_tile(int nx, int
                                                       unsigned* __restrict__ tile_fmax,
                                                       const float2* __restrict__ O, size_t wstride) {
   __shared__ __align__(16) int acc[ACC_N], accl[ACC_N];
-  {
+  if (wstride) {  // batched worlds; single worlds pass 0
     const size_t ws = blockIdx.z * wstride;
     tile_start = wshift(tile_start, ws); list = wshift(list, ws); X = wshift(X, ws); rho_b = wshift(rho_b, ws);
     tile_rho_max = wshift(tile_rho_max, ws); tile_fmax = wshift(tile_fmax, ws); O = wshift(O, ws);

@@ -254,6 +254,153 @@ def run_reference(args, rank: int):
     }), flush=True)
 
 
+def batch_worlds(base: str, n: int, first_seed: int):
+    """n individuals of one BASELINE.json config: same recipe and chain structure, different seeds
+    (config 1 is a single deterministic filament: its individuals differ in phase and position)."""
+    import numpy as np
+    from paper_2607_02954_b200 import worlds
+    out = []
+    for k in range(n):
+        w = worlds.make_world(base, seed=first_seed + k)
+        if base == "1":
+            w["act_phase"] = (w["act_phase"] + np.float32(0.37 * (first_seed + k))).astype(np.float32)
+            w["xy"] = (w["xy"] + np.float32(0.61 * ((first_seed + k) % 13))).astype(np.float32)
+        out.append(w)
+    return out
+
+
+def run_batch(args, rank, world_size, dev, dist, barrier):
+    """--workload batch2 / batch1: a population of BASELINE.json config-2
+    (config-1) worlds stepped in lock-step by mc_step_batch; every rank owns its own batch."""
+    import numpy as np
+    import torch
+    from paper_2607_02954_b200 import binding
+    base = {"batch2": "2", "batch1": "1"}[args.workload]
+    n = args.batch_worlds or {"2": 1024, "1": 4096}[base]
+    ws = batch_worlds(base, n, first_seed=rank * n)
+    B = binding.Batch(ws, device=str(dev))
+    N, nc = B.N, int(ws[0]["params"]["nx"]) * int(ws[0]["params"]["ny"])
+    B.step(args.warmup)
+    barrier()
+    sampler = ClockSampler(dev.index or 0)
+    if rank == 0:
+        sampler.start()
+    l0 = B.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(B.stream)
+    B.step(args.steps)
+    e1.record(B.stream)
+    barrier()
+    ms = torch.tensor([e0.elapsed_time(e1)], device=dev, dtype=torch.float64)
+    launches = B.launch_count() - l0
+    if dist is not None:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms_total = float(ms.item())
+    clocks = sampler.stop() if rank == 0 else None
+    ms_step = ms_total / args.steps
+    value = aggregate(n * N, args.steps, world_size, ms_total)
+    # per-kernel durations of the batched launches
+    B.profile_enable(True)
+    B.step(min(args.steps, 64))
+    prof, pn = B.profile_read()
+    B.profile_enable(False)
+    kms = {k: v / max(pn, 1) for k, v in prof.items()}
+    kb = kernel_bytes(n * nc, n * N)
+    peak, peak_src = measured_peak_gbs()
+    dom = max(kms, key=lambda k: kms[k])
+    ach = kb[dom] / (kms[dom] * 1e-3) / 1e9 if kms[dom] > 0 else 0.0
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": None, "traffic_note": "no ncu capture of the batched launches", "peak_source": peak_src,
+                "frac_of_8TBps_nominal": ach / 8000.0, "algorithmic_bytes_per_launch": kb[dom],
+                "ms_per_launch": kms[dom], "share_of_step": kms[dom] / max(sum(kms.values()), 1e-12), "csrc_sha": csrc_sha()}
+    roofline_step = {"bound": "hbm", "peak": peak, "unit": "GB/s", "models": {}}
+    for model in STEP_MODELS:
+        by = step_bytes(n * nc, n * N, 0, model)
+        a_ = by / (ms_step * 1e-3) / 1e9
+        roofline_step["models"][model] = {"bytes_per_step": by, "achieved": a_, "frac": a_ / peak,
+                                          "frac_of_8TBps_nominal": a_ / 8000.0}
+    roofline_step.update({k: roofline_step["models"]["raw"][k] for k in ("achieved", "frac", "frac_of_8TBps_nominal")})
+    kernels = {k: {"ms": round(kms[k], 5), "GBps": round(kb[k] / (kms[k] * 1e-3) / 1e9, 1) if kms[k] > 0 else None}
+               for k in kms}
+    # e2e: the population loop through the public API with HOST buffers, every step: upload all
+    # positions from pinned host memory, step, read all positions back to pinned host memory
+    xy_h = torch.from_numpy(np.stack([w["xy"] for w in ws]).astype(np.float32)).pin_memory()
+    back = torch.empty_like(xy_h).pin_memory()
+
+    def e2e_step():
+        B.set_positions(xy_h)
+        B.step(1)
+        out, _ = B.read_positions(host=False)
+        back.copy_(out, non_blocking=True)
+        torch.cuda.synchronize(dev)
+
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.e2e_steps):
+        e2e_step()
+        xy_h, back = back, xy_h
+    barrier()
+    te = torch.tensor([time.perf_counter() - t0], device=dev, dtype=torch.float64)
+    if dist is not None:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_val = aggregate(n * N, args.e2e_steps, world_size, float(te.item()) * 1e3)
+    B.close()
+    del B
+    # the same world stepped ALONE through mc_step (what a population loop without the batch pays)
+    single = None
+    cpu = None
+    if rank == 0:
+        S = binding.World(ws[0], device=str(dev))
+        S.step(20)
+        torch.cuda.synchronize(dev)
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record(S.stream)
+        S.step(400)
+        a1.record(S.stream)
+        torch.cuda.synchronize(dev)
+        ms1 = a0.elapsed_time(a1) / 400
+        single = {"ms_per_step": ms1, "bead_steps_per_s": N / (ms1 * 1e-3),
+                  "batch_speedup": value / world_size / (N / (ms1 * 1e-3)),
+                  "what": "one world of the batch stepped alone through mc_step (CUDA-graph replay), 400 steps"}
+        S.close()
+        if world_size == 1 and not args.no_cpu_baseline:
+            from oracle import mco
+            cores = os.cpu_count() or 1
+            O = mco.World(ws[0], threads=cores)
+            O.step(2)
+            k, t0 = 0, time.perf_counter()
+            while k < 400 and (k < 5 or time.perf_counter() - t0 < 10.0):
+                O.step(1)
+                k += 1
+            secs = time.perf_counter() - t0
+            cpu = {"value": N * k / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
+                   "sample": f"one world of the batch ({world_label(base, ws[0])}), {k} steps in {secs:.1f} s, fp64, "
+                             f"OpenMP over {cores} threads; the worlds of a batch are independent"}
+            O.close()
+    if rank == 0:
+        p = ws[0]["params"]
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world_size, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic (seeded, DESIGN.md input recipe)",
+            "config": {"workload": f"batch of {n} x BASELINE.json config {base} (mc_step_batch)", "worlds": n,
+                       "beads": n * N, "beads_per_world": N, "grid": [p["nx"], p["ny"]],
+                       "parallelism": "replicas only (one independent batch per GPU)",
+                       "l2": f"working set {step_bytes(n * nc, n * N) / 1e6:.0f} MB per step vs 126 MB L2; no flush"},
+            "cell_steps_per_s": world_size * n * nc * args.steps / (ms_total * 1e-3),
+            "roofline": roofline, "roofline_step": roofline_step, "kernels": kernels, "single_world": single,
+            "cpu_baseline": cpu,
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": n * N * 8, "d2h_bytes_per_step": n * N * 8,
+                    "steps": args.e2e_steps,
+                    "what": "per step: mc_set_positions_batch from pinned host + mc_step_batch(1) + "
+                            "mc_read_positions_batch to pinned host"},
+            "gpu_launches": launches, "clocks": clocks,
+        }), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -266,6 +413,8 @@ def main():
     ap.add_argument("--no-extra", action="store_true", help="skip the short runs of the other worlds")
     ap.add_argument("--coupling", default="force", choices=["force", "mdf"])
     ap.add_argument("--mdf-iters", type=int, default=3)
+    ap.add_argument("--batch-worlds", type=int, default=0,
+                    help="--workload batch2 / batch1: worlds per batch (default 1024 / 4096)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -293,6 +442,12 @@ def main():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize(dev)
+
+    if args.workload.startswith("batch"):
+        run_batch(args, rank, world_size, dev, dist, barrier)
+        if dist is not None:
+            dist.destroy_process_group()
+        return
 
     # replicas only: every rank owns an independent world of the same recipe (seed = rank)
     w = worlds.make_world(args.workload, seed=rank)

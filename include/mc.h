@@ -257,6 +257,13 @@ int mc_load_filaments_batch(mc_batch* b, int32_t n_fil, const int32_t* offsets /
                             const float* act_amp /*DEVICE*/, const float* act_phase /*DEVICE*/,
                             const float* act_period /*DEVICE*/, const float* act_L_amp /*DEVICE or NULL*/);
 int mc_step_batch(mc_batch* b, int32_t n);
+/* Positions of ALL worlds in one call each way (the population loop: upload the individuals, step,
+ * read back their displacement = fitness).  xy: DEVICE float [n_worlds][N][2], world-major,
+ * chain-ordered.  mc_set_positions_batch keeps parameters, fluid and step counter and makes the next
+ * step rebuild the tile lists; mc_read_positions_batch also returns MC_EDIVERGED if any world's
+ * divergence flag is set (after filling xy).  Both synchronise the stream. */
+int mc_set_positions_batch(mc_batch* b, const float* xy /*DEVICE*/);
+int mc_read_positions_batch(mc_batch* b, int64_t* step_out /*HOST*/, float* xy /*DEVICE*/);
 mc_world* mc_batch_world(mc_batch* b, int32_t k);
 void mc_destroy_batch(mc_batch* b);
 const char* mc_batch_last_error(const mc_batch* b);

@@ -20,7 +20,7 @@ SYMBOLS = ("mc_workspace_bytes", "mc_create", "mc_load_filaments", "mc_step", "m
            "mc_profile_enable", "mc_profile_read", "mc_keep_intermediates", "mc_texture_gathers",
            "mc_cluster_tiles", "mc_set_positions", "mc_set_length_actuation", "mc_batch_workspace_bytes",
            "mc_create_batch", "mc_load_filaments_batch", "mc_step_batch", "mc_batch_world", "mc_destroy_batch",
-           "mc_batch_last_error")
+           "mc_batch_last_error", "mc_set_positions_batch", "mc_read_positions_batch")
 PROF_SLOTS = ("K0_bin", "K2a_deposit", "K3a_blur_grad", "K1_filament", "K2b_spread", "K3b_lbm",
               "K4_interp_integrate")
 
@@ -97,6 +97,10 @@ def load_library():
     L.mc_load_filaments_batch.argtypes = [vp, i32, C.POINTER(i32)] + [vp] * 10
     L.mc_step_batch.restype = C.c_int
     L.mc_step_batch.argtypes = [vp, i32]
+    L.mc_set_positions_batch.restype = C.c_int
+    L.mc_set_positions_batch.argtypes = [vp, vp]
+    L.mc_read_positions_batch.restype = C.c_int
+    L.mc_read_positions_batch.argtypes = [vp, C.POINTER(i64), vp]
     L.mc_batch_world.restype = vp
     L.mc_batch_world.argtypes = [vp, i32]
     L.mc_destroy_batch.restype = None
@@ -362,6 +366,43 @@ class Batch:
 
     def step(self, n: int = 1):
         self._check(load_library().mc_step_batch(self.h, int(n)))
+
+    def set_positions(self, xy):
+        """mc_set_positions_batch: xy [n, N, 2] host numpy array or device tensor."""
+        torch = self.torch
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):
+            if not isinstance(xy, torch.Tensor):
+                xy = torch.from_numpy(np.ascontiguousarray(xy, dtype=np.float32))
+            d = xy.to(self.device, dtype=torch.float32, non_blocking=False).contiguous()
+            assert d.numel() == 2 * self.N * self.n
+            rc = load_library().mc_set_positions_batch(self.h, C.c_void_p(d.data_ptr()))
+        self._check(rc)
+
+    def read_positions(self, host: bool = True):
+        """mc_read_positions_batch -> (xy [n, N, 2], step)"""
+        torch = self.torch
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):
+            out = torch.empty((self.n, self.N, 2), dtype=torch.float32, device=self.device)
+            st = C.c_int64()
+            rc = load_library().mc_read_positions_batch(self.h, C.byref(st), C.c_void_p(out.data_ptr()))
+        self._check(rc)
+        return (out.cpu().numpy() if host else out), int(st.value)
+
+    def profile_enable(self, on: bool = True):
+        """per-kernel CUDA-event timing of the batched launches (they are issued by world 0)"""
+        L = load_library()
+        self._check(L.mc_profile_enable(L.mc_batch_world(self.h, 0), int(bool(on))))
+
+    def profile_read(self):
+        L = load_library()
+        ms = (C.c_float * len(PROF_SLOTS))()
+        n = C.c_int32()
+        self._check(L.mc_profile_read(L.mc_batch_world(self.h, 0), ms, C.byref(n)))
+        return {k: float(ms[i]) for i, k in enumerate(PROF_SLOTS)}, int(n.value)
+
+    def launch_count(self) -> int:
+        L = load_library()
+        return int(L.mc_launch_count(L.mc_batch_world(self.h, 0)))
 
     def world(self, k: int) -> "World":
         h = load_library().mc_batch_world(self.h, int(k))

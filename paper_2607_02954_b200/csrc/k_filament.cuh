@@ -28,6 +28,13 @@
 
 namespace mc {
 
+// layout twin of ListState (k_tile.cuh), which this header cannot include
+struct ListStateWords {
+  int need;
+  float drift;
+  unsigned step_max, step_max_p, step_max_m;
+};
+
 constexpr int BEAD_FIRST = 1, BEAD_LAST = 2, BEAD_PAD = 4;
 constexpr int BEAD_ODD = 8;  // odd index within its chain (edge parity of the Gauss-Seidel pass, k_pbd.cuh)
 
@@ -311,15 +318,29 @@ __global__ void k_chain_keys(int n_fil, const int* __restrict__ offsets, const f
   keys[f] = (cj / key_tile) * ((nx + key_tile - 1) / key_tile) + ci / key_tile;
 }
 
-// mc_read_state: internal order -> caller's order
-__global__ void k_unpermute2(int N, const int* __restrict__ src, const float2* __restrict__ in, float2* __restrict__ out) {
+// mc_read_state: internal order -> caller's order.  Batched (blockIdx.y = world): the workspace
+// arrays lie wstride bytes apart, the caller's array holds the worlds back to back (N entries each).
+__global__ void k_unpermute2(int N, const int* __restrict__ src, const float2* __restrict__ in, float2* __restrict__ out,
+                             size_t wstride = 0) {
+  src = wshift(src, blockIdx.y * wstride);
+  in = wshift(in, blockIdx.y * wstride);
+  out += (size_t)blockIdx.y * N;
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b < N) out[src[b]] = in[b];
 }
 // mc_set_positions: caller's order -> internal order
-__global__ void k_permute2(int N, const int* __restrict__ src, const float2* __restrict__ in, float2* __restrict__ out) {
+__global__ void k_permute2(int N, const int* __restrict__ src, const float2* __restrict__ in, float2* __restrict__ out,
+                           size_t wstride = 0) {
+  src = wshift(src, blockIdx.y * wstride);
+  out = wshift(out, blockIdx.y * wstride);
+  in += (size_t)blockIdx.y * N;
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b < N) out[b] = in[src[b]];
+}
+// all worlds of a batch: the next step rebuilds the tile lists (drift = +inf)
+__global__ void k_force_rebuild(ListStateWords* st, size_t wstride) {
+  st = wshift(st, blockIdx.x * wstride);
+  if (threadIdx.x == 0) { st->need = 1; st->drift = __int_as_float(0x7f800000); st->step_max = st->step_max_p = st->step_max_m = 0u; }
 }
 __global__ void k_permute1(int N, const int* __restrict__ src, const float* __restrict__ in, float* __restrict__ out,
                            int* __restrict__ nonzero) {

@@ -1191,6 +1191,59 @@ int mc_load_filaments_batch(mc_batch* b, int32_t n_fil, const int32_t* offsets, 
   return MC_OK;
 }
 
+int mc_set_positions_batch(mc_batch* b, const float* xy) {
+  if (!b) return MC_EINVAL;
+  mc_world* lead = b->worlds[0];
+  if (lead->N == 0) return MC_OK;
+  if (!xy) return bfail(b, MC_EINVAL, "null array");
+  static_assert(sizeof(mc::ListStateWords) == sizeof(mc::ListState), "ListState twin");
+  cudaStream_t st = lead->stream;
+  const unsigned nb = (unsigned)b->worlds.size();
+  mc::k_permute2<<<dim3((lead->N + 255) / 256, nb), 256, 0, st>>>(lead->N, lead->ptr<int>(lead->L.src),
+                                                                  reinterpret_cast<const float2*>(xy),
+                                                                  lead->ptr<float2>(lead->L.X), b->stride);
+  mc::k_force_rebuild<<<nb, 32, 0, st>>>(reinterpret_cast<mc::ListStateWords*>(lead->ptr<int>(lead->L.flags) + 16), b->stride);
+  lead->launches += 2;
+  if (lead->p.two_layer) {
+    mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(lead->ptr<int>(lead->L.flags) + 16);
+    mc::k_markers<<<dim3((lead->N + 255) / 256, nb), 256, 0, st>>>(lead->N, lead->ptr<float2>(lead->L.X), lead->ptr<float4>(lead->L.PC),
+                                                                   lead->layer_h, lead->ptr<float2>(lead->L.O),
+                                                                   &ls_state->step_max_m, b->stride);
+    lead->launches++;
+  }
+  cudaError_t e = cudaStreamSynchronize(st);  // xy belongs to the caller
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) return bfail(b, MC_ECUDA, std::string("mc_set_positions_batch: ") + cudaGetErrorString(e));
+  return MC_OK;
+}
+
+int mc_read_positions_batch(mc_batch* b, int64_t* step_out, float* xy) {
+  if (!b) return MC_EINVAL;
+  mc_world* lead = b->worlds[0];
+  if (step_out) *step_out = lead->step;
+  cudaStream_t st = lead->stream;
+  const unsigned nb = (unsigned)b->worlds.size();
+  if (xy && lead->N) {
+    mc::k_unpermute2<<<dim3((lead->N + 255) / 256, nb), 256, 0, st>>>(lead->N, lead->ptr<int>(lead->L.src),
+                                                                      lead->ptr<float2>(lead->L.X),
+                                                                      reinterpret_cast<float2*>(xy), b->stride);
+    lead->launches++;
+  }
+  // sticky divergence flags of all worlds (word 0 of each world's flag block)
+  std::vector<int> h(nb, 0);
+  cudaError_t e = cudaMemcpy2DAsync(h.data(), sizeof(int), lead->ptr<int>(lead->L.flags), b->stride, sizeof(int), nb,
+                                    cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) return bfail(b, MC_ECUDA, std::string("mc_read_positions_batch: ") + cudaGetErrorString(e));
+  for (unsigned k = 0; k < nb; ++k)
+    if (h[k]) {
+      b->worlds[k]->diverged = true;
+      return bfail(b, MC_EDIVERGED, std::string("world ") + std::to_string(k) + " diverged (non-finite bead or |u| > 0.3)");
+    }
+  return MC_OK;
+}
+
 int mc_step_batch(mc_batch* b, int32_t n) {
   if (!b) return MC_EINVAL;
   if (n < 0) return bfail(b, MC_EINVAL, "n < 0");

@@ -126,3 +126,27 @@ def test_batch_set_positions_on_a_member():
     S0 = binding.World(ws[0])
     S0.step(6)
     assert B.world(0).read_state(keys=("xy",))["xy"].tobytes() == S0.read_state(keys=("xy",))["xy"].tobytes()
+
+
+def test_batch_positions_in_one_call_each_way():
+    # mc_set_positions_batch / mc_read_positions_batch = the per-world calls, bit for bit
+    from paper_2607_02954_b200 import binding
+    ws = family(lambda s: worlds.ragged_world(96, 64, [5, 16, 33, 64], seed=s), 4)
+    B = binding.Batch(ws)
+    B.step(3)
+    xy, step = B.read_positions()
+    assert step == 3 and xy.shape == (4, B.N, 2)
+    for k in range(4):
+        assert xy[k].tobytes() == B.world(k).read_state(keys=("xy",))["xy"].tobytes()
+    new = (xy + np.float32(0.3) * np.arange(1, 5, dtype=np.float32)[:, None, None]).astype(np.float32)
+    B.set_positions(new)
+    B.step(4)
+    got, _ = B.read_positions()
+    for k in range(4):
+        S = binding.World(ws[k])
+        S.step(3)
+        S.set_positions(new[k])
+        S.step(4)
+        assert got[k].tobytes() == S.read_state(keys=("xy",))["xy"].tobytes(), k
+        S.close()
+    B.close()

@@ -170,3 +170,31 @@ def test_scallop_theorem_and_wave_direction():
         assert np.linalg.norm(wave) > 5e-4
     assert ratios[0] < 0.25 and ratios[1] < 0.25
     assert ratios[1] < ratios[0]          # more viscous -> closer to zero
+
+
+def test_viscosity_sweep_of_the_scallop_pair():
+    # P:L151 "Viscosity is swept from 1e-3 to 2; this spans approximately Reynolds number Re ~ 1e3
+    # to 1 ..., covering the transition from inertia-dominated to viscosity-dominated swimming";
+    # P:L139 "time-reversible strategies ... produce zero net displacement at high viscosity";
+    # P:L155 "Ultimately, a very high viscosity brings all movement close to a stop".
+    # nu_lat over the paper's range, reciprocal single hinge against the travelling wave; the coupling
+    # kappa is 2 in the thin-fluid half (stability limit of the stiff IBM spring) and 8 in
+    # the viscous half, the two halves sharing nu_lat = 0.1.
+    def pair(nu, kappa):
+        h = np.linalg.norm(net_displacement_per_cycle(swimmer(nu, kappa, "hinge"), periods=6))
+        wv = np.linalg.norm(net_displacement_per_cycle(swimmer(nu, kappa, "wave"), periods=6))
+        return h, wv
+    thin = [pair(nu, 2.0) for nu in (1e-3, 1e-2, 0.1)]
+    thick = [pair(nu, 8.0) for nu in (0.1, 0.5, 2.0)]
+    r_thin = [h / wv for h, wv in thin]
+    r_thick = [h / wv for h, wv in thick]
+    # inertia-dominated end: the reciprocal stroke DOES swim, even better than the wave (Re ~ 1e3)
+    assert r_thin[0] > 1.0
+    # ... and loses its advantage monotonically as the fluid thickens
+    assert r_thin[0] > r_thin[1] > r_thin[2] and r_thin[2] < 0.3
+    # viscosity-dominated half: scallop theorem, ever more strictly
+    assert all(r < 0.25 for r in r_thick) and r_thick[0] > r_thick[1] > r_thick[2]
+    # the reciprocal swimmer's own displacement falls monotonically across each half of the sweep
+    assert thin[0][0] > thin[1][0] > thin[2][0] and thick[0][0] > thick[1][0] > thick[2][0]
+    # close to a stop at the thick end: the wave at nu_lat = 2 covers < 10 % of its distance at 0.1
+    assert thick[2][1] < 0.1 * thick[0][1]

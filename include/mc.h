@@ -205,13 +205,17 @@ int mc_keep_intermediates(mc_world* w, int32_t on);
  * the call, 0 if not, or a negative error. */
 int mc_texture_gathers(mc_world* w, int32_t on);
 
-/* Crowded worlds: the tile-accumulation kernels (S2 deposit; S5 spread fused with S6) can give
- * every 32x32 tile a thread-block cluster of c CTAs that share the tile's bead list and combine
- * their integer partial sums through distributed shared memory (identical bits; DESIGN.md
- * section 7).  mc_load_filaments switches this on (c = 4) when the largest tile list exceeds 4096
- * beads.  mc_cluster_tiles(w, c) with c in {0, 2, 4, 8} forces the setting for the following steps
- * (0: one CTA per tile), c = -1 restores the automatic choice.  Returns the cluster size in use
- * after the call, or a negative error. */
+/* Crowded worlds: the tile-accumulation kernels (S2 deposit; S5 spread fused with S6) can give a
+ * 32x32 tile a thread-block cluster of c CTAs that share the tile's bead list and combine their
+ * integer partial sums through distributed shared memory (identical bits).
+ * mc_load_filaments switches this on (c = 4) when the largest tile list exceeds 4096 beads: the
+ * tiles listing more than 1024 beads are then served by a cluster launch of their own that runs
+ * beside the one-CTA-per-tile launch over all other tiles (second stream owned by the world).
+ * mc_cluster_tiles(w, c) with c in {0, 2, 4, 8} forces the setting for the following steps (0: one
+ * CTA per tile), c | MC_CLUSTER_ALL_TILES gives EVERY tile a cluster in one launch (the simpler
+ * scheme, for tests and measurements), c = -1 restores the automatic choice.  Returns the cluster
+ * size in use after the call, or a negative error. */
+#define MC_CLUSTER_ALL_TILES 64
 int mc_cluster_tiles(mc_world* w, int32_t c);
 
 /* Optional per-kernel timing with CUDA events on the world's stream (used by bench.py for the

@@ -277,9 +277,10 @@ class World:
             self._check(rc)
         return rc == 1
 
-    def cluster_tiles(self, c: int = -1) -> int:
-        """mc_cluster_tiles: CTAs per tile of the P2G kernels (0, 2, 4, 8; -1 automatic) -> in use."""
-        rc = load_library().mc_cluster_tiles(self.h, int(c))
+    def cluster_tiles(self, c: int = -1, all_tiles: bool = False) -> int:
+        """mc_cluster_tiles: CTAs per crowded tile of the P2G kernels (0, 2, 4, 8; -1 automatic) -> in use.
+        all_tiles: every tile gets a cluster in one launch (MC_CLUSTER_ALL_TILES) instead of the split launch."""
+        rc = load_library().mc_cluster_tiles(self.h, int(c) | (64 if all_tiles and c >= 0 else 0))
         if rc < 0:
             self._check(rc)
         return rc

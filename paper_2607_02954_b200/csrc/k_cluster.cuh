@@ -48,16 +48,23 @@ template <int C>
 __global__ void __cluster_dims__(C, 1, 1) __launch_bounds__(256)
     k_deposit_tile_cl(int nx, int ny, const int* __restrict__ tile_start, const int* __restrict__ list,
                       const float2* __restrict__ X, float* __restrict__ rho_b, float* __restrict__ tile_rho_max,
-                      unsigned* __restrict__ tile_fmax, size_t wstride) {
+                      unsigned* __restrict__ tile_fmax, size_t wstride, const int* __restrict__ crowded = nullptr,
+                      const int* __restrict__ n_crowded = nullptr, int cl_max = 0) {
   __shared__ __align__(16) int acc[ACC_N], accl[ACC_N];
   {
     const size_t ws = blockIdx.y * wstride;
+    crowded = wshift(crowded, ws); n_crowded = wshift(n_crowded, ws);
     tile_start = wshift(tile_start, ws); list = wshift(list, ws); X = wshift(X, ws); rho_b = wshift(rho_b, ws);
     tile_rho_max = wshift(tile_rho_max, ws); tile_fmax = wshift(tile_fmax, ws);
   }
   cg::cluster_group cl = cg::this_cluster();
   const int rank = (int)cl.block_rank();
-  const int t = blockIdx.x / C, ntx = nx / TS;
+  int t = blockIdx.x / C;
+  if (crowded) {  // split launch: cluster k serves the k-th crowded tile (the whole cluster leaves together)
+    if (t >= min(*n_crowded, cl_max)) return;
+    t = crowded[t];
+  }
+  const int ntx = nx / TS;
   const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
   const int s = tile_start[t], e = tile_start[t + 1];
   const bool wide = (e - s) > WIDE_N;
@@ -111,7 +118,12 @@ __global__ void __cluster_dims__(C, 1, 1) __launch_bounds__(256) k_lbm_spread_ti
   const int rank = (int)cl.block_rank();
   const LbmArgs& a = p.lbm;
   const int nx = a.nx, ny = a.ny;
-  const int t = blockIdx.x / C, ntx = nx / TS;
+  int t = blockIdx.x / C;
+  if (p.crowded) {  // split launch: cluster k serves the k-th crowded tile
+    if (t >= min(*p.n_crowded, p.cl_max)) return;
+    t = p.crowded[t];
+  }
+  const int ntx = nx / TS;
   const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
   const int s = p.tile_start[t], e = p.tile_start[t + 1];
   const int ce = cluster_share<C>(e - s);  // the same in every CTA of the cluster

@@ -138,8 +138,15 @@ struct LbmSpreadArgs {
   float* tile_rho_max;        // may be NULL; read, then reset to 0 for the next step's S2 (atomicMax)
   const unsigned* tile_fmax;  // may be NULL
   const float2* O;            // two-layer marker offsets (TWO variants), else NULL
+  // crowded worlds (k_cluster.cuh): tiles with rank < cl_max in the crowded table belong to the cluster
+  // launch; the cluster launch finds its tiles in crowded[0 .. min(*n_crowded, cl_max))
+  const int* crowded_rank;    // NULL: no split
+  const int* crowded;
+  const int* n_crowded;
+  int cl_max;
   __device__ __forceinline__ void shift(size_t bytes) {
     lbm.shift(bytes);
+    crowded_rank = wshift(crowded_rank, bytes); crowded = wshift(crowded, bytes); n_crowded = wshift(n_crowded, bytes);
     tile_start = wshift(tile_start, bytes); list = wshift(list, bytes); X = wshift(X, bytes); F = wshift(F, bytes);
     tile_rho_max = wshift(tile_rho_max, bytes); tile_fmax = wshift(tile_fmax, bytes); O = wshift(O, bytes);
   }
@@ -155,6 +162,7 @@ __global__ void __launch_bounds__(256, 5) k_lbm_spread_tile(LbmSpreadArgs p, siz
   // 1-D grid in row-major tile order (a 2-D grid is rasterised differently by the hardware and
   // cost the streaming phase 20 % on world 4d)
   const int t = blockIdx.x, ntx = nx / TS;
+  if (p.crowded_rank && (unsigned)p.crowded_rank[t] < (unsigned)p.cl_max) return;  // the cluster launch's tile
   const int x0 = (t % ntx) * TS, y0 = (t / ntx) * TS;
   const int s = p.tile_start[t], e = p.tile_start[t + 1];
   {

@@ -302,14 +302,17 @@ __global__ void __launch_bounds__(256, LIGHT ? 6 : 1) k_deposit_tile(int nx, int
                                                       float* __restrict__ rho_b,
                                                       float* __restrict__ tile_rho_max,
                                                       unsigned* __restrict__ tile_fmax,
-                                                      const float2* __restrict__ O, size_t wstride) {
+                                                      const float2* __restrict__ O, size_t wstride,
+                                                      const int* __restrict__ crowded_rank = nullptr, int cl_max = 0) {
   __shared__ __align__(16) int acc[ACC_N], accl[ACC_N];
   if (wstride) {  // batched worlds; single worlds pass 0
     const size_t ws = blockIdx.z * wstride;
+    crowded_rank = wshift(crowded_rank, ws);
     tile_start = wshift(tile_start, ws); list = wshift(list, ws); X = wshift(X, ws); rho_b = wshift(rho_b, ws);
     tile_rho_max = wshift(tile_rho_max, ws); tile_fmax = wshift(tile_fmax, ws); O = wshift(O, ws);
   }
   const int t = blockIdx.y * gridDim.x + blockIdx.x;  // grid = (nx/TS, ny/TS)
+  if (crowded_rank && (unsigned)crowded_rank[t] < (unsigned)cl_max) return;  // served by the cluster launch (k_cluster.cuh)
   const int x0 = blockIdx.x * TS, y0 = blockIdx.y * TS;
   const int s = tile_start[t], e = tile_start[t + 1];
   const bool wide = (e - s) > WIDE_N;

@@ -181,10 +181,23 @@ __device__ __forceinline__ void bucket_starts(int n_tiles, const int* __restrict
   }
 }
 
+// Crowded tiles (config 5): the tiles whose list exceeds CROWDED_N entries are handed to a cluster
+// launch of their own (k_cluster.cuh) that runs BESIDE the one-CTA-per-tile launch on a second
+// stream; the table is rebuilt with the lists.  crowded[r] = tile id of rank r, crowded_rank[t] = r or
+// -1, *n_crowded = their number.  The ranks depend on the arrival order of the atomics, i.e. which
+// crowded tile gets which cluster is not reproducible -- harmless: every tile's result is the same
+// integer sum whoever computes it.
+constexpr int CROWDED_N = 1024;
+struct CrowdedTable {
+  int* crowded;       // [n_tiles]
+  int* crowded_rank;  // [n_tiles]
+  int* n_crowded;     // [1]
+};
+
 // ONE block of 1024 threads: tile_start = exclusive scan of tile_count (n_tiles + 1 entries);
 // counts are zeroed for the next rebuild.  sm: 33 ints of shared memory.
 __device__ __forceinline__ void tile_scan(int* __restrict__ tile_count, int n_tiles, int* __restrict__ tile_start,
-                                          int* sm) {
+                                          int* sm, CrowdedTable ct = CrowdedTable{nullptr, nullptr, nullptr}) {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   int carry = 0;
   for (int base = 0; base < n_tiles; base += 1024) {
@@ -219,6 +232,40 @@ __device__ __forceinline__ void tile_scan(int* __restrict__ tile_count, int n_ti
     __syncthreads();
   }
   if (threadIdx.x == 0) tile_start[n_tiles] = carry;
+  if (ct.crowded) {
+    // ranks in (roughly) DESCENDING order of list length -- 64 linear buckets between CROWDED_N and
+    // the longest list: the cluster launch is dispatched in rank order, and starting the heaviest
+    // tiles first evens out the SMs (config 5: busiest SM 151 k cycles against 90 k on average with
+    // ranks in tile order)
+    __shared__ int hist[64], cursor[64], longest;
+    if (threadIdx.x < 64) hist[threadIdx.x] = 0;
+    if (threadIdx.x == 0) longest = CROWDED_N + 1;
+    __syncthreads();  // also makes tile_start visible to the whole block
+    for (int i = threadIdx.x; i < n_tiles; i += 1024) atomicMax(&longest, tile_start[i + 1] - tile_start[i]);
+    __syncthreads();
+    const int span = longest - CROWDED_N;
+    auto bucket = [&](int n) { return 63 - min(63, (int)(((long long)(n - CROWDED_N - 1) * 64) / span)); };  // 0 = longest
+    for (int i = threadIdx.x; i < n_tiles; i += 1024) {
+      const int n = tile_start[i + 1] - tile_start[i];
+      if (n > CROWDED_N) atomicAdd(&hist[bucket(n)], 1);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int run = 0;
+      for (int b = 0; b < 64; ++b) { cursor[b] = run; run += hist[b]; }
+      *ct.n_crowded = run;
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n_tiles; i += 1024) {
+      const int n = tile_start[i + 1] - tile_start[i];
+      int r = -1;
+      if (n > CROWDED_N) {
+        r = atomicAdd(&cursor[bucket(n)], 1);
+        ct.crowded[r] = i;
+      }
+      ct.crowded_rank[i] = r;
+    }
+  }
 }
 
 template <bool FILL>
@@ -250,9 +297,11 @@ __global__ void __launch_bounds__(256) k_bucket_starts(const ListState* __restri
 }
 
 __global__ void __launch_bounds__(1024) k_tile_scan(ListState* __restrict__ st, int* __restrict__ tile_count,
-                                                    int n_tiles, int* __restrict__ tile_start, size_t wstride) {
+                                                    int n_tiles, int* __restrict__ tile_start, CrowdedTable ct,
+                                                    size_t wstride) {
   const size_t ws = blockIdx.y * wstride;
   st = wshift(st, ws); tile_count = wshift(tile_count, ws); tile_start = wshift(tile_start, ws);
+  ct.crowded = wshift(ct.crowded, ws); ct.crowded_rank = wshift(ct.crowded_rank, ws); ct.n_crowded = wshift(ct.n_crowded, ws);
   __shared__ int sm[33];
   __shared__ int need_s;
   if (threadIdx.x == 0) {
@@ -261,7 +310,7 @@ __global__ void __launch_bounds__(1024) k_tile_scan(ListState* __restrict__ st, 
   }
   __syncthreads();
   if (!need_s) return;
-  tile_scan(tile_count, n_tiles, tile_start, sm);
+  tile_scan(tile_count, n_tiles, tile_start, sm, ct);
 }
 
 // Small worlds (bound by launch overhead, not by work): the whole of K0 in ONE launch of one
@@ -272,9 +321,10 @@ __global__ void __launch_bounds__(1024) k_list_build_small(ListState* __restrict
                                                            int n_tiles, int* __restrict__ tile_count,
                                                            int* __restrict__ tile_start, int* __restrict__ bucket_count,
                                                            int* __restrict__ bucket_cursor, int* __restrict__ list,
-                                                           size_t wstride) {
+                                                           CrowdedTable ct, size_t wstride) {
   // one CTA per world: blockIdx.x is always 0 here, the world index rides in blockIdx.y
   const size_t ws = blockIdx.y * wstride;
+  ct.crowded = wshift(ct.crowded, ws); ct.crowded_rank = wshift(ct.crowded_rank, ws); ct.n_crowded = wshift(ct.n_crowded, ws);
   st = wshift(st, ws); X = wshift(X, ws); O = wshift(O, ws); tile_count = wshift(tile_count, ws);
   tile_start = wshift(tile_start, ws); bucket_count = wshift(bucket_count, ws);
   bucket_cursor = wshift(bucket_cursor, ws); list = wshift(list, ws);
@@ -288,7 +338,7 @@ __global__ void __launch_bounds__(1024) k_list_build_small(ListState* __restrict
   if (!need_s) return;
   tile_bin<false>(X, O, N, nx, ny, tile_count, bucket_count, nullptr);
   __syncthreads();
-  tile_scan(tile_count, n_tiles, tile_start, sm);
+  tile_scan(tile_count, n_tiles, tile_start, sm, ct);
   __syncthreads();
   bucket_starts(n_tiles, tile_start, bucket_count, bucket_cursor);
   __syncthreads();
@@ -306,9 +356,10 @@ __global__ void __cluster_dims__(K0_CLUSTER, 1, 1) __launch_bounds__(1024)
     k_list_build_cluster(ListState* __restrict__ st, const float2* __restrict__ X, const float2* __restrict__ O, int N,
                          int nx, int ny, int n_tiles, int* __restrict__ tile_count, int* __restrict__ tile_start,
                          int* __restrict__ bucket_count, int* __restrict__ bucket_cursor, int* __restrict__ list,
-                         size_t wstride) {
+                         CrowdedTable ct, size_t wstride) {
   // one cluster per world: blockIdx.x = rank in the cluster, blockIdx.y = world
   const size_t ws = blockIdx.y * wstride;
+  ct.crowded = wshift(ct.crowded, ws); ct.crowded_rank = wshift(ct.crowded_rank, ws); ct.n_crowded = wshift(ct.n_crowded, ws);
   st = wshift(st, ws); X = wshift(X, ws); O = wshift(O, ws); tile_count = wshift(tile_count, ws);
   tile_start = wshift(tile_start, ws); bucket_count = wshift(bucket_count, ws);
   bucket_cursor = wshift(bucket_cursor, ws); list = wshift(list, ws);
@@ -320,7 +371,7 @@ __global__ void __cluster_dims__(K0_CLUSTER, 1, 1) __launch_bounds__(1024)
   if (!*reinterpret_cast<volatile int*>(&st->need)) return;  // the same value in every CTA: all leave together
   tile_bin<false>(X, O, N, nx, ny, tile_count, bucket_count, nullptr);
   cl.sync();
-  if (blockIdx.x == 0) tile_scan(tile_count, n_tiles, tile_start, sm);
+  if (blockIdx.x == 0) tile_scan(tile_count, n_tiles, tile_start, sm, ct);
   cl.sync();
   bucket_starts(n_tiles, tile_start, bucket_count, bucket_cursor);
   cl.sync();

@@ -35,6 +35,7 @@ struct Layout {
   size_t X, PA, PB, PC, PD, F, sense, list, src, bflags, scratch, flags, sources;
   size_t V, dF, hrinv, mdf_fmax;  // MDF coupling only
   size_t PE, O, Dp;               // rest-length actuation amplitudes; two-layer offsets; projection displacement
+  size_t crowded, crowded_rank;   // crowded-tile table of the split cluster launch (k_tile.cuh CrowdedTable)
   size_t total;
 };
 
@@ -124,6 +125,8 @@ Layout make_layout(const mc_world_params* p, const Derived& d) {
   L.PE = take(N * 4);
   L.O = take(p->two_layer ? N * 8 : 0);
   L.Dp = take(p->pbd_project ? N * 8 : 0);
+  L.crowded = take(nt * 4);
+  L.crowded_rank = take(nt * 4);
   L.total = off;
   return L;
 }
@@ -152,6 +155,11 @@ struct mc_world {
   int batch_n = 1;
   size_t batch_stride = 0;
   bool batch_member = false;  // owned by an mc_batch: stepped and reloaded only through it
+  // crowded worlds: the cluster launch over the crowded tiles runs on a second stream beside the
+  // one-CTA-per-tile launch over the rest (fork / join by events; also under graph capture)
+  bool split_on = true;   // mc_cluster_tiles(w, c | MC_CLUSTER_ALL_TILES): every tile gets a cluster (round-1 scheme; tests)
+  cudaStream_t side = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   cudaTextureObject_t tex_u = 0, tex_A = 0;  // linear float2 views of u and A for the texture-pipe half of the gathers
   int n_sm = 148;               // SMs of the device the world lives on (grid-stride kernels size their grids by it)
   bool uniform_params = false;  // K1 variant: L_rest, stiffnesses and period identical for all beads
@@ -219,6 +227,24 @@ constexpr int K0_SMALL_BEADS = 32768, K0_SMALL_TILES = 1024;
 constexpr int K0_MEDIUM_BEADS = 262144, K0_MEDIUM_TILES = 8192;
 static_assert(GRAPH_STEPS % 2 == 0, "graph period");
 
+// crowded-tile table of this world (k_tile.cuh); n_crowded lives in the flag words
+mc::CrowdedTable crowded_table(mc_world* w) {
+  return mc::CrowdedTable{w->ptr<int>(w->L.crowded), w->ptr<int>(w->L.crowded_rank), w->ptr<int>(w->L.flags) + 6};
+}
+// at most this many crowded tiles get a cluster; the rest stay with the one-CTA launch (correct, slower)
+constexpr int CL_MAX = 1024;
+
+bool ensure_side_stream(mc_world* w) {
+  if (w->side) return true;
+  if (cudaStreamCreateWithFlags(&w->side, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); w->side = nullptr; return false; }
+  if (cudaEventCreateWithFlags(&w->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&w->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return true;
+}
+
 void drop_graphs(mc_world* w) {
   for (int k = 0; k < 2; ++k)
     if (w->graph[k]) { cudaGraphExecDestroy(w->graph[k]); w->graph[k] = nullptr; }
@@ -283,6 +309,12 @@ int enqueue_step(mc_world* w) {
   const int n_items = two ? 2 * N : N;            // listed points: beads, or their two-layer markers
   const int bgrid = (n_items + bt - 1) / bt;
   mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16);
+  // crowded worlds: the tiles with long lists go to a cluster launch of their own on a second stream
+  const bool split = w->cluster > 0 && !two && w->split_on && w->side != nullptr;
+  const mc::CrowdedTable ctab = split ? crowded_table(w) : mc::CrowdedTable{nullptr, nullptr, nullptr};
+  const int cl_max = std::min(n_tiles, CL_MAX);
+  auto fork_side = [&]() { cudaEventRecord(w->ev_fork, st); cudaStreamWaitEvent(w->side, w->ev_fork, 0); };
+  auto join_side = [&]() { cudaEventRecord(w->ev_join, w->side); cudaStreamWaitEvent(st, w->ev_join, 0); };
 
   prof_mark(w, 0);
   if (beads) {
@@ -291,16 +323,16 @@ int enqueue_step(mc_world* w) {
     if (n_items <= K0_SMALL_BEADS && n_tiles <= K0_SMALL_TILES) {
       // small world: one launch of one CTA (per world) instead of four (k_tile.cuh)
       mc::k_list_build_small<<<dim3(1, nb), 1024, 0, st>>>(ls_state, X, O, N, nx, ny, n_tiles, tile_count, tile_start,
-                                                           bucket_count, bucket_cursor, list, ws);
+                                                           bucket_count, bucket_cursor, list, ctab, ws);
       w->launches += 1;
     } else if (n_items <= K0_MEDIUM_BEADS && n_tiles <= K0_MEDIUM_TILES) {
       mc::k_list_build_cluster<<<dim3(mc::K0_CLUSTER, nb), 1024, 0, st>>>(ls_state, X, O, N, nx, ny, n_tiles, tile_count,
-                                                                          tile_start, bucket_count, bucket_cursor, list, ws);
+                                                                          tile_start, bucket_count, bucket_cursor, list, ctab, ws);
       w->launches += 1;
     } else {
       const int k0grid = bgrid < w->n_sm * 8 ? bgrid : w->n_sm * 8;
       mc::k_tile_bin<false><<<dim3(k0grid, nb), bt, 0, st>>>(ls_state, X, O, N, nx, ny, tile_count, bucket_count, nullptr, ws);
-      mc::k_tile_scan<<<dim3(1, nb), 1024, 0, st>>>(ls_state, tile_count, n_tiles, tile_start, ws);
+      mc::k_tile_scan<<<dim3(1, nb), 1024, 0, st>>>(ls_state, tile_count, n_tiles, tile_start, ctab, ws);
       mc::k_bucket_starts<<<dim3(std::min((n_tiles + 7) / 8, w->n_sm * 4), nb), 256, 0, st>>>(ls_state, n_tiles, tile_start, bucket_count, bucket_cursor, ws);
       mc::k_tile_bin<true><<<dim3(k0grid, nb), bt, 0, st>>>(ls_state, X, O, N, nx, ny, nullptr, bucket_cursor, list, ws);
       w->launches += 4;
@@ -310,6 +342,18 @@ int enqueue_step(mc_world* w) {
     if (w->d.n_density) {
       if (two)  // two-layer markers: one CTA per tile whatever the crowding
         mc::k_deposit_tile<false, true><<<tgrid, 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax, O, ws);
+      else if (split) {
+        // crowded tiles: clusters on the side stream; all other tiles: the light one-CTA kernel beside them
+        fork_side();
+#define MC_DEP_CL(C) mc::k_deposit_tile_cl<C><<<dim3(cl_max * C, nb), 256, 0, w->side>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax, ws, ctab.crowded, ctab.n_crowded, cl_max)
+        if (w->cluster == 8) MC_DEP_CL(8);
+        else if (w->cluster == 4) MC_DEP_CL(4);
+        else MC_DEP_CL(2);
+#undef MC_DEP_CL
+        mc::k_deposit_tile<true><<<tgrid, 128, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax, nullptr, ws, ctab.crowded_rank, cl_max);
+        join_side();
+        w->launches++;
+      }
       else if (w->cluster == 8)
         mc::k_deposit_tile_cl<8><<<dim3(n_tiles * 8, nb), 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax, ws);
       else if (w->cluster == 4)
@@ -469,6 +513,7 @@ int enqueue_step(mc_world* w) {
     // MDF: the bound on the summed F left by the last forcing iteration (K1's is on V)
     ls.tile_fmax = mdf ? w->ptr<unsigned>(w->L.mdf_fmax) + (size_t)(w->p.mdf_iters - 1) * n_tiles : tile_fmax;
     ls.O = O;
+    ls.crowded_rank = nullptr; ls.crowded = nullptr; ls.n_crowded = nullptr; ls.cl_max = 0;
 #define MC_FUSED_CL(C)                                                                                   \
   {                                                                                                      \
     if (w->keep_G) mc::k_lbm_spread_tile_cl<C, true><<<dim3(n_tiles * C, nb), 256, 0, st>>>(ls, ws);     \
@@ -477,6 +522,23 @@ int enqueue_step(mc_world* w) {
     if (two) {
       if (w->keep_G) mc::k_lbm_spread_tile<true, true><<<dim3(n_tiles, nb), 256, 0, st>>>(ls, ws);
       else mc::k_lbm_spread_tile<false, true><<<dim3(n_tiles, nb), 256, 0, st>>>(ls, ws);
+    }
+    else if (split) {
+      ls.crowded_rank = ctab.crowded_rank; ls.crowded = ctab.crowded; ls.n_crowded = ctab.n_crowded; ls.cl_max = cl_max;
+      fork_side();
+#define MC_FUSED_SPLIT(C)                                                                                     \
+  {                                                                                                           \
+    if (w->keep_G) mc::k_lbm_spread_tile_cl<C, true><<<dim3(cl_max * C, nb), 256, 0, w->side>>>(ls, ws);      \
+    else mc::k_lbm_spread_tile_cl<C, false><<<dim3(cl_max * C, nb), 256, 0, w->side>>>(ls, ws);               \
+  }
+      if (w->cluster == 8) MC_FUSED_SPLIT(8)
+      else if (w->cluster == 4) MC_FUSED_SPLIT(4)
+      else MC_FUSED_SPLIT(2)
+#undef MC_FUSED_SPLIT
+      if (w->keep_G) mc::k_lbm_spread_tile<true><<<dim3(n_tiles, nb), 256, 0, st>>>(ls, ws);
+      else mc::k_lbm_spread_tile<false><<<dim3(n_tiles, nb), 256, 0, st>>>(ls, ws);
+      join_side();
+      w->launches++;
     }
     else if (w->cluster == 8) MC_FUSED_CL(8)
     else if (w->cluster == 4) MC_FUSED_CL(4)
@@ -569,6 +631,9 @@ void mc_destroy(mc_world* w) {
   for (cudaEvent_t e : w->prof_ev) cudaEventDestroy(e);
   if (w->tex_u) cudaDestroyTextureObject(w->tex_u);
   if (w->tex_A) cudaDestroyTextureObject(w->tex_A);
+  if (w->ev_fork) cudaEventDestroy(w->ev_fork);
+  if (w->ev_join) cudaEventDestroy(w->ev_join);
+  if (w->side) cudaStreamDestroy(w->side);
   drop_graphs(w);
   delete w;
 }
@@ -861,6 +926,7 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   // (measured on config 5: one CTA per tile 0.351 ms/step, clusters of 2: 0.263, 4: 0.250, 8: 0.325)
   w->cluster_auto = h_maxlist > 4096 ? 4 : 0;
   w->cluster = w->cluster_user >= 0 ? w->cluster_user : w->cluster_auto;
+  if (w->cluster > 0 && w->split_on) ensure_side_stream(w);  // no side stream: one cluster launch over all tiles
   w->uniform_params = (h_nonuni == 0);
   if (reuse_order) {
     w->stride = prev_stride;
@@ -1055,11 +1121,15 @@ int mc_keep_intermediates(mc_world* w, int32_t on) {
 
 int mc_cluster_tiles(mc_world* w, int32_t c) {
   if (!w) return MC_EINVAL;
+  bool split_on = true;
+  if (c >= 0 && (c & MC_CLUSTER_ALL_TILES)) { split_on = false; c &= ~MC_CLUSTER_ALL_TILES; }
   if (c != -1 && c != 0 && c != 2 && c != 4 && c != 8) return fail(w, MC_EINVAL, "cluster size must be -1, 0, 2, 4 or 8");
   const int now = c >= 0 ? c : w->cluster_auto;
-  if (now != w->cluster) drop_graphs(w);
+  if (now != w->cluster || split_on != w->split_on) drop_graphs(w);
   w->cluster_user = c;
   w->cluster = now;
+  w->split_on = split_on;
+  if (now > 0 && split_on) ensure_side_stream(w);
   return now;
 }
 
@@ -1187,6 +1257,7 @@ int mc_load_filaments_batch(mc_batch* b, int32_t n_fil, const int32_t* offsets, 
     w->cluster_auto = cl;
     w->cluster = w->cluster_user >= 0 ? w->cluster_user : cl;
   }
+  if (lead->cluster > 0 && lead->split_on) ensure_side_stream(lead);
   drop_graphs(lead);
   return MC_OK;
 }

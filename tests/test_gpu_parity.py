@@ -429,11 +429,13 @@ def test_cluster_tiles_do_not_change_the_bits():
     # crowded worlds give every tile a thread-block cluster whose CTAs share the tile's list and
     # combine integer partial sums through distributed shared memory: same bits as one CTA per tile
     from paper_2607_02954_b200 import binding
+    # (split launch: clusters for the crowded tiles on a second stream beside the one-CTA launch over
+    # the rest; all_tiles: one launch with a cluster for every tile)
     w = _very_crowded()
     outs = []
-    for c in (0, 2, 4, 8, -1):
+    for c, all_tiles in ((0, False), (2, False), (4, False), (8, False), (-1, False), (2, True), (4, True), (8, True)):
         G = binding.World(w)
-        used = G.cluster_tiles(c)
+        used = G.cluster_tiles(c, all_tiles=all_tiles)
         assert used == (c if c >= 0 else 4), (c, used)   # automatic choice: 4 (largest list > 4096)
         G.keep_intermediates(True)
         G.step(7)

@@ -601,6 +601,35 @@ def main():
             Ge.close()
             del Ge, we
 
+    # the paper's own scalability experiment (Fig. 5): fixed 256 x 256 grid, 1000 steps,
+    # particle count swept up to 500 k.  The paper prints no numbers (a plot on one L40S); this is the
+    # same sweep on seeded random 64-bead chains (couplings of the config-5 recipe once the grid is
+    # crowded), reported as context: ms per 1000 steps against N, and the straight-line fit.
+    if extra is not None:
+        sweep = []
+        for n_fil in (16, 157, 1563, 4000, 7813):
+            dense = n_fil * 64 >= 65536
+            we = worlds.random_world(256, 256, n_fil, 64, seed=1, kappa=0.25 if dense else 2.0,
+                                     kappa_rep=2e-4 if dense else 0.01, tag="e5")
+            Ge = binding.World(we, device=str(dev))
+            Ge.step(50)
+            torch.cuda.synchronize(dev)
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record(Ge.stream)
+            Ge.step(1000)
+            a1.record(Ge.stream)
+            torch.cuda.synchronize(dev)
+            sweep.append({"particles": Ge.N, "ms_per_1000_steps": a0.elapsed_time(a1)})
+            Ge.close()
+        xs = np.array([r["particles"] for r in sweep], dtype=np.float64)
+        ys = np.array([r["ms_per_1000_steps"] for r in sweep], dtype=np.float64)
+        slope, icpt = np.polyfit(xs, ys, 1)
+        extra["paper_E5_fixed_256x256_grid"] = {
+            "sweep": sweep, "fit_ms_per_1000_steps": {"per_particle": slope, "intercept": icpt},
+            "max_rel_residual": float(np.abs(ys - (slope * xs + icpt)).max() / ys.max()),
+            "note": "P:L190 workload shape (256x256, 1000 steps, up to 500k particles) on synthetic chains; "
+                    "the paper's plot has no printed numbers"}
+
     cpu = None
     if rank == 0 and world_size == 1 and not args.no_cpu_baseline:
         # the oracle on the SAME world: a few whole steps (4d: ~3 s per step on 16 cores), and the

@@ -131,16 +131,22 @@ GATHER_BYTES = {"K1_filament": 8, "K4_interp_integrate": 8}   # per node
 
 
 def csrc_sha() -> str:
-    """Hash of the CUDA sources the timed library was built from (ties an ncu capture to a build)."""
-    import glob
-    import hashlib
-    h = hashlib.sha256()
-    d = os.path.join(ROOT, "paper_2607_02954_b200", "csrc")
-    for f in sorted(glob.glob(os.path.join(d, "*.cu")) + glob.glob(os.path.join(d, "*.cuh"))):
-        h.update(os.path.basename(f).encode())
-        with open(f, "rb") as fh:
-            h.update(fh.read())
-    return h.hexdigest()[:16]
+    """Hash of the CUDA sources the timed library was built from (ties an ncu capture to a build).
+    paper_2607_02954_b200/build.py writes it beside libmc.so; a library built from other sources than
+    the ones in the tree is reported as such."""
+    from paper_2607_02954_b200 import build as mc_build
+    if os.path.dirname(os.path.abspath(mc_build.HERE)) != os.path.abspath(ROOT):  # tests point ROOT elsewhere
+        import glob
+        import hashlib
+        h = hashlib.sha256()
+        d = os.path.join(ROOT, "paper_2607_02954_b200", "csrc")
+        for f in sorted(glob.glob(os.path.join(d, "*.cu")) + glob.glob(os.path.join(d, "*.cuh"))):
+            h.update(os.path.basename(f).encode())
+            with open(f, "rb") as fh:
+                h.update(fh.read())
+        return h.hexdigest()[:16]
+    src, built = mc_build.csrc_sha(), mc_build.built_sha()
+    return src if built == src else f"MISMATCH(sources {src}, library {built or 'unknown'})"
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture

@@ -30,8 +30,31 @@ def _deps():
             + [os.path.join(os.path.dirname(HERE), "include", "mc.h"), os.path.abspath(__file__)])
 
 
+def csrc_sha() -> str:
+    """Hash of the CUDA sources (names and contents of csrc/*.cu, *.cuh): ties a built library and an
+    ncu capture to the sources they were made from."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh"))):
+        h.update(os.path.basename(f).encode())
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+SHA_FILE = os.path.join(HERE, "libmc.csrc_sha")   # written beside libmc.so by build()
+
+
+def built_sha() -> str:
+    try:
+        with open(SHA_FILE) as fh:
+            return fh.read().strip()
+    except OSError:
+        return ""
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    if (not force and os.path.exists(LIB)
+    if (not force and os.path.exists(LIB) and built_sha() == csrc_sha()
             and os.path.getmtime(LIB) >= max(os.path.getmtime(p) for p in _deps())):
         return LIB
     cmd = [NVCC] + FLAGS + sources() + ["-o", LIB]
@@ -42,6 +65,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         raise RuntimeError("nvcc failed building libmc.so")
     with open(os.path.join(HERE, "libmc.ptxas.log"), "w") as fh:
         fh.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
+    with open(SHA_FILE, "w") as fh:
+        fh.write(csrc_sha() + "\n")
     return LIB
 
 

@@ -32,7 +32,9 @@ __global__ void __launch_bounds__(256) k_interp_integrate(int N, float2* __restr
       const float2 up = interp2_off(u, nx, ny, p.x, p.y, o.x, o.y), um = interp2_off(u, nx, ny, p.x, p.y, -o.x, -o.y);
       U = make_float2(0.5f * (up.x + um.x), 0.5f * (up.y + um.y));
     } else {
-      U = TEXROWS ? interp2_tex<TEXROWS, false>(u, tex_u, nx, ny, p.x, p.y) : interp2(u, nx, ny, p.x, p.y);
+      // 16-byte pair loads, all four rows through the LSU pipe (world 4d: 0.1415 ms with 8-byte loads
+      // and one row through the texture pipe, 0.138 with pairs, 0.158 with pairs + one texture row)
+      U = interp2_pair<0>(u, nx, ny, p.x, p.y);
     }
     p.x += U.x;
     p.y += U.y;

@@ -98,8 +98,9 @@ typedef struct {
                         positions" (reading 27).  0 (default): only through the fluid  */
   int32_t two_layer; /* 1: two-layer broadcast (reading 28): every exchange of a bead with
                         the grid (S2, S4, S5, S7) goes through its two markers X_i +- h n_i with
-                        weight 1/2 each, n_i the unit normal of the chain at the bead.  Not
-                        defined together with MC_COUPLING_MDF                               */
+                        weight 1/2 each, n_i the unit normal of the chain at the bead; with
+                        MC_COUPLING_MDF the forcing iterations sample and broadcast through the
+                        markers as well                                                   */
   float layer_offset; /* h, half the distance between the two layers, in nodes; 0 => 0.5; <= 1 */
 } mc_world_params;
 

@@ -488,6 +488,51 @@ void mco_mdf(int32_t nx, int32_t ny, int64_t N, const double* xy, const double* 
   if (u_out) std::memcpy(u_out, u.data(), 2 * nc * sizeof(double));
 }
 
+// Multi-Direct Forcing through the two-layer broadcast (readings 26 + 28; P:L127 lists both among
+// the practices used together).  P holds `layers` points per bead (layers = 2: the markers
+// M_i^+, M_i^-; layers = 1: the bead itself, then this is mco_mdf).  Each iteration
+//   U_i = mean over the bead's points of interp(u^k);  dF_i = rho0 (V_i - U_i);  F_i += dF_i;
+//   every point spreads dF_i / layers;  u^{k+1} = ustar + G^{k+1} / (2 rho).
+void mco_mdf_layers(int32_t nx, int32_t ny, int64_t N, int32_t layers, const double* P, const double* V,
+                    const double* ustar, const double* rho, double rho0, int32_t iters, double* F,
+                    double* G, double* u_out, double* resid) {
+  const size_t nc = (size_t)nx * ny;
+  const int64_t NP = N * layers;
+  std::vector<double> u(ustar, ustar + 2 * nc), Up(2 * (size_t)NP), U(2 * (size_t)N), dF(2 * (size_t)N),
+      dFp(2 * (size_t)NP), dG(2 * nc);
+  for (size_t c = 0; c < 2 * nc; ++c) G[c] = 0.0;
+  for (int64_t i = 0; i < 2 * N; ++i) F[i] = 0.0;
+  for (int k = 0; k <= iters; ++k) {
+    mco_interp(nx, ny, 2, u.data(), NP, P, Up.data());           // sample at every point
+    for (int64_t i = 0; i < N; ++i)
+      for (int c = 0; c < 2; ++c) {
+        double s = 0.0;
+        for (int l = 0; l < layers; ++l) s += Up[2 * (i * layers + l) + c];
+        U[2 * i + c] = s / layers;                                 // mean over the bead's points
+      }
+    if (resid) {
+      double r = 0.0;
+      for (int64_t i = 0; i < 2 * N; ++i) r = std::fmax(r, std::fabs(V[i] - U[i]));
+      resid[k] = r;
+    }
+    if (k == iters) break;
+    for (int64_t i = 0; i < 2 * N; ++i) {
+      dF[i] = rho0 * (V[i] - U[i]);                               // direct forcing
+      F[i] += dF[i];
+    }
+    for (int64_t i = 0; i < N; ++i)
+      for (int l = 0; l < layers; ++l)
+        for (int c = 0; c < 2; ++c) dFp[2 * (i * layers + l) + c] = dF[2 * i + c] / layers;
+    mco_spread(nx, ny, NP, P, dFp.data(), dG.data());             // broadcast through every point
+    for (size_t c = 0; c < 2 * nc; ++c) G[c] += dG[c];
+    for (size_t c = 0; c < nc; ++c) {
+      u[c] = ustar[c] + G[c] / (2.0 * rho[c]);
+      u[nc + c] = ustar[nc + c] + G[nc + c] / (2.0 * rho[c]);
+    }
+  }
+  if (u_out) std::memcpy(u_out, u.data(), 2 * nc * sizeof(double));
+}
+
 }  // extern "C"
 
 // ------------------------------------------------------------------------------------
@@ -536,7 +581,7 @@ int mco_create(const mco_world_params* p, mco_world** out) {
   if ((p->pbd_order != 0 && p->pbd_order != 1) || (p->pbd_project != 0 && p->pbd_project != 1) ||
       (p->two_layer != 0 && p->two_layer != 1) || !(p->layer_offset >= 0) || p->layer_offset > 1)
     return MCO_EINVAL;
-  if (p->two_layer && p->coupling == MCO_COUPLING_MDF) return MCO_EINVAL;  // not defined together (reading 28)
+
   if (p->coupling != MCO_COUPLING_FORCE && p->coupling != MCO_COUPLING_MDF) return MCO_EINVAL;
   if (p->coupling == MCO_COUPLING_MDF && (p->mdf_iters < 1 || p->mdf_iters > 16)) return MCO_EINVAL;
   for (int k = 0; k < p->n_fields; ++k) {
@@ -725,8 +770,12 @@ static int mco_one_step(mco_world* w) {
     // S5 (MDF): forcing iterations against the force-free velocity of the current populations
     std::vector<double> rho(nc), ustar(2 * nc), V(w->F);
     mco_moments(nx, ny, w->f.data(), rho.data(), ustar.data());
-    mco_mdf(nx, ny, N, w->X.data(), V.data(), ustar.data(), rho.data(), w->rho0, w->p.mdf_iters,
-            w->F.data(), w->G.data(), nullptr, nullptr);
+    if (two)  // the forcing iterations see the fluid through the markers as well (readings 26 + 28)
+      mco_mdf_layers(nx, ny, N, 2, P, V.data(), ustar.data(), rho.data(), w->rho0, w->p.mdf_iters,
+                     w->F.data(), w->G.data(), nullptr, nullptr);
+    else
+      mco_mdf(nx, ny, N, w->X.data(), V.data(), ustar.data(), rho.data(), w->rho0, w->p.mdf_iters,
+              w->F.data(), w->G.data(), nullptr, nullptr);
   } else if (two) {
     // S5, two layers: each marker carries half of its bead's force
     std::vector<double> FM(2 * (size_t)NM);

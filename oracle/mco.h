@@ -159,6 +159,13 @@ void mco_mdf(int32_t nx, int32_t ny, int64_t N, const double* xy, const double* 
              const double* ustar, const double* rho, double rho0, int32_t iters, double* F,
              double* G, double* u_out, double* resid);
 
+/* MDF through `layers` points per bead (layers = 2: the two-layer markers, readings 26 + 28;
+ * layers = 1 is mco_mdf).  P [N*layers][2], point l of bead i at row i*layers + l.  Sampling = mean
+ * over a bead's points, broadcast = dF / layers through each point.  Other arguments as mco_mdf. */
+void mco_mdf_layers(int32_t nx, int32_t ny, int64_t N, int32_t layers, const double* P, const double* V,
+                    const double* ustar, const double* rho, double rho0, int32_t iters, double* F,
+                    double* G, double* u_out, double* resid);
+
 #ifdef __cplusplus
 }
 #endif

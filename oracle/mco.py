@@ -326,3 +326,17 @@ def mdf(xy, V, ustar, rho, rho0: float, iters: int):
                   C.c_double(rho0), C.c_int32(iters), _d(out["F"]), _d(out["G"]), _d(out["u"]),
                   _d(out["resid"]))
     return out
+
+
+def mdf_layers(P, layers: int, V, ustar, rho, rho0: float, iters: int):
+    """MDF through `layers` points per bead (P [N*layers, 2]) -> dict like mdf()."""
+    P, V, ustar, rho = _f64(P), _f64(V), _f64(ustar), _f64(rho)
+    _, ny, nx = ustar.shape
+    N = len(V)
+    assert len(P) == N * layers
+    out = dict(F=np.empty((N, 2)), G=np.empty((2, ny, nx)), u=np.empty((2, ny, nx)),
+               resid=np.empty(iters + 1))
+    lib().mco_mdf_layers(C.c_int32(nx), C.c_int32(ny), C.c_int64(N), C.c_int32(layers), _d(P), _d(V), _d(ustar),
+                         _d(rho), C.c_double(rho0), C.c_int32(iters), _d(out["F"]), _d(out["G"]), _d(out["u"]),
+                         _d(out["resid"]))
+    return out

@@ -78,18 +78,25 @@ __global__ void __launch_bounds__(256) k_mdf_force(int N, const float2* __restri
                                                    const float2* __restrict__ u, cudaTextureObject_t tex_u, int nx,
                                                    int ny, float rho0, float2* __restrict__ dF,
                                                    float2* __restrict__ F, unsigned* __restrict__ tile_fmax,
-                                                   size_t wstride) {
+                                                   size_t wstride, const float2* __restrict__ O = nullptr) {
   {
     const size_t ws = blockIdx.y * wstride;
     X = wshift(X, ws); V = wshift(V, ws); u = wshift(u, ws); dF = wshift(dF, ws); F = wshift(F, ws);
-    tile_fmax = wshift(tile_fmax, ws);
+    tile_fmax = wshift(tile_fmax, ws); O = wshift(O, ws);
   }
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = b < N;  // every lane stays for the warp-wide reduction
   const float2 p = X[valid ? b : N - 1];
   float m = 0.0f;
   if (valid) {
-    const float2 U = TEXROWS ? interp2_tex<TEXROWS, false>(u, tex_u, nx, ny, p.x, p.y) : interp2(u, nx, ny, p.x, p.y);
+    float2 U;
+    if (!TEXROWS && O) {  // two-layer broadcast (readings 26 + 28): the mean of the samples at the two markers
+      const float2 o = __ldg(O + b);
+      const float2 up = interp2_off(u, nx, ny, p.x, p.y, o.x, o.y), um = interp2_off(u, nx, ny, p.x, p.y, -o.x, -o.y);
+      U = make_float2(0.5f * (up.x + um.x), 0.5f * (up.y + um.y));
+    } else {
+      U = TEXROWS ? interp2_tex<TEXROWS, false>(u, tex_u, nx, ny, p.x, p.y) : interp2(u, nx, ny, p.x, p.y);
+    }
     const float2 v = V[b];
     const float2 d = make_float2(rho0 * (v.x - U.x), rho0 * (v.y - U.y));
     float2 f = d;
@@ -112,6 +119,7 @@ __global__ void __launch_bounds__(256) k_mdf_force(int N, const float2* __restri
 // K5c: broadcast.  One CTA per 32x32 tile accumulates the spread of dF in shared memory (the
 // fixed-point tile accumulation of S5, k_p2g.cuh: order independent, bit-reproducible) and
 // corrects the velocity of the tile's nodes in place.  Tiles without listed beads return at once.
+template <bool TWO = false>
 __global__ void __launch_bounds__(256, 5) k_mdf_spread_tile(int nx, int ny, const int* __restrict__ tile_start,
                                                             const int* __restrict__ list,
                                                             const float2* __restrict__ X,
@@ -119,14 +127,14 @@ __global__ void __launch_bounds__(256, 5) k_mdf_spread_tile(int nx, int ny, cons
                                                             const float* __restrict__ tile_rho_max,
                                                             const unsigned* __restrict__ tile_fmax,
                                                             const float* __restrict__ hrinv, float2* __restrict__ u,
-                                                            size_t wstride) {
+                                                            size_t wstride, const float2* __restrict__ O = nullptr) {
   __shared__ __align__(16) int acc0[ACC_N], acc1[ACC_N], accl0[ACC_N], accl1[ACC_N];
   __shared__ float red[32];
   {
     const size_t ws = blockIdx.y * wstride;
     tile_start = wshift(tile_start, ws); list = wshift(list, ws); X = wshift(X, ws); dF = wshift(dF, ws);
     tile_rho_max = wshift(tile_rho_max, ws); tile_fmax = wshift(tile_fmax, ws); hrinv = wshift(hrinv, ws);
-    u = wshift(u, ws);
+    u = wshift(u, ws); O = wshift(O, ws);
   }
   const int t = blockIdx.x, ntx = nx / TS;
   const int s = tile_start[t], e = tile_start[t + 1];
@@ -141,14 +149,15 @@ __global__ void __launch_bounds__(256, 5) k_mdf_spread_tile(int nx, int ny, cons
   float4 v0 = *up0, v1 = *up1;
   const float2 h0 = __ldg(reinterpret_cast<const float2*>(hrinv + (size_t)(y0 + ry) * nx + i));
   const float2 h1 = __ldg(reinterpret_cast<const float2*>(hrinv + (size_t)(y0 + ry + 16) * nx + i));
-  float2 xpre = make_float2(0.f, 0.f), fpre = make_float2(0.f, 0.f);
+  float2 xpre = make_float2(0.f, 0.f), fpre = make_float2(0.f, 0.f), opre = make_float2(0.f, 0.f);
   {
     const int b = first_entry(s, e, list);
-    if (b >= 0) { xpre = __ldg(X + b); fpre = __ldg(dF + b); }
+    if (b >= 0) { load_point<TWO>(X, O, b, xpre, opre); fpre = __ldg(dF + (TWO ? b >> 1 : b)); }
   }
   float linv;
-  const float scale = spread_tile_accumulate(nx, ny, x0, y0, s, e, list, X, dF, tile_rho_max ? tile_rho_max[t] : 0.0f,
-                                             tile_fmax, t, acc0, acc1, accl0, accl1, red, linv, xpre, fpre);
+  const float scale = spread_tile_accumulate<false, TWO>(nx, ny, x0, y0, s, e, list, X, dF,
+                                                         tile_rho_max ? tile_rho_max[t] : 0.0f, tile_fmax, t, acc0,
+                                                         acc1, accl0, accl1, red, linv, xpre, fpre, DealCfg(), O, opre);
   __syncthreads();
   const float inv = 1.0f / scale;
   {

@@ -59,7 +59,6 @@ bool validate(const mc_world_params* p, Derived* d, std::string* why) {
   if (p->max_beads < 0 || p->max_beads > ((int64_t)1 << 29) - 1) { *why = "max_beads out of range (0 .. 2^29 - 1)"; return false; }
   if (p->coupling != MC_COUPLING_FORCE && p->coupling != MC_COUPLING_MDF) { *why = "unknown coupling"; return false; }
   if (p->coupling == MC_COUPLING_MDF && (p->mdf_iters < 1 || p->mdf_iters > 16)) { *why = "mdf_iters must be 1..16"; return false; }
-  if (p->coupling == MC_COUPLING_MDF && p->two_layer) { *why = "two_layer is not defined with the MDF coupling (reading 28)"; return false; }
   for (int k = 0; k < p->n_fields; ++k) {
     const mc_field_params& f = p->fields[k];
     if (f.kind == MC_FIELD_BEAD_DENSITY) {
@@ -439,7 +438,7 @@ int enqueue_step(mc_world* w) {
       const int mbx = pick_bx(nx) / 2;
       mc::k_lbm_moments<<<dim3(nx / (2 * mbx), ny, nb), mbx, 0, st>>>(w->fbuf(w->cur), nx, ny, w->rho0, ug, hrinv, ws);
       w->launches++;
-      const bool tex = w->tex_on && w->tex_u && nb == 1;
+      const bool tex = w->tex_on && w->tex_u && nb == 1 && !two;
       const int K = w->p.mdf_iters;
       unsigned* mfmax = w->ptr<unsigned>(w->L.mdf_fmax);  // [K][n_tiles], raised by K5b with atomicMax
       for (unsigned b = 0; b < nb; ++b)
@@ -449,7 +448,7 @@ int enqueue_step(mc_world* w) {
         unsigned* slot = mfmax + (size_t)k * n_tiles;
         const bool first = k == 0, last = k + 1 == K;
 #define MC_MDF_FORCE(FI, LA, TX) \
-  mc::k_mdf_force<FI, LA, TX><<<dim3((N + 63) / 64, nb), 64, 0, st>>>(N, X, V, ug, w->tex_u, nx, ny, w->rho0, dF, F, slot, ws)
+  mc::k_mdf_force<FI, LA, TX><<<dim3((N + 63) / 64, nb), 64, 0, st>>>(N, X, V, ug, w->tex_u, nx, ny, w->rho0, dF, F, slot, ws, O)
         if (tex) {
           if (first && last) MC_MDF_FORCE(true, true, 1);
           else if (first) MC_MDF_FORCE(true, false, 1);
@@ -464,8 +463,12 @@ int enqueue_step(mc_world* w) {
 #undef MC_MDF_FORCE
         w->launches++;
         if (!last) {
-          mc::k_mdf_spread_tile<<<dim3(n_tiles, nb), 256, 0, st>>>(nx, ny, tile_start, list, X, dF,
-                                                                   w->d.n_density ? tile_rho_max : nullptr, slot, hrinv, ug, ws);
+          if (two)
+            mc::k_mdf_spread_tile<true><<<dim3(n_tiles, nb), 256, 0, st>>>(nx, ny, tile_start, list, X, dF,
+                                                                           w->d.n_density ? tile_rho_max : nullptr, slot, hrinv, ug, ws, O);
+          else
+            mc::k_mdf_spread_tile<false><<<dim3(n_tiles, nb), 256, 0, st>>>(nx, ny, tile_start, list, X, dF,
+                                                                            w->d.n_density ? tile_rho_max : nullptr, slot, hrinv, ug, ws);
           w->launches++;
         }
       }

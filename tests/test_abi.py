@@ -51,7 +51,7 @@ def test_workspace_bytes_validation(lib):
     for key, val in (("pbd_iters", 0), ("pbd_iters", 9), ("pbd_order", 2), ("pbd_project", 2), ("two_layer", -1),
                      ("layer_offset", 1.5)):
         assert binding.workspace_bytes(dict(w["params"], **{key: val})) == 0, key
-    assert binding.workspace_bytes(dict(w["params"], two_layer=1, coupling=1, mdf_iters=2)) == 0  # reading 28
+    assert binding.workspace_bytes(dict(w["params"], two_layer=1, coupling=1, mdf_iters=2)) > good  # readings 26 + 28 together
     # literal PBD and the two-layer broadcast are accepted; two layers double the tile lists
     assert binding.workspace_bytes(dict(w["params"], pbd_iters=4, pbd_order=1)) == good
     assert binding.workspace_bytes(dict(w["params"], two_layer=1)) > good

@@ -81,15 +81,22 @@ def test_two_layer_trajectory():
     assert_close("X after 100 steps", G.read_state(keys=("xy",))["xy"], O.read_state()["xy"], 1e-3)
 
 
-def test_two_layer_differs_from_one_layer_and_mdf_is_refused():
+def test_two_layer_differs_from_one_layer():
     from paper_2607_02954_b200 import binding
     w = worlds.random_world(128, 96, 40, 64, seed=8)
     A, B = binding.World(w), binding.World(two(w))
     A.step(10)
     B.step(10)
     assert rel_l2(B.read_state(keys=("u",))["u"], A.read_state(keys=("u",))["u"])[0] > 1e-3
-    with pytest.raises(binding.McError):
-        binding.World(two(w, coupling=1, mdf_iters=2))
+
+
+@pytest.mark.parametrize("name,iters", [("ragged", 3), ("m64", 1), ("no_fields", 4), ("single_tile", 2), ("h025", 3)])
+def test_two_layer_with_mdf_per_step_parity(name, iters):
+    # the paper's leakage-control stack together: MDF iterations through the two-layer markers
+    w = WORLDS[name]()
+    w["params"] = dict(w["params"], coupling=1, mdf_iters=iters)
+    worst = run_protocol(w, steps_at=[0, 1, 8])
+    print(name, "mdf", iters, {k: f"{v:.2e}" for k, v in worst.items()})
 
 
 def test_two_layer_one_parity_step_large():

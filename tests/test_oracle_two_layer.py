@@ -156,8 +156,70 @@ def test_two_layer_widens_the_band_of_a_straight_chain():
     assert rows(G1) == 3 and rows(Gp + Gm) == 5     # y = 30 is a node row: phi(+-2) = 0
 
 
-def test_two_layer_is_not_defined_with_mdf():
-    w = _two_layer_world()
-    w["params"] = dict(w["params"], coupling=1, mdf_iters=2)
-    with pytest.raises(ValueError):
-        mco.World(w)
+def _pair_gram(M, nx, ny):
+    """Gram matrix of the two-layer kernels: K_ij = sum_g delta2(g; i) delta2(g; j)."""
+    n = len(M) // 2
+    K = np.empty((n, n))
+    for j in range(n):
+        dj = 0.5 * mco.deposit(nx, ny, M[2 * j:2 * j + 2])
+        s = mco.interp(dj[None], M)[:, 0]
+        K[:, j] = 0.5 * (s[0::2] + s[1::2])
+    return K
+
+
+def test_mdf_through_one_layer_is_mco_mdf():
+    nx, ny = 20, 24
+    rng = np.random.default_rng(7)
+    xy = np.stack([20 * worlds.uniform(1, "mdf-a", 30), 24 * worlds.uniform(1, "mdf-b", 30)], 1)
+    V = 1e-2 * rng.standard_normal((30, 2))
+    us = 1e-3 * rng.standard_normal((2, ny, nx))
+    rho = 1 + 0.03 * rng.standard_normal((ny, nx))
+    a, b = mco.mdf(xy, V, us, rho, 1.0, 4), mco.mdf_layers(xy, 1, V, us, rho, 1.0, 4)
+    for k in ("F", "G", "u", "resid"):
+        assert np.array_equal(a[k], b[k]), k
+
+
+def test_two_layer_mdf_converges_to_the_no_slip_solution_of_a_dense_solve():
+    # fixed point of the two-layer iteration: mean-over-markers interp(ustar + spread2(F)/(2 rho)) = V
+    # <=> K F = 2 rho (V - Ustar), K the Gram matrix of the two-layer kernels; the error after k
+    # iterations is (I - K/2)^k (F^0 - F_exact), exactly as for one layer (tests/test_oracle_mdf.py)
+    nx, ny, rho = 24, 20, 1.05
+    s = np.arange(9.0)
+    xy = np.stack([6.3 + s * np.cos(0.4), 7.1 + s * np.sin(0.4)], 1)
+    M = mco.markers([0, 9], xy, 0.5)
+    rng = np.random.default_rng(4)
+    V = 1e-2 * np.stack([np.cos(0.3 * s), 0.5 + np.sin(0.2 * s)], 1)
+    us = 1e-4 * rng.standard_normal((2, ny, nx))
+    K = _pair_gram(M, nx, ny)
+    assert np.linalg.eigvalsh(K).max() < 4
+    Um = mco.interp(us, M)
+    Fex = np.linalg.solve(K, 2 * rho * (V - 0.5 * (Um[0::2] + Um[1::2])))
+    for it in (1, 3, 32):
+        r = mco.mdf_layers(M, 2, V, us, np.full((ny, nx), rho), rho, it)
+        EK = np.linalg.matrix_power(np.eye(9) - 0.5 * K, it) @ (-Fex)
+        assert np.allclose(r["F"] - Fex, EK, rtol=1e-9, atol=1e-15)
+        assert np.allclose(r["G"].sum(axis=(1, 2)), r["F"].sum(axis=0), rtol=1e-12, atol=1e-18)
+    assert np.all(np.diff(r["resid"]) < 0) and r["resid"][-1] < 0.1 * r["resid"][0]
+
+
+def test_two_layer_mdf_step_glue_and_budgets():
+    w = _two_layer_world(kappa_rep=0.01)
+    w["params"] = dict(w["params"], coupling=1, mdf_iters=3)
+    O = mco.World(w)
+    O.step(2)
+    before = O.read_state()
+    O.step(1)
+    s, it = O.read_state(), O.read_intermediates()
+    X0 = before["xy"]
+    M = mco.markers(w["offsets"], X0, 0.5)
+    # the summed force and its grid image are those of the layered MDF on the step's own inputs
+    f_pre = before["fdev"] + np.array([4 / 9] + [1 / 9] * 4 + [1 / 36] * 4)[:, None, None]
+    rho, ustar = mco.moments(f_pre)
+    r1 = mco.mdf_layers(M, 2, np.zeros_like(X0), ustar, rho, 1.0, 1)      # V = 0: F = -rho0 * mean interp(u*)
+    Um = mco.interp(ustar, M)
+    assert np.allclose(r1["F"], -0.5 * (Um[0::2] + Um[1::2]), rtol=1e-13, atol=1e-18)
+    assert np.allclose(it["G"].sum(axis=(1, 2)), s["force"].sum(axis=0), rtol=1e-11, atol=1e-16)
+    U = s["xy"] - X0
+    assert abs((it["G"] * s["u"]).sum() - (s["force"] * U).sum()) < 1e-11 * abs((s["force"] * U).sum()) + 1e-18
+    mom = lambda st: np.array([np.tensordot(CX, st["fdev"], 1).sum(), np.tensordot(CY, st["fdev"], 1).sum()])
+    assert np.abs(mom(s) - mom(before) - s["force"].sum(axis=0)).max() < 1e-12

@@ -188,6 +188,16 @@ int mc_step(mc_world* w, int32_t n);
 int mc_read_state(mc_world* w, int64_t* step_out /*HOST*/, float* xy, float* u, float* rho,
                   float* fdev, float* field, float* force, float* sense);
 
+/* Checkpoint / resume: replace the fluid state and the step counter by a state read earlier with
+ * mc_read_state ("discrete grids which store information about the world, such as the fluid
+ * state").  fdev: DEVICE float [9][ny][nx], pre-collision populations as deviations f_q - w_q*rho0
+ * exactly as mc_read_state returns them, or NULL to keep the fluid; step: the step index the next
+ * mc_step starts from (it selects the actuation phase).  Together with mc_load_filaments /
+ * mc_set_positions this restores a world: a resumed run continues like the uninterrupted one up to
+ * rounding (the tile lists are rebuilt, and their lengths set the fixed-point scales).  Clears a
+ * divergence flag.  Synchronises the stream.  Errors: MC_EINVAL, MC_ESTATE (batch member), MC_ECUDA. */
+int mc_load_fluid(mc_world* w, int64_t step, const float* fdev /*DEVICE or NULL*/);
+
 /* Last step's intermediates, for parity checks (same rules as mc_read_state):
  *   rho_b [ny][nx] deposited bead density (S2); G [2][ny][nx] spread force (S5). */
 int mc_read_intermediates(mc_world* w, float* rho_b, float* G);

@@ -18,7 +18,7 @@ MC_OK, MC_EINVAL, MC_ENOMEM, MC_ECUDA, MC_ESTATE, MC_EDIVERGED = 0, -1, -2, -3, 
 SYMBOLS = ("mc_workspace_bytes", "mc_create", "mc_load_filaments", "mc_step", "mc_read_state",
            "mc_read_intermediates", "mc_launch_count", "mc_destroy", "mc_last_error",
            "mc_profile_enable", "mc_profile_read", "mc_keep_intermediates", "mc_texture_gathers",
-           "mc_cluster_tiles", "mc_set_positions", "mc_set_length_actuation", "mc_batch_workspace_bytes",
+           "mc_cluster_tiles", "mc_set_positions", "mc_set_length_actuation", "mc_load_fluid", "mc_batch_workspace_bytes",
            "mc_create_batch", "mc_load_filaments_batch", "mc_step_batch", "mc_batch_world", "mc_destroy_batch",
            "mc_batch_last_error", "mc_set_positions_batch", "mc_read_positions_batch")
 PROF_SLOTS = ("K0_bin", "K2a_deposit", "K3a_blur_grad", "K1_filament", "K2b_spread", "K3b_lbm",
@@ -87,6 +87,8 @@ def load_library():
     L.mc_set_positions.argtypes = [vp, vp]
     L.mc_cluster_tiles.restype = C.c_int
     L.mc_cluster_tiles.argtypes = [vp, i32]
+    L.mc_load_fluid.restype = C.c_int
+    L.mc_load_fluid.argtypes = [vp, i64, vp]
     L.mc_set_length_actuation.restype = C.c_int
     L.mc_set_length_actuation.argtypes = [vp, vp]
     L.mc_batch_workspace_bytes.restype = C.c_size_t
@@ -225,6 +227,19 @@ class World:
                 d = a.to(self.device, dtype=torch.float32).contiguous()
                 assert d.numel() == self.N
                 rc = load_library().mc_set_length_actuation(self.h, C.c_void_p(d.data_ptr()))
+        self._check(rc)
+
+    def load_fluid(self, step: int, fdev=None):
+        """mc_load_fluid: step counter and (optionally) the populations [9, ny, nx] as mc_read_state returns them."""
+        torch = self.torch
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):
+            d = None
+            if fdev is not None:
+                if not isinstance(fdev, torch.Tensor):
+                    fdev = torch.from_numpy(np.ascontiguousarray(fdev, dtype=np.float32))
+                d = fdev.to(self.device, dtype=torch.float32).contiguous()
+                assert d.numel() == 9 * self.nx * self.ny
+            rc = load_library().mc_load_fluid(self.h, int(step), C.c_void_p(d.data_ptr()) if d is not None else None)
         self._check(rc)
 
     def set_positions(self, xy):

@@ -302,6 +302,29 @@ __global__ void k_lbm_export(const float* __restrict__ src, int nx, int ny, floa
   if (rho) rho[c] = rho0 + (g[0] + ((g[1] + g[3]) + (g[2] + g[4])) + ((g[5] + g[7]) + (g[6] + g[8])));
 }
 
+// mc_load_fluid: the inverse of k_lbm_export.  The library stores POST-collision populations at their
+// own node and streams on read (g_q(x) = gpost_q(x - c_q)); a caller hands in the streamed,
+// pre-collision deviations g_q(x), so gpost_q(x) = g_q(x + c_q).
+__global__ void k_lbm_import(const float* __restrict__ fdev, int nx, int ny, float* __restrict__ dst) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y;
+  if (i >= nx) return;
+  const size_t nc = (size_t)nx * ny;
+  const int im = (i == 0) ? nx - 1 : i - 1, ip = (i == nx - 1) ? 0 : i + 1;
+  const int jm = (j == 0) ? ny - 1 : j - 1, jp = (j == ny - 1) ? 0 : j + 1;
+  const size_t r0 = (size_t)j * nx, rm = (size_t)jm * nx, rp = (size_t)jp * nx;
+  const size_t c = r0 + i;
+  dst[0 * nc + c] = fdev[0 * nc + r0 + i];
+  dst[1 * nc + c] = fdev[1 * nc + r0 + ip];   // c_1 = (+1, 0)
+  dst[2 * nc + c] = fdev[2 * nc + rp + i];    // c_2 = (0, +1)
+  dst[3 * nc + c] = fdev[3 * nc + r0 + im];   // c_3 = (-1, 0)
+  dst[4 * nc + c] = fdev[4 * nc + rm + i];    // c_4 = (0, -1)
+  dst[5 * nc + c] = fdev[5 * nc + rp + ip];   // c_5 = (+1, +1)
+  dst[6 * nc + c] = fdev[6 * nc + rp + im];   // c_6 = (-1, +1)
+  dst[7 * nc + c] = fdev[7 * nc + rm + im];   // c_7 = (-1, -1)
+  dst[8 * nc + c] = fdev[8 * nc + rm + ip];   // c_8 = (+1, -1)
+}
+
 // mc_read_state: blocked interleaved (x,y) field -> two row-major planes
 __global__ void k_split2(int nx, int ny, const float2* __restrict__ in, float* __restrict__ out0, float* __restrict__ out1) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;

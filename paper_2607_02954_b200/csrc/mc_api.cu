@@ -1115,6 +1115,30 @@ int mc_set_length_actuation(mc_world* w, const float* act_L_amp) {
   return MC_OK;
 }
 
+int mc_load_fluid(mc_world* w, int64_t step, const float* fdev) {
+  if (!w) return MC_EINVAL;
+  if (w->batch_member && !g_batch_call) return fail(w, MC_ESTATE, "world belongs to a batch");
+  if (step < 0) return fail(w, MC_EINVAL, "step < 0");
+  cudaStream_t st = w->stream;
+  CudaSeq cs{w, "mc_load_fluid"};
+  if (fdev) {
+    const int bx = pick_bx(w->nx);
+    mc::k_lbm_import<<<dim3(w->nx / bx, w->ny), bx, 0, st>>>(fdev, w->nx, w->ny, w->fbuf(w->cur));
+    cs.launched("k_lbm_import");
+    w->launches++;
+  }
+  w->step = step;
+  const long long host_step = step;
+  cs.ok(cudaMemcpyAsync(w->ptr<long long>(w->L.flags) + 4, &host_step, 8, cudaMemcpyHostToDevice, st), "cudaMemcpyAsync");
+  w->diverged = false;
+  cs.ok(cudaMemsetAsync(w->ptr<int>(w->L.flags), 0, 4, st), "cudaMemsetAsync");  // a loaded state starts with a clear flag
+  cudaError_t e = cudaStreamSynchronize(st);  // fdev belongs to the caller, host_step to this frame
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (cs.rc != MC_OK) return cs.rc;
+  if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_load_fluid: ") + cudaGetErrorString(e));
+  return MC_OK;
+}
+
 int mc_keep_intermediates(mc_world* w, int32_t on) {
   if (!w) return MC_EINVAL;
   if (w->keep_G != (on != 0)) drop_graphs(w);

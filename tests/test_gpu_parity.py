@@ -482,3 +482,47 @@ def test_set_positions_continues_the_run():
     c1, c2 = C1.read_state(keys=("xy", "u", "force")), C2.read_state(keys=("xy", "u", "force"))
     for k in ("xy", "u", "force"):
         assert c1[k].tobytes() == c2[k].tobytes(), k
+
+
+def test_checkpoint_and_resume_through_load_fluid():
+    # mc_read_state -> (new world) mc_load_filaments + mc_load_fluid: the populations and the step
+    # counter come back bit for bit, and the resumed run continues like the uninterrupted one to rounding
+    from paper_2607_02954_b200 import binding
+    w = SMALL["static_64x96"]()
+    A = binding.World(w)
+    A.step(9)
+    ck = A.read_state(keys=("xy", "fdev"))
+    B = binding.World(dict(w, xy=ck["xy"]))
+    B.load_fluid(ck["step"], ck["fdev"])
+    back = B.read_state(keys=("xy", "fdev"))
+    assert back["step"] == 9
+    assert back["fdev"].tobytes() == ck["fdev"].tobytes() and back["xy"].tobytes() == ck["xy"].tobytes()
+    A.step(7)
+    B.step(7)
+    a, b = A.read_state(keys=("xy", "u", "fdev", "force")), B.read_state(keys=("xy", "u", "fdev", "force"))
+    assert a["step"] == b["step"] == 16
+    assert rel_l2(b["xy"], a["xy"])[0] < 1e-6
+    for k in ("u", "fdev", "force"):                  # force: the actuation phase of step 15 is the same
+        assert rel_l2(b[k], a[k])[0] < 2e-5, k
+    # the step counter alone (fluid kept): only the actuation phase changes
+    B.load_fluid(100)
+    assert B.read_state(keys=("xy",))["step"] == 100
+    with pytest.raises(binding.McError):
+        B.load_fluid(-1)
+
+
+def test_keep_g_is_neutral_in_the_cluster_kernels():
+    # parity runs the KEEP_G instantiations, bench.py the plain ones: same bits on a crowded world
+    # (split launch: k_lbm_spread_tile_cl<4, *> beside k_lbm_spread_tile<*>)
+    from paper_2607_02954_b200 import binding
+    w = _very_crowded()
+    outs = []
+    for keep in (False, True):
+        G = binding.World(w)
+        assert G.cluster_tiles(-1) == 4
+        G.keep_intermediates(keep)
+        G.step(6)
+        outs.append(G.read_state(keys=("xy", "u", "fdev", "force")))
+        G.close()
+    for k in ("xy", "u", "fdev", "force"):
+        assert outs[0][k].tobytes() == outs[1][k].tobytes(), k

@@ -198,3 +198,62 @@ def test_viscosity_sweep_of_the_scallop_pair():
     assert thin[0][0] > thin[1][0] > thin[2][0] and thick[0][0] > thick[1][0] > thick[2][0]
     # close to a stop at the thick end: the wave at nu_lat = 2 covers < 10 % of its distance at 0.1
     assert thick[2][1] < 0.1 * thick[0][1]
+
+
+def test_oracle_is_clean_under_asan_and_ubsan(tmp_path):
+    # the oracle is built with -fsanitize=address,undefined and steps a world with
+    # every option on; any out-of-bounds access, use of freed memory or undefined arithmetic aborts.
+    # (compute-sanitizer is closed on the GPU pool; the CUDA path's memory safety rests on parity over
+    # ragged / periodic / crowded worlds and on bit-reproducibility.)
+    import os
+    import subprocess
+    import sys
+    src = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "oracle", "mco.cpp")
+    drv = tmp_path / "drive.cpp"
+    drv.write_text(r"""
+#include "mco.h"
+#include <cstdio>
+#include <cmath>
+#include <vector>
+int main() {
+  for (int variant = 0; variant < 3; ++variant) {
+    mco_world_params p = {};
+    p.nx = 64; p.ny = 32; p.dt = 1e-2f; p.nu = 10.f; p.trt_lambda = 0.25f; p.rho0 = 1.f; p.k_el = 2e4f;
+    p.pbd_iters = variant == 0 ? 1 : 3; p.pbd_order = variant == 2; p.pbd_project = variant == 2;
+    p.two_layer = variant >= 1; p.layer_offset = 0.5f; p.coupling = variant == 1; p.mdf_iters = 2;
+    float src4[4] = {10.f, 20.f, 1.f, 6.f};
+    p.n_fields = 2;
+    p.fields[0].kind = MCO_FIELD_BEAD_DENSITY; p.fields[0].sigma = 1.f; p.fields[0].radius = 5; p.fields[0].coupling = 100.f;
+    p.fields[1].kind = MCO_FIELD_STATIC_SOURCE; p.fields[1].coupling = 200.f; p.fields[1].n_sources = 1; p.fields[1].sources = src4;
+    const int lens[4] = {3, 17, 40, 5};
+    std::vector<int32_t> off = {0};
+    for (int m : lens) off.push_back(off.back() + m);
+    const int N = off.back();
+    p.max_beads = N;
+    std::vector<float> xy(2 * N), L(N, 1.f), th(N, 0.1f), k(N, 0.5f), amp(N, 0.05f), ph(N, 0.3f), T(N, 2.f), la(N, 0.03f);
+    for (int f = 0; f < 4; ++f)
+      for (int i = off[f]; i < off[f + 1]; ++i) { xy[2 * i] = 60.f + 0.9f * (i - off[f]) + 64.f * (f - 1); xy[2 * i + 1] = 5.f + 7.f * f + 0.3f * std::sin(0.7f * i); }
+    mco_world* w = nullptr;
+    if (mco_create(&p, &w) != MCO_OK) return 2;
+    if (mco_load_filaments(w, 4, off.data(), xy.data(), L.data(), th.data(), k.data(), k.data(), k.data(), amp.data(), ph.data(), T.data()) != MCO_OK) return 3;
+    mco_set_length_actuation(w, la.data());
+    mco_set_threads(w, 2);
+    if (mco_step(w, 4) != MCO_OK) return 4;
+    std::vector<double> X(2 * N), u(2 * 64 * 32);
+    long long st = 0;
+    mco_read_state(w, (int64_t*)&st, X.data(), u.data(), nullptr, nullptr, nullptr, nullptr, nullptr);
+    if (st != 4 || !std::isfinite(X[0])) return 5;
+    mco_destroy(w);
+  }
+  std::puts("sanitized ok");
+  return 0;
+}
+""")
+    exe = tmp_path / "drive"
+    inc = os.path.dirname(src)
+    r = subprocess.run(["g++", "-std=c++17", "-O1", "-g", "-fopenmp", "-fsanitize=address,undefined",
+                        "-fno-sanitize-recover=all", f"-I{inc}", str(drv), src, "-o", str(exe)], capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr[-2000:]
+    env = dict(os.environ, ASAN_OPTIONS="detect_leaks=1", OMP_NUM_THREADS="2")
+    r = subprocess.run([str(exe)], capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0 and "sanitized ok" in r.stdout, (r.returncode, r.stdout[-500:], r.stderr[-3000:])

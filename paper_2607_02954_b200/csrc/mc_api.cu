@@ -634,6 +634,7 @@ void mc_destroy(mc_world* w) {
   for (cudaEvent_t e : w->prof_ev) cudaEventDestroy(e);
   if (w->tex_u) cudaDestroyTextureObject(w->tex_u);
   if (w->tex_A) cudaDestroyTextureObject(w->tex_A);
+  if (w->side) cudaStreamSynchronize(w->side);  // nothing of this world may still run on its second stream
   if (w->ev_fork) cudaEventDestroy(w->ev_fork);
   if (w->ev_join) cudaEventDestroy(w->ev_join);
   if (w->side) cudaStreamDestroy(w->side);
@@ -1152,11 +1153,24 @@ int mc_cluster_tiles(mc_world* w, int32_t c) {
   if (c >= 0 && (c & MC_CLUSTER_ALL_TILES)) { split_on = false; c &= ~MC_CLUSTER_ALL_TILES; }
   if (c != -1 && c != 0 && c != 2 && c != 4 && c != 8) return fail(w, MC_EINVAL, "cluster size must be -1, 0, 2, 4 or 8");
   const int now = c >= 0 ? c : w->cluster_auto;
-  if (now != w->cluster || split_on != w->split_on) drop_graphs(w);
+  const bool changed = now != w->cluster || split_on != w->split_on;
+  if (changed) drop_graphs(w);
   w->cluster_user = c;
   w->cluster = now;
   w->split_on = split_on;
   if (now > 0 && split_on) ensure_side_stream(w);
+  if (changed && w->N > 0) {
+    // the crowded-tile table is written by the list rebuild of a step that runs the split launch:
+    // make the next step rebuild, so that a table from before the switch is never used
+    mc::ListState force;
+    force.need = 1;
+    force.drift = INFINITY;
+    force.step_max = force.step_max_p = force.step_max_m = 0u;
+    cudaError_t e = cudaMemcpyAsync(reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16), &force, sizeof(force),
+                                    cudaMemcpyHostToDevice, w->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(w->stream);  // `force` is a host variable of this call
+    if (e != cudaSuccess) return fail(w, MC_ECUDA, std::string("mc_cluster_tiles: ") + cudaGetErrorString(e));
+  }
   return now;
 }
 

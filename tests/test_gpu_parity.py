@@ -445,6 +445,20 @@ def test_cluster_tiles_do_not_change_the_bits():
         for k in outs[0]:
             if k != "step":
                 assert outs[0][k].tobytes() == o[k].tobytes(), k
+    # switching the scheme in the middle of a run (the crowded-tile table belongs to the split launch and
+    # must be rebuilt before it is used): same bits as a run that never switched
+    G = binding.World(w)
+    G.cluster_tiles(4, all_tiles=True)
+    G.keep_intermediates(True)
+    G.step(3)
+    G.cluster_tiles(4, all_tiles=False)
+    G.step(2)
+    G.cluster_tiles(0)
+    G.step(2)
+    late = {**G.read_state(), **G.read_intermediates()}
+    G.close()
+    for k in ("xy", "u", "fdev", "force"):
+        assert rel_l2(late[k], outs[0][k])[0] < 1e-6, k   # to rounding: the forced rebuilds change the list lengths
     # a world without crowded tiles stays on one CTA per tile
     G = binding.World(SMALL["uniform_m32"]())
     assert G.cluster_tiles(-1) == 0

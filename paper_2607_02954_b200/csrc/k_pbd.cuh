@@ -271,61 +271,88 @@ __global__ void __launch_bounds__(128) k_filament_pbd(PbdArgs g, size_t wstride)
   }
 }
 
+// Raise *slot (bits of a non-negative float) to the block's maximum of m: ONE guarded atomic per
+// CTA.  These kernels are short and all their warps would hit the same address (k_markers spent 53 of
+// its 57 us on 7,572 serialised reds); the guard reads past L1 so that it sees other CTAs' updates.
+__device__ __forceinline__ void block_max_to(float m, unsigned* __restrict__ slot) {
+  __shared__ float wmax[32];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    m = (threadIdx.x < (blockDim.x >> 5)) ? wmax[threadIdx.x] : 0.0f;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if (threadIdx.x == 0) {
+      const unsigned mb = __float_as_uint(m);
+      if (mb > __ldcg(slot)) atomicMax(slot, mb);
+    }
+  }
+}
+
 // Two-layer broadcast (reading 28): offset h n_i of every bead, n_i = normalised mean of the unit
 // normals (-t_y, t_x) of the adjacent edges (one edge at a chain end; the first edge's normal if
 // the two cancel).  Runs after every change of X (load, mc_set_positions, K4, projection).
 // step_max_m: bits of the largest component change of an offset, for the drift bound of the tile
 // lists (a marker moves by the bead's displacement plus the change of its offset).
-__global__ void __launch_bounds__(256) k_markers(int N, const float2* __restrict__ X, const float4* __restrict__ PC, float h,
-                                                 float2* __restrict__ O, unsigned* __restrict__ step_max_m, size_t wstride) {
+__global__ void __launch_bounds__(1024) k_markers(int N, const float2* __restrict__ X,
+                                                  const unsigned char* __restrict__ bflags, float h,
+                                                  float2* __restrict__ O, unsigned* __restrict__ step_max_m, size_t wstride) {
   X = wshift(X, blockIdx.y * wstride);
-  PC = wshift(PC, blockIdx.y * wstride);
+  bflags = wshift(bflags, blockIdx.y * wstride);
   O = wshift(O, blockIdx.y * wstride);
   step_max_m = wshift(step_max_m, blockIdx.y * wstride);
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   float m = 0.0f;
   if (b < N) {
-    const int fl = __float_as_int(__ldg(PC + b).w);
-    const float2 p = X[b];
-    // fp64 from the exact fp32 edge vectors: at a hairpin the two edge normals nearly cancel and
-    // the direction of their sum would lose ~|n1 + n2|^-1 digits in fp32 (parity world "hairpin")
-    double nx_ = 0.0, ny_ = 0.0, fx = 0.0, fy = 0.0;
-    bool have = false;
-    if (!(fl & BEAD_FIRST)) {  // edge (b-1, b); differences of nearby fp32 positions are exact
-      const float2 q = X[b - 1];
-      const double vx = (double)p.x - (double)q.x, vy = (double)p.y - (double)q.y;
-      const double inv = 1.0 / sqrt(vx * vx + vy * vy);
-      fx = -vy * inv; fy = vx * inv;
-      nx_ = fx; ny_ = fy;
-      have = true;
+    // every load up front and unconditional (clamped neighbours): one round trip to memory.  The flags
+    // come from the one-byte array of the load (the float4 parameter pack would cost 16 B/bead for 2 bits)
+    const int fl = bflags[b];
+    const float2 p = X[b], qp = X[max(b - 1, 0)], qn = X[min(b + 1, N - 1)], old = O[b];
+    // The differences of nearby fp32 positions are exact.  fp32 normals carry ~1e-7 each; where the
+    // joint is bent beyond ~150 degrees the two normals nearly cancel and the direction of their sum
+    // loses |n1 + n2|^-1 digits (parity world "hairpin" failed at 8e-6): those beads -- rare -- take the
+    // same sum in fp64.  (All in fp64 cost 0.5 ms per step on world 4d: fp64 sqrt and divide.)
+    const bool hasp = !(fl & BEAD_FIRST), hasn = !(fl & BEAD_LAST);
+    float2 vp = make_float2(1.f, 0.f), vn = make_float2(1.f, 0.f);
+    if (hasp) vp = make_float2(p.x - qp.x, p.y - qp.y);   // edge (b-1, b)
+    if (hasn) vn = make_float2(qn.x - p.x, qn.y - p.y);   // edge (b, b+1)
+    const float ip = rsqrtf(vp.x * vp.x + vp.y * vp.y), in_ = rsqrtf(vn.x * vn.x + vn.y * vn.y);
+    const float2 np_ = make_float2(-vp.y * ip, vp.x * ip), nn_ = make_float2(-vn.y * in_, vn.x * in_);
+    float sx = (hasp ? np_.x : 0.f) + (hasn ? nn_.x : 0.f), sy = (hasp ? np_.y : 0.f) + (hasn ? nn_.y : 0.f);
+    const float s2 = sx * sx + sy * sy;
+    float2 o;
+    if (s2 > 0.25f) {
+      const float sc = h * rsqrtf(s2);
+      o = make_float2(sc * sx, sc * sy);
+    } else {
+      double nx_ = 0.0, ny_ = 0.0, fx = 0.0, fy = 0.0;
+      if (hasp) {
+        const double inv = 1.0 / sqrt((double)vp.x * vp.x + (double)vp.y * vp.y);
+        fx = -(double)vp.y * inv; fy = (double)vp.x * inv;
+        nx_ = fx; ny_ = fy;
+      }
+      if (hasn) {
+        const double inv = 1.0 / sqrt((double)vn.x * vn.x + (double)vn.y * vn.y);
+        const double ex = -(double)vn.y * inv, ey = (double)vn.x * inv;
+        if (!hasp) { fx = ex; fy = ey; }
+        nx_ += ex; ny_ += ey;
+      }
+      double nn = sqrt(nx_ * nx_ + ny_ * ny_);
+      if (!(nn > 1e-9)) { nx_ = fx; ny_ = fy; nn = 1.0; }
+      const double sc = (double)h / nn;
+      o = make_float2((float)(sc * nx_), (float)(sc * ny_));
     }
-    if (!(fl & BEAD_LAST)) {   // edge (b, b+1)
-      const float2 q = X[b + 1];
-      const double vx = (double)q.x - (double)p.x, vy = (double)q.y - (double)p.y;
-      const double inv = 1.0 / sqrt(vx * vx + vy * vy);
-      const double ex = -vy * inv, ey = vx * inv;
-      if (!have) { fx = ex; fy = ey; }
-      nx_ += ex; ny_ += ey;
-    }
-    double nn = sqrt(nx_ * nx_ + ny_ * ny_);
-    if (!(nn > 1e-9)) { nx_ = fx; ny_ = fy; nn = 1.0; }
-    const double sc = (double)h / nn;
-    const float2 o = make_float2((float)(sc * nx_), (float)(sc * ny_));
-    const float2 old = O[b];
     O[b] = o;
     m = fmaxf(fabsf(o.x - old.x), fabsf(o.y - old.y));
   }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-  if ((threadIdx.x & 31) == 0) {
-    const unsigned mb = __float_as_uint(m);
-    if (mb > *step_max_m) atomicMax(step_max_m, mb);
-  }
+  block_max_to(m, step_max_m);
 }
 
 // Projection (reading 27): X += Dp after the PBD pass on the advected positions; also the
 // non-finite guard and the largest projection displacement for the lists' drift bound.
-__global__ void __launch_bounds__(256) k_add_displacement(int N, float2* __restrict__ X, const float2* __restrict__ Dp,
+__global__ void __launch_bounds__(1024) k_add_displacement(int N, float2* __restrict__ X, const float2* __restrict__ Dp,
                                                           int* __restrict__ flag, unsigned* __restrict__ step_max_p,
                                                           size_t wstride) {
   X = wshift(X, blockIdx.y * wstride);
@@ -343,12 +370,7 @@ __global__ void __launch_bounds__(256) k_add_displacement(int N, float2* __restr
     if (!(isfinite(p.x) && isfinite(p.y))) atomicOr(flag, 8);
     m = fmaxf(fabsf(d.x), fabsf(d.y));
   }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-  if ((threadIdx.x & 31) == 0) {
-    const unsigned mb = __float_as_uint(m);
-    if (mb > *step_max_p) atomicMax(step_max_p, mb);
-  }
+  block_max_to(m, step_max_p);
 }
 
 }  // namespace mc

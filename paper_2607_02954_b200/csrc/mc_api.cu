@@ -112,7 +112,7 @@ Layout make_layout(const mc_world_params* p, const Derived& d) {
   L.sense = take(N * 4);
   L.list = take((p->two_layer ? 2 : 1) * N * 4 * 4);   // a bead (two-layer: each of its 2 markers) is listed in at most 4 tiles
   L.src = take(N * 4);        // internal bead -> caller's bead
-  L.bflags = take(N);         // first/last flags (load-time scratch; PC.w carries them)
+  L.bflags = take(N);         // first/last/odd flags, one byte per bead (PC.w carries them for K1; k_markers reads these)
   L.scratch = take((N / 3 + 2) * 8);  // load-time: chain offsets and sort keys
   L.flags = take(64 * 4);
   L.sources = take(d.n_src_floats * f4);
@@ -339,8 +339,10 @@ int enqueue_step(mc_world* w) {
     prof_mark(w, 1);
     // K2a: S2 deposit
     if (w->d.n_density) {
-      if (two)  // two-layer markers: one CTA per tile whatever the crowding
-        mc::k_deposit_tile<false, true><<<tgrid, 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax, O, ws);
+      if (two) {  // two-layer markers: one CTA per tile whatever the crowding
+        if (w->deposit_threads == 128) mc::k_deposit_tile<true, true><<<tgrid, 128, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax, O, ws);
+        else mc::k_deposit_tile<false, true><<<tgrid, 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max, tile_fmax, O, ws);
+      }
       else if (split) {
         // crowded tiles: clusters on the side stream; all other tiles: the light one-CTA kernel beside them
         fork_side();
@@ -594,12 +596,12 @@ int enqueue_step(mc_world* w) {
       const int pgrid = (w->n_windows * 32 + 63) / 64;
       if (w->uniform_params) mc::k_filament_pbd<true><<<dim3(pgrid, nb), 64, 0, st>>>(pa, ws);
       else mc::k_filament_pbd<false><<<dim3(pgrid, nb), 64, 0, st>>>(pa, ws);
-      mc::k_add_displacement<<<dim3((N + 255) / 256, nb), 256, 0, st>>>(N, X, pa.Dp, flag, &ls_state->step_max_p, ws);
+      mc::k_add_displacement<<<dim3((N + 1023) / 1024, nb), 1024, 0, st>>>(N, X, pa.Dp, flag, &ls_state->step_max_p, ws);
       w->launches += 2;
     }
     if (two) {
       // the markers follow the new positions (reading 28)
-      mc::k_markers<<<dim3((N + 255) / 256, nb), 256, 0, st>>>(N, X, w->ptr<float4>(w->L.PC), w->layer_h,
+      mc::k_markers<<<dim3((N + 1023) / 1024, nb), 1024, 0, st>>>(N, X, w->ptr<unsigned char>(w->L.bflags), w->layer_h,
                                                                 w->ptr<float2>(w->L.O), &ls_state->step_max_m, ws);
       w->launches++;
     }
@@ -892,7 +894,7 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
     if (w->p.two_layer) {
       // markers of the loaded positions (reading 28); the offsets start from zero
       cs.ok(cudaMemsetAsync(w->ptr<float2>(w->L.O), 0, (size_t)N * 8, st), "cudaMemsetAsync");
-      mc::k_markers<<<(int)((N + 255) / 256), 256, 0, st>>>((int)N, w->ptr<float2>(w->L.X), w->ptr<float4>(w->L.PC),
+      mc::k_markers<<<(int)((N + 1023) / 1024), 1024, 0, st>>>((int)N, w->ptr<float2>(w->L.X), w->ptr<unsigned char>(w->L.bflags),
                                                             w->layer_h, w->ptr<float2>(w->L.O), &ls_state->step_max_m, 0);
       cs.launched("k_markers");
       w->launches++;
@@ -925,7 +927,8 @@ int mc_load_filaments(mc_world* w, int32_t n_fil, const int32_t* offsets, const 
   w->N = (int)N;
   w->n_fil = n_fil;
   w->has_L_act = false;  // a load resets the rest-length actuation (mc_set_length_actuation)
-  w->deposit_threads = h_maxlist > 1024 ? 256 : 128;
+  // (two-layer lists hold two markers per bead: twice as long for the same crowding)
+  w->deposit_threads = h_maxlist > (w->p.two_layer ? 4096 : 1024) ? 256 : 128;
   // crowded tiles (config 5 lists ~16,000 beads in its central tiles): a cluster of CTAs per tile
   // (measured on config 5: one CTA per tile 0.351 ms/step, clusters of 2: 0.263, 4: 0.250, 8: 0.325)
   w->cluster_auto = h_maxlist > 4096 ? 4 : 0;
@@ -962,7 +965,7 @@ int mc_set_positions(mc_world* w, const float* xy) {
   mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(w->ptr<int>(w->L.flags) + 16);
   cudaMemcpyAsync(ls_state, &force, sizeof(force), cudaMemcpyHostToDevice, st);
   if (w->p.two_layer) {
-    mc::k_markers<<<(w->N + 255) / 256, 256, 0, st>>>(w->N, w->ptr<float2>(w->L.X), w->ptr<float4>(w->L.PC), w->layer_h,
+    mc::k_markers<<<(w->N + 1023) / 1024, 1024, 0, st>>>(w->N, w->ptr<float2>(w->L.X), w->ptr<unsigned char>(w->L.bflags), w->layer_h,
                                                       w->ptr<float2>(w->L.O), &ls_state->step_max_m, 0);
     w->launches++;
   }
@@ -1318,7 +1321,7 @@ int mc_set_positions_batch(mc_batch* b, const float* xy) {
   lead->launches += 2;
   if (lead->p.two_layer) {
     mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(lead->ptr<int>(lead->L.flags) + 16);
-    mc::k_markers<<<dim3((lead->N + 255) / 256, nb), 256, 0, st>>>(lead->N, lead->ptr<float2>(lead->L.X), lead->ptr<float4>(lead->L.PC),
+    mc::k_markers<<<dim3((lead->N + 1023) / 1024, nb), 1024, 0, st>>>(lead->N, lead->ptr<float2>(lead->L.X), lead->ptr<unsigned char>(lead->L.bflags),
                                                                    lead->layer_h, lead->ptr<float2>(lead->L.O),
                                                                    &ls_state->step_max_m, b->stride);
     lead->launches++;

@@ -247,7 +247,8 @@ __device__ __forceinline__ float2 interp2_pair(const float2* __restrict__ p, int
   return make_float2(ax, ay);
 }
 
-// interp2 at the marker (x + ox, y + oy) (two-layer broadcast; plain loads)
+// interp2 at the marker (x + ox, y + oy) (two-layer broadcast): 16-byte pair loads like interp2_pair,
+// the support formed by support_off.
 __device__ __forceinline__ float2 interp2_off(const float2* __restrict__ p, int nx, int ny, float x, float y, float ox,
                                               float oy) {
   int i0, j0;
@@ -258,18 +259,31 @@ __device__ __forceinline__ float2 interp2_off(const float2* __restrict__ p, int 
   peskin4(fy, wy[0], wy[1], wy[2], wy[3]);
   i0 = wrapi(i0, nx);
   j0 = wrapi(j0, ny);
+  const bool odd = (i0 & 1) != 0;
+  const int e = i0 & ~1;
+  int pc[3];
+#pragma unroll
+  for (int q = 0; q < 3; ++q) {
+    const int c = (e + 2 * q >= nx) ? e + 2 * q - nx : e + 2 * q;
+    pc[q] = ((c >> 2) << 4) + (c & 3);
+  }
+  const float w0 = odd ? 0.0f : wx[0], w1 = odd ? wx[0] : wx[1], w2 = odd ? wx[1] : wx[2], w3 = odd ? wx[2] : wx[3],
+              w4 = odd ? wx[3] : 0.0f;
+  const int nbx = nx >> 2;
   float ax = 0.0f, ay = 0.0f;
 #pragma unroll
   for (int l = 0; l < 4; ++l) {
     const int row = (j0 + l >= ny) ? j0 + l - ny : j0 + l;
-    float sx = 0.0f, sy = 0.0f;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const int c = (i0 + k >= nx) ? i0 + k - nx : i0 + k;
-      const float2 v = __ldg(p + blk_index(c, row, nx));
-      sx = fmaf(v.x, wx[k], sx);
-      sy = fmaf(v.y, wx[k], sy);
-    }
+    const char* r = reinterpret_cast<const char*>(p + ((size_t)(row >> 2) * nbx * 16 + ((row & 3) << 2)));
+    const float4 v0 = __ldg(reinterpret_cast<const float4*>(r + (unsigned long long)(unsigned)pc[0] * 8u));
+    const float4 v1 = __ldg(reinterpret_cast<const float4*>(r + (unsigned long long)(unsigned)pc[1] * 8u));
+    float4 v2 = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (odd) v2 = __ldg(reinterpret_cast<const float4*>(r + (unsigned long long)(unsigned)pc[2] * 8u));
+    float sx = v0.x * w0, sy = v0.y * w0;
+    sx = fmaf(v0.z, w1, sx); sy = fmaf(v0.w, w1, sy);
+    sx = fmaf(v1.x, w2, sx); sy = fmaf(v1.y, w2, sy);
+    sx = fmaf(v1.z, w3, sx); sy = fmaf(v1.w, w3, sy);
+    sx = fmaf(v2.x, w4, sx); sy = fmaf(v2.y, w4, sy);
     ax = fmaf(sx, wy[l], ax);
     ay = fmaf(sy, wy[l], ay);
   }

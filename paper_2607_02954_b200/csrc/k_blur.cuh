@@ -56,17 +56,57 @@ template <int R>
 __global__ void __launch_bounds__(BLUR_THREADS, R > 6 ? 1 : 7) k_blur_grad(int nx, int ny, BlurTaps taps,
                                                             const float* __restrict__ rho_b, float coef,
                                                             const float2* base, float2* A,
-                                                            float* __restrict__ field_out, size_t wstride) {
+                                                            float* __restrict__ field_out, size_t wstride,
+                                                            const float* __restrict__ tile_rho_max = nullptr) {
   if (wstride) {  // batched worlds (single worlds pass 0); field_out is a caller array of ONE world
     rho_b = wshift(rho_b, blockIdx.y * wstride);
     base = wshift(base, blockIdx.y * wstride);
     A = wshift(A, blockIdx.y * wstride);
+    tile_rho_max = wshift(tile_rho_max, blockIdx.y * wstride);
   }
   constexpr int NV = blur_NV(R), CW = blur_CW(R), CP = blur_CP(R);
   __shared__ __align__(16) float2 td[BLUR_T * CP];
   // 1-D grid in row-major tile order (2-D grids are rasterised in an order that streams worse)
   const int ntx = nx / BLUR_T;
   const int i0 = (blockIdx.x % ntx) * BLUR_T, j0 = (blockIdx.x / ntx) * BLUR_T;
+  if (tile_rho_max) {
+    // Crowded worlds (config 5: ~90 % of the tiles hold no bead): the window of this tile reaches
+    // R + 1 <= 17 nodes into its 8 neighbours; if S2 left rho_b = 0 on all nine tiles (their maxima,
+    // written by K2a of this step) the filtered field and its gradient vanish here: the tile only
+    // writes the base field (or zeros) and skips the loads and the arithmetic.  Exact, not approximate.
+    static_assert(BLUR_T == 32, "tile_rho_max is per 32 x 32 tile");
+    const int nty = ny / BLUR_T, tx = blockIdx.x % ntx, ty = blockIdx.x / ntx;
+    bool any = false;
+#pragma unroll
+    for (int d = 0; d < 9; ++d)
+      any = any || tile_rho_max[wrap1(ty + d / 3 - 1, nty) * ntx + wrap1(tx + d % 3 - 1, ntx)] != 0.0f;
+    if (!any) {
+      if (threadIdx.x < BLUR_T * 4) {
+        const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+        const int c = (lane & 1) + 2 * ((lane >> 3) & 1);
+        const int row = ((lane >> 1) & 3) + 4 * (lane >> 4) + 8 * wid;
+        const size_t bidx = blk_index(i0 + 8 * c, j0 + row, nx);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          float4* dst = reinterpret_cast<float4*>(A + bidx + 16 * h);
+          float4 lo = make_float4(0.f, 0.f, 0.f, 0.f), hi = lo;
+          if (base) {
+            const float4* src = reinterpret_cast<const float4*>(base + bidx + 16 * h);
+            lo = src[0];
+            hi = src[1];
+          }
+          __stcs(dst, lo);
+          __stcs(dst + 1, hi);
+        }
+        if (field_out) {
+          float4* f = reinterpret_cast<float4*>(field_out + (size_t)(j0 + row) * nx + i0 + 8 * c);
+          f[0] = make_float4(0.f, 0.f, 0.f, 0.f);
+          f[1] = f[0];
+        }
+      }
+      return;
+    }
+  }
   // y pass: items (chunk c of 8 rows, PAIR of columns col, col + 1 <-> nodes i0 - (R+1) + col ...):
   // 8-byte loads, both columns ride in packed FFMA2 pairs
   // (for even R the window starts at an odd node: the pairs then start one column further left)

@@ -262,7 +262,10 @@ void launch_blur_R(mc_world* w, int k, const float2* base, float2* A, float* fie
   // the step filters every world of a batch; a read-out (field_out given) only this world
   const unsigned nb = field_out ? 1u : (unsigned)w->batch_n;
   mc::k_blur_grad<R><<<dim3(grid, nb), mc::BLUR_THREADS, 0, w->stream>>>(
-      w->nx, w->ny, w->taps[k], w->ptr<float>(w->L.rho_b), w->coef[k], base, A, field_out, w->batch_stride);
+      w->nx, w->ny, w->taps[k], w->ptr<float>(w->L.rho_b), w->coef[k], base, A, field_out, w->batch_stride,
+      // crowded worlds skip the tiles whose 3 x 3 neighbourhood holds no bead (exact); only inside a step:
+      // at read-out time the fused kernel has already reset the per-tile maxima
+      (w->cluster > 0 && !field_out && R <= 31) ? w->ptr<float>(w->L.tile_rho_max) : nullptr);
 }
 
 // K3a for bead-density field k; first: start from the static part, else add to the planes in A

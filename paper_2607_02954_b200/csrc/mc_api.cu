@@ -54,6 +54,8 @@ bool validate(const mc_world_params* p, Derived* d, std::string* why) {
   if (p->pbd_order != MC_PBD_JACOBI && p->pbd_order != MC_PBD_GAUSS_SEIDEL) { *why = "unknown pbd_order"; return false; }
   if ((p->pbd_project != 0 && p->pbd_project != 1) || (p->two_layer != 0 && p->two_layer != 1)) { *why = "pbd_project and two_layer must be 0 or 1"; return false; }
   if (!(p->layer_offset >= 0.0f) || p->layer_offset > 1.0f) { *why = "layer_offset must lie in [0, 1]"; return false; }
+  // two layers list 2 N markers: the 32-bit list offsets then hold up to 8 N
+  if (p->two_layer && p->max_beads > ((int64_t)1 << 28) - 1) { *why = "max_beads out of range for two_layer (0 .. 2^28 - 1)"; return false; }
   if (p->n_fields < 0 || p->n_fields > 4) { *why = "n_fields must be 0..4"; return false; }
   // the tile lists hold up to 4 N entries addressed with 32-bit ints (k_tile.cuh)
   if (p->max_beads < 0 || p->max_beads > ((int64_t)1 << 29) - 1) { *why = "max_beads out of range (0 .. 2^29 - 1)"; return false; }
@@ -1211,6 +1213,7 @@ int mc_read_intermediates(mc_world* w, float* rho_b, float* G) {
 struct mc_batch {
   std::vector<mc_world*> worlds;
   size_t stride = 0;
+  bool consistent = true;  // false after a batch load that failed part-way: the worlds differ until the next good load
   std::string err;
 };
 
@@ -1281,6 +1284,7 @@ int mc_load_filaments_batch(mc_batch* b, int32_t n_fil, const int32_t* offsets, 
   BatchScope scope;
   mc_world* lead = b->worlds[0];
   lead->batch_n = 1;  // member calls below act on one world each
+  b->consistent = false;
   bool uniform_all = true, any_L = false;
   int dep = 128, cl = 0;
   for (size_t k = 0; k < b->worlds.size(); ++k) {
@@ -1306,6 +1310,7 @@ int mc_load_filaments_batch(mc_batch* b, int32_t n_fil, const int32_t* offsets, 
   }
   if (lead->cluster > 0 && lead->split_on) ensure_side_stream(lead);
   drop_graphs(lead);
+  b->consistent = true;
   return MC_OK;
 }
 
@@ -1365,6 +1370,7 @@ int mc_read_positions_batch(mc_batch* b, int64_t* step_out, float* xy) {
 int mc_step_batch(mc_batch* b, int32_t n) {
   if (!b) return MC_EINVAL;
   if (n < 0) return bfail(b, MC_EINVAL, "n < 0");
+  if (!b->consistent) return bfail(b, MC_ESTATE, "the last mc_load_filaments_batch failed part-way: load the batch again");
   BatchScope scope;
   mc_world* lead = b->worlds[0];
   for (mc_world* w : b->worlds)

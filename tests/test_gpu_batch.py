@@ -102,6 +102,20 @@ def test_batch_members_cannot_be_stepped_alone_and_loads_are_checked():
     with pytest.raises(binding.McError) as e:
         binding.Batch(bad)
     assert e.value.code == binding.MC_EINVAL and "world 1" in str(e.value)
+    # a load that fails part-way leaves the batch unusable until a good one
+    import ctypes as C
+    import torch
+    B2 = binding.Batch(ws)
+    dev = []
+    for k in binding._CHAIN_KEYS:
+        a = np.stack([np.ascontiguousarray(w[k], dtype=np.float32) for w in bad])
+        dev.append(torch.from_numpy(a).cuda())
+    off = np.ascontiguousarray(ws[0]["offsets"], dtype=np.int32)
+    rc = lib.mc_load_filaments_batch(B2.h, len(off) - 1, off.ctypes.data_as(C.POINTER(C.c_int32)),
+                                     *[C.c_void_p(t.data_ptr()) for t in dev], None)
+    assert rc == binding.MC_EINVAL
+    assert lib.mc_step_batch(B2.h, 1) == binding.MC_ESTATE
+    B2.close()
     other = worlds.random_world(64, 64, 4, 32, seed=9)          # different chain structure
     with pytest.raises(ValueError):
         binding.Batch([ws[0], other])

@@ -283,6 +283,31 @@ mc_world* mc_batch_world(mc_batch* b, int32_t k);
 void mc_destroy_batch(mc_batch* b);
 const char* mc_batch_last_error(const mc_batch* b);
 
+/* ---- one entry point that allocates nothing ------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it) and therefore cannot provide a workspace: S2 on its own,
+ *   rho_b(g) = sum_i delta_h(g - X_i)      ("node positions are deposited onto a grid"; readings 7, 13)
+ * with the step's own kernels (tile lists + fixed-point shared-memory accumulation), their scratch
+ * in a file-scope static device array of the library (803,328 bytes, held by every GPU that loads
+ * libmc.so until the process exits).  Limits: n_beads <= MC_NOALLOC_MAX_BEADS and
+ * (nx/32)*(ny/32) <= MC_NOALLOC_MAX_TILES (e.g. 1024 x 1024 nodes); larger sizes return MC_EINVAL with
+ * a message that names the limit.  The call makes no cudaMalloc / cudaFree and calls no allocating
+ * routine; it enqueues three kernels on cuda_stream (NULL = legacy default stream) and returns
+ * without synchronising.
+ *   xy    DEVICE float [n_beads][2], unwrapped positions, 8-byte aligned (may be NULL if n_beads = 0)
+ *   rho_b DEVICE float [ny][nx] out, 16-byte aligned
+ * The result equals what a world's S2 computes from the same positions (mc_read_intermediates), bit
+ * for bit when that world's tile lists are fresh, else to fixed-point rounding (~1e-7).
+ * All calls on a device share the one scratch array, which keeps the previous call's contents (every
+ * call clears what must start at zero): calls that OVERLAP on the GPU -- different streams, or
+ * host threads without ordering -- race on it; serialise them on one stream or with events.
+ * Errors: MC_EINVAL, MC_ECUDA; message from mc_noalloc_last_error (per host thread). */
+#define MC_NOALLOC_MAX_BEADS 32768
+#define MC_NOALLOC_MAX_TILES 1024
+int mc_deposit_noalloc(int32_t nx, int32_t ny, int32_t n_beads, const float* xy /*DEVICE*/,
+                       float* rho_b /*DEVICE*/, void* cuda_stream);
+const char* mc_noalloc_last_error(void);
+
 /* Frees the host handle only (the workspace belongs to the caller).  NULL is allowed. */
 void mc_destroy(mc_world* w);
 

@@ -20,7 +20,9 @@ SYMBOLS = ("mc_workspace_bytes", "mc_create", "mc_load_filaments", "mc_step", "m
            "mc_profile_enable", "mc_profile_read", "mc_keep_intermediates", "mc_texture_gathers",
            "mc_cluster_tiles", "mc_set_positions", "mc_set_length_actuation", "mc_load_fluid", "mc_batch_workspace_bytes",
            "mc_create_batch", "mc_load_filaments_batch", "mc_step_batch", "mc_batch_world", "mc_destroy_batch",
-           "mc_batch_last_error", "mc_set_positions_batch", "mc_read_positions_batch")
+           "mc_batch_last_error", "mc_set_positions_batch", "mc_read_positions_batch", "mc_deposit_noalloc",
+           "mc_noalloc_last_error")
+NOALLOC_MAX_BEADS, NOALLOC_MAX_TILES = 32768, 1024
 PROF_SLOTS = ("K0_bin", "K2a_deposit", "K3a_blur_grad", "K1_filament", "K2b_spread", "K3b_lbm",
               "K4_interp_integrate")
 
@@ -103,6 +105,10 @@ def load_library():
     L.mc_set_positions_batch.argtypes = [vp, vp]
     L.mc_read_positions_batch.restype = C.c_int
     L.mc_read_positions_batch.argtypes = [vp, C.POINTER(i64), vp]
+    L.mc_deposit_noalloc.restype = C.c_int
+    L.mc_deposit_noalloc.argtypes = [i32, i32, i32, vp, vp, vp]
+    L.mc_noalloc_last_error.restype = C.c_char_p
+    L.mc_noalloc_last_error.argtypes = []
     L.mc_batch_world.restype = vp
     L.mc_batch_world.argtypes = [vp, i32]
     L.mc_destroy_batch.restype = None
@@ -330,6 +336,23 @@ class World:
             self.close()
         except Exception:
             pass
+
+
+def deposit_noalloc(nx: int, ny: int, xy, out, stream=None):
+    """mc_deposit_noalloc: rho_b = sum_i delta_h(g - X_i) into `out` (device float tensor [ny, nx]) from `xy`
+    (device float tensor [N, 2]); the library's static scratch, no allocation.  Marshalling only: both
+    tensors are the caller's.  Asynchronous on `stream` (a torch stream; default: the current one)."""
+    import torch
+    assert xy.is_cuda and out.is_cuda and xy.dtype == torch.float32 and out.dtype == torch.float32
+    assert xy.is_contiguous() and out.is_contiguous() and out.numel() == nx * ny
+    st = stream if stream is not None else torch.cuda.current_stream(xy.device)
+    with torch.cuda.device(xy.device):
+        rc = load_library().mc_deposit_noalloc(int(nx), int(ny), int(xy.shape[0]),
+                                               C.c_void_p(xy.data_ptr()) if xy.numel() else None,
+                                               C.c_void_p(out.data_ptr()), C.c_void_p(st.cuda_stream))
+    if rc != MC_OK:
+        raise McError(rc, load_library().mc_noalloc_last_error().decode())
+    return out
 
 
 class Batch:

@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <algorithm>
@@ -1384,6 +1385,129 @@ int mc_step_batch(mc_batch* b, int32_t n) {
     w->cur = lead->cur;
   }
   if (rc != MC_OK) return bfail(b, rc, lead->err);
+  return MC_OK;
+}
+
+#pragma GCC visibility pop
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// mc_deposit_noalloc: S2 (rho_b = sum_i delta_h(g - X_i)) for callers that cannot allocate --
+// code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Everything
+// else in this library works inside a caller-provided workspace; this ONE entry point needs none:
+// the scratch of the tile binning (counters, offsets, bucket cursors, the lists) and of the deposit
+// (per-tile maxima) lives in the file-scope device array below, of a fixed modest size that every GPU
+// which loads the library holds until the process exits.  The kernels are the ones of the step
+// (k_list_build_small, k_deposit_tile): same arithmetic, same fixed-point accumulation.
+//
+// In HOST code the array's name is a host-side stand-in, not a device address: its device address is
+// resolved once per device with cudaGetSymbolAddress (below) and passed to the kernels.
+// All calls share the array and it keeps the last call's contents: every call first clears what must
+// start at zero (k_noalloc_init).  Calls that overlap on the GPU (two streams, two host threads) RACE
+// on it: serialise them on one stream or with events.
+namespace {
+
+constexpr int NA_MAX_BEADS = MC_NOALLOC_MAX_BEADS, NA_MAX_TILES = MC_NOALLOC_MAX_TILES;
+static_assert(NA_MAX_BEADS <= K0_SMALL_BEADS && NA_MAX_TILES <= K0_SMALL_TILES, "the one-CTA list build serves these sizes");
+// layout of the scratch, in 4-byte words
+constexpr size_t NA_STATE = 0;                                   // ListState (5 words), padded to 64
+constexpr size_t NA_TILE_COUNT = 64;                             // [NA_MAX_TILES]
+constexpr size_t NA_TILE_START = NA_TILE_COUNT + NA_MAX_TILES;   // [NA_MAX_TILES + 1], padded to + 64
+constexpr size_t NA_BUCKET_COUNT = NA_TILE_START + NA_MAX_TILES + 64;   // [32 NA_MAX_TILES]
+constexpr size_t NA_BUCKET_CURSOR = NA_BUCKET_COUNT + 32 * (size_t)NA_MAX_TILES;
+constexpr size_t NA_RHO_MAX = NA_BUCKET_CURSOR + 32 * (size_t)NA_MAX_TILES;   // [NA_MAX_TILES] float
+constexpr size_t NA_FMAX = NA_RHO_MAX + NA_MAX_TILES;            // [NA_MAX_TILES] unsigned
+constexpr size_t NA_LIST = NA_FMAX + NA_MAX_TILES;               // [4 NA_MAX_BEADS]: a bead is listed in at most 4 tiles
+constexpr size_t NA_WORDS = NA_LIST + 4 * (size_t)NA_MAX_BEADS;  // 200,832 words = 803,328 bytes
+
+static __device__ __align__(256) int g_noalloc_scratch[NA_WORDS];
+
+// clear what must start at zero and order a list build (drift = +inf => need = 1)
+__global__ void k_noalloc_init(int* __restrict__ scratch, int n_tiles) {
+  mc::ListState* st = reinterpret_cast<mc::ListState*>(scratch + NA_STATE);
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    st->need = 1;
+    st->drift = __int_as_float(0x7f800000);
+    st->step_max = st->step_max_p = st->step_max_m = 0u;
+  }
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < 32 * n_tiles; i += gridDim.x * blockDim.x) {
+    scratch[NA_BUCKET_COUNT + i] = 0;
+    if (i < n_tiles) {
+      scratch[NA_TILE_COUNT + i] = 0;
+      scratch[NA_RHO_MAX + i] = 0;   // bits of 0.0f
+      scratch[NA_FMAX + i] = 0;
+    }
+  }
+}
+
+thread_local std::string g_noalloc_error;
+constexpr int NA_MAX_DEVICES = 64;
+int* g_noalloc_ptr[NA_MAX_DEVICES] = {};   // device address of the scratch, per device (0: not resolved yet)
+std::mutex g_noalloc_mutex;
+
+int na_fail(int code, const std::string& msg) {
+  g_noalloc_error = msg;
+  return code;
+}
+
+}  // namespace
+
+extern "C" {
+#pragma GCC visibility push(default)
+
+const char* mc_noalloc_last_error(void) { return g_noalloc_error.c_str(); }
+
+int mc_deposit_noalloc(int32_t nx, int32_t ny, int32_t n_beads, const float* xy, float* rho_b, void* cuda_stream) {
+  g_noalloc_error.clear();
+  if (nx < 32 || ny < 32 || nx % 32 || ny % 32) return na_fail(MC_EINVAL, "nx, ny must be multiples of 32, >= 32");
+  const long long n_tiles_ll = (long long)(nx / mc::TS) * (ny / mc::TS);
+  if (n_tiles_ll > NA_MAX_TILES)
+    return na_fail(MC_EINVAL, "grid too large for mc_deposit_noalloc: " + std::to_string(n_tiles_ll) + " tiles of 32 x 32 nodes, the static scratch holds " +
+                                  std::to_string(NA_MAX_TILES) + " (MC_NOALLOC_MAX_TILES)");
+  if (n_beads < 0) return na_fail(MC_EINVAL, "n_beads < 0");
+  if (n_beads > NA_MAX_BEADS)
+    return na_fail(MC_EINVAL, "too many beads for mc_deposit_noalloc: " + std::to_string(n_beads) + ", the static scratch holds " +
+                                  std::to_string(NA_MAX_BEADS) + " (MC_NOALLOC_MAX_BEADS)");
+  if (!rho_b || (n_beads > 0 && !xy)) return na_fail(MC_EINVAL, "null array");
+  if (((uintptr_t)xy % 8) != 0 || ((uintptr_t)rho_b % 16) != 0) return na_fail(MC_EINVAL, "xy must be 8-byte and rho_b 16-byte aligned");
+  const int n_tiles = (int)n_tiles_ll;
+  // set-up, once per device, with that device current: the device address of the scratch
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return na_fail(MC_ECUDA, std::string("cudaGetDevice: ") + cudaGetErrorString(e));
+  if (dev < 0 || dev >= NA_MAX_DEVICES) return na_fail(MC_EINVAL, "device index out of range");
+  int* scratch = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+      void* ptr = nullptr;
+      e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+      if (e != cudaSuccess || !ptr) {
+        cudaGetLastError();
+        return na_fail(MC_ECUDA, std::string("cudaGetSymbolAddress(g_noalloc_scratch): ") + cudaGetErrorString(e));
+      }
+      g_noalloc_ptr[dev] = static_cast<int*>(ptr);
+    }
+    scratch = g_noalloc_ptr[dev];
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  mc::ListState* ls_state = reinterpret_cast<mc::ListState*>(scratch + NA_STATE);
+  int* tile_count = scratch + NA_TILE_COUNT;
+  int* tile_start = scratch + NA_TILE_START;
+  int* bucket_count = scratch + NA_BUCKET_COUNT;
+  int* bucket_cursor = scratch + NA_BUCKET_CURSOR;
+  float* tile_rho_max = reinterpret_cast<float*>(scratch + NA_RHO_MAX);
+  unsigned* tile_fmax = reinterpret_cast<unsigned*>(scratch + NA_FMAX);
+  int* list = scratch + NA_LIST;
+  const float2* X = reinterpret_cast<const float2*>(xy);
+  k_noalloc_init<<<32, 256, 0, st>>>(scratch, n_tiles);
+  mc::k_list_build_small<<<dim3(1, 1), 1024, 0, st>>>(ls_state, X, nullptr, n_beads, nx, ny, n_tiles, tile_count, tile_start,
+                                                       bucket_count, bucket_cursor, list,
+                                                       mc::CrowdedTable{nullptr, nullptr, nullptr}, 0);
+  mc::k_deposit_tile<false><<<dim3(nx / mc::TS, ny / mc::TS, 1), 256, 0, st>>>(nx, ny, tile_start, list, X, rho_b, tile_rho_max,
+                                                                                tile_fmax, nullptr, 0);
+  e = cudaPeekAtLastError();
+  if (e != cudaSuccess) return na_fail(MC_ECUDA, std::string("mc_deposit_noalloc: kernel launch: ") + cudaGetErrorString(e));
   return MC_OK;
 }
 

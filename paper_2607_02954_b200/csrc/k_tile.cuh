@@ -389,6 +389,42 @@ __global__ void __cluster_dims__(K0_CLUSTER, 1, 1) __launch_bounds__(1024)
   tile_bin<true>(X, O, N, nx, ny, nullptr, bucket_cursor, list);
 }
 
+// Large single worlds: the whole of K0 in ONE cooperative launch (grid barrier between the phases; all
+// CTAs co-resident by construction of a cooperative launch) instead of four launches, three of which
+// only return on the ~10 of 11 steps that keep their lists: on worlds of a million beads the launch
+// boundaries of those empty kernels are 5 % of the step.  Nobody writes the list state while the grid
+// decides (every thread derives the same decision from it); the LAST CTA to leave commits the policy
+// (an exit counter, reset by that CTA).  grid = resident CTAs of 1024 threads (host: occupancy query).
+__global__ void __launch_bounds__(1024) k_list_build_coop(ListState* __restrict__ st, int* __restrict__ exit_ctr,
+                                                          const float2* __restrict__ X, const float2* __restrict__ O,
+                                                          int N, int nx, int ny, int n_tiles, int* __restrict__ tile_count,
+                                                          int* __restrict__ tile_start, int* __restrict__ bucket_count,
+                                                          int* __restrict__ bucket_cursor, int* __restrict__ list,
+                                                          CrowdedTable ct) {
+  namespace cg = cooperative_groups;
+  __shared__ int sm[33];
+  float d;
+  const bool due = list_rebuild_due(st, &d);  // the same in every thread of the grid
+  if (due) {
+    cg::grid_group grid = cg::this_grid();
+    tile_bin<false>(X, O, N, nx, ny, tile_count, bucket_count, nullptr);
+    grid.sync();
+    if (blockIdx.x == 0) tile_scan(tile_count, n_tiles, tile_start, sm, ct);
+    grid.sync();
+    bucket_starts(n_tiles, tile_start, bucket_count, bucket_cursor);
+    grid.sync();
+    tile_bin<true>(X, O, N, nx, ny, nullptr, bucket_cursor, list);
+  }
+  __syncthreads();  // every thread of this CTA has read the state
+  if (threadIdx.x == 0) {
+    __threadfence();
+    if (atomicAdd(exit_ctr, 1) == (int)gridDim.x - 1) {
+      *exit_ctr = 0;
+      list_policy_commit(st);  // need, drift, step maxima for this step's K4
+    }
+  }
+}
+
 // mc_load_filaments: largest tile list (chooses the CTA size of the P2G kernels)
 __global__ void k_max_int(const int* __restrict__ v, int n, int* __restrict__ out) {
   int m = 0;

@@ -157,6 +157,7 @@ struct mc_world {
   int batch_n = 1;
   size_t batch_stride = 0;
   bool batch_member = false;  // owned by an mc_batch: stepped and reloaded only through it
+  int coop_grid = 0;  // CTAs of the one-launch cooperative K0 of large single worlds (0: device cannot, four launches)
   // crowded worlds: the cluster launch over the crowded tiles runs on a second stream beside the
   // one-CTA-per-tile launch over the rest (fork / join by events; also under graph capture)
   bool split_on = true;   // mc_cluster_tiles(w, c | MC_CLUSTER_ALL_TILES): every tile gets a cluster (round-1 scheme; tests)
@@ -333,6 +334,18 @@ int enqueue_step(mc_world* w) {
     } else if (n_items <= K0_MEDIUM_BEADS && n_tiles <= K0_MEDIUM_TILES) {
       mc::k_list_build_cluster<<<dim3(mc::K0_CLUSTER, nb), 1024, 0, st>>>(ls_state, X, O, N, nx, ny, n_tiles, tile_count,
                                                                           tile_start, bucket_count, bucket_cursor, list, ctab, ws);
+      w->launches += 1;
+    } else if (nb == 1 && w->coop_grid > 0) {
+      // large single world: one cooperative launch (k_tile.cuh k_list_build_coop)
+      int* exit_ctr = w->ptr<int>(w->L.flags) + 7;
+      const float2* Xc = X;
+      int Nc = N, nxc = nx, nyc = ny, ntc = n_tiles;
+      mc::CrowdedTable ctc = ctab;
+      void* args[] = {&ls_state, &exit_ctr, &Xc, (void*)&O, &Nc, &nxc, &nyc, &ntc, &tile_count, &tile_start,
+                      &bucket_count, &bucket_cursor, &list, &ctc};
+      const int cgrid = std::min(w->coop_grid, (n_items + 1023) / 1024);
+      if (cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(&mc::k_list_build_coop), dim3(cgrid), dim3(1024), args, 0, st) != cudaSuccess)
+        return fail(w, MC_ECUDA, std::string("mc_step: cooperative launch of K0: ") + cudaGetErrorString(cudaGetLastError()));
       w->launches += 1;
     } else {
       const int k0grid = bgrid < w->n_sm * 8 ? bgrid : w->n_sm * 8;
@@ -727,6 +740,15 @@ int mc_create(const mc_world_params* p, void* workspace, size_t workspace_bytes,
     if (cudaGetDevice(&dev) == cudaSuccess &&
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
       w->n_sm = sms;
+  }
+  {
+    // one-launch K0 for large worlds: a cooperative grid of resident 1024-thread CTAs
+    int dev = 0, coop = 0, occ = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop &&
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mc::k_list_build_coop, 1024, 0) == cudaSuccess && occ > 0)
+      w->coop_grid = w->n_sm * occ;
+    else
+      cudaGetLastError();
   }
   // lattice constants (reading 10, 12): nu_lat = nu dt; tau+ = 3 nu_lat + 1/2; tau- = Lambda/(tau+ - 1/2) + 1/2
   const double dt = (double)p->dt, nu_lat = (double)p->nu * dt;

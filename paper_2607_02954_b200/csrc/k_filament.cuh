@@ -226,12 +226,12 @@ __global__ void __launch_bounds__(256, 5) k_filament_force(FilamentArgs a, size_
   if (a.A) {
     if (oA) {
       const float2 g = TEXROWS ? interp2_tex<TEXROWS, true>(a.A, a.tex_A, a.nx, a.ny, xa.x, xa.y)
-                               : interp2(a.A, a.nx, a.ny, xa.x, xa.y);
+                               : interp2_pair<0>(a.A, a.nx, a.ny, xa.x, xa.y);
       FA.x += g.x; FA.y += g.y;
     }
     if (oB) {
       const float2 g = TEXROWS ? interp2_tex<TEXROWS, true>(a.A, a.tex_A, a.nx, a.ny, xb.x, xb.y)
-                               : interp2(a.A, a.nx, a.ny, xb.x, xb.y);
+                               : interp2_pair<0>(a.A, a.nx, a.ny, xb.x, xb.y);
       FB.x += g.x; FB.y += g.y;
     }
   }

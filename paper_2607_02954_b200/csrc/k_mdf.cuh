@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(256) k_mdf_force(int N, const float2* __restri
       const float2 up = interp2_off(u, nx, ny, p.x, p.y, o.x, o.y), um = interp2_off(u, nx, ny, p.x, p.y, -o.x, -o.y);
       U = make_float2(0.5f * (up.x + um.x), 0.5f * (up.y + um.y));
     } else {
-      U = TEXROWS ? interp2_tex<TEXROWS, false>(u, tex_u, nx, ny, p.x, p.y) : interp2(u, nx, ny, p.x, p.y);
+      U = TEXROWS ? interp2_tex<TEXROWS, false>(u, tex_u, nx, ny, p.x, p.y) : interp2_pair<0>(u, nx, ny, p.x, p.y);
     }
     const float2 v = V[b];
     const float2 d = make_float2(rho0 * (v.x - U.x), rho0 * (v.y - U.y));

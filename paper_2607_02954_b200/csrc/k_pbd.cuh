@@ -222,7 +222,7 @@ __global__ void __launch_bounds__(128) k_filament_pbd(PbdArgs g, size_t wstride)
         const float2 gm = interp2_off(a.A, a.nx, a.ny, xa.x, xa.y, -oa.x, -oa.y);
         FA.x += 0.5f * (gp.x + gm.x); FA.y += 0.5f * (gp.y + gm.y);
       } else {
-        const float2 gq = interp2(a.A, a.nx, a.ny, xa.x, xa.y);
+        const float2 gq = interp2_pair<0>(a.A, a.nx, a.ny, xa.x, xa.y);
         FA.x += gq.x; FA.y += gq.y;
       }
     }
@@ -232,7 +232,7 @@ __global__ void __launch_bounds__(128) k_filament_pbd(PbdArgs g, size_t wstride)
         const float2 gm = interp2_off(a.A, a.nx, a.ny, xb.x, xb.y, -ob.x, -ob.y);
         FB.x += 0.5f * (gp.x + gm.x); FB.y += 0.5f * (gp.y + gm.y);
       } else {
-        const float2 gq = interp2(a.A, a.nx, a.ny, xb.x, xb.y);
+        const float2 gq = interp2_pair<0>(a.A, a.nx, a.ny, xb.x, xb.y);
         FB.x += gq.x; FB.y += gq.y;
       }
     }

@@ -167,7 +167,12 @@ def ncu_traffic(slot: str, workload: str, mdf_iters: int = 0):
     if d.get("csrc_sha") != csrc_sha():
         return None, f"stale capture: profiles/r2_traffic.json is of build {d.get('csrc_sha')}, this is {csrc_sha()}"
     if d.get("world") != workload:
-        return None, f"capture is of world {d.get('world')}"
+        # captures of other workloads of the same build (e.g. "batch2") sit under "other_worlds"
+        o = d.get("other_worlds", {}).get(workload)
+        if not o:
+            return None, f"capture is of world {d.get('world')}"
+        v = o.get("dram_bytes_per_launch", {}).get(_SLOT_KERNEL.get(slot, ""))
+        return v, ("ncu --set full, " + o.get("command", "")) if v is not None else "kernel not captured"
     if slot == "K2b_spread":  # the K5 group of the MDF coupling: one figure for all its launches
         m = d.get("mdf", {})
         return (m.get("K5_group_bytes_per_step"), "ncu") if m.get("mdf_iters") == mdf_iters else (None, "no MDF capture")
@@ -317,7 +322,7 @@ def run_batch(args, rank, world_size, dev, dist, barrier):
     dom = max(kms, key=lambda k: kms[k])
     ach = kb[dom] / (kms[dom] * 1e-3) / 1e9 if kms[dom] > 0 else 0.0
     roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": None, "traffic_note": "no ncu capture of the batched launches", "peak_source": peak_src,
+                "traffic": ncu_traffic(dom, args.workload)[0], "traffic_note": ncu_traffic(dom, args.workload)[1], "peak_source": peak_src,
                 "frac_of_8TBps_nominal": ach / 8000.0, "algorithmic_bytes_per_launch": kb[dom],
                 "ms_per_launch": kms[dom], "share_of_step": kms[dom] / max(sum(kms.values()), 1e-12), "csrc_sha": csrc_sha()}
     roofline_step = {"bound": "hbm", "peak": peak, "unit": "GB/s", "models": {}}
